@@ -1,0 +1,121 @@
+/*
+ * wolff.h -- C-ABI boundary of the B200-native Wolff single-cluster hot path.
+ *
+ * Method: Y. Komura, Y. Okabe, "GPU-based single-cluster algorithm for the
+ * simulation of the Ising model", arXiv 1110.0899.  Citations below are
+ * "PAPER.md:<line> (section)" into the paper text this build was written from.
+ * DESIGN.md section 3 lists the readings (R1..R15) taken where the paper is
+ * silent; they are the same on both sides of the parity tests.
+ *
+ * What one update computes (section 2, steps i-v; Hamiltonian and
+ * periodic boundaries PAPER.md:36-40, Eq. 2; wave-front parallel growth
+ * PAPER.md:84-98, section 4): choose a site i0; let s0 be its spin; the cluster is
+ * the connected component of i0 in the graph whose edges are the lattice bonds
+ * between two spins equal to s0 whose bond variable is active (probability
+ * p = 1 - exp(-2J/T)); flip every spin of the cluster.  Bond
+ * variables are a pure function of (seed, update index, undirected edge), so the
+ * result does not depend on traversal order or thread schedule.
+ *
+ * Conventions
+ *   - Lattice: N = L^dim sites, int8 spins +1 / -1, site id i = x + L*y (+ L*L*z),
+ *     x fastest; periodic in every direction.
+ *   - All device state is owned by the library and lives on the CUDA device that is
+ *     current when wolff_create is called.  Every output buffer and the stream are
+ *     owned by the caller.  Pointers marked "host or device" may be either (they are
+ *     classified with cudaPointerGetAttributes); pageable host memory is allowed.
+ *   - Every call returns 0 (WOLFF_OK) or a negative error code; the reason is kept in
+ *     a thread-local string returned by wolff_last_error().  Nothing aborts, throws or
+ *     prints.  A CUDA error is sticky on the handle (later calls return WOLFF_ECUDA).
+ *   - A handle is not thread-safe; distinct handles are independent.
+ *   - There is no CPU fallback: without a usable CUDA device wolff_create fails.
+ */
+#ifndef WOLFF_B200_H
+#define WOLFF_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define WOLFF_API __attribute__((visibility("default")))
+#else
+#define WOLFF_API
+#endif
+
+#define WOLFF_OK      0
+#define WOLFF_EINVAL (-1)   /* bad argument */
+#define WOLFF_ENOMEM (-2)   /* device or host allocation failed */
+#define WOLFF_ECUDA  (-3)   /* CUDA runtime error (sticky on the handle) */
+#define WOLFF_EINTERNAL (-4) /* device-side watchdog fired (a barrier did not complete) */
+
+typedef struct wolff_ctx *wolff_handle;   /* opaque, library-owned */
+
+/* Create a chain.  dim = 2 (square) or 3 (simple cubic); L >= 2; N = L^dim <= 2^31;
+ * J >= 0 and T > 0 finite (J and T act only through the integer bond
+ * threshold floor((1 - exp(-2J/T)) * 2^32)).  Allocates the lattice, the
+ * cluster list (uint32 x N, the "ic/in" list of PAPER.md:50) and control words on the
+ * current device, fills the lattice with the seed-derived random +/-1 start
+ * (BASELINE.json configs: "random start from seed"), sets the update index to 0.
+ * Returns NULL on failure (see wolff_last_error). */
+WOLFF_API wolff_handle wolff_create(int dim, int L, double J, double T, uint64_t seed);
+
+/* Enqueue n_updates single-cluster updates (PAPER.md:42-48 steps i-v, grown wave-front
+ * parallel as in PAPER.md:84-98) on cuda_stream (a cudaStream_t passed as void*; NULL =
+ * the legacy default stream) as ONE persistent kernel launch, and return without waiting.
+ * Update indices continue from the handle's counter: run(a); run(b) equals run(a+b).
+ * n_updates == 0 is a no-op.  The per-update cluster sizes of this call are kept on the
+ * device until the next wolff_run (see wolff_observables). */
+WOLFF_API int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream);
+
+/* Wait for the handle's queued work, then compute on the device, from the CURRENT lattice,
+ * E = - sum over bonds s_i s_j (each bond once, units of J; Eq. 2) and
+ * M = sum s_i ("measurement of energy and magnetization"), and, if
+ * cluster_sizes != NULL, copy the n_updates cluster sizes of the MOST RECENT wolff_run
+ * (uint32 each; the final value of the counter "ic" of PAPER.md:50).  Any of the three
+ * pointers may be NULL; each may be host or device memory.  Blocks until done. */
+WOLFF_API int wolff_observables(wolff_handle h, int64_t *E, int64_t *M, uint32_t *cluster_sizes);
+
+/* Copy the lattice (N bytes, +1/-1, x fastest) to dst (host or device).  Blocks. */
+WOLFF_API int wolff_get_spins(wolff_handle h, int8_t *dst);
+
+/* Load a lattice (N bytes, each +1 or -1; host or device).  Used for cold starts, crafted
+ * cases and resuming.  Values other than +/-1 give WOLFF_EINVAL and leave the lattice
+ * unchanged.  Blocks. */
+WOLFF_API int wolff_set_spins(wolff_handle h, const int8_t *src);
+
+/* Update index (number of updates done since creation, or as set) and the integer bond
+ * threshold in [0, 2^32].  Either pointer may be NULL (host pointers). */
+WOLFF_API int wolff_get_state(wolff_handle h, uint64_t *update_index, uint64_t *threshold);
+
+/* Set the update index (to resume a chain: lattice + index + seed is the whole state). */
+WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
+
+/* Tuning / test knobs; never change the result.  Keys:
+ *   "mode"           0 = auto (default), 1 = force every level grid-wide, 2 = force one-CTA
+ *                    levels whenever the frontier fits the shared-memory queue
+ *   "up_threshold"   frontier width above which growth leaves one-CTA mode (1..queue cap)
+ *   "down_threshold" frontier width at or below which grid-wide growth returns to one CTA
+ *   "grid_ctas"      number of CTAs of the persistent kernel (0 = one per SM)
+ * Unknown key or out-of-range value: WOLFF_EINVAL. */
+WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);
+
+/* Counters of the most recent wolff_run, for the latency roofline (host pointer, 8 values):
+ *   [0] updates  [1] flipped spins  [2] one-CTA levels  [3] grid-wide levels
+ *   [4] switches one-CTA -> grid    [5] switches grid -> one-CTA
+ *   [6] claim attempts (atomics)    [7] widest frontier seen
+ * Blocks until the run has finished. */
+#define WOLFF_NSTATS 8
+WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
+
+/* Free everything.  NULL is allowed. */
+WOLFF_API int wolff_destroy(wolff_handle h);
+
+/* Reason for the last failure on this thread (static storage, never NULL). */
+WOLFF_API const char *wolff_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WOLFF_B200_H */

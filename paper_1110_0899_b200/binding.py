@@ -1,0 +1,181 @@
+"""ctypes binding of include/wolff.h -- argument marshalling only; every step runs in the CUDA library.
+
+PyTorch appears here only as a source of device pointers (`tensor.data_ptr()`) and streams
+(`torch.cuda.current_stream().cuda_stream`).  If `libwolff_b200.so` is missing this module raises; there is no
+CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import threading
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libwolff_b200.so")
+
+WOLFF_OK, WOLFF_EINVAL, WOLFF_ENOMEM, WOLFF_ECUDA, WOLFF_EINTERNAL = 0, -1, -2, -3, -4
+NSTATS = 8
+STAT_NAMES = ("updates", "flipped", "levels_cta", "levels_grid", "switch_up", "switch_down", "claim_attempts",
+              "widest_frontier")
+
+# every symbol include/wolff.h declares (tests/test_abi.py checks the header against this table)
+_SIGNATURES = {
+    "wolff_create": (ctypes.c_void_p, [ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_uint64]),
+    "wolff_run": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p]),
+    "wolff_observables": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_get_spins": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_set_spins": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]),
+    "wolff_set_update_index": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_uint64]),
+    "wolff_set_option": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_char_p, ctypes.c_int64]),
+    "wolff_get_stats": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]),
+    "wolff_destroy": (ctypes.c_int, [ctypes.c_void_p]),
+    "wolff_last_error": (ctypes.c_char_p, []),
+}
+
+_lock = threading.Lock()
+_lib = None
+
+
+class WolffError(RuntimeError):
+    def __init__(self, code: int, message: str):
+        super().__init__("wolff error %d: %s" % (code, message))
+        self.code = code
+
+
+def load() -> ctypes.CDLL:
+    """Load libwolff_b200.so (built in-tree by `paper_1110_0899_b200.build`).  Fails loudly when absent."""
+    global _lib
+    with _lock:
+        if _lib is None:
+            if not os.path.exists(LIB_PATH):
+                raise ImportError(
+                    "%s is missing: build it with `python -m paper_1110_0899_b200.build` "
+                    "(needs nvcc; there is no CPU fallback)" % LIB_PATH)
+            lib = ctypes.CDLL(LIB_PATH)
+            for name, (restype, argtypes) in _SIGNATURES.items():
+                fn = getattr(lib, name)        # AttributeError if the symbol is not exported
+                fn.restype, fn.argtypes = restype, argtypes
+            _lib = lib
+        return _lib
+
+
+def last_error() -> str:
+    return load().wolff_last_error().decode()
+
+
+def _ptr(buf):
+    """Raw address of a torch tensor (host or device), a numpy array, an int address, or None."""
+    if buf is None:
+        return None
+    if isinstance(buf, int):
+        return buf
+    if isinstance(buf, np.ndarray):
+        return buf.ctypes.data
+    if hasattr(buf, "data_ptr"):
+        return buf.data_ptr()
+    raise TypeError("expected a torch tensor, numpy array, int address or None")
+
+
+def _stream_handle(stream):
+    if stream is None:
+        return None
+    if isinstance(stream, int):
+        return stream
+    return stream.cuda_stream            # torch.cuda.Stream
+
+
+class Wolff:
+    """One Wolff single-cluster chain on the current CUDA device (wolff_create .. wolff_destroy)."""
+
+    def __init__(self, dim: int, L: int, J: float, T: float, seed: int):
+        self._lib = load()
+        self._h = self._lib.wolff_create(int(dim), int(L), float(J), float(T), int(seed))
+        if not self._h:
+            raise WolffError(WOLFF_EINVAL, last_error())
+        self.dim, self.L, self.N = int(dim), int(L), int(L) ** int(dim)
+        self.last_n = 0
+
+    # -- lifetime
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.wolff_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int):
+        if rc != WOLFF_OK:
+            raise WolffError(rc, last_error())
+
+    # -- the four calls north_star names
+    def run(self, n_updates: int, stream=None):
+        """wolff_run: enqueue n_updates updates on `stream` (torch.cuda.Stream, raw handle or None) and return."""
+        self._check(self._lib.wolff_run(self._h, int(n_updates), _stream_handle(stream)))
+        if n_updates:
+            self.last_n = int(n_updates)
+
+    def observables_into(self, E=None, M=None, cluster_sizes=None):
+        """wolff_observables with caller-owned buffers (torch tensors on host/device, numpy arrays, or None)."""
+        self._check(self._lib.wolff_observables(self._h, _ptr(E), _ptr(M), _ptr(cluster_sizes)))
+
+    def observables(self, sizes: bool = False):
+        """(E, M) of the current lattice, plus the last run's cluster sizes when sizes=True (numpy, host)."""
+        em = np.zeros(2, dtype=np.int64)
+        out = np.empty(self.last_n, dtype=np.uint32) if sizes and self.last_n else None
+        self._check(self._lib.wolff_observables(self._h, em.ctypes.data, em.ctypes.data + 8, _ptr(out)))
+        if sizes:
+            return int(em[0]), int(em[1]), (out if out is not None else np.empty(0, dtype=np.uint32))
+        return int(em[0]), int(em[1])
+
+    def get_spins_into(self, dst):
+        self._check(self._lib.wolff_get_spins(self._h, _ptr(dst)))
+
+    def get_spins(self) -> np.ndarray:
+        out = np.empty(self.N, dtype=np.int8)
+        self.get_spins_into(out)
+        return out
+
+    # -- hooks
+    def set_spins(self, src):
+        if isinstance(src, np.ndarray):
+            src = np.ascontiguousarray(src, dtype=np.int8).reshape(-1)
+            if src.size != self.N:
+                raise ValueError("need N = %d spins" % self.N)
+        self._check(self._lib.wolff_set_spins(self._h, _ptr(src)))
+
+    @property
+    def update_index(self) -> int:
+        u = ctypes.c_uint64()
+        self._check(self._lib.wolff_get_state(self._h, ctypes.byref(u), None))
+        return int(u.value)
+
+    @update_index.setter
+    def update_index(self, u: int):
+        self._check(self._lib.wolff_set_update_index(self._h, int(u)))
+
+    @property
+    def threshold(self) -> int:
+        t = ctypes.c_uint64()
+        self._check(self._lib.wolff_get_state(self._h, None, ctypes.byref(t)))
+        return int(t.value)
+
+    def set_option(self, key: str, value: int):
+        self._check(self._lib.wolff_set_option(self._h, key.encode(), int(value)))
+
+    def stats(self) -> dict:
+        buf = (ctypes.c_uint64 * NSTATS)()
+        self._check(self._lib.wolff_get_stats(self._h, buf))
+        return dict(zip(STAT_NAMES, (int(x) for x in buf)))

@@ -1,0 +1,345 @@
+// api.cu -- the extern "C" boundary declared in include/wolff.h (host side only).
+#include <cmath>
+#include <cstdarg>
+#include <cstddef>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/wolff.h"
+#include "internal.h"
+
+using namespace wolff;
+
+namespace {
+
+thread_local char g_error[512] = "";
+
+void set_error(const char *fmt, ...) __attribute__((format(printf, 1, 2)));
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_error, sizeof(g_error), fmt, ap);
+    va_end(ap);
+}
+
+}  // namespace
+
+struct wolff_ctx {
+    int dim = 0, L = 0;
+    double J = 0, T = 0;
+    uint64_t seed = 0;
+    uint64_t N = 0;
+    uint64_t thr = 0;
+    uint64_t u = 0;                 // next update index
+    int device = 0;
+    int num_sms = 0;
+    Geometry geo{};
+    int8_t *spins = nullptr;
+    uint32_t *clist = nullptr;
+    uint32_t *sizes = nullptr;
+    uint64_t sizes_cap = 0;         // entries allocated
+    uint64_t last_n = 0;            // updates in the most recent wolff_run
+    Control *ctl = nullptr;
+    cudaStream_t last_stream = nullptr;
+    bool cuda_failed = false;
+    bool ran = false;
+    // knobs
+    int mode = 0;
+    uint32_t qcap = 0;
+    uint32_t up = 0, down = 0;
+    int grid_ctas = 0;              // 0 = one per SM
+    int max_ctas = 0;               // co-resident limit
+    size_t smem_bytes = 0;
+};
+
+namespace {
+
+int fail_cuda(wolff_ctx *h, cudaError_t e, const char *what)
+{
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    if (h) h->cuda_failed = true;
+    return WOLFF_ECUDA;
+}
+
+#define CHECK_CUDA(h, call, what)                                   \
+    do {                                                            \
+        cudaError_t e_ = (call);                                    \
+        if (e_ != cudaSuccess) return fail_cuda((h), e_, (what));   \
+    } while (0)
+
+int check_handle(wolff_ctx *h)
+{
+    if (!h) { set_error("null handle"); return WOLFF_EINVAL; }
+    if (h->cuda_failed) { set_error("handle is in a failed CUDA state"); return WOLFF_ECUDA; }
+    cudaError_t e = cudaSetDevice(h->device);
+    if (e != cudaSuccess) return fail_cuda(h, e, "cudaSetDevice");
+    return WOLFF_OK;
+}
+
+// Reading R7: p = -expm1(-2J/T) in IEEE double, thr = floor(p * 2^32) in [0, 2^32].
+uint64_t bond_threshold(double J, double T)
+{
+    const double p = -std::expm1(-2.0 * J / T);
+    if (!(p > 0.0)) return 0;
+    const double scaled = std::floor(std::ldexp(p, 32));
+    if (scaled >= 4294967296.0) return 4294967296ull;
+    return (uint64_t)scaled;
+}
+
+void effective_thresholds(const wolff_ctx *h, uint32_t *up, uint32_t *down)
+{
+    const uint32_t up_max = h->qcap / (2u * (uint32_t)h->dim);   // the next level must fit one queue buffer
+    if (h->mode == 1) { *up = 0; *down = 0; return; }            // every level grid-wide
+    if (h->mode == 2) { *up = up_max; *down = up_max; return; }  // one CTA whenever it fits
+    uint32_t u = h->up < up_max ? h->up : up_max;
+    uint32_t d = h->down < u ? h->down : u;
+    *up = u; *down = d;
+}
+
+int sync_and_check(wolff_ctx *h)
+{
+    CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+    if (h->ran) {
+        unsigned int err = 0;
+        CHECK_CUDA(h, cudaMemcpy(&err, &h->ctl->error, sizeof(err), cudaMemcpyDeviceToHost), "read error flag");
+        if (err != 0) {
+            set_error("device watchdog: a grid barrier did not complete (error flag %u)", err);
+            h->cuda_failed = true;
+            return WOLFF_EINTERNAL;
+        }
+    }
+    return WOLFF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *wolff_last_error(void) { return g_error; }
+
+wolff_handle wolff_create(int dim, int L, double J, double T, uint64_t seed)
+{
+    if (dim != 2 && dim != 3) { set_error("dim must be 2 or 3 (got %d)", dim); return nullptr; }
+    if (L < 2) { set_error("L must be >= 2 (got %d)", L); return nullptr; }
+    if (!(J >= 0.0) || !std::isfinite(J)) { set_error("J must be finite and >= 0"); return nullptr; }
+    if (!(T > 0.0) || !std::isfinite(T)) { set_error("T must be finite and > 0"); return nullptr; }
+    uint64_t N = 1;
+    for (int k = 0; k < dim; ++k) {
+        N *= (uint64_t)L;
+        if (N > (1ull << 31)) { set_error("N = L^dim exceeds 2^31"); return nullptr; }
+    }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        set_error("no usable CUDA device (%s); this library has no CPU fallback", cudaGetErrorString(e));
+        return nullptr;
+    }
+    wolff_ctx *h = new (std::nothrow) wolff_ctx();
+    if (!h) { set_error("out of host memory"); return nullptr; }
+    h->dim = dim; h->L = L; h->J = J; h->T = T; h->seed = seed; h->N = N;
+    h->thr = bond_threshold(J, T);
+    h->geo.L = (uint32_t)L;
+    h->geo.N = (uint32_t)N;
+    h->geo.LL = (uint32_t)((uint64_t)L * (uint64_t)L);
+    h->geo.pow2 = ((L & (L - 1)) == 0) ? 1u : 0u;
+    h->geo.logL = 0;
+    if (h->geo.pow2) while ((1u << h->geo.logL) < (uint32_t)L) ++h->geo.logL;
+
+    cudaDeviceProp prop{};
+    bool ok = cudaGetDevice(&h->device) == cudaSuccess && cudaGetDeviceProperties(&prop, h->device) == cudaSuccess;
+    if (!ok) { set_error("cudaGetDeviceProperties failed"); delete h; return nullptr; }
+    if (!prop.cooperativeLaunch) { set_error("device lacks cooperative launch"); delete h; return nullptr; }
+    h->num_sms = prop.multiProcessorCount;
+
+    h->qcap = 8192;                       // entries per queue buffer: 2 x 32 KiB of shared memory
+    h->smem_bytes = 2ull * h->qcap * sizeof(uint32_t);
+    h->up = 256; h->down = 96;
+    int per_sm = 0;
+    e = growth_max_ctas(dim, h->geo.pow2 != 0, h->smem_bytes, &per_sm);
+    if (e != cudaSuccess || per_sm < 1) {
+        set_error("growth kernel cannot be made resident: %s", cudaGetErrorString(e));
+        delete h; return nullptr;
+    }
+    h->max_ctas = per_sm * h->num_sms;
+
+    // N spins padded to a multiple of 16 bytes; N list entries; control block
+    const size_t lattice_bytes = (size_t)((N + 15ull) & ~15ull);
+    if (cudaMalloc(&h->spins, lattice_bytes) != cudaSuccess || cudaMalloc(&h->clist, (size_t)N * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&h->ctl, sizeof(Control)) != cudaSuccess) {
+        set_error("device allocation failed for N = %llu", (unsigned long long)N);
+        wolff_destroy(h);
+        return nullptr;
+    }
+    e = cudaMemset(h->ctl, 0, sizeof(Control));
+    if (e == cudaSuccess) e = cudaMemset(h->spins, 0, lattice_bytes);
+    if (e == cudaSuccess) e = launch_init_lattice(h->spins, h->geo.N, seed, nullptr);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        set_error("lattice initialisation failed: %s", cudaGetErrorString(e));
+        wolff_destroy(h);
+        return nullptr;
+    }
+    return h;
+}
+
+int wolff_destroy(wolff_handle h)
+{
+    if (!h) return WOLFF_OK;
+    cudaSetDevice(h->device);
+    if (h->last_stream || h->ran) cudaStreamSynchronize(h->last_stream);
+    cudaFree(h->spins);
+    cudaFree(h->clist);
+    cudaFree(h->sizes);
+    cudaFree(h->ctl);
+    delete h;
+    return WOLFF_OK;
+}
+
+int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (n_updates == 0) return WOLFF_OK;
+    if (n_updates > (1ull << 32)) { set_error("n_updates too large for one call (max 2^32)"); return WOLFF_EINVAL; }
+    if (h->ran && stream != h->last_stream) {
+        // the size log and control block are about to be reused: finish the previous run first
+        CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+    }
+    if (n_updates > h->sizes_cap) {
+        if (h->ran) CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+        uint64_t cap = h->sizes_cap ? h->sizes_cap : 1024;
+        while (cap < n_updates) cap *= 2;
+        uint32_t *fresh = nullptr;
+        if (cudaMalloc(&fresh, (size_t)cap * sizeof(uint32_t)) != cudaSuccess) {
+            cudaGetLastError();
+            set_error("cannot allocate the cluster-size log for %llu updates", (unsigned long long)n_updates);
+            return WOLFF_ENOMEM;
+        }
+        cudaFree(h->sizes);
+        h->sizes = fresh;
+        h->sizes_cap = cap;
+    }
+    GrowthParams p{};
+    p.spins = h->spins; p.clist = h->clist; p.sizes = h->sizes; p.ctl = h->ctl; p.geo = h->geo;
+    p.key0 = (uint32_t)h->seed; p.key1 = (uint32_t)(h->seed >> 32);
+    p.thr = h->thr; p.u0 = h->u; p.n_updates = n_updates; p.qcap = h->qcap;
+    effective_thresholds(h, &p.up, &p.down);
+    int ctas = h->grid_ctas > 0 ? h->grid_ctas : h->num_sms;
+    if (ctas > h->max_ctas) ctas = h->max_ctas;
+    // control words of the growth kernel start from zero at every launch (generation 0)
+    CHECK_CUDA(h, cudaMemsetAsync(h->ctl, 0, offsetof(Control, acc_unequal), stream), "cudaMemsetAsync(control)");
+    CHECK_CUDA(h, launch_growth(p, h->dim, ctas, h->smem_bytes, stream), "launch growth kernel");
+    h->u += n_updates;
+    h->last_n = n_updates;
+    h->last_stream = stream;
+    h->ran = true;
+    return WOLFF_OK;
+}
+
+int wolff_observables(wolff_handle h, int64_t *E, int64_t *M, uint32_t *cluster_sizes)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    rc = sync_and_check(h);
+    if (rc) return rc;
+    cudaStream_t s = h->last_stream;
+    if (E || M) {
+        CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, h->num_sms, s), "launch E/M reduction");
+        if (E) CHECK_CUDA(h, cudaMemcpyAsync(E, &h->ctl->E, sizeof(int64_t), cudaMemcpyDefault, s), "copy E");
+        if (M) CHECK_CUDA(h, cudaMemcpyAsync(M, &h->ctl->M, sizeof(int64_t), cudaMemcpyDefault, s), "copy M");
+    }
+    if (cluster_sizes && h->last_n > 0)
+        CHECK_CUDA(h, cudaMemcpyAsync(cluster_sizes, h->sizes, (size_t)h->last_n * sizeof(uint32_t), cudaMemcpyDefault, s),
+                   "copy cluster sizes");
+    CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_get_spins(wolff_handle h, int8_t *dst)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    if (!dst) { set_error("dst is NULL"); return WOLFF_EINVAL; }
+    rc = sync_and_check(h);
+    if (rc) return rc;
+    CHECK_CUDA(h, cudaMemcpyAsync(dst, h->spins, (size_t)h->N, cudaMemcpyDefault, h->last_stream), "copy lattice out");
+    CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_set_spins(wolff_handle h, const int8_t *src)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    if (!src) { set_error("src is NULL"); return WOLFF_EINVAL; }
+    rc = sync_and_check(h);
+    if (rc) return rc;
+    cudaStream_t s = h->last_stream;
+    // stage in the cluster list (N * 4 bytes, idle between runs), validate there, then commit
+    int8_t *staging = reinterpret_cast<int8_t *>(h->clist);
+    CHECK_CUDA(h, cudaMemcpyAsync(staging, src, (size_t)h->N, cudaMemcpyDefault, s), "copy lattice in");
+    CHECK_CUDA(h, cudaMemsetAsync(&h->ctl->invalid, 0, sizeof(unsigned int), s), "reset validation flag");
+    CHECK_CUDA(h, launch_validate(staging, h->geo.N, h->ctl, s), "launch validation");
+    unsigned int invalid = 0;
+    CHECK_CUDA(h, cudaMemcpyAsync(&invalid, &h->ctl->invalid, sizeof(invalid), cudaMemcpyDeviceToHost, s), "read validation flag");
+    CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    if (invalid) { set_error("set_spins: every byte must be +1 or -1"); return WOLFF_EINVAL; }
+    CHECK_CUDA(h, cudaMemcpyAsync(h->spins, staging, (size_t)h->N, cudaMemcpyDeviceToDevice, s), "commit lattice");
+    CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_get_state(wolff_handle h, uint64_t *update_index, uint64_t *threshold)
+{
+    if (!h) { set_error("null handle"); return WOLFF_EINVAL; }
+    if (update_index) *update_index = h->u;
+    if (threshold) *threshold = h->thr;
+    return WOLFF_OK;
+}
+
+int wolff_set_update_index(wolff_handle h, uint64_t update_index)
+{
+    if (!h) { set_error("null handle"); return WOLFF_EINVAL; }
+    h->u = update_index;
+    return WOLFF_OK;
+}
+
+int wolff_set_option(wolff_handle h, const char *key, int64_t value)
+{
+    if (!h || !key) { set_error("null handle or key"); return WOLFF_EINVAL; }
+    const uint32_t up_max = h->qcap / (2u * (uint32_t)h->dim);
+    if (!strcmp(key, "mode")) {
+        if (value < 0 || value > 2) { set_error("mode must be 0, 1 or 2"); return WOLFF_EINVAL; }
+        h->mode = (int)value;
+    } else if (!strcmp(key, "up_threshold")) {
+        if (value < 1 || value > (int64_t)up_max) { set_error("up_threshold must be in [1, %u]", up_max); return WOLFF_EINVAL; }
+        h->up = (uint32_t)value;
+    } else if (!strcmp(key, "down_threshold")) {
+        if (value < 0 || value > (int64_t)up_max) { set_error("down_threshold must be in [0, %u]", up_max); return WOLFF_EINVAL; }
+        h->down = (uint32_t)value;
+    } else if (!strcmp(key, "grid_ctas")) {
+        if (value < 0 || value > h->max_ctas) { set_error("grid_ctas must be in [0, %d]", h->max_ctas); return WOLFF_EINVAL; }
+        h->grid_ctas = (int)value;
+    } else {
+        set_error("unknown option '%s'", key);
+        return WOLFF_EINVAL;
+    }
+    return WOLFF_OK;
+}
+
+int wolff_get_stats(wolff_handle h, uint64_t *stats)
+{
+    int rc = check_handle(h);
+    if (rc) return rc;
+    if (!stats) { set_error("stats is NULL"); return WOLFF_EINVAL; }
+    rc = sync_and_check(h);
+    if (rc) return rc;
+    if (!h->ran) { memset(stats, 0, WOLFF_NSTATS * sizeof(uint64_t)); return WOLFF_OK; }
+    CHECK_CUDA(h, cudaMemcpy(stats, h->ctl->stats, WOLFF_NSTATS * sizeof(uint64_t), cudaMemcpyDeviceToHost), "read stats");
+    return WOLFF_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,140 @@
+// device_common.cuh -- device-side building blocks shared by the kernels of libwolff_b200.
+//
+// Nothing here is shared with oracle/: the oracle has its own plain-C statement of the same
+// definitions (readings R5-R11).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace wolff {
+
+// ---------------------------------------------------------------- Philox4x32-10 (reading R11)
+// Salmon et al., SC'11.  One round maps (c0,c1,c2,c3) to
+// (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)); the key is bumped by the Weyl
+// constants between rounds.  Written as two 32x32->64 multiplies per round (IMAD.WIDE.U32).
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u;
+constexpr uint32_t kPhiloxM1 = 0xCD9E8D57u;
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u;
+constexpr uint32_t kPhiloxW1 = 0xBB67AE85u;
+
+// Domain tags (bits 31:30 of counter word 1) keep the three streams disjoint (reading R10).
+constexpr uint32_t kDomainBond = 0u << 30;
+constexpr uint32_t kDomainSite = 1u << 30;
+constexpr uint32_t kDomainInit = 2u << 30;
+
+__device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                               uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * (uint64_t)c0;
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * (uint64_t)c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+        k0 += kPhiloxW0;
+        k1 += kPhiloxW1;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+__device__ __forceinline__ uint32_t word_of(const uint4 &v, int d)
+{
+    return d == 0 ? v.x : (d == 1 ? v.y : (d == 2 ? v.z : v.w));
+}
+
+// ---------------------------------------------------------------- lattice geometry (reading R5)
+// Site id i = x + L*y (+ L*L*z).  nbr[2d] is the +d neighbour, nbr[2d+1] the -d neighbour,
+// coordinates wrap periodically.
+struct Geometry {
+    uint32_t L;      // linear size
+    uint32_t N;      // L^dim   (N <= 2^31)
+    uint32_t LL;     // L*L
+    uint32_t logL;   // log2 L when L is a power of two, else 0
+    uint32_t pow2;   // 1 when L is a power of two
+};
+
+template <int DIM, bool POW2>
+__device__ __forceinline__ void neighbours(const Geometry &g, uint32_t i, uint32_t (&nbr)[2 * DIM])
+{
+    uint32_t x, y, z = 0;
+    if (POW2) {
+        const uint32_t mask = g.L - 1u;
+        x = i & mask;
+        y = (i >> g.logL) & mask;
+        if (DIM == 3) z = i >> (2u * g.logL);
+    } else {
+        x = i % g.L;
+        const uint32_t t = i / g.L;
+        y = t % g.L;
+        if (DIM == 3) z = t / g.L;
+    }
+    const uint32_t Lm1 = g.L - 1u;
+    nbr[0] = (x == Lm1) ? i - Lm1 : i + 1u;
+    nbr[1] = (x == 0u) ? i + Lm1 : i - 1u;
+    const uint32_t ywrap = g.LL - g.L;                 // L*(L-1)
+    nbr[2] = (y == Lm1) ? i - ywrap : i + g.L;
+    nbr[3] = (y == 0u) ? i + ywrap : i - g.L;
+    if (DIM == 3) {
+        const uint32_t zwrap = g.N - g.LL;             // L*L*(L-1)
+        nbr[4] = (z == Lm1) ? i - zwrap : i + g.LL;
+        nbr[5] = (z == 0u) ? i + zwrap : i - g.LL;
+    }
+}
+
+// ---------------------------------------------------------------- spins
+// int8 storage, +1 = 0x01, -1 = 0xFF.  All lattice reads in the growth kernel bypass L1
+// (ld.global.cg): the kernel is persistent across updates, and an L1 line cached during an
+// earlier update could show a spin with its old sign.
+__device__ __forceinline__ int load_spin_l2(const int8_t *spins, uint32_t i)
+{
+    return (int)__ldcg(reinterpret_cast<const signed char *>(spins) + i);
+}
+
+// Claim-and-flip: one atomic on the 32-bit word containing byte j that
+// sets the byte to -s0 and returns whether THIS thread changed it from s0.  CUDA has no 8-bit
+// CAS; with +1 = 0x01 and -1 = 0xFF the transition s0 -> -s0 is an idempotent bit operation
+// (OR 0xFE for +1 -> -1, AND 0x01 for -1 -> +1), so a single atom.or / atom.and has exactly
+// the semantics of CAS(s0 -> -s0) and never needs a retry when a sibling byte changes.
+__device__ __forceinline__ bool claim_and_flip(int8_t *spins, uint32_t j, int s0)
+{
+    unsigned int *word = reinterpret_cast<unsigned int *>(spins) + (j >> 2);
+    const unsigned int shift = (j & 3u) * 8u;
+    unsigned int old;
+    if (s0 > 0) old = atomicOr(word, 0xFEu << shift);
+    else        old = atomicAnd(word, ~(0xFEu << shift));
+    return ((old >> shift) & 0xFFu) == ((unsigned int)s0 & 0xFFu);
+}
+
+// ---------------------------------------------------------------- inter-CTA synchronisation words
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p)
+{
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_u64(unsigned long long *p, unsigned long long v)
+{
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned int atom_add_acq_rel_u32(unsigned int *p, unsigned int v)
+{
+    unsigned int old;
+    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
+    return old;
+}
+__device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int *p)
+{
+    unsigned int v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed_u32(unsigned int *p, unsigned int v)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+}  // namespace wolff

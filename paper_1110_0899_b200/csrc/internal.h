@@ -1,0 +1,72 @@
+// internal.h -- host/device shared declarations of libwolff_b200 (not part of the public ABI).
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "device_common.cuh"
+
+namespace wolff {
+
+// Phases carried in the barrier word (bits 39:32).
+enum Phase : unsigned int {
+    kPhaseGrid = 1,    // next level is grid-wide
+    kPhaseToCta = 2,   // frontier shrank: CTA 0 continues alone from the window [lo, hi)
+    kPhaseDone = 3,    // the frontier is empty: the update's cluster is complete
+    kPhaseExit = 4,    // all updates of this launch are done
+    kPhaseAbort = 5    // watchdog fired
+};
+
+// Global-memory control block of one handle.  Every hot word sits in its own 128-byte line.
+struct alignas(128) Control {
+    // [gen:24 | phase:8 | hi:32]; polled by every CTA, written by the last arriver / by CTA 0.
+    unsigned long long bar;
+    unsigned char pad0[120];
+    unsigned int arrive;          // grid barrier arrival counter
+    unsigned char pad1[124];
+    unsigned int tail;            // append cursor of the cluster list
+    unsigned char pad2[124];
+    // descriptor of a grid phase, written by CTA 0 before it releases the other CTAs
+    unsigned int lo;
+    int s0;
+    unsigned long long u;
+    unsigned char pad3[112];
+    unsigned int error;           // nonzero: a barrier timed out
+    unsigned int pad4;
+    unsigned long long stats[8];  // see WOLFF_NSTATS in wolff.h
+    unsigned char pad5[56];
+    // E/M reduction scratch
+    unsigned long long acc_unequal;
+    unsigned long long acc_negative;
+    unsigned int ticket;
+    unsigned int invalid;         // set_spins validation
+    long long E;
+    long long M;
+};
+
+struct GrowthParams {
+    int8_t *spins;
+    uint32_t *clist;        // cluster list, N entries
+    uint32_t *sizes;        // per-update cluster sizes of this launch
+    Control *ctl;
+    Geometry geo;
+    uint32_t key0, key1;    // Philox key = seed
+    unsigned long long thr; // bond threshold in [0, 2^32]
+    unsigned long long u0;  // first update index of this launch
+    unsigned long long n_updates;
+    uint32_t up;            // leave one-CTA mode when the frontier is wider than this
+    uint32_t down;          // return to one-CTA mode when the frontier is at most this wide
+    uint32_t qcap;          // entries per shared-memory queue buffer
+};
+
+constexpr int kGrowthThreads = 512;
+
+// launchers (defined next to their kernels)
+cudaError_t launch_growth(const GrowthParams &p, int dim, int grid_ctas, size_t smem_bytes, cudaStream_t stream);
+cudaError_t growth_max_ctas(int dim, bool pow2, size_t smem_bytes, int *ctas_per_sm);
+cudaError_t growth_prepare(int dim, bool pow2, size_t smem_bytes);
+cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, cudaStream_t stream);
+cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, cudaStream_t stream);
+cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo, int dim, Control *ctl,
+                                        int num_sms, cudaStream_t stream);
+
+}  // namespace wolff

@@ -1,0 +1,129 @@
+"""GPU-vs-oracle parity through the C-ABI: lattice bytes, per-update cluster sizes, integer E and M, bit-exact.
+
+Tolerance: none.  Everything on the path is integer (int8 spins, uint32 bond words against a uint32 threshold,
+int64 sums); the one floating-point step, the threshold, is compared first (reading R7).
+"""
+import numpy as np
+import pytest
+
+from paper_1110_0899_b200 import workloads as wl
+from parity_util import assert_same_state, compare_batched, compare_stepwise, make_pair
+
+pytestmark = pytest.mark.gpu
+
+MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 0, "up_threshold": 8, "down_threshold": 3},
+         {"mode": 1, "grid_ctas": 3}, {"mode": 0, "up_threshold": 40, "down_threshold": 40, "grid_ctas": 16}]
+
+
+# ------------------------------------------------------------------ BASELINE config C1, exactly as written
+@pytest.mark.parametrize("options", MODES[:3])
+def test_config_c1_every_update(options):
+    c = wl.CONFIGS["C1"]
+    gpu, ref = make_pair(*c.create_args(), options=options)
+    assert_same_state(gpu, ref, "start lattice (reading R9)")
+    compare_stepwise(gpu, ref, c.n_meas, lattice_every=100)
+
+
+# ------------------------------------------------------------------ small and degenerate lattices, every growth mode
+SMALL = [(2, 2, 2.0), (2, 3, 2.0), (2, 4, wl.TC_2D), (2, 6, 1.8), (2, 5, 3.0), (3, 2, 4.0), (3, 3, wl.TC_3D),
+         (3, 4, wl.TC_3D), (3, 6, 4.0), (2, 16, wl.TC_2D), (3, 8, wl.TC_3D), (2, 48, 2.1), (3, 12, 4.2)]
+
+
+@pytest.mark.parametrize("options", MODES)
+@pytest.mark.parametrize("dim,L,T", SMALL)
+def test_small_lattices_stepwise(dim, L, T, options):
+    gpu, ref = make_pair(dim, L, 1.0, T, seed=7 + L, options=options)
+    assert_same_state(gpu, ref, "start")
+    compare_stepwise(gpu, ref, 60)
+
+
+@pytest.mark.parametrize("options", MODES)
+@pytest.mark.parametrize("dim,L", [(2, 64), (2, 100), (3, 16), (3, 20)])
+def test_p_one_cold_start_widest_frontiers(dim, L, options):
+    # thr = 2^32: the first update flips all N spins; frontiers are as wide as they get and every mode switch fires
+    N = L ** dim
+    gpu, ref = make_pair(dim, L, 1.0, 0.04, seed=3, start=wl.cold(N), options=options)
+    assert gpu.threshold == 1 << 32
+    compare_batched(gpu, ref, [1, 1, 3])
+    gpu.set_spins(wl.blobs(dim, L, seed=5))
+    ref.set_spins(wl.blobs(dim, L, seed=5))
+    compare_batched(gpu, ref, [1] * 6)
+
+
+@pytest.mark.parametrize("dim,L", [(2, 32), (3, 8)])
+def test_p_zero_only_the_seed_site_flips(dim, L):
+    gpu, ref = make_pair(dim, L, 0.0, 1.0, seed=11)
+    assert gpu.threshold == 0
+    gpu.run(200)
+    E, M, sz = gpu.observables(sizes=True)
+    assert np.all(sz == 1)
+    assert np.array_equal(sz, ref.run(200))
+    assert_same_state(gpu, ref)
+
+
+@pytest.mark.parametrize("maker", ["checkerboard", "stripes", "blobs", "random"])
+@pytest.mark.parametrize("dim,L,T", [(2, 64, 1.5), (3, 16, 3.0)])
+def test_crafted_start_lattices(dim, L, T, maker):
+    N = L ** dim
+    start = {"checkerboard": lambda: wl.checkerboard(dim, L), "stripes": lambda: wl.stripes(dim, L, 3, axis=1),
+             "blobs": lambda: wl.blobs(dim, L, 9), "random": lambda: wl.random_pm1(N, 4, 0.7)}[maker]()
+    gpu, ref = make_pair(dim, L, 1.0, T, seed=21, start=start)
+    compare_batched(gpu, ref, [1, 2, 17, 80])
+
+
+def test_split_run_equivalence_and_resume():
+    c = wl.CONFIGS["C1"]
+    a, ref = make_pair(*c.create_args())
+    b, _ = make_pair(*c.create_args())
+    a.run(7); a.run(13); a.run(1)
+    b.run(21)
+    assert np.array_equal(a.get_spins(), b.get_spins()) and a.observables() == b.observables()
+    ref.run(21)
+    assert_same_state(a, ref)
+    # resume: lattice + update index + seed is the whole state
+    c2, _ = make_pair(*c.create_args())
+    c2.set_spins(a.get_spins())
+    c2.update_index = a.update_index
+    a.run(50); c2.run(50); ref.run(50)
+    assert np.array_equal(a.get_spins(), c2.get_spins())
+    assert_same_state(c2, ref)
+
+
+def test_seeds_and_large_update_index():
+    gpu, ref = make_pair(2, 32, 1.0, wl.TC_2D, seed=(0xDEADBEEF << 32) | 0x12345678)
+    gpu.update_index = ref.update_index = (1 << 40) + 12345        # exercises u_hi in the Philox counter
+    compare_batched(gpu, ref, [40])
+
+
+# ------------------------------------------------------------------ medium sizes: several tiles, ragged tails
+@pytest.mark.parametrize("options", [{"mode": 0}, {"mode": 1}])
+@pytest.mark.parametrize("name,n", [("C2", 40), ("C4", 40)])
+def test_medium_configs_equilibrated_variant(name, n, options):
+    c = wl.CONFIGS[name]
+    gpu, ref = make_pair(*c.create_args(), start=wl.cold(c.N), options=options)
+    compare_batched(gpu, ref, [1, 4, n])
+
+
+@pytest.mark.parametrize("name", ["C2", "C4"])
+def test_medium_configs_literal_random_start(name):
+    c = wl.CONFIGS[name]
+    gpu, ref = make_pair(*c.create_args())
+    assert_same_state(gpu, ref, "start lattice")
+    compare_batched(gpu, ref, [1000])
+
+
+# ------------------------------------------------------------------ BASELINE full sizes in the bench's launch configuration
+@pytest.mark.parametrize("name,batches", [("C3", [1, 5]), ("C5a", [1, 8]), ("C5b", [2, 30])])
+def test_full_size_configs_equilibrated_variant(name, batches):
+    # cold start (the bench's 'equilibrated' variant): the first clusters span the lattice, then shrink towards T_c sizes
+    c = wl.CONFIGS[name]
+    gpu, ref = make_pair(*c.create_args(), start=wl.cold(c.N))
+    compare_batched(gpu, ref, batches)
+
+
+@pytest.mark.parametrize("name", ["C3", "C5a", "C5b"])
+def test_full_size_configs_literal_random_start(name):
+    c = wl.CONFIGS[name]
+    gpu, ref = make_pair(*c.create_args())
+    assert_same_state(gpu, ref, "start lattice")
+    compare_batched(gpu, ref, [1000, 2000])
