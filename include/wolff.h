@@ -109,6 +109,17 @@ WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);
 #define WOLFF_NSTATS 8
 WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
 
+/* Dependent-latency microbenchmarks on the current device (the links of one BFS level of the
+ * growth kernel, timed in isolation; they define the latency roofline bench.py reports).  Writes
+ * WOLFF_NMICRO doubles, nanoseconds each, to a host pointer:
+ *   [0] dependent L2 load, one lane (ld.global.cg over an L2-resident 16 MiB buffer)
+ *   [1] dependent L2 load, one warp, 32 scattered lines   [2] dependent atom.or with return, one lane
+ *   [3] dependent atom.or, one warp, 32 scattered words   [4] __syncthreads at 512 threads
+ *   [5] three Philox4x32-10 blocks, one warp              [6] the library's grid barrier, one CTA per SM
+ * Not part of the measured path. */
+#define WOLFF_NMICRO 7
+WOLFF_API int wolff_microbench(double *out_ns, int n_out);
+
 /* Free everything.  NULL is allowed. */
 WOLFF_API int wolff_destroy(wolff_handle h);
 

@@ -31,6 +31,7 @@ _SIGNATURES = {
     "wolff_set_update_index": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_uint64]),
     "wolff_set_option": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_char_p, ctypes.c_int64]),
     "wolff_get_stats": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]),
+    "wolff_microbench": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.c_int]),
     "wolff_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "wolff_last_error": (ctypes.c_char_p, []),
 }
@@ -85,6 +86,19 @@ def _stream_handle(stream):
     if isinstance(stream, int):
         return stream
     return stream.cuda_stream            # torch.cuda.Stream
+
+
+MICRO_NAMES = ("l2_load_lane_ns", "l2_load_warp_ns", "l2_atomic_lane_ns", "l2_atomic_warp_ns", "syncthreads_ns",
+               "philox_x3_ns", "grid_barrier_ns")
+
+
+def microbench() -> dict:
+    """wolff_microbench: the dependent latencies that bound one BFS level (nanoseconds)."""
+    buf = (ctypes.c_double * len(MICRO_NAMES))()
+    rc = load().wolff_microbench(buf, len(MICRO_NAMES))
+    if rc != WOLFF_OK:
+        raise WolffError(rc, "wolff_microbench failed")
+    return dict(zip(MICRO_NAMES, (float(x) for x in buf)))
 
 
 class Wolff:

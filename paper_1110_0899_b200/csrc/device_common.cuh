@@ -41,6 +41,36 @@ __device__ __forceinline__ uint4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_
     return make_uint4(c0, c1, c2, c3);
 }
 
+// K independent blocks with the rounds interleaved: the ten rounds of one block form a dependent
+// chain (IMAD.WIDE -> LOP3 -> IMAD.WIDE ...), so running K chains side by side costs about the
+// latency of one.  All blocks share counter words 1..3 and the key; only word 0 differs.
+template <int K>
+__device__ __forceinline__ void philox4x32_10_multi(const uint32_t (&ctr0)[K], uint32_t c1_, uint32_t c2_, uint32_t c3_,
+                                                    uint32_t k0, uint32_t k1, uint4 (&out)[K])
+{
+    uint32_t c0[K], c1[K], c2[K], c3[K];
+#pragma unroll
+    for (int j = 0; j < K; ++j) { c0[j] = ctr0[j]; c1[j] = c1_; c2[j] = c2_; c3[j] = c3_; }
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+#pragma unroll
+        for (int j = 0; j < K; ++j) {
+            const uint64_t p0 = (uint64_t)kPhiloxM0 * (uint64_t)c0[j];
+            const uint64_t p1 = (uint64_t)kPhiloxM1 * (uint64_t)c2[j];
+            const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1[j] ^ k0;
+            const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3[j] ^ k1;
+            c1[j] = (uint32_t)p1;
+            c3[j] = (uint32_t)p0;
+            c0[j] = n0;
+            c2[j] = n2;
+        }
+        k0 += kPhiloxW0;
+        k1 += kPhiloxW1;
+    }
+#pragma unroll
+    for (int j = 0; j < K; ++j) out[j] = make_uint4(c0[j], c1[j], c2[j], c3[j]);
+}
+
 __device__ __forceinline__ uint32_t word_of(const uint4 &v, int d)
 {
     return d == 0 ? v.x : (d == 1 ? v.y : (d == 2 ? v.z : v.w));
@@ -126,6 +156,13 @@ __device__ __forceinline__ unsigned int atom_add_acq_rel_u32(unsigned int *p, un
     asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
     return old;
 }
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long *p)
+{
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
 __device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int *p)
 {
     unsigned int v;

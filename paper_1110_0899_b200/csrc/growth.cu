@@ -35,7 +35,7 @@ __device__ __forceinline__ unsigned int bar_hi(unsigned long long w) { return (u
 __device__ __noinline__ unsigned long long wait_generation(Control *ctl, unsigned int want, bool bounded)
 {
     unsigned int polls = 0;
-    unsigned int ns = 20;
+    unsigned int ns = 32;
     for (;;) {
         const unsigned long long w = ld_acquire_u64(&ctl->bar);
         if (bar_gen(w) == (want & 0xFFFFFFu)) return w;
@@ -49,23 +49,25 @@ __device__ __noinline__ unsigned long long wait_generation(Control *ctl, unsigne
         }
         if (!bounded) {
             __nanosleep(ns);
-            if (ns < 160) ns += 20;
+            if (ns < 640) ns += ns >> 1;
         }
     }
 }
 
 // Expand one frontier site per lane (A2-A5): gather the 2*DIM neighbour spins, decide the bonds,
-// claim-and-flip, and append the winners to dst[] with ONE shared-memory atomic per warp
-// (ballot/popc aggregation).  Must be called by all 32 lanes of a warp.
+// claim-and-flip, and append the winners to dst[] with ONE atomic per warp on *dst_count
+// (ballot/popc aggregation).  dst/dst_count are the shared-memory queue in one-CTA mode and the
+// global cluster list and its tail in grid mode.  Must be called by all 32 lanes of a warp.
 template <int DIM, bool POW2>
 __device__ __forceinline__ void expand_sites(const GrowthParams &p, int s0, uint32_t u_lo, uint32_t u_hi,
                                              bool valid, uint32_t i, uint32_t *dst, unsigned int *dst_count,
                                              unsigned int &attempts)
 {
     uint32_t nbr[2 * DIM];
-    bool won[2 * DIM];
+    bool cand[2 * DIM];
+    unsigned int old[2 * DIM];
 #pragma unroll
-    for (int k = 0; k < 2 * DIM; ++k) { nbr[k] = 0u; won[k] = false; }
+    for (int k = 0; k < 2 * DIM; ++k) { nbr[k] = 0u; cand[k] = false; old[k] = 0u; }
 
     if (valid) {
         neighbours<DIM, POW2>(p.geo, i, nbr);
@@ -83,34 +85,44 @@ __device__ __forceinline__ void expand_sites(const GrowthParams &p, int s0, uint
             const uint4 bwd = philox4x32_10(nbr[2 * d + 1], kDomainBond, u_lo, u_hi, p.key0, p.key1);
             bondword[2 * d + 1] = word_of(bwd, d);
         }
-        // A4: claim-and-flip the same-sign neighbours behind active bonds
 #pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k) {
-            const bool candidate = (sp[k] == s0) && ((unsigned long long)bondword[k] < p.thr);
-            if (candidate) {
-                won[k] = claim_and_flip(p.spins, nbr[k], s0);
-                ++attempts;
-            }
-        }
+        for (int k = 0; k < 2 * DIM; ++k) cand[k] = (sp[k] == s0) && ((unsigned long long)bondword[k] < p.thr);
     }
 
-    // A5: warp-aggregated append
+    // A4: claim-and-flip the same-sign neighbours behind active bonds.  All atomics of a lane are
+    // issued before any result is looked at, so their L2 round trips overlap.
+    unsigned int *const words = reinterpret_cast<unsigned int *>(p.spins);
+    if (s0 > 0) {   // uniform for the whole update
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k)
+            if (cand[k]) old[k] = atomicOr(words + (nbr[k] >> 2), 0xFEu << ((nbr[k] & 3u) * 8u));
+    } else {
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k)
+            if (cand[k]) old[k] = atomicAnd(words + (nbr[k] >> 2), ~(0xFEu << ((nbr[k] & 3u) * 8u)));
+    }
+    const unsigned int s0_byte = (unsigned int)s0 & 0xFFu;
     unsigned int ballots[2 * DIM];
     unsigned int total = 0;
 #pragma unroll
     for (int k = 0; k < 2 * DIM; ++k) {
-        ballots[k] = __ballot_sync(kFullMask, won[k]);
+        const bool won = cand[k] && (((old[k] >> ((nbr[k] & 3u) * 8u)) & 0xFFu) == s0_byte);
+        attempts += cand[k] ? 1u : 0u;
+        ballots[k] = __ballot_sync(kFullMask, won);
         total += __popc(ballots[k]);
     }
+
+    // A5: warp-aggregated append
     if (total != 0u) {   // warp-uniform
         const unsigned int lane = threadIdx.x & 31u;
         unsigned int base = 0;
         if (lane == 0u) base = atomicAdd(dst_count, total);
         base = __shfl_sync(kFullMask, base, 0);
-        const unsigned int lt = (1u << lane) - 1u;
+        const unsigned int bit = 1u << lane;
+        const unsigned int lt = bit - 1u;
 #pragma unroll
         for (int k = 0; k < 2 * DIM; ++k) {
-            if (won[k]) dst[base + __popc(ballots[k] & lt)] = nbr[k];
+            if (ballots[k] & bit) dst[base + __popc(ballots[k] & lt)] = nbr[k];
             base += __popc(ballots[k]);
         }
     }
@@ -118,8 +130,6 @@ __device__ __forceinline__ void expand_sites(const GrowthParams &p, int s0, uint
 
 struct SharedState {
     unsigned int cnt[3];       // rotating level counters of the one-CTA queues
-    unsigned int stage_cnt;    // entries staged by this CTA in a grid-wide pass
-    unsigned int base;         // broadcast: slot returned by the global append
     int s0;                    // broadcast: seed spin of the current update
     unsigned long long word;   // broadcast: barrier word
 };
@@ -127,7 +137,7 @@ struct SharedState {
 // Grid-wide level loop over the global cluster list (A2-A6, grid mode).  Called by every CTA with
 // identical (lo, hi, gen); returns with the window/phase decided by the last CTA to arrive.
 template <int DIM, bool POW2>
-__device__ __forceinline__ unsigned int grid_levels(const GrowthParams &p, SharedState &sh, uint32_t *stage,
+__device__ __forceinline__ unsigned int grid_levels(const GrowthParams &p, SharedState &sh,
                                                     int s0, unsigned long long u, uint32_t &lo, uint32_t &hi,
                                                     unsigned int &gen, unsigned int &attempts,
                                                     unsigned long long &levels, uint32_t &widest)
@@ -148,23 +158,14 @@ __device__ __forceinline__ unsigned int grid_levels(const GrowthParams &p, Share
             const uint32_t begin = (uint32_t)begin64;
             const uint32_t end = (n - begin < per) ? n : begin + per;
             for (uint32_t pass = begin; pass < end; pass += T) {
-                if (tid == 0) sh.stage_cnt = 0u;
-                __syncthreads();
                 const uint32_t idx = pass + tid;
                 const bool valid = idx < end;
                 const uint32_t site = valid ? __ldcg(p.clist + lo + idx) : 0u;
-                expand_sites<DIM, POW2>(p, s0, u_lo, u_hi, valid, site, stage, &sh.stage_cnt, attempts);
-                __syncthreads();
-                const unsigned int c = sh.stage_cnt;
-                if (c != 0u) {   // CTA-uniform
-                    if (tid == 0) sh.base = atomicAdd(&ctl->tail, c);
-                    __syncthreads();
-                    const unsigned int base = sh.base;
-                    for (unsigned int k = tid; k < c; k += T) p.clist[base + k] = stage[k];
-                }
+                // winners go straight to the global list: one atomic on the tail per warp
+                expand_sites<DIM, POW2>(p, s0, u_lo, u_hi, valid, site, p.clist, &ctl->tail, attempts);
             }
-            __threadfence();
         }
+        // every thread's list writes happen-before thread 0's release (bar.sync, then atom.acq_rel)
         __syncthreads();
         // A6: grid barrier; the last CTA to arrive decides what the next level is
         if (tid == 0) {
@@ -221,7 +222,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
             uint32_t hi = bar_hi(w);
             const int s0 = (int)ld_relaxed_u32(reinterpret_cast<unsigned int *>(&ctl->s0));
             const unsigned long long u = __ldcg(&ctl->u);
-            const unsigned int out = grid_levels<DIM, POW2>(p, sh, q0, s0, u, lo, hi, gen, attempts, levels_grid, widest);
+            const unsigned int out = grid_levels<DIM, POW2>(p, sh, s0, u, lo, hi, gen, attempts, levels_grid, widest);
             if (out == kPhaseAbort) break;
         }
         if (attempts) atomicAdd(&ctl->stats[6], (unsigned long long)attempts);
@@ -270,7 +271,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
                 ++gen;
                 ++ups;
                 uint32_t lo = 0u, hi = n;
-                const unsigned int out = grid_levels<DIM, POW2>(p, sh, q0, s0, u, lo, hi, gen, attempts, levels_grid, widest);
+                const unsigned int out = grid_levels<DIM, POW2>(p, sh, s0, u, lo, hi, gen, attempts, levels_grid, widest);
                 size += (unsigned long long)(hi - n);
                 if (out == kPhaseAbort) { aborted = true; break; }
                 if (out == kPhaseDone) break;

@@ -16,12 +16,14 @@ enum Phase : unsigned int {
     kPhaseAbort = 5    // watchdog fired
 };
 
+constexpr int kMaxCtas = 1024;   // upper bound on co-resident CTAs of the persistent kernel
+
 // Global-memory control block of one handle.  Every hot word sits in its own 128-byte line.
 struct alignas(128) Control {
     // [gen:24 | phase:8 | hi:32]; polled by every CTA, written by the last arriver / by CTA 0.
     unsigned long long bar;
     unsigned char pad0[120];
-    unsigned int arrive;          // grid barrier arrival counter
+    unsigned int arrive;          // arrival counter (microbenchmark of the central-counter barrier only)
     unsigned char pad1[124];
     unsigned int tail;            // append cursor of the cluster list
     unsigned char pad2[124];
@@ -34,6 +36,11 @@ struct alignas(128) Control {
     unsigned int pad4;
     unsigned long long stats[8];  // see WOLFF_NSTATS in wolff.h
     unsigned char pad5[56];
+    // Level barrier of the grid phase ("quasi-block synchronisation"): CTA b publishes
+    // [level generation : 32 | entries it appended this level : 32] in its own slot, every CTA reads all
+    // slots.  Two banks alternate with the generation's parity so that a CTA arriving at barrier k+1
+    // never overwrites a slot somebody is still reading for barrier k.
+    unsigned long long flags[2][kMaxCtas];
     // E/M reduction scratch
     unsigned long long acc_unequal;
     unsigned long long acc_negative;
