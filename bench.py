@@ -156,7 +156,7 @@ def run_b200(args, rank: int, world: int):
                 growth_ms.append(e0.elapsed_time(e1))
                 st = h.stats()
                 flipped += st["flipped"]; attempts += st["claim_attempts"]
-                levels += st["levels_cta"] + st["levels_grid"]
+                levels += st["levels_cta"] + st["levels_cluster"] + st["levels_grid"]
                 assert int(sizes_d.sum().item()) == st["flipped"]
 
         for _ in range(warmup):

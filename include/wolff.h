@@ -92,21 +92,30 @@ WOLFF_API int wolff_get_state(wolff_handle h, uint64_t *update_index, uint64_t *
 /* Set the update index (to resume a chain: lattice + index + seed is the whole state). */
 WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
 
-/* Tuning / test knobs; never change the result.  Keys:
- *   "mode"           0 = auto (default), 1 = force every level grid-wide, 2 = force one-CTA
- *                    levels whenever the frontier fits the shared-memory queue
- *   "up_threshold"   frontier width above which growth leaves one-CTA mode (1..queue cap)
- *   "down_threshold" frontier width at or below which grid-wide growth returns to one CTA
- *   "grid_ctas"      number of CTAs of the persistent kernel (0 = one per SM)
- * Unknown key or out-of-range value: WOLFF_EINVAL. */
+/* Tuning / test knobs; never change the result.  The growth kernel runs each BFS level in one of
+ * three tiers by frontier width n: one CTA (n <= up), one thread-block cluster (n <= cluster_up), the
+ * whole grid (above).  Keys:
+ *   "mode"                 0 = auto (default), 1 = every level grid-wide, 2 = one CTA whenever the frontier
+ *                          fits its shared-memory queue, 3 = the cluster whenever it fits
+ *   "up_threshold"         frontier width above which growth leaves one-CTA mode and wakes the cluster
+ *   "down_threshold"       frontier width at or below which cluster growth returns to one CTA
+ *   "cluster_up_threshold" frontier width above which growth leaves cluster mode for a grid phase
+ *   "grid_down_threshold"  frontier width at or below which a grid phase returns to cluster mode
+ *   "balance_min"          cluster mode: a CTA holding more than max(balance_min, 2 x fair share) entries
+ *                          makes the level redistribute the frontier through distributed shared memory
+ *   "cluster_ctas"         CTAs per thread-block cluster: 1, 2, 4, 8 or 16 (default 16)
+ *   "grid_ctas"            total CTAs of the persistent kernel (0 = as many clusters as can be co-resident)
+ *   "cooperative"          1 (default) = cooperative launch, 0 = plain launch of a grid sized to be co-resident
+ * Thresholds are clamped to what the shared-memory queues can hold.  Unknown key or out-of-range
+ * value: WOLFF_EINVAL. */
 WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);
 
-/* Counters of the most recent wolff_run, for the latency roofline (host pointer, 8 values):
- *   [0] updates  [1] flipped spins  [2] one-CTA levels  [3] grid-wide levels
- *   [4] switches one-CTA -> grid    [5] switches grid -> one-CTA
- *   [6] claim attempts (atomics)    [7] widest frontier seen
+/* Counters of the most recent wolff_run, for the latency roofline (host pointer, WOLFF_NSTATS values):
+ *   [0] updates            [1] flipped spins        [2] one-CTA levels       [3] cluster levels
+ *   [4] grid-wide levels   [5] cluster wake-ups     [6] rebalanced cluster levels
+ *   [7] claim attempts (atomics)                    [8] widest frontier seen [9] reserved
  * Blocks until the run has finished. */
-#define WOLFF_NSTATS 8
+#define WOLFF_NSTATS 10
 WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
 
 /* Dependent-latency microbenchmarks on the current device (the links of one BFS level of the

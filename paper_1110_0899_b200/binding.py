@@ -16,9 +16,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libwolff_b200.so")
 
 WOLFF_OK, WOLFF_EINVAL, WOLFF_ENOMEM, WOLFF_ECUDA, WOLFF_EINTERNAL = 0, -1, -2, -3, -4
-NSTATS = 8
-STAT_NAMES = ("updates", "flipped", "levels_cta", "levels_grid", "switch_up", "switch_down", "claim_attempts",
-              "widest_frontier")
+NSTATS = 10
+STAT_NAMES = ("updates", "flipped", "levels_cta", "levels_cluster", "levels_grid", "cluster_wakeups",
+              "levels_rebalanced", "claim_attempts", "widest_frontier", "reserved")
 
 # every symbol include/wolff.h declares (tests/test_abi.py checks the header against this table)
 _SIGNATURES = {

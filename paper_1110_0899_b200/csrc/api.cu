@@ -48,9 +48,15 @@ struct wolff_ctx {
     // knobs
     int mode = 0;
     uint32_t qcap = 0;
-    uint32_t up = 0, down = 0;
-    int grid_ctas = 0;              // 0 = one per SM
-    int max_ctas = 0;               // co-resident limit
+    uint32_t up = 0, down = 0;      // one CTA <-> cluster
+    uint32_t cl_up = 0, grid_down = 0;   // cluster <-> grid
+    uint32_t bal_min = 0;
+    int grid_ctas = 0;              // requested total CTAs, 0 = as many clusters as fit
+    int cluster_ctas = 0;           // CTAs per cluster
+    int cooperative = 1;
+    // launch shape derived from the knobs (recomputed when shape_dirty)
+    bool shape_dirty = true;
+    int max_clusters = 0;           // co-resident limit for this cluster size
     size_t smem_bytes = 0;
 };
 
@@ -88,14 +94,39 @@ uint64_t bond_threshold(double J, double T)
     return (uint64_t)scaled;
 }
 
-void effective_thresholds(const wolff_ctx *h, uint32_t *up, uint32_t *down)
+uint32_t cta_capacity(const wolff_ctx *h) { return h->qcap / (2u * (uint32_t)h->dim); }   // next level must fit one buffer
+uint32_t cluster_capacity(const wolff_ctx *h) { return (uint32_t)h->cluster_ctas * (cta_capacity(h) & ~31u); }
+
+void effective_thresholds(const wolff_ctx *h, GrowthParams *p)
 {
-    const uint32_t up_max = h->qcap / (2u * (uint32_t)h->dim);   // the next level must fit one queue buffer
-    if (h->mode == 1) { *up = 0; *down = 0; return; }            // every level grid-wide
-    if (h->mode == 2) { *up = up_max; *down = up_max; return; }  // one CTA whenever it fits
-    uint32_t u = h->up < up_max ? h->up : up_max;
-    uint32_t d = h->down < u ? h->down : u;
-    *up = u; *down = d;
+    const uint32_t up_max = cta_capacity(h), cl_max = cluster_capacity(h);
+    p->bal_min = h->bal_min;
+    if (h->mode == 1) { p->up = p->down = p->cl_up = p->grid_down = 0; return; }      // every level grid-wide
+    uint32_t up = h->up < up_max ? h->up : up_max;
+    uint32_t down = h->down < up ? h->down : up;
+    uint32_t cl_up = h->cl_up < cl_max ? h->cl_up : cl_max;
+    if (h->mode == 2) { up = up_max; down = up_max; }                                 // one CTA whenever it fits
+    if (h->mode == 3) { up = 0; down = 0; cl_up = cl_max; }                           // the cluster whenever it fits
+    p->up = up; p->down = down; p->cl_up = cl_up;
+    p->grid_down = h->grid_down < cl_up ? h->grid_down : cl_up;
+}
+
+// (Re)derive the launch shape from the knobs: kernel attributes and the co-resident cluster limit.
+int refresh_shape(wolff_ctx *h)
+{
+    if (!h->shape_dirty) return WOLFF_OK;
+    GrowthLaunch l{h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0};
+    int clusters = 0;
+    cudaError_t e = growth_max_clusters(h->dim, h->geo.pow2 != 0, l, &clusters);
+    if (e != cudaSuccess || clusters < 1) {
+        cudaGetLastError();
+        set_error("growth kernel cannot be made resident with clusters of %d CTAs: %s", h->cluster_ctas,
+                  e != cudaSuccess ? cudaGetErrorString(e) : "no cluster fits");
+        return WOLFF_EINVAL;
+    }
+    h->max_clusters = clusters;
+    h->shape_dirty = false;
+    return WOLFF_OK;
 }
 
 int sync_and_check(wolff_ctx *h)
@@ -153,16 +184,18 @@ wolff_handle wolff_create(int dim, int L, double J, double T, uint64_t seed)
     if (!prop.cooperativeLaunch) { set_error("device lacks cooperative launch"); delete h; return nullptr; }
     h->num_sms = prop.multiProcessorCount;
 
-    h->qcap = 8192;                       // entries per queue buffer: 2 x 32 KiB of shared memory
+    h->qcap = 16384;                      // entries per queue buffer: 2 x 64 KiB of shared memory per CTA
     h->smem_bytes = 2ull * h->qcap * sizeof(uint32_t);
-    h->up = 256; h->down = 96;
-    int per_sm = 0;
-    e = growth_max_ctas(dim, h->geo.pow2 != 0, h->smem_bytes, &per_sm);
-    if (e != cudaSuccess || per_sm < 1) {
-        set_error("growth kernel cannot be made resident: %s", cudaGetErrorString(e));
-        delete h; return nullptr;
+    h->cluster_ctas = 16;
+    h->up = 64; h->down = 24;
+    h->cl_up = 32768; h->grid_down = 8192;
+    h->bal_min = 64;
+    if (refresh_shape(h) != WOLFF_OK) {
+        // clusters of 16 need the non-portable size; fall back to the portable maximum
+        h->cluster_ctas = 8;
+        h->shape_dirty = true;
+        if (refresh_shape(h) != WOLFF_OK) { delete h; return nullptr; }
     }
-    h->max_ctas = per_sm * h->num_sms;
 
     // N spins padded to a multiple of 16 bytes; N list entries; control block
     const size_t lattice_bytes = (size_t)((N + 15ull) & ~15ull);
@@ -226,12 +259,16 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     p.spins = h->spins; p.clist = h->clist; p.sizes = h->sizes; p.ctl = h->ctl; p.geo = h->geo;
     p.key0 = (uint32_t)h->seed; p.key1 = (uint32_t)(h->seed >> 32);
     p.thr = h->thr; p.u0 = h->u; p.n_updates = n_updates; p.qcap = h->qcap;
-    effective_thresholds(h, &p.up, &p.down);
-    int ctas = h->grid_ctas > 0 ? h->grid_ctas : h->num_sms;
-    if (ctas > h->max_ctas) ctas = h->max_ctas;
+    effective_thresholds(h, &p);
+    rc = refresh_shape(h);
+    if (rc) return rc;
+    int clusters = h->grid_ctas > 0 ? h->grid_ctas / h->cluster_ctas : h->max_clusters;
+    if (clusters > h->max_clusters) clusters = h->max_clusters;
+    if (clusters < 1) clusters = 1;
+    const GrowthLaunch shape{clusters * h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0};
     // control words of the growth kernel start from zero at every launch (generation 0)
     CHECK_CUDA(h, cudaMemsetAsync(h->ctl, 0, offsetof(Control, acc_unequal), stream), "cudaMemsetAsync(control)");
-    CHECK_CUDA(h, launch_growth(p, h->dim, ctas, h->smem_bytes, stream), "launch growth kernel");
+    CHECK_CUDA(h, launch_growth(p, h->dim, shape, stream), "launch growth kernel");
     h->u += n_updates;
     h->last_n = n_updates;
     h->last_stream = stream;
@@ -310,19 +347,44 @@ int wolff_set_update_index(wolff_handle h, uint64_t update_index)
 int wolff_set_option(wolff_handle h, const char *key, int64_t value)
 {
     if (!h || !key) { set_error("null handle or key"); return WOLFF_EINVAL; }
-    const uint32_t up_max = h->qcap / (2u * (uint32_t)h->dim);
+    const uint32_t up_max = cta_capacity(h);
     if (!strcmp(key, "mode")) {
-        if (value < 0 || value > 2) { set_error("mode must be 0, 1 or 2"); return WOLFF_EINVAL; }
+        if (value < 0 || value > 3) { set_error("mode must be 0, 1, 2 or 3"); return WOLFF_EINVAL; }
         h->mode = (int)value;
     } else if (!strcmp(key, "up_threshold")) {
-        if (value < 1 || value > (int64_t)up_max) { set_error("up_threshold must be in [1, %u]", up_max); return WOLFF_EINVAL; }
+        if (value < 0 || value > (int64_t)up_max) { set_error("up_threshold must be in [0, %u]", up_max); return WOLFF_EINVAL; }
         h->up = (uint32_t)value;
     } else if (!strcmp(key, "down_threshold")) {
         if (value < 0 || value > (int64_t)up_max) { set_error("down_threshold must be in [0, %u]", up_max); return WOLFF_EINVAL; }
         h->down = (uint32_t)value;
+    } else if (!strcmp(key, "cluster_up_threshold")) {
+        if (value < 0 || value > (int64_t)0x7FFFFFFF) { set_error("cluster_up_threshold must be in [0, 2^31)"); return WOLFF_EINVAL; }
+        h->cl_up = (uint32_t)value;
+    } else if (!strcmp(key, "grid_down_threshold")) {
+        if (value < 0 || value > (int64_t)0x7FFFFFFF) { set_error("grid_down_threshold must be in [0, 2^31)"); return WOLFF_EINVAL; }
+        h->grid_down = (uint32_t)value;
+    } else if (!strcmp(key, "balance_min")) {
+        if (value < 0 || value > (int64_t)0x7FFFFFFF) { set_error("balance_min must be in [0, 2^31)"); return WOLFF_EINVAL; }
+        h->bal_min = (uint32_t)value;
     } else if (!strcmp(key, "grid_ctas")) {
-        if (value < 0 || value > h->max_ctas) { set_error("grid_ctas must be in [0, %d]", h->max_ctas); return WOLFF_EINVAL; }
+        if (value < 0 || value > 1 << 20) { set_error("grid_ctas must be in [0, 2^20]"); return WOLFF_EINVAL; }
         h->grid_ctas = (int)value;
+    } else if (!strcmp(key, "cluster_ctas")) {
+        if (value != 1 && value != 2 && value != 4 && value != 8 && value != 16) {
+            set_error("cluster_ctas must be 1, 2, 4, 8 or 16");
+            return WOLFF_EINVAL;
+        }
+        const int before = h->cluster_ctas;
+        h->cluster_ctas = (int)value;
+        h->shape_dirty = true;
+        if (check_handle(h) != WOLFF_OK || refresh_shape(h) != WOLFF_OK) {
+            h->cluster_ctas = before;
+            h->shape_dirty = true;
+            return WOLFF_EINVAL;
+        }
+    } else if (!strcmp(key, "cooperative")) {
+        if (value != 0 && value != 1) { set_error("cooperative must be 0 or 1"); return WOLFF_EINVAL; }
+        h->cooperative = (int)value;
     } else {
         set_error("unknown option '%s'", key);
         return WOLFF_EINVAL;

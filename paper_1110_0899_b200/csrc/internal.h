@@ -10,20 +10,18 @@ namespace wolff {
 // Phases carried in the barrier word (bits 39:32).
 enum Phase : unsigned int {
     kPhaseGrid = 1,    // next level is grid-wide
-    kPhaseToCta = 2,   // frontier shrank: CTA 0 continues alone from the window [lo, hi)
+    kPhaseToCluster = 2,   // frontier narrowed: cluster 0 continues from the window [lo, hi)
     kPhaseDone = 3,    // the frontier is empty: the update's cluster is complete
     kPhaseExit = 4,    // all updates of this launch are done
     kPhaseAbort = 5    // watchdog fired
 };
-
-constexpr int kMaxCtas = 1024;   // upper bound on co-resident CTAs of the persistent kernel
 
 // Global-memory control block of one handle.  Every hot word sits in its own 128-byte line.
 struct alignas(128) Control {
     // [gen:24 | phase:8 | hi:32]; polled by every CTA, written by the last arriver / by CTA 0.
     unsigned long long bar;
     unsigned char pad0[120];
-    unsigned int arrive;          // arrival counter (microbenchmark of the central-counter barrier only)
+    unsigned int arrive;          // grid barrier arrival counter
     unsigned char pad1[124];
     unsigned int tail;            // append cursor of the cluster list
     unsigned char pad2[124];
@@ -34,13 +32,8 @@ struct alignas(128) Control {
     unsigned char pad3[112];
     unsigned int error;           // nonzero: a barrier timed out
     unsigned int pad4;
-    unsigned long long stats[8];  // see WOLFF_NSTATS in wolff.h
-    unsigned char pad5[56];
-    // Level barrier of the grid phase ("quasi-block synchronisation"): CTA b publishes
-    // [level generation : 32 | entries it appended this level : 32] in its own slot, every CTA reads all
-    // slots.  Two banks alternate with the generation's parity so that a CTA arriving at barrier k+1
-    // never overwrites a slot somebody is still reading for barrier k.
-    unsigned long long flags[2][kMaxCtas];
+    unsigned long long stats[12]; // see WOLFF_NSTATS in wolff.h
+    unsigned char pad5[24];
     // E/M reduction scratch
     unsigned long long acc_unequal;
     unsigned long long acc_negative;
@@ -60,17 +53,28 @@ struct GrowthParams {
     unsigned long long thr; // bond threshold in [0, 2^32]
     unsigned long long u0;  // first update index of this launch
     unsigned long long n_updates;
-    uint32_t up;            // leave one-CTA mode when the frontier is wider than this
+    uint32_t up;            // leave one-CTA mode (wake the cluster) when the frontier is wider than this
     uint32_t down;          // return to one-CTA mode when the frontier is at most this wide
+    uint32_t cl_up;         // leave cluster mode (grid phase) when the frontier is wider than this
+    uint32_t grid_down;     // return from a grid phase to cluster mode when the frontier is at most this wide
+    uint32_t bal_min;       // cluster mode: a CTA holding more than max(bal_min, 2 x fair share) triggers rebalancing
     uint32_t qcap;          // entries per shared-memory queue buffer
+};
+
+// Launch shape of the persistent kernel.
+struct GrowthLaunch {
+    int grid_ctas;          // total CTAs, a multiple of cluster_ctas
+    int cluster_ctas;       // CTAs per thread-block cluster (1, 2, 4, 8 or 16)
+    size_t smem_bytes;      // dynamic shared memory per CTA (the two queue buffers)
+    bool cooperative;       // launch with the cooperative attribute (co-residency guaranteed by the driver)
 };
 
 constexpr int kGrowthThreads = 512;
 
 // launchers (defined next to their kernels)
-cudaError_t launch_growth(const GrowthParams &p, int dim, int grid_ctas, size_t smem_bytes, cudaStream_t stream);
-cudaError_t growth_max_ctas(int dim, bool pow2, size_t smem_bytes, int *ctas_per_sm);
-cudaError_t growth_prepare(int dim, bool pow2, size_t smem_bytes);
+cudaError_t launch_growth(const GrowthParams &p, int dim, const GrowthLaunch &l, cudaStream_t stream);
+// sets the kernel's attributes for this launch shape and reports how many clusters can be co-resident
+cudaError_t growth_max_clusters(int dim, bool pow2, const GrowthLaunch &l, int *max_clusters);
 cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, cudaStream_t stream);
 cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, cudaStream_t stream);
 cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo, int dim, Control *ctl,

@@ -11,12 +11,18 @@ from parity_util import assert_same_state, compare_batched, compare_stepwise, ma
 
 pytestmark = pytest.mark.gpu
 
-MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 0, "up_threshold": 8, "down_threshold": 3},
-         {"mode": 1, "grid_ctas": 3}, {"mode": 0, "up_threshold": 40, "down_threshold": 40, "grid_ctas": 16}]
+# growth tiers forced in turn: auto, grid, one CTA, cluster; then threshold sets that make every tier switch fire
+# on small lattices (CTA <-> cluster <-> grid), odd cluster sizes and grid sizes, and the rebalancing path
+MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 3},
+         {"mode": 0, "up_threshold": 8, "down_threshold": 3, "cluster_up_threshold": 40, "grid_down_threshold": 20},
+         {"mode": 1, "grid_ctas": 3, "cluster_ctas": 1},
+         {"mode": 0, "up_threshold": 2, "down_threshold": 1, "cluster_ctas": 4, "balance_min": 0},
+         {"mode": 3, "cluster_ctas": 8, "cluster_up_threshold": 100, "grid_down_threshold": 100, "grid_ctas": 16},
+         {"mode": 3, "cluster_ctas": 2, "balance_min": 1000000, "cooperative": 0}]
 
 
 # ------------------------------------------------------------------ BASELINE config C1, exactly as written
-@pytest.mark.parametrize("options", MODES[:3])
+@pytest.mark.parametrize("options", MODES[:4])
 def test_config_c1_every_update(options):
     c = wl.CONFIGS["C1"]
     gpu, ref = make_pair(*c.create_args(), options=options)
@@ -96,7 +102,7 @@ def test_seeds_and_large_update_index():
 
 
 # ------------------------------------------------------------------ medium sizes: several tiles, ragged tails
-@pytest.mark.parametrize("options", [{"mode": 0}, {"mode": 1}])
+@pytest.mark.parametrize("options", [{"mode": 0}, {"mode": 1}, {"mode": 3}])
 @pytest.mark.parametrize("name,n", [("C2", 40), ("C4", 40)])
 def test_medium_configs_equilibrated_variant(name, n, options):
     c = wl.CONFIGS[name]
