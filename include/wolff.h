@@ -115,7 +115,7 @@ WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);
  *   [4] grid-wide levels   [5] cluster wake-ups     [6] rebalanced cluster levels
  *   [7] claim attempts (atomics)                    [8] widest frontier seen [9] reserved
  * Blocks until the run has finished. */
-#define WOLFF_NSTATS 10
+#define WOLFF_NSTATS 16
 WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
 
 /* Dependent-latency microbenchmarks on the current device (the links of one BFS level of the

@@ -54,6 +54,7 @@ struct wolff_ctx {
     int grid_ctas = 0;              // requested total CTAs, 0 = as many clusters as fit
     int cluster_ctas = 0;           // CTAs per cluster
     int cooperative = 1;
+    int spec = 0;                   // speculative claims (no neighbour gather)
     // launch shape derived from the knobs (recomputed when shape_dirty)
     bool shape_dirty = true;
     int max_clusters = 0;           // co-resident limit for this cluster size
@@ -115,7 +116,7 @@ void effective_thresholds(const wolff_ctx *h, GrowthParams *p)
 int refresh_shape(wolff_ctx *h)
 {
     if (!h->shape_dirty) return WOLFF_OK;
-    GrowthLaunch l{h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0};
+    GrowthLaunch l{h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0, h->spec != 0};
     int clusters = 0;
     cudaError_t e = growth_max_clusters(h->dim, h->geo.pow2 != 0, l, &clusters);
     if (e != cudaSuccess || clusters < 1) {
@@ -265,7 +266,7 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     int clusters = h->grid_ctas > 0 ? h->grid_ctas / h->cluster_ctas : h->max_clusters;
     if (clusters > h->max_clusters) clusters = h->max_clusters;
     if (clusters < 1) clusters = 1;
-    const GrowthLaunch shape{clusters * h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0};
+    const GrowthLaunch shape{clusters * h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0, h->spec != 0};
     // control words of the growth kernel start from zero at every launch (generation 0)
     CHECK_CUDA(h, cudaMemsetAsync(h->ctl, 0, offsetof(Control, acc_unequal), stream), "cudaMemsetAsync(control)");
     CHECK_CUDA(h, launch_growth(p, h->dim, shape, stream), "launch growth kernel");
@@ -382,6 +383,11 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
             h->shape_dirty = true;
             return WOLFF_EINVAL;
         }
+    } else if (!strcmp(key, "speculative")) {
+        if (value != 0 && value != 1) { set_error("speculative must be 0 or 1"); return WOLFF_EINVAL; }
+        h->spec = (int)value;
+        h->shape_dirty = true;
+        if (check_handle(h) != WOLFF_OK || refresh_shape(h) != WOLFF_OK) return WOLFF_EINVAL;
     } else if (!strcmp(key, "cooperative")) {
         if (value != 0 && value != 1) { set_error("cooperative must be 0 or 1"); return WOLFF_EINVAL; }
         h->cooperative = (int)value;

@@ -1,0 +1,153 @@
+// expand.cuh -- expansion of one cluster site per lane, shared by the
+// level-synchronous kernel (growth.cu) and the barrier-free kernel (growth_async.cu).
+//
+// PAPER.md:45-46 (steps ii/iii): every neighbour of a newly added spin that is parallel to the seed
+// spin and not yet a member joins with probability p = 1 - exp(-2J/T).  Here the random number of a
+// bond is a function of (seed, update, bond) (readings R6, R10), and "join" is one atomic that flips
+// the spin (reading R3), so the order in which sites are expanded cannot show in the result.
+#pragma once
+#include "internal.h"
+
+namespace wolff {
+
+constexpr unsigned int kFullMask = 0xFFFFFFFFu;
+
+// Coordinates of site i (reading R5).
+template <int DIM, bool POW2>
+__device__ __forceinline__ void site_coords(const Geometry &g, uint32_t i, uint32_t &x, uint32_t &y, uint32_t &z)
+{
+    z = 0;
+    if (POW2) {
+        const uint32_t mask = g.L - 1u;
+        x = i & mask;
+        y = (i >> g.logL) & mask;
+        if (DIM == 3) z = i >> (2u * g.logL);
+    } else {
+        x = i % g.L;
+        const uint32_t t = i / g.L;
+        y = t % g.L;
+        if (DIM == 3) z = t / g.L;
+    }
+}
+
+// nbr[2d] = +d neighbour, nbr[2d+1] = -d neighbour of site i at (x, y, z), periodic.
+template <int DIM>
+__device__ __forceinline__ void neighbours_at(const Geometry &g, uint32_t i, uint32_t x, uint32_t y, uint32_t z,
+                                              uint32_t (&nbr)[2 * DIM])
+{
+    const uint32_t Lm1 = g.L - 1u;
+    nbr[0] = (x == Lm1) ? i - Lm1 : i + 1u;
+    nbr[1] = (x == 0u) ? i + Lm1 : i - 1u;
+    const uint32_t ywrap = g.LL - g.L;                 // L*(L-1)
+    nbr[2] = (y == Lm1) ? i - ywrap : i + g.L;
+    nbr[3] = (y == 0u) ? i + ywrap : i - g.L;
+    if (DIM == 3) {
+        const uint32_t zwrap = g.N - g.LL;             // L*L*(L-1)
+        nbr[4] = (z == Lm1) ? i - zwrap : i + g.LL;
+        nbr[5] = (z == 0u) ? i + zwrap : i - g.LL;
+    }
+}
+
+// A2-A4 for one site per lane.  On return nbr[] holds the 2*DIM neighbour ids, bit k of `won` is set
+// when THIS lane flipped nbr[k] from s0 to -s0 (so nbr[k] is a new member of the cluster), and
+// (x, y, z) are the site's coordinates.  Lanes with valid == false do nothing and return won = 0.
+//
+// SPEC == false: gather the neighbour spins first (A2, ld.global.cg, in flight while the Philox rounds
+//   execute) and issue the claim atomic only for same-sign neighbours behind active bonds.
+// SPEC == true: no gather.  The claim atomic is idempotent on a spin that is not s0 (OR 0xFE on 0xFF,
+//   AND 0x01.. on 0x01 change nothing) and returns the old byte, so it is issued for every active bond
+//   and the returned byte says whether the neighbour was parallel: the dependent chain of one hop
+//   loses the L2 load (about 2*dim*p atomics per site instead of about 1.1, on an idle atomic unit).
+template <int DIM, bool POW2, bool SPEC>
+__device__ __forceinline__ void claim_neighbours(const GrowthParams &p, int s0, uint32_t u_lo, uint32_t u_hi, bool valid,
+                                                 uint32_t i, uint32_t (&nbr)[2 * DIM], unsigned int &won, uint32_t &x,
+                                                 uint32_t &y, uint32_t &z, unsigned int &attempts)
+{
+    bool cand[2 * DIM];
+    unsigned int old[2 * DIM];
+#pragma unroll
+    for (int k = 0; k < 2 * DIM; ++k) { nbr[k] = 0u; cand[k] = false; old[k] = 0u; }
+    x = y = z = 0u;
+    won = 0u;
+
+    if (valid) {
+        site_coords<DIM, POW2>(p.geo, i, x, y, z);
+        neighbours_at<DIM>(p.geo, i, x, y, z, nbr);
+        int sp[2 * DIM];
+        if (!SPEC) {
+#pragma unroll
+            for (int k = 0; k < 2 * DIM; ++k) sp[k] = load_spin_l2(p.spins, nbr[k]);
+        }
+        // A3: the bond to the +d neighbour is owned by this site (word d of the site's block); the bond
+        // to the -d neighbour is owned by that neighbour (word d of ITS block).  The 1 + DIM blocks are
+        // independent chains and run with their rounds interleaved.
+        uint32_t ctr0[1 + DIM];
+        uint4 blk[1 + DIM];
+        ctr0[0] = i;
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) ctr0[1 + d] = nbr[2 * d + 1];
+        philox4x32_10_multi<1 + DIM>(ctr0, kDomainBond, u_lo, u_hi, p.key0, p.key1, blk);
+#pragma unroll
+        for (int d = 0; d < DIM; ++d) {
+            cand[2 * d] = (unsigned long long)word_of(blk[0], d) < p.thr;
+            cand[2 * d + 1] = (unsigned long long)word_of(blk[1 + d], d) < p.thr;
+            if (!SPEC) {
+                cand[2 * d] = cand[2 * d] && (sp[2 * d] == s0);
+                cand[2 * d + 1] = cand[2 * d + 1] && (sp[2 * d + 1] == s0);
+            }
+        }
+    }
+
+    // A4: all atomics of a lane are issued before any result is looked at, so their L2 round trips overlap.
+    unsigned int *const words = reinterpret_cast<unsigned int *>(p.spins);
+    if (s0 > 0) {   // uniform for the whole update
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k)
+            if (cand[k]) old[k] = atomicOr(words + (nbr[k] >> 2), 0xFEu << ((nbr[k] & 3u) * 8u));
+    } else {
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k)
+            if (cand[k]) old[k] = atomicAnd(words + (nbr[k] >> 2), ~(0xFEu << ((nbr[k] & 3u) * 8u)));
+    }
+    const unsigned int s0_byte = (unsigned int)s0 & 0xFFu;
+#pragma unroll
+    for (int k = 0; k < 2 * DIM; ++k) {
+        const bool w = cand[k] && (((old[k] >> ((nbr[k] & 3u) * 8u)) & 0xFFu) == s0_byte);
+        attempts += cand[k] ? 1u : 0u;
+        won |= w ? (1u << k) : 0u;
+    }
+}
+
+// A2-A5 for one site per lane: claim_neighbours, then append the winners to dst[] with ONE atomic per
+// warp on *dst_count (ballot/popc aggregation).  Must be called by all 32 lanes of a warp.
+template <int DIM, bool POW2, bool SPEC>
+__device__ __forceinline__ void expand_sites(const GrowthParams &p, int s0, uint32_t u_lo, uint32_t u_hi, bool valid,
+                                             uint32_t i, uint32_t *dst, unsigned int *dst_count, unsigned int &attempts)
+{
+    uint32_t nbr[2 * DIM];
+    unsigned int won;
+    uint32_t x, y, z;
+    claim_neighbours<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, i, nbr, won, x, y, z, attempts);
+    unsigned int ballots[2 * DIM];
+    unsigned int total = 0;
+#pragma unroll
+    for (int k = 0; k < 2 * DIM; ++k) {
+        ballots[k] = __ballot_sync(kFullMask, (won >> k) & 1u);
+        total += __popc(ballots[k]);
+    }
+    if (total != 0u) {   // warp-uniform
+        const unsigned int lane = threadIdx.x & 31u;
+        unsigned int base = 0;
+        if (lane == 0u) base = atomicAdd(dst_count, total);
+        base = __shfl_sync(kFullMask, base, 0);
+        const unsigned int bit = 1u << lane;
+        const unsigned int lt = bit - 1u;
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k) {
+            if (ballots[k] & bit) dst[base + __popc(ballots[k] & lt)] = nbr[k];
+            base += __popc(ballots[k]);
+        }
+    }
+}
+
+}  // namespace wolff

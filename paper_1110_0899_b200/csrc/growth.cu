@@ -20,13 +20,13 @@
 // append -> barrier).  One SM sustains only ~0.5 scattered L2 requests per clock, so a frontier of a
 // few hundred sites already takes microseconds on one CTA; sixteen SMs of a cluster take it in one
 // pass, and their barrier costs ~0.2 us instead of the ~1.8 us of a grid-wide one.
+#include "expand.cuh"
 #include "internal.h"
 
 namespace wolff {
 
 namespace {
 
-constexpr unsigned int kFullMask = 0xFFFFFFFFu;
 constexpr int kMaxClusterCtas = 16;
 
 __device__ __forceinline__ unsigned long long pack_bar(unsigned int gen, unsigned int phase, unsigned int hi)
@@ -107,82 +107,6 @@ __device__ __noinline__ unsigned long long wait_generation(Control *ctl, unsigne
     }
 }
 
-// Expand one frontier site per lane (A2-A5): gather the 2*DIM neighbour spins, decide the bonds,
-// claim-and-flip, and append the winners to dst[] with ONE atomic per warp on *dst_count
-// (ballot/popc aggregation).  dst/dst_count are a shared-memory queue in one-CTA and cluster mode
-// and the global cluster list and its tail in grid mode.  Must be called by all 32 lanes of a warp.
-template <int DIM, bool POW2>
-__device__ __forceinline__ void expand_sites(const GrowthParams &p, int s0, uint32_t u_lo, uint32_t u_hi,
-                                             bool valid, uint32_t i, uint32_t *dst, unsigned int *dst_count,
-                                             unsigned int &attempts)
-{
-    uint32_t nbr[2 * DIM];
-    bool cand[2 * DIM];
-    unsigned int old[2 * DIM];
-#pragma unroll
-    for (int k = 0; k < 2 * DIM; ++k) { nbr[k] = 0u; cand[k] = false; old[k] = 0u; }
-
-    if (valid) {
-        neighbours<DIM, POW2>(p.geo, i, nbr);
-        // A2: neighbour spins (L2 loads; in flight while the Philox rounds below execute)
-        int sp[2 * DIM];
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k) sp[k] = load_spin_l2(p.spins, nbr[k]);
-        // A3: bond variables.  The bond to the +d neighbour is owned by this site (word d of the
-        // site's block); the bond to the -d neighbour is owned by that neighbour (word d of ITS
-        // block).  The 1 + DIM blocks are independent chains and run with their rounds interleaved.
-        uint32_t ctr0[1 + DIM];
-        uint4 blk[1 + DIM];
-        ctr0[0] = i;
-#pragma unroll
-        for (int d = 0; d < DIM; ++d) ctr0[1 + d] = nbr[2 * d + 1];
-        philox4x32_10_multi<1 + DIM>(ctr0, kDomainBond, u_lo, u_hi, p.key0, p.key1, blk);
-#pragma unroll
-        for (int d = 0; d < DIM; ++d) {
-            cand[2 * d] = (sp[2 * d] == s0) && ((unsigned long long)word_of(blk[0], d) < p.thr);
-            cand[2 * d + 1] = (sp[2 * d + 1] == s0) && ((unsigned long long)word_of(blk[1 + d], d) < p.thr);
-        }
-    }
-
-    // A4: claim-and-flip the same-sign neighbours behind active bonds.  All atomics of a lane are
-    // issued before any result is looked at, so their L2 round trips overlap.
-    unsigned int *const words = reinterpret_cast<unsigned int *>(p.spins);
-    if (s0 > 0) {   // uniform for the whole update
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k)
-            if (cand[k]) old[k] = atomicOr(words + (nbr[k] >> 2), 0xFEu << ((nbr[k] & 3u) * 8u));
-    } else {
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k)
-            if (cand[k]) old[k] = atomicAnd(words + (nbr[k] >> 2), ~(0xFEu << ((nbr[k] & 3u) * 8u)));
-    }
-    const unsigned int s0_byte = (unsigned int)s0 & 0xFFu;
-    unsigned int ballots[2 * DIM];
-    unsigned int total = 0;
-#pragma unroll
-    for (int k = 0; k < 2 * DIM; ++k) {
-        const bool won = cand[k] && (((old[k] >> ((nbr[k] & 3u) * 8u)) & 0xFFu) == s0_byte);
-        attempts += cand[k] ? 1u : 0u;
-        ballots[k] = __ballot_sync(kFullMask, won);
-        total += __popc(ballots[k]);
-    }
-
-    // A5: warp-aggregated append
-    if (total != 0u) {   // warp-uniform
-        const unsigned int lane = threadIdx.x & 31u;
-        unsigned int base = 0;
-        if (lane == 0u) base = atomicAdd(dst_count, total);
-        base = __shfl_sync(kFullMask, base, 0);
-        const unsigned int bit = 1u << lane;
-        const unsigned int lt = bit - 1u;
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k) {
-            if (ballots[k] & bit) dst[base + __popc(ballots[k] & lt)] = nbr[k];
-            base += __popc(ballots[k]);
-        }
-    }
-}
-
 // Command block, written by the master CTA into every CTA of cluster 0 (through distributed shared
 // memory) right before the cluster barrier that wakes the helpers.
 struct Command {
@@ -212,11 +136,14 @@ struct Counters {
     unsigned int attempts = 0;
     unsigned long long levels_grid = 0, levels_cluster = 0, levels_rebalanced = 0;
     uint32_t widest = 0;
+#ifdef WOLFF_PROFILE
+    long long prof[4] = {0, 0, 0, 0};   // cycles of a cluster level: head, expansion, CTA barrier + count exchange, cluster barrier
+#endif
 };
 
 // Grid-wide level loop over the global cluster list (A2-A6, grid mode).  Called by every CTA with
 // identical (lo, hi, gen); returns with the window/phase decided by the last CTA to arrive.
-template <int DIM, bool POW2>
+template <int DIM, bool POW2, bool SPEC>
 __device__ __forceinline__ unsigned int grid_levels(const GrowthParams &p, SharedState &sh, int s0, uint32_t u_lo,
                                                     uint32_t u_hi, uint32_t &lo, uint32_t &hi, Counters &c)
 {
@@ -239,7 +166,7 @@ __device__ __forceinline__ unsigned int grid_levels(const GrowthParams &p, Share
                 const bool valid = idx < end;
                 const uint32_t site = valid ? __ldcg(p.clist + lo + idx) : 0u;
                 // winners go straight to the global list: one atomic on the tail per warp
-                expand_sites<DIM, POW2>(p, s0, u_lo, u_hi, valid, site, p.clist, &ctl->tail, c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, p.clist, &ctl->tail, c.attempts);
             }
         }
         // every thread's list writes happen-before thread 0's release (bar.sync, then atom.acq_rel)
@@ -282,7 +209,7 @@ enum Outcome : unsigned int { kOutDone = 0, kOutToCta = 1, kOutAbort = 2 };
 // queues can hold) leave for a grid phase and come back when they narrow to grid_down.
 // Returns kOutDone (frontier empty), kOutToCta (frontier <= down: the master CTA has gathered it
 // into its buffer 0, sh.lcnt[0] holds the count) or kOutAbort.  `added` accumulates the spins added.
-template <int DIM, bool POW2>
+template <int DIM, bool POW2, bool SPEC>
 __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, SharedState &sh, uint32_t *q0, uint32_t *q1,
                                                        unsigned int R, unsigned int r, int s0, uint32_t u_lo, uint32_t u_hi,
                                                        unsigned int par, unsigned long long &added, Counters &c)
@@ -294,6 +221,9 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
     const uint32_t sh_q0 = smem_addr(q0), sh_q1 = smem_addr(q1);
     bool first = true;
     for (;;) {
+#ifdef WOLFF_PROFILE
+        const long long pt0 = clock64();
+#endif
         // ---- counts of this level (local shared memory; the peers stored them before the barrier)
         unsigned int cq[kMaxClusterCtas];
         unsigned int n = 0, maxq = 0, mine = 0, before = 0;
@@ -347,7 +277,7 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
             if (r == 0u && tid == 0) st_release_u64(&ctl->bar, pack_bar(c.gen + 1u, kPhaseGrid, n));
             ++c.gen;
             uint32_t lo = 0u, hi = n;
-            const unsigned int out = grid_levels<DIM, POW2>(p, sh, s0, u_lo, u_hi, lo, hi, c);
+            const unsigned int out = grid_levels<DIM, POW2, SPEC>(p, sh, s0, u_lo, u_hi, lo, hi, c);
             added += (unsigned long long)(hi - n);
             if (out == kPhaseAbort) return kOutAbort;
             if (out == kPhaseDone) return kOutDone;
@@ -373,12 +303,15 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
         ++c.levels_cluster;
         const bool local = fits_local && maxq <= (2u * per > p.bal_min ? 2u * per : p.bal_min);
         unsigned int *const dst_count = &sh.acnt[par ^ 1u];
+#ifdef WOLFF_PROFILE
+        const long long pt1 = clock64();
+#endif
         if (local) {
             for (unsigned int pass = 0; pass < mine; pass += T) {
                 const unsigned int idx = pass + tid;
                 const bool valid = idx < mine;
                 const uint32_t site = valid ? cur[idx] : 0u;
-                expand_sites<DIM, POW2>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, c.attempts);
             }
         } else {
             ++c.levels_rebalanced;
@@ -398,13 +331,22 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
                     }
                     site = (owner == r) ? cur[off] : ld_dsmem_u32(map_to_rank(sh_cur, owner) + 4u * off);
                 }
-                expand_sites<DIM, POW2>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, c.attempts);
             }
         }
+#ifdef WOLFF_PROFILE
+        const long long pt2 = clock64();
+#endif
         __syncthreads();                           // all appends of this CTA are done
         if (tid < R) st_dsmem_u32(map_to_rank(sh_cnt + 4u * ((par ^ 1u) * kMaxClusterCtas + r), tid), *dst_count);
         if (tid == 32) sh.acnt[par] = 0u;          // the buffer this level read becomes the next append target
+#ifdef WOLFF_PROFILE
+        const long long pt3 = clock64();
+#endif
         cluster_sync();                            // A6: level barrier of the cluster
+#ifdef WOLFF_PROFILE
+        c.prof[0] += pt1 - pt0; c.prof[1] += pt2 - pt1; c.prof[2] += pt3 - pt2; c.prof[3] += clock64() - pt3;
+#endif
         par ^= 1u;
     }
 }
@@ -432,7 +374,7 @@ __device__ __forceinline__ void begin_cluster_phase(SharedState &sh, unsigned in
     __syncthreads();
 }
 
-template <int DIM, bool POW2>
+template <int DIM, bool POW2, bool SPEC>
 __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthParams p)
 {
     constexpr int T = kGrowthThreads;
@@ -458,7 +400,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
             uint32_t lo = 0u, hi = bar_hi(w);
             const int s0 = (int)ld_relaxed_u32(reinterpret_cast<unsigned int *>(&ctl->s0));
             const unsigned long long u = __ldcg(&ctl->u);
-            const unsigned int out = grid_levels<DIM, POW2>(p, sh, s0, (uint32_t)u, (uint32_t)(u >> 32), lo, hi, c);
+            const unsigned int out = grid_levels<DIM, POW2, SPEC>(p, sh, s0, (uint32_t)u, (uint32_t)(u >> 32), lo, hi, c);
             if (out == kPhaseAbort) break;
         }
         if (c.attempts) atomicAdd(&ctl->stats[7], (unsigned long long)c.attempts);
@@ -476,7 +418,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
             const uint32_t u_lo = sh.cmd.u_lo, u_hi = sh.cmd.u_hi;
             begin_cluster_phase(sh, par, sh.cmd.n);
             unsigned long long added = 0;
-            const unsigned int out = cluster_levels<DIM, POW2>(p, sh, q0, q1, R, r, s0, u_lo, u_hi, par, added, c);
+            const unsigned int out = cluster_levels<DIM, POW2, SPEC>(p, sh, q0, q1, R, r, s0, u_lo, u_hi, par, added, c);
             if (out == kOutAbort) break;
         }
         if (c.attempts) atomicAdd(&ctl->stats[7], (unsigned long long)c.attempts);
@@ -519,7 +461,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
                 cluster_sync();
                 begin_cluster_phase(sh, par, n);
                 unsigned long long added = 0;
-                const unsigned int out = cluster_levels<DIM, POW2>(p, sh, q0, q1, R, 0u, s0, u_lo, u_hi, par, added, c);
+                const unsigned int out = cluster_levels<DIM, POW2, SPEC>(p, sh, q0, q1, R, 0u, s0, u_lo, u_hi, par, added, c);
                 size += added;
                 if (out == kOutAbort) { aborted = true; break; }
                 if (out == kOutDone) break;
@@ -535,7 +477,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
                 const unsigned int idx = pass + tid;
                 const bool valid = idx < n;
                 const uint32_t site = valid ? cur[idx] : 0u;
-                expand_sites<DIM, POW2>(p, s0, u_lo, u_hi, valid, site, nxt, &sh.lcnt[lvl1], c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, &sh.lcnt[lvl1], c.attempts);
             }
             __syncthreads();
             size += sh.lcnt[lvl1];
@@ -561,11 +503,14 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
         ctl->stats[5] = to_cluster;
         ctl->stats[6] = c.levels_rebalanced;
         ctl->stats[8] = c.widest;
+#ifdef WOLFF_PROFILE
+        for (int k = 0; k < 4; ++k) ctl->stats[10 + k] = (unsigned long long)c.prof[k];
+#endif
     }
     if (c.attempts) atomicAdd(&ctl->stats[7], (unsigned long long)c.attempts);
 }
 
-template <int DIM, bool POW2>
+template <int DIM, bool POW2, bool SPEC>
 cudaError_t launch_one(const GrowthParams &p, const GrowthLaunch &l, cudaStream_t stream)
 {
     cudaLaunchConfig_t cfg{};
@@ -582,13 +527,13 @@ cudaError_t launch_one(const GrowthParams &p, const GrowthLaunch &l, cudaStream_
     attrs[1].val.cooperative = 1;
     cfg.attrs = attrs;
     cfg.numAttrs = l.cooperative ? 2 : 1;
-    return cudaLaunchKernelEx(&cfg, growth_kernel<DIM, POW2>, p);
+    return cudaLaunchKernelEx(&cfg, growth_kernel<DIM, POW2, SPEC>, p);
 }
 
-template <int DIM, bool POW2>
+template <int DIM, bool POW2, bool SPEC>
 cudaError_t prepare_one(const GrowthLaunch &l, int *max_clusters)
 {
-    const void *fn = reinterpret_cast<const void *>(&growth_kernel<DIM, POW2>);
+    const void *fn = reinterpret_cast<const void *>(&growth_kernel<DIM, POW2, SPEC>);
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)l.smem_bytes);
     if (e != cudaSuccess) return e;
     if (l.cluster_ctas > 8) {
@@ -607,24 +552,36 @@ cudaError_t prepare_one(const GrowthLaunch &l, int *max_clusters)
         attr.val.clusterDim.z = 1;
         cfg.attrs = &attr;
         cfg.numAttrs = 1;
-        e = cudaOccupancyMaxActiveClusters(max_clusters, growth_kernel<DIM, POW2>, &cfg);
+        e = cudaOccupancyMaxActiveClusters(max_clusters, growth_kernel<DIM, POW2, SPEC>, &cfg);
     }
     return e;
 }
 
 }  // namespace
 
+#define WOLFF_GROWTH_DISPATCH(CALL)                                                     \
+    do {                                                                               \
+        if (dim == 2) {                                                                \
+            if (pow2) return l.spec ? CALL(2, true, true) : CALL(2, true, false);      \
+            return l.spec ? CALL(2, false, true) : CALL(2, false, false);              \
+        }                                                                              \
+        if (pow2) return l.spec ? CALL(3, true, true) : CALL(3, true, false);          \
+        return l.spec ? CALL(3, false, true) : CALL(3, false, false);                  \
+    } while (0)
+
 cudaError_t launch_growth(const GrowthParams &p, int dim, const GrowthLaunch &l, cudaStream_t stream)
 {
     const bool pow2 = p.geo.pow2 != 0u;
-    if (dim == 2) return pow2 ? launch_one<2, true>(p, l, stream) : launch_one<2, false>(p, l, stream);
-    return pow2 ? launch_one<3, true>(p, l, stream) : launch_one<3, false>(p, l, stream);
+#define WOLFF_CALL(D, P, S) launch_one<D, P, S>(p, l, stream)
+    WOLFF_GROWTH_DISPATCH(WOLFF_CALL);
+#undef WOLFF_CALL
 }
 
 cudaError_t growth_max_clusters(int dim, bool pow2, const GrowthLaunch &l, int *max_clusters)
 {
-    if (dim == 2) return pow2 ? prepare_one<2, true>(l, max_clusters) : prepare_one<2, false>(l, max_clusters);
-    return pow2 ? prepare_one<3, true>(l, max_clusters) : prepare_one<3, false>(l, max_clusters);
+#define WOLFF_CALL(D, P, S) prepare_one<D, P, S>(l, max_clusters)
+    WOLFF_GROWTH_DISPATCH(WOLFF_CALL);
+#undef WOLFF_CALL
 }
 
 }  // namespace wolff
