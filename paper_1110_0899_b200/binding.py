@@ -18,8 +18,8 @@ LIB_PATH = os.path.join(HERE, "libwolff_b200.so")
 WOLFF_OK, WOLFF_EINVAL, WOLFF_ENOMEM, WOLFF_ECUDA, WOLFF_EINTERNAL = 0, -1, -2, -3, -4
 NSTATS = 16
 STAT_NAMES = ("updates", "flipped", "levels_cta", "levels_cluster", "levels_grid", "cluster_wakeups",
-              "levels_rebalanced", "claim_attempts", "widest_frontier", "reserved",
-              "s10", "s11", "s12", "s13", "s14", "s15")
+              "levels_rebalanced", "claim_attempts", "widest_frontier", "monitor_polls",
+              "s10", "messages", "ring_pushes", "warp_passes", "spills", "s15")
 
 # every symbol include/wolff.h declares (tests/test_abi.py checks the header against this table)
 _SIGNATURES = {

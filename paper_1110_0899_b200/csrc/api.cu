@@ -59,6 +59,18 @@ struct wolff_ctx {
     bool shape_dirty = true;
     int max_clusters = 0;           // co-resident limit for this cluster size
     size_t smem_bytes = 0;
+    // shared-memory-resident kernel (growth_tiles.cu): knobs, plan, and the device state that goes with the plan
+    int tile_log_opt = 0;           // 0 = auto
+    int tile_ctas_opt = 0;          // 0 = one CTA per SM
+    uint32_t ring_cap = 8192;
+    size_t smem_optin = 0;          // shared memory one CTA may use
+    bool plan_dirty = true;
+    bool plan_ok = false;
+    TileParams tp{};
+    size_t tile_smem = 0;
+    unsigned long long *tile_inbox = nullptr;
+    unsigned long long *tile_ctr = nullptr;     // gtail[G], gdone[G], gspill[G], added
+    uint32_t *tile_spill = nullptr;
 };
 
 namespace {
@@ -130,6 +142,83 @@ int refresh_shape(wolff_ctx *h)
     return WOLFF_OK;
 }
 
+void free_tile_state(wolff_ctx *h)
+{
+    cudaFree(h->tile_inbox); h->tile_inbox = nullptr;
+    cudaFree(h->tile_ctr); h->tile_ctr = nullptr;
+    cudaFree(h->tile_spill); h->tile_spill = nullptr;
+}
+
+uint32_t ceil_log2(uint64_t v) { uint32_t l = 0; while ((1ull << l) < v) ++l; return l; }
+
+// (Re)derive the tiling of growth_tiles.cu from the knobs and allocate its inboxes, spill lists and counters.
+// plan_ok == false (L not a power of two, L < 4, or the lattice does not fit the chip's shared memory) is not an
+// error: wolff_run then uses the level-synchronous kernel of growth.cu.
+int refresh_plan(wolff_ctx *h)
+{
+    if (!h->plan_dirty) return WOLFF_OK;
+    if (h->ran) CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+    free_tile_state(h);
+    h->plan_ok = false;
+    h->plan_dirty = false;
+    if (!h->geo.pow2 || h->L < 4) return WOLFF_OK;
+    const uint32_t dim = (uint32_t)h->dim, logL = h->geo.logL;
+    uint32_t b = h->tile_log_opt > 0 ? (uint32_t)h->tile_log_opt : (dim == 2 ? 6u : 4u);
+    if (b > logL) b = logL;
+    const uint64_t ntiles = 1ull << (dim * (logL - b));
+    if (ntiles > (1ull << 24)) return WOLFF_OK;
+    uint32_t G = (uint32_t)h->num_sms;
+    if (h->tile_ctas_opt > 0 && (uint32_t)h->tile_ctas_opt < G) G = (uint32_t)h->tile_ctas_opt;
+    if (ntiles < G) G = (uint32_t)ntiles;
+    const uint32_t slots = (uint32_t)((ntiles + G - 1) / G);
+    const size_t smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap);
+    if (smem + 256 > h->smem_optin) return WOLFF_OK;
+    int per_sm = 0;
+    cudaError_t e = tiles_prepare(h->dim, smem, &per_sm);
+    if (e != cudaSuccess || per_sm < 1) { cudaGetLastError(); return WOLFF_OK; }
+
+    TileParams &tp = h->tp;
+    tp = TileParams{};
+    tp.tile_log = b;
+    tp.ntiles = (uint32_t)ntiles;
+    tp.permA = (0x9E3779B1u & (uint32_t)(ntiles - 1)) | 1u;
+    uint32_t inv = tp.permA;                      // Newton iteration for the inverse of an odd number mod 2^32
+    for (int it = 0; it < 5; ++it) inv *= 2u - tp.permA * inv;
+    tp.permAinv = inv & (uint32_t)(ntiles - 1);
+    tp.G = G;
+    tp.magicG = ((1ull << 40) + G - 1) / G;
+    tp.slots = slots;
+    // messages one update can send to one CTA: every bond across the surface of its tiles once, the seed, the exit
+    const uint64_t surface = (uint64_t)slots * 2ull * dim * (1ull << ((dim - 1) * b));
+    tp.in_log = ceil_log2(surface + 4);
+    tp.in_cap = 1u << tp.in_log;
+    tp.spill_log = ceil_log2((uint64_t)slots << (dim * b));
+    tp.ring_cap = h->ring_cap;
+    tp.watchdog_ns = 20ull * 1000ull * 1000ull * 1000ull;
+    h->tile_smem = smem;
+
+    const size_t inbox_bytes = ((size_t)G << tp.in_log) * sizeof(unsigned long long);
+    const size_t ctr_bytes = (3 * (size_t)G + 1) * sizeof(unsigned long long);
+    const size_t spill_bytes = ((size_t)G << tp.spill_log) * sizeof(uint32_t);
+    if (cudaMalloc(&h->tile_inbox, inbox_bytes) != cudaSuccess || cudaMalloc(&h->tile_ctr, ctr_bytes) != cudaSuccess ||
+        cudaMalloc(&h->tile_spill, spill_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        free_tile_state(h);
+        return WOLFF_OK;      // not enough memory for the tiled kernel's queues: the level-synchronous kernel needs none
+    }
+    CHECK_CUDA(h, cudaMemset(h->tile_inbox, 0, inbox_bytes), "clear inboxes");
+    CHECK_CUDA(h, cudaMemset(h->tile_ctr, 0, ctr_bytes), "clear counters");
+    CHECK_CUDA(h, cudaMemset(h->tile_spill, 0, spill_bytes), "clear spill lists");
+    tp.inbox = h->tile_inbox;
+    tp.gtail = h->tile_ctr;
+    tp.gdone = h->tile_ctr + G;
+    tp.gspill = h->tile_ctr + 2 * (size_t)G;
+    tp.added = h->tile_ctr + 3 * (size_t)G;
+    tp.spill = h->tile_spill;
+    h->plan_ok = true;
+    return WOLFF_OK;
+}
+
 int sync_and_check(wolff_ctx *h)
 {
     CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
@@ -184,6 +273,7 @@ wolff_handle wolff_create(int dim, int L, double J, double T, uint64_t seed)
     if (!ok) { set_error("cudaGetDeviceProperties failed"); delete h; return nullptr; }
     if (!prop.cooperativeLaunch) { set_error("device lacks cooperative launch"); delete h; return nullptr; }
     h->num_sms = prop.multiProcessorCount;
+    h->smem_optin = prop.sharedMemPerBlockOptin;
 
     h->qcap = 16384;                      // entries per queue buffer: 2 x 64 KiB of shared memory per CTA
     h->smem_bytes = 2ull * h->qcap * sizeof(uint32_t);
@@ -227,6 +317,7 @@ int wolff_destroy(wolff_handle h)
     cudaFree(h->clist);
     cudaFree(h->sizes);
     cudaFree(h->ctl);
+    free_tile_state(h);
     delete h;
     return WOLFF_OK;
 }
@@ -260,16 +351,33 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     p.spins = h->spins; p.clist = h->clist; p.sizes = h->sizes; p.ctl = h->ctl; p.geo = h->geo;
     p.key0 = (uint32_t)h->seed; p.key1 = (uint32_t)(h->seed >> 32);
     p.thr = h->thr; p.u0 = h->u; p.n_updates = n_updates; p.qcap = h->qcap;
-    effective_thresholds(h, &p);
-    rc = refresh_shape(h);
-    if (rc) return rc;
-    int clusters = h->grid_ctas > 0 ? h->grid_ctas / h->cluster_ctas : h->max_clusters;
-    if (clusters > h->max_clusters) clusters = h->max_clusters;
-    if (clusters < 1) clusters = 1;
-    const GrowthLaunch shape{clusters * h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0, h->spec != 0};
-    // control words of the growth kernel start from zero at every launch (generation 0)
+    // control words of the growth kernels start from zero at every launch (generation 0, no error, no stats)
     CHECK_CUDA(h, cudaMemsetAsync(h->ctl, 0, offsetof(Control, acc_unequal), stream), "cudaMemsetAsync(control)");
-    CHECK_CUDA(h, launch_growth(p, h->dim, shape, stream), "launch growth kernel");
+    if (h->mode == 0) {
+        rc = refresh_plan(h);
+        if (rc) return rc;
+    }
+    if (h->mode == 0 && h->plan_ok) {
+        // shared-memory-resident kernel; a message carries the update index relative to the launch in 29 bits
+        const uint64_t chunk = (1ull << 29) - 1;
+        for (uint64_t done = 0; done < n_updates; done += chunk) {
+            TileParams tp = h->tp;
+            tp.g = p;
+            tp.g.u0 = h->u + done;
+            tp.g.n_updates = n_updates - done < chunk ? n_updates - done : chunk;
+            tp.g.sizes = h->sizes + done;
+            CHECK_CUDA(h, launch_growth_tiles(tp, h->dim, h->tile_smem, stream), "launch tiled growth kernel");
+        }
+    } else {
+        effective_thresholds(h, &p);
+        rc = refresh_shape(h);
+        if (rc) return rc;
+        int clusters = h->grid_ctas > 0 ? h->grid_ctas / h->cluster_ctas : h->max_clusters;
+        if (clusters > h->max_clusters) clusters = h->max_clusters;
+        if (clusters < 1) clusters = 1;
+        const GrowthLaunch shape{clusters * h->cluster_ctas, h->cluster_ctas, h->smem_bytes, h->cooperative != 0, h->spec != 0};
+        CHECK_CUDA(h, launch_growth(p, h->dim, shape, stream), "launch growth kernel");
+    }
     h->u += n_updates;
     h->last_n = n_updates;
     h->last_stream = stream;
@@ -350,8 +458,20 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
     if (!h || !key) { set_error("null handle or key"); return WOLFF_EINVAL; }
     const uint32_t up_max = cta_capacity(h);
     if (!strcmp(key, "mode")) {
-        if (value < 0 || value > 3) { set_error("mode must be 0, 1, 2 or 3"); return WOLFF_EINVAL; }
+        if (value < 0 || value > 4) { set_error("mode must be 0, 1, 2, 3 or 4"); return WOLFF_EINVAL; }
         h->mode = (int)value;
+    } else if (!strcmp(key, "tile_log")) {
+        if (value != 0 && (value < 2 || value > 12)) { set_error("tile_log must be 0 (auto) or in [2, 12]"); return WOLFF_EINVAL; }
+        h->tile_log_opt = (int)value;
+        h->plan_dirty = true;
+    } else if (!strcmp(key, "tile_ctas")) {
+        if (value < 0 || value > 1 << 16) { set_error("tile_ctas must be in [0, 65536]"); return WOLFF_EINVAL; }
+        h->tile_ctas_opt = (int)value;
+        h->plan_dirty = true;
+    } else if (!strcmp(key, "ring_cap")) {
+        if (value < 32 || value > 32768 || (value & (value - 1)) != 0) { set_error("ring_cap must be a power of two in [32, 32768]"); return WOLFF_EINVAL; }
+        h->ring_cap = (uint32_t)value;
+        h->plan_dirty = true;
     } else if (!strcmp(key, "up_threshold")) {
         if (value < 0 || value > (int64_t)up_max) { set_error("up_threshold must be in [0, %u]", up_max); return WOLFF_EINVAL; }
         h->up = (uint32_t)value;

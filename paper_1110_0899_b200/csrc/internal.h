@@ -23,14 +23,10 @@ struct alignas(128) Control {
     alignas(128) unsigned long long bar;
     alignas(128) unsigned int arrive;          // grid barrier arrival counter
     alignas(128) unsigned int tail;            // append cursor of the cluster list
-    // descriptor of a grid phase / of a barrier-free phase, written by CTA 0 before it releases the others
+    // descriptor of a grid phase, written by CTA 0 before it releases the others
     alignas(128) unsigned int lo;
     int s0;
     unsigned long long u;
-    // barrier-free kernel: [seq:32 | .. | s0<0:1 | op:8]; seq = 2g when phase g starts, 2g+1 when it is over
-    alignas(128) unsigned long long state;
-    alignas(128) unsigned long long added;     // barrier-free kernel: spins claimed in the running phase
-    alignas(128) unsigned long long acks;      // barrier-free kernel: phase ends seen, summed over helper CTAs
     alignas(128) unsigned int error;           // nonzero: a barrier / phase timed out
     unsigned int pad4;
     unsigned long long stats[16];              // see WOLFF_NSTATS in wolff.h
@@ -61,22 +57,28 @@ struct GrowthParams {
     uint32_t qcap;          // entries per shared-memory queue buffer
 };
 
-// Barrier-free kernel (growth_async.cu): the lattice is cut into tiles of 2^tile_log sites per side, tile
-// (tx, ty, tz) belongs to CTA (tx + hashA*ty + hashB*tz) mod G, and a claimed site is expanded by the CTA that
-// owns its tile.  Sites that cross into another CTA's tile travel through that CTA's inbox, a segment of one
-// global array sized by the number of sites the CTA owns (a site is handed over at most once per update).
-struct AsyncParams {
+// Shared-memory-resident barrier-free kernel (growth_tiles.cu).  The lattice (L a power of two) is cut into tiles of
+// 2^tile_log sites per side; tile t belongs to CTA ((t * permA) mod ntiles) mod G and sits in that CTA's shared
+// memory for the length of the launch.  A claim that crosses into another CTA's territory travels as a 64-bit
+// message through that CTA's inbox (global memory).  All counters below run on across launches (nothing is reset).
+struct TileParams {
     GrowthParams g;
-    uint32_t *inbox;                 // N entries, every one kEmpty between phases
-    const uint32_t *seg;             // [G + 1] first inbox entry of each CTA
-    unsigned long long *gtail;       // [G] entries pushed into CTA c's inbox since the launch began
-    unsigned long long *gdone;       // [G] of those, how many are completely processed (with all local descendants)
+    unsigned long long *inbox;       // G segments of in_cap messages; slot validity by lap parity, never cleared
+    unsigned long long *gtail;       // [G] messages ever pushed into CTA c's inbox
+    unsigned long long *gdone;       // [G] of those, how many are consumed with their whole local progeny expanded
+    unsigned long long *gspill;      // [G] running position of CTA c's spill list
+    unsigned long long *added;       // spins ever claimed (sum over CTAs, published with gdone)
+    uint32_t *spill;                 // G segments of 2^spill_log entries: overflow of the shared-memory ring
+    unsigned long long magicG;       // ceil(2^40 / G)
     uint32_t tile_log;
-    uint32_t hashA, hashB;
+    uint32_t ntiles;                 // (L >> tile_log)^dim, a power of two
+    uint32_t permA, permAinv;        // odd multiplier and its inverse mod ntiles
+    uint32_t G;                      // CTAs (one per SM, all co-resident)
+    uint32_t slots;                  // tiles per CTA (upper bound)
+    uint32_t in_log, in_cap;         // inbox entries per CTA (a power of two above the messages one update can send it)
+    uint32_t spill_log;              // spill entries per CTA (at least the sites the CTA owns)
     uint32_t ring_cap;               // entries of the shared-memory ring (power of two)
-    uint32_t lvl_cap;                // entries per one-CTA level buffer
-    uint32_t zero;                   // always 0: makes the second pass of the termination check depend on the first
-    unsigned long long watchdog_ns;  // a phase longer than this aborts the launch
+    unsigned long long watchdog_ns;  // an update longer than this aborts the launch
 };
 
 // Launch shape of the persistent kernel.
@@ -89,14 +91,16 @@ struct GrowthLaunch {
 };
 
 constexpr int kGrowthThreads = 512;
+constexpr int kTileThreads = 512;
 
 // launchers (defined next to their kernels)
 cudaError_t launch_growth(const GrowthParams &p, int dim, const GrowthLaunch &l, cudaStream_t stream);
 // sets the kernel's attributes for this launch shape and reports how many clusters can be co-resident
 cudaError_t growth_max_clusters(int dim, bool pow2, const GrowthLaunch &l, int *max_clusters);
-// barrier-free kernel: sets attributes, reports co-resident CTAs per SM; launches `ctas` CTAs cooperatively
-cudaError_t async_prepare(int dim, bool pow2, bool spec, size_t smem_bytes, int *ctas_per_sm);
-cudaError_t launch_growth_async(const AsyncParams &p, int dim, bool spec, int ctas, size_t smem_bytes, cudaStream_t stream);
+// shared-memory-resident kernel: shared memory needed, attributes + co-resident CTAs per SM, cooperative launch of tp.G CTAs
+size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap);
+cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm);
+cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, cudaStream_t stream);
 cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, cudaStream_t stream);
 cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo, int dim, Control *ctl,
