@@ -234,16 +234,17 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
             if (lane == 0) {
                 unsigned int idle = 0;
                 for (;;) {
-                    const unsigned int t = ld_vol(&sh.tail);
+                    // head before tail: tail only grows and head never passes it, so t - h >= 0 whatever happens in between
                     h = ld_vol(&sh.head);
+                    const unsigned int t = ld_vol(&sh.tail);
                     if (t != h) {
                         k = t - h < 32u ? t - h : 32u;
                         if (atomicCAS(&sh.head, h, h + k) == h) break;
                         k = 0;
                         continue;
                     }
-                    const unsigned long long st = ld_vol64(&sh.spill_tail);
                     sh_pos = ld_vol64(&sh.spill_head);
+                    const unsigned long long st = ld_vol64(&sh.spill_tail);
                     if (st != sh_pos) {
                         k = st - sh_pos < 32ull ? (unsigned int)(st - sh_pos) : 32u;
                         if (atomicCAS(&sh.spill_head, sh_pos, sh_pos + k) == sh_pos) { from_spill = 1; break; }
