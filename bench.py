@@ -127,6 +127,8 @@ def run_b200(args, rank: int, world: int):
         c = wl.CONFIGS[cfg_name]
         seed = c.seed + rank
         h = binding.Wolff(c.dim, c.L, c.J, c.T, seed)
+        if args.mode:
+            h.set_option("mode", args.mode)
         if cold:
             h.set_spins(wl.cold(c.N))
         if equil:
@@ -337,6 +339,7 @@ def main():
     ap.add_argument("--equil", type=int, default=1000, help="untimed equilibration updates after the cold start")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--reference-updates", type=int, default=3)
+    ap.add_argument("--mode", type=int, default=0, help="growth kernel: 0 = default (shared-memory-resident), 4 = level-synchronous tiers")
     ap.add_argument("--no-secondary", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
