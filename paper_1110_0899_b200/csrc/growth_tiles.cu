@@ -38,7 +38,7 @@ namespace {
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;
 constexpr int kT = kTileThreads;
 constexpr int kWarps = kT / 32;
-constexpr int kStage = 32 * 6;                     // winners one warp can produce in one pass (2*dim per lane)
+constexpr int kStage = 32;                         // winners one warp can produce in one pass (one per lane)
 
 // message = [kind:2 | lap:1 | k:29] [site:31 | s0<0:1]
 enum Kind : unsigned int { kKindNone = 0, kKindClaim = 1, kKindSeed = 2, kKindExit = 3 };
@@ -91,6 +91,10 @@ struct Tally {
     unsigned int ring_pushes = 0;       // sites handed to the ring (per lane)
     unsigned int spills = 0;            // sites spilled to global memory (per lane)
     unsigned int passes = 0;            // warp passes (lane 0)
+#ifdef WOLFF_PROFILE
+    unsigned long long cyc_pass = 0;    // cycles inside passes (lane 0)
+    unsigned long long lanes = 0;       // sites expanded (lane 0)
+#endif
 };
 
 // ------------------------------------------------------------------------------------------ geometry of the tiling
@@ -208,28 +212,40 @@ __device__ __forceinline__ void raise_abort(Control *ctl, unsigned int code) { s
 
 // ------------------------------------------------------------------------------------------ worker warp
 // Expands sites owned by this CTA until the launch is over (A2-A5 on shared memory).
+//
+// One LANE PER BOND: a warp holds up to S = 32 / (2*DIM) sites per pass (8 in 2D, 5 in 3D) and lane (q, k) tests the
+// bond from site q to its neighbour k (k = 2d: +d, k = 2d + 1: -d).  The frontier inside one CTA is a handful of
+// sites wide, so lanes are cheap and the dependent instruction chain of a pass is what an update waits for: per lane
+// one neighbour address, one Philox block (the bond owner's), one LDS, one ATOMS, one ballot for the whole warp.
 template <int DIM>
 __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, int8_t *lat, uint32_t *ring, uint32_t *stage,
                                             unsigned int c, Tally &tl)
 {
+    constexpr unsigned int ND = 2u * DIM, S = 32u / ND;
     const GrowthParams &p = tp.g;
     const Tiling<DIM> tg(tp);
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned int bit = 1u << lane, lt = bit - 1u;
+    const unsigned int q = lane / ND, k = lane - q * ND, d = k >> 1, sgn = k & 1u;
+    const bool alive = q < S;
+    const uint32_t sh_d = d * tg.logL, fmask = tg.Lmask << sh_d, delta = sgn ? 0xFFFFFFFFu : 1u;
     const uint32_t rmask = tp.ring_cap - 1u;
     const uint32_t tile_sites_log = DIM * tp.tile_log;
     const uint32_t in_mask = tp.in_cap - 1u;
+    const uint32_t thr32 = (uint32_t)p.thr;
+    const bool always = (p.thr >> 32) != 0ull;          // thr = 2^32: every bond is active
     unsigned int *const words = reinterpret_cast<unsigned int *>(lat);
     uint32_t site = 0;
-    bool have = false;
+    unsigned int nsites = 0;     // sites held by the warp (warp-uniform); lanes of group q < nsites work
     int s0 = 1;
+    unsigned int s0_byte = 1u;
     uint32_t u_lo = 0, u_hi = 0, krel = 0;
     unsigned int mywon = 0;      // spins this lane claimed since the warp last ran dry
 
     for (;;) {
-        if (!__any_sync(kFullMask, have)) {
-            // ---- take up to 32 sites from the ring, else from the spill list
-            unsigned int k = 0, h = 0, from_spill = 0;
+        if (nsites == 0u) {
+            // ---- take up to S sites from the ring, else from the spill list
+            unsigned int n = 0, h = 0, from_spill = 0;
             unsigned long long sh_pos = 0;
             if (lane == 0) {
                 unsigned int idle = 0;
@@ -238,36 +254,37 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
                     h = ld_vol(&sh.head);
                     const unsigned int t = ld_vol(&sh.tail);
                     if (t != h) {
-                        k = t - h < 32u ? t - h : 32u;
-                        if (atomicCAS(&sh.head, h, h + k) == h) break;
-                        k = 0;
+                        n = t - h < S ? t - h : S;
+                        if (atomicCAS(&sh.head, h, h + n) == h) break;
+                        n = 0;
                         continue;
                     }
                     sh_pos = ld_vol64(&sh.spill_head);
                     const unsigned long long st = ld_vol64(&sh.spill_tail);
                     if (st != sh_pos) {
-                        k = st - sh_pos < 32ull ? (unsigned int)(st - sh_pos) : 32u;
-                        if (atomicCAS(&sh.spill_head, sh_pos, sh_pos + k) == sh_pos) { from_spill = 1; break; }
-                        k = 0;
+                        n = st - sh_pos < (unsigned long long)S ? (unsigned int)(st - sh_pos) : S;
+                        if (atomicCAS(&sh.spill_head, sh_pos, sh_pos + n) == sh_pos) { from_spill = 1; break; }
+                        n = 0;
                         continue;
                     }
                     if (ld_vol(&sh.stop)) break;
-                    if (++idle > 16u) __nanosleep(40);
+                    if (++idle > 16u) __nanosleep(20);
                 }
             }
-            k = __shfl_sync(kFullMask, k, 0);
+            n = __shfl_sync(kFullMask, n, 0);
             h = __shfl_sync(kFullMask, h, 0);
             from_spill = __shfl_sync(kFullMask, from_spill, 0);
             sh_pos = __shfl_sync(kFullMask, sh_pos, 0);
-            if (k == 0) break;                                   // launch over
-            if (lane < k) {
+            if (n == 0u) break;                                  // launch over
+            uint32_t ent = 0;
+            if (lane < n) {
                 unsigned int spins = 0;
                 if (!from_spill) {
                     uint32_t *slot = ring + ((h + lane) & rmask);
                     do {
-                        site = atomicExch(slot, kEmpty);         // the producer reserved it; its store is on the way
-                        if (site == kEmpty && ++spins > (1u << 26)) { raise_abort(p.ctl, 4u); site = 0u; }
-                    } while (site == kEmpty);
+                        ent = atomicExch(slot, kEmpty);          // the producer reserved it; its store is on the way
+                        if (ent == kEmpty && ++spins > (1u << 26)) { raise_abort(p.ctl, 4u); ent = 0u; }
+                    } while (ent == kEmpty);
                 } else {
                     const unsigned long long pos = sh_pos + (unsigned long long)lane;
                     const uint32_t *slot = tp.spill + ((size_t)c << tp.spill_log) + ((uint32_t)pos & ((1u << tp.spill_log) - 1u));
@@ -277,123 +294,64 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
                         v = ld_relaxed_u32(slot);
                         if ((v & 1u) != tag && ++spins > (1u << 24)) { raise_abort(p.ctl, 5u); v = tag; }
                     } while ((v & 1u) != tag);
-                    site = v >> 1;
+                    ent = v >> 1;
                 }
-                have = true;
             }
+            site = __shfl_sync(kFullMask, ent, q);
+            nsites = n;
             // the update these sites belong to (written by the receiver before it fed the ring)
             s0 = *reinterpret_cast<volatile int *>(&sh.s0);
+            s0_byte = (unsigned int)s0 & 0xFFu;
             u_lo = ld_vol(&sh.u_lo);
             u_hi = ld_vol(&sh.u_hi);
             krel = (uint32_t)((((unsigned long long)u_hi << 32) | u_lo) - p.u0);
         }
+#ifdef WOLFF_PROFILE
+        const long long tp0 = clock64();
+#endif
+        const unsigned int expanded = nsites;
+        const bool have = alive && q < nsites;
 
-        // ---- A2: neighbours; which of them live in this CTA's shared memory, and where
-        const unsigned int expanded = __popc(__ballot_sync(kFullMask, have));
-        uint32_t nbr[2 * DIM];
-        uint32_t where[2 * DIM];     // local: byte address in lat[]; remote: owner CTA
-        unsigned int local = 0;      // bit k: nbr[k] is owned by this CTA
-        unsigned int cand = 0;       // bit k: bond active (and, if local, neighbour parallel to s0)
-        unsigned int won = 0;
-        if (have) {
-            uint32_t x, y, z;
-            tg.coords(site, x, y, z);
-            neighbours_at<DIM>(p.geo, site, x, y, z, nbr);
-            const uint32_t t0 = tg.tile_of(x, y, z);
-            uint32_t own0, slot0;
-            tg.place(t0, own0, slot0);
-            const uint32_t base0 = (slot0 << tile_sites_log);
-            const uint32_t w0 = tg.within(x, y, z);
-            const uint32_t crd[3] = {x, y, z};
-#pragma unroll
-            for (int d = 0; d < DIM; ++d) {
-                const uint32_t cm = crd[d] & tg.m;
-                const uint32_t stride = 1u << (d * tg.b);
-                const uint32_t tcoord = (crd[d] >> tg.b);
-                const uint32_t tclear = t0 & ~(tg.nt_mask << (d * tg.nt_log));
-#pragma unroll
-                for (int sgn = 0; sgn < 2; ++sgn) {
-                    const int k = 2 * d + sgn;
-                    const bool inside = sgn == 0 ? (cm != tg.m) : (cm != 0u);
-                    if (inside) {
-                        where[k] = base0 + (sgn == 0 ? w0 + stride : w0 - stride);
-                        local |= 1u << k;
-                    } else {
-                        const uint32_t tn = tclear | (((sgn == 0 ? tcoord + 1u : tcoord - 1u) & tg.nt_mask) << (d * tg.nt_log));
-                        uint32_t own, slot;
-                        tg.place(tn, own, slot);
-                        const uint32_t wn = sgn == 0 ? w0 - tg.m * stride : w0 + tg.m * stride;
-                        if (own == c) { where[k] = (slot << tile_sites_log) + wn; local |= 1u << k; }
-                        else where[k] = own;
-                    }
-                }
-            }
-            // gather of the local neighbours (LDS), in flight while the Philox rounds execute
-            int sp[2 * DIM];
-#pragma unroll
-            for (int k = 0; k < 2 * DIM; ++k) sp[k] = ((local >> k) & 1u) ? (int)*reinterpret_cast<volatile signed char *>(lat + where[k]) : s0;
-            // A3: the bond to the +d neighbour is owned by this site, the bond to the -d neighbour by that neighbour
-            uint32_t ctr0[1 + DIM];
-            uint4 blk[1 + DIM];
-            ctr0[0] = site;
-#pragma unroll
-            for (int d = 0; d < DIM; ++d) ctr0[1 + d] = nbr[2 * d + 1];
-            philox4x32_10_multi<1 + DIM>(ctr0, kDomainBond, u_lo, u_hi, p.key0, p.key1, blk);
-#pragma unroll
-            for (int d = 0; d < DIM; ++d) {
-                if ((unsigned long long)word_of(blk[0], d) < p.thr && sp[2 * d] == s0) cand |= 1u << (2 * d);
-                if ((unsigned long long)word_of(blk[1 + d], d) < p.thr && sp[2 * d + 1] == s0) cand |= 1u << (2 * d + 1);
-            }
-        } else {
-#pragma unroll
-            for (int k = 0; k < 2 * DIM; ++k) { nbr[k] = 0u; where[k] = 0u; }
-        }
+        // ---- A2: this lane's neighbour; is it in this CTA's shared memory, and where
+        const uint32_t nid = (site & ~fmask) | ((((site >> sh_d) + delta) & tg.Lmask) << sh_d);
+        uint32_t nx, ny, nz, own, slot;
+        tg.coords(nid, nx, ny, nz);
+        tg.place(tg.tile_of(nx, ny, nz), own, slot);
+        const uint32_t addr = (slot << tile_sites_log) + tg.within(nx, ny, nz);
+        const bool local = own == c;
+        const unsigned int shift = (addr & 3u) * 8u;
+        // gather (LDS), in flight while the Philox rounds execute
+        unsigned int spw = 0;
+        if (have && local) spw = *reinterpret_cast<volatile unsigned int *>(words + (addr >> 2));
+        // ---- A3: the bond to the +d neighbour is owned by this site, the bond to the -d neighbour by that neighbour
+        const uint4 blk = philox4x32_10(sgn ? nid : site, kDomainBond, u_lo, u_hi, p.key0, p.key1);
+        const uint32_t r = d == 0u ? blk.x : (d == 1u ? blk.y : blk.z);
+        const bool active = have && (always || r < thr32);
+        const bool cand_l = active && local && (((spw >> shift) & 0xFFu) == s0_byte);
+        const bool cand_r = active && !local;
 
-        // ---- A4 across the territory border: a message to the owner (slot by one L2 atomic, then one 8-byte store).
-        // Issued first, so that the L2 round trips overlap the shared-memory claims below.
-        const unsigned int remote = cand & ~local;
-        unsigned long long pos[2 * DIM];
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k)
-            if ((remote >> k) & 1u) pos[k] = atomicAdd(tp.gtail + where[k], 1ull);
+        // ---- A4 across the territory border: a message to the owner (slot by one L2 atomic, then one 8-byte store)
+        unsigned long long pos = 0;
+        if (cand_r) pos = atomicAdd(tp.gtail + own, 1ull);
         // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
-        const unsigned int lc = cand & local;
-        unsigned int old[2 * DIM];
-        if (s0 > 0) {
-#pragma unroll
-            for (int k = 0; k < 2 * DIM; ++k)
-                if ((lc >> k) & 1u) old[k] = atomicOr(words + (where[k] >> 2), 0xFEu << ((where[k] & 3u) * 8u));
-        } else {
-#pragma unroll
-            for (int k = 0; k < 2 * DIM; ++k)
-                if ((lc >> k) & 1u) old[k] = atomicAnd(words + (where[k] >> 2), ~(0xFEu << ((where[k] & 3u) * 8u)));
+        bool won = false;
+        if (cand_l) {
+            const unsigned int old = s0 > 0 ? atomicOr(words + (addr >> 2), 0xFEu << shift) : atomicAnd(words + (addr >> 2), ~(0xFEu << shift));
+            won = ((old >> shift) & 0xFFu) == s0_byte;
+            ++tl.attempts;
         }
-        const unsigned int s0_byte = (unsigned int)s0 & 0xFFu;
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k)
-            if (((lc >> k) & 1u) && (((old[k] >> ((where[k] & 3u) * 8u)) & 0xFFu) == s0_byte)) won |= 1u << k;
-        tl.attempts += __popc(lc);
-        mywon += __popc(won);
+        mywon += won ? 1u : 0u;
         if (lane == 0) ++tl.passes;
 
-        // ---- A5: compact the winners; the first 32 are this warp's next pass
-        unsigned int total = 0;
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k) {
-            const bool mine = (won >> k) & 1u;
-            const unsigned int b = __ballot_sync(kFullMask, mine);
-            if (mine) stage[total + __popc(b & lt)] = nbr[k];
-            total += __popc(b);
-        }
+        // ---- A5: compact the winners; the first S are this warp's next pass
+        const unsigned int wb = __ballot_sync(kFullMask, won);
+        const unsigned int total = __popc(wb);
+        if (won) stage[__popc(wb & lt)] = nid;
         // messages leave before this pass is accounted for
-#pragma unroll
-        for (int k = 0; k < 2 * DIM; ++k) {
-            if ((remote >> k) & 1u) {
-                const unsigned int lap = (unsigned int)(pos[k] >> tp.in_log) & 1u;
-                st_relaxed_u64(tp.inbox + ((size_t)where[k] << tp.in_log) + ((uint32_t)pos[k] & in_mask),
-                               pack_msg(kKindClaim, lap, krel, nbr[k], s0));
-                ++tl.messages;
-            }
+        if (cand_r) {
+            const unsigned int lap = (unsigned int)(pos >> tp.in_log) & 1u;
+            st_relaxed_u64(tp.inbox + ((size_t)own << tp.in_log) + ((uint32_t)pos & in_mask), pack_msg(kKindClaim, lap, krel, nid, s0));
+            ++tl.messages;
         }
         __syncwarp();
         // ---- accounting: the new sites are counted before any of them can be seen by another warp
@@ -410,10 +368,14 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
         } else if (total != expanded) {
             if (lane == 0) atomicAdd(&sh.pending, total - expanded);
         }
-        have = lane < total;
-        if (have) site = stage[lane];
-        if (total > 32u) hand_over(tp, sh, ring, stage + 32, total - 32u, c, tl);
+        nsites = total < S ? total : S;
+        if (alive && q < nsites) site = stage[q];
+        if (total > S) hand_over(tp, sh, ring, stage + S, total - S, c, tl);
         __syncwarp();      // stage[] is rewritten in the next pass
+#ifdef WOLFF_PROFILE
+        tl.cyc_pass += (unsigned long long)(clock64() - tp0);
+        tl.lanes += expanded;
+#endif
     }
 }
 
@@ -641,6 +603,10 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         if (rp) atomicAdd(&ctl->stats[12], (unsigned long long)rp);
         if (tl.passes) atomicAdd(&ctl->stats[13], (unsigned long long)tl.passes);
         if (sp) atomicAdd(&ctl->stats[14], (unsigned long long)sp);
+#ifdef WOLFF_PROFILE
+        if (tl.cyc_pass) atomicAdd(&ctl->stats[15], tl.cyc_pass);
+        if (tl.lanes) atomicAdd(&ctl->stats[10], tl.lanes);
+#endif
     }
 }
 
