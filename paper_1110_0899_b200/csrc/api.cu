@@ -64,6 +64,7 @@ struct wolff_ctx {
     int tile_ctas_opt = 0;          // 0 = one CTA per SM
     uint32_t ring_cap = 8192;
     uint64_t watchdog_ms = 20000;
+    uint32_t idle_ns = 1000;
     size_t smem_optin = 0;          // shared memory one CTA may use
     bool plan_dirty = true;
     bool plan_ok = false;
@@ -196,6 +197,9 @@ int refresh_plan(wolff_ctx *h)
     tp.spill_log = ceil_log2((uint64_t)slots << (dim * b));
     tp.ring_cap = h->ring_cap;
     tp.watchdog_ns = h->watchdog_ms * 1000000ull;
+    tp.idle_ns = h->idle_ns;
+    tp.thr32 = (uint32_t)h->thr;
+    tp.thr_all = (h->thr >> 32) != 0 ? 1u : 0u;
     h->tile_smem = smem;
 
     const size_t inbox_bytes = ((size_t)G << tp.in_log) * sizeof(unsigned long long);
@@ -472,6 +476,10 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
     } else if (!strcmp(key, "watchdog_ms")) {
         if (value < 1 || value > 3600000) { set_error("watchdog_ms must be in [1, 3600000]"); return WOLFF_EINVAL; }
         h->watchdog_ms = (uint64_t)value;
+        h->plan_dirty = true;
+    } else if (!strcmp(key, "idle_ns")) {
+        if (value < 0 || value > 1000000) { set_error("idle_ns must be in [0, 1000000]"); return WOLFF_EINVAL; }
+        h->idle_ns = (uint32_t)value;
         h->plan_dirty = true;
     } else if (!strcmp(key, "ring_cap")) {
         if (value < 32 || value > 32768 || (value & (value - 1)) != 0) { set_error("ring_cap must be a power of two in [32, 32768]"); return WOLFF_EINVAL; }

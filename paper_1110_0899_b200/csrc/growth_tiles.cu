@@ -72,9 +72,33 @@ __device__ __forceinline__ void st_relaxed_u64(unsigned long long *p, unsigned l
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+// Branch-free forms for the dependent chain of a worker pass (predicated instructions instead of divergent regions).
+__device__ __forceinline__ uint32_t selp_u32(uint32_t a, uint32_t b, bool pick_a)
+{
+    uint32_t r;
+    asm("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n selp.u32 %0, %1, %2, p;\n}" : "=r"(r) : "r"(a), "r"(b), "r"((unsigned int)pick_a));
+    return r;
+}
+// Claim on shared memory: OR (s0 = +1) or AND (s0 = -1) on the word at shared address saddr, when `go`; returns the old word.
+__device__ __forceinline__ unsigned int atoms_claim(uint32_t saddr, unsigned int mask_or, bool go_or, bool go_and)
+{
+    unsigned int old = 0;
+    asm volatile("{\n .reg .pred p, q;\n .reg .b32 m;\n setp.ne.u32 p, %3, 0;\n setp.ne.u32 q, %4, 0;\n not.b32 m, %2;\n"
+                 " @p atom.shared.or.b32 %0, [%1], %2;\n @q atom.shared.and.b32 %0, [%1], m;\n}"
+                 : "+r"(old) : "r"(saddr), "r"(mask_or), "r"((unsigned int)go_or), "r"((unsigned int)go_and) : "memory");
+    return old;
+}
+__device__ __forceinline__ unsigned long long atomg_inc_if(unsigned long long *p, bool go)
+{
+    unsigned long long old = 0;
+    asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %2, 0;\n @p atom.global.add.u64 %0, [%1], 1;\n}"
+                 : "+l"(old) : "l"(p), "r"((unsigned int)go) : "memory");
+    return old;
+}
+
 // Per-CTA shared state.
-struct TShared {
-    unsigned int head, tail;            // ring: entries [head, tail) wait for a worker warp
+struct alignas(16) TShared {
+    unsigned int head, tail;            // ring: entries [head, tail) wait for a worker warp (one aligned 64-bit word)
     unsigned int pending;               // sites claimed by this CTA and not yet expanded (+ receiver tokens)
     unsigned int claimed;               // spins claimed since the last publish
     unsigned int stop;                  // leave: exit message seen, or the launch is aborted
@@ -94,6 +118,7 @@ struct Tally {
 #ifdef WOLFF_PROFILE
     unsigned long long cyc_pass = 0;    // cycles inside passes (lane 0)
     unsigned long long lanes = 0;       // sites expanded (lane 0)
+    unsigned long long cyc1 = 0, n1 = 0, cyc1r = 0, cyc2 = 0, cyc3 = 0, cyc23c = 0, n23c = 0;
 #endif
 };
 
@@ -232,9 +257,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
     const uint32_t rmask = tp.ring_cap - 1u;
     const uint32_t tile_sites_log = DIM * tp.tile_log;
     const uint32_t in_mask = tp.in_cap - 1u;
-    const uint32_t thr32 = (uint32_t)p.thr;
-    const bool always = (p.thr >> 32) != 0ull;          // thr = 2^32: every bond is active
-    unsigned int *const words = reinterpret_cast<unsigned int *>(lat);
+    const uint32_t lat_s = (uint32_t)__cvta_generic_to_shared(lat);
     uint32_t site = 0;
     unsigned int nsites = 0;     // sites held by the warp (warp-uniform); lanes of group q < nsites work
     int s0 = 1;
@@ -250,25 +273,30 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
             if (lane == 0) {
                 unsigned int idle = 0;
                 for (;;) {
-                    // head before tail: tail only grows and head never passes it, so t - h >= 0 whatever happens in between
-                    h = ld_vol(&sh.head);
-                    const unsigned int t = ld_vol(&sh.tail);
+                    // one 64-bit load: a consistent (head, tail) pair; the three loads of an idle poll are independent
+                    const unsigned long long ht = ld_vol64(reinterpret_cast<const unsigned long long *>(&sh.head));
+                    sh_pos = ld_vol64(&sh.spill_head);
+                    const unsigned long long st = ld_vol64(&sh.spill_tail);
+                    const unsigned int stop = ld_vol(&sh.stop);
+                    h = (unsigned int)ht;
+                    const unsigned int t = (unsigned int)(ht >> 32);
                     if (t != h) {
                         n = t - h < S ? t - h : S;
                         if (atomicCAS(&sh.head, h, h + n) == h) break;
                         n = 0;
                         continue;
                     }
-                    sh_pos = ld_vol64(&sh.spill_head);
-                    const unsigned long long st = ld_vol64(&sh.spill_tail);
                     if (st != sh_pos) {
                         n = st - sh_pos < (unsigned long long)S ? (unsigned int)(st - sh_pos) : S;
                         if (atomicCAS(&sh.spill_head, sh_pos, sh_pos + n) == sh_pos) { from_spill = 1; break; }
                         n = 0;
                         continue;
                     }
-                    if (ld_vol(&sh.stop)) break;
-                    if (++idle > 16u) __nanosleep(20);
+                    if (stop) break;
+                    // idle warps share the SM's load/store pipe with the working ones: back off (the warps of a CTA are
+                    // staggered by their idle counts, so one of them polls every few tens of nanoseconds)
+                    ++idle;
+                    if (idle > 2u) __nanosleep(idle < 8u ? 64u : (idle < 16u ? 256u : tp.idle_ns));
                 }
             }
             n = __shfl_sync(kFullMask, n, 0);
@@ -321,27 +349,29 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
         const bool local = own == c;
         const unsigned int shift = (addr & 3u) * 8u;
         // gather (LDS), in flight while the Philox rounds execute
+        const uint32_t saddr = lat_s + (addr & ~3u);
         unsigned int spw = 0;
-        if (have && local) spw = *reinterpret_cast<volatile unsigned int *>(words + (addr >> 2));
+        if (have && local) asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(spw) : "r"(saddr));
         // ---- A3: the bond to the +d neighbour is owned by this site, the bond to the -d neighbour by that neighbour
         const uint4 blk = philox4x32_10(sgn ? nid : site, kDomainBond, u_lo, u_hi, p.key0, p.key1);
-        const uint32_t r = d == 0u ? blk.x : (d == 1u ? blk.y : blk.z);
-        const bool active = have && (always || r < thr32);
+        const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
+        const bool active = have && (r < tp.thr32 || tp.thr_all != 0u);
         const bool cand_l = active && local && (((spw >> shift) & 0xFFu) == s0_byte);
         const bool cand_r = active && !local;
 
         // ---- A4 across the territory border: a message to the owner (slot by one L2 atomic, then one 8-byte store)
-        unsigned long long pos = 0;
-        if (cand_r) pos = atomicAdd(tp.gtail + own, 1ull);
+        const unsigned long long pos = atomg_inc_if(tp.gtail + own, cand_r);
         // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
-        bool won = false;
-        if (cand_l) {
-            const unsigned int old = s0 > 0 ? atomicOr(words + (addr >> 2), 0xFEu << shift) : atomicAnd(words + (addr >> 2), ~(0xFEu << shift));
-            won = ((old >> shift) & 0xFFu) == s0_byte;
-            ++tl.attempts;
-        }
+        const unsigned int old = atoms_claim(saddr, 0xFEu << shift, cand_l && s0 > 0, cand_l && s0 < 0);
+        const bool won = cand_l && (((old >> shift) & 0xFFu) == s0_byte);
+        tl.attempts += cand_l ? 1u : 0u;
         mywon += won ? 1u : 0u;
         if (lane == 0) ++tl.passes;
+#ifdef WOLFF_PROFILE
+        const long long tp1 = clock64();
+        const bool anyr = __any_sync(kFullMask, cand_r);
+        if (anyr) tl.cyc1r += (unsigned long long)(tp1 - tp0); else { tl.cyc1 += (unsigned long long)(tp1 - tp0); ++tl.n1; }
+#endif
 
         // ---- A5: compact the winners; the first S are this warp's next pass
         const unsigned int wb = __ballot_sync(kFullMask, won);
@@ -354,6 +384,10 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
             ++tl.messages;
         }
         __syncwarp();
+#ifdef WOLFF_PROFILE
+        const long long tp2 = clock64();
+        tl.cyc2 += (unsigned long long)(tp2 - tp1);
+#endif
         // ---- accounting: the new sites are counted before any of them can be seen by another warp
         if (total == 0u) {
             // the warp runs dry: its claims become visible to the publisher before its sites stop being pending
@@ -373,7 +407,10 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, i
         if (total > S) hand_over(tp, sh, ring, stage + S, total - S, c, tl);
         __syncwarp();      // stage[] is rewritten in the next pass
 #ifdef WOLFF_PROFILE
-        tl.cyc_pass += (unsigned long long)(clock64() - tp0);
+        const long long tp3 = clock64();
+        tl.cyc_pass += (unsigned long long)(tp3 - tp0);
+        tl.cyc3 += (unsigned long long)(tp3 - tp2);
+        if (total != 0u && total <= S && !anyr) { tl.cyc23c += (unsigned long long)(tp3 - tp1); ++tl.n23c; }
         tl.lanes += expanded;
 #endif
     }
@@ -523,7 +560,9 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
     if (lane == 0) {
         ctl->stats[0] += p.n_updates;
         ctl->stats[1] += flipped;
+#ifndef WOLFF_PROFILE
         ctl->stats[9] += polls_total;
+#endif
     }
 }
 
@@ -606,6 +645,13 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
 #ifdef WOLFF_PROFILE
         if (tl.cyc_pass) atomicAdd(&ctl->stats[15], tl.cyc_pass);
         if (tl.lanes) atomicAdd(&ctl->stats[10], tl.lanes);
+        if (tl.cyc1) atomicAdd(&ctl->stats[2], tl.cyc1);
+        if (tl.n1) atomicAdd(&ctl->stats[3], tl.n1);
+        if (tl.cyc1r) atomicAdd(&ctl->stats[4], tl.cyc1r);
+        if (tl.cyc2) atomicAdd(&ctl->stats[5], tl.cyc2);
+        if (tl.cyc3) atomicAdd(&ctl->stats[6], tl.cyc3);
+        if (tl.cyc23c) atomicAdd(&ctl->stats[8], tl.cyc23c);
+        if (tl.n23c) atomicAdd(&ctl->stats[9], tl.n23c);
 #endif
     }
 }

@@ -79,6 +79,8 @@ struct TileParams {
     uint32_t spill_log;              // spill entries per CTA (at least the sites the CTA owns)
     uint32_t ring_cap;               // entries of the shared-memory ring (power of two)
     unsigned long long watchdog_ns;  // an update longer than this aborts the launch
+    uint32_t thr32, thr_all;         // low word of the bond threshold; thr_all = 1 when thr = 2^32 (every bond active)
+    uint32_t idle_ns;                // longest sleep of an idle worker warp between two polls of the ring
 };
 
 // Launch shape of the persistent kernel.
