@@ -43,8 +43,10 @@ def measured_peak_hbm():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-# ncu `--set full` DRAM traffic of the growth kernel per launch, bytes; see profiles/.  None until captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = None
+# ncu `--set full` DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of one launch of the growth kernel,
+# bytes: profiles/r1_growth_tiles_C3.md (a 10-update C3 launch: the 16 MiB lattice is read once in the prologue; the
+# write-back and all queue traffic stay in L2).  It does not grow with the updates per launch.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 22557696 + 536576
 
 
 class ClockSampler:
@@ -104,6 +106,28 @@ def algorithmic_bytes(dim: int, flipped: int, attempts: int) -> int:
     return flipped * (2 * dim + 8) + 4 * attempts
 
 
+# ====================================================================== N > 1: replicas only
+
+def all_reduce_scalar(x, op: str, world: int, device=None):
+    """Sum / max of one number over the ranks (no-op at world 1).  The only collective of the bench: the data path
+    has none, every rank runs its own chain."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM if op == "sum" else dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_replicas(flipped: int, updates: int, total_ms: float, world: int, device=None):
+    """Whole-job throughput of N independent replicas: units of all ranks / the slowest rank's device time."""
+    ms = all_reduce_scalar(total_ms, "max", world, device)
+    f = all_reduce_scalar(flipped, "sum", world, device)
+    u = all_reduce_scalar(updates, "sum", world, device)
+    return {"total_ms": ms, "flipped": f, "updates": u, "value": f / (ms * 1e-3), "updates_per_s": u / (ms * 1e-3)}
+
+
 # ====================================================================== the CUDA arm
 
 def run_b200(args, rank: int, world: int):
@@ -139,9 +163,20 @@ def run_b200(args, rank: int, world: int):
         sizes_d = torch.zeros(updates, dtype=torch.int32, device=dev)
         flipped = attempts = levels = 0
         step_ms, growth_ms = [], []
+        # BFS depth of the clusters the timed steps grow (a property of the workload): the
+        # level-synchronous kernel (mode 4) replays the same updates from the same lattice, untimed, and counts levels
+        twin = None
+        if args.mode == 0 and not args.no_depth:
+            twin = binding.Wolff(c.dim, c.L, c.J, c.T, seed)
+            twin.set_option("mode", 4)
+            snapshot = torch.empty(c.N, dtype=torch.int8, device=dev)
 
         def one_step(timed: bool):
             nonlocal flipped, attempts, levels
+            if timed and twin is not None:
+                h.get_spins_into(snapshot)
+                twin.set_spins(snapshot)
+                twin.update_index = h.update_index
             with torch.cuda.stream(stream):
                 flush.fill_(1)                     # L2 flush between steps, outside the timed events
                 e0 = torch.cuda.Event(enable_timing=True)
@@ -158,8 +193,13 @@ def run_b200(args, rank: int, world: int):
                 growth_ms.append(e0.elapsed_time(e1))
                 st = h.stats()
                 flipped += st["flipped"]; attempts += st["claim_attempts"]
-                levels += st["levels_cta"] + st["levels_cluster"] + st["levels_grid"]
                 assert int(sizes_d.sum().item()) == st["flipped"]
+                if twin is not None:
+                    twin.run(updates, stream=stream)
+                    ts = twin.stats()
+                    assert ts["flipped"] == st["flipped"]
+                    st = ts
+                levels += st["levels_cta"] + st["levels_cluster"] + st["levels_grid"]
 
         for _ in range(warmup):
             one_step(False)
@@ -170,6 +210,8 @@ def run_b200(args, rank: int, world: int):
                 one_step(True)
             barrier()
         wall = time.perf_counter() - t0
+        if twin is not None:
+            twin.close()
         res = {"cfg": c, "h": h, "flipped": flipped, "attempts": attempts, "levels": levels, "updates": updates * steps,
                "step_ms": step_ms, "growth_ms": growth_ms, "wall_s": wall, "clocks": clocks.summary()}
         return res
@@ -199,29 +241,16 @@ def run_b200(args, rank: int, world: int):
         dt = time.perf_counter() - t0
         return {"flipped": flipped, "seconds": dt, "h2d": c.N, "d2h": c.N + 16 + 4 * updates}
 
-    import torch.distributed as dist
-
     def reduce_sum(x):
-        if world == 1:
-            return x
-        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        return float(t.item())
+        return all_reduce_scalar(x, "sum", world, dev)
 
     def reduce_max(x):
-        if world == 1:
-            return x
-        t = torch.tensor([float(x)], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+        return all_reduce_scalar(x, "max", world, dev)
 
     primary = measure(args.workload, args.updates, args.equil, args.steps, args.warmup, cold=True)
     c = primary["cfg"]
-    total_ms = reduce_max(sum(primary["step_ms"]))
-    growth_ms_total = reduce_max(sum(primary["growth_ms"]))
-    flipped_all = reduce_sum(primary["flipped"])
-    updates_all = reduce_sum(primary["updates"])
-    value = flipped_all / (total_ms * 1e-3)
+    agg = aggregate_replicas(primary["flipped"], primary["updates"], sum(primary["step_ms"]), world, dev)
+    total_ms, updates_all, value = agg["total_ms"], agg["updates"], agg["value"]
 
     e = e2e(args.workload, args.updates, args.steps, args.warmup, primary["h"])
     e2e_value = reduce_sum(e["flipped"]) / reduce_max(e["seconds"])
@@ -241,16 +270,17 @@ def run_b200(args, rank: int, world: int):
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "updates_per_s": updates_all / (total_ms * 1e-3),
         "mean_cluster": primary["flipped"] / primary["updates"],
-        "levels_per_update": primary["levels"] / primary["updates"],
-        "us_per_level": sum(primary["growth_ms"]) * 1e3 / max(primary["levels"], 1),
+        "bfs_depth_per_update": primary["levels"] / primary["updates"],
+        "us_per_bfs_level": sum(primary["growth_ms"]) * 1e3 / max(primary["levels"], 1),
         "clocks": primary["clocks"],
         "gpu_launches": 2 * args.steps,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"]},
-        "roofline": {"bound": "hbm", "kernel": "growth_kernel (persistent, one launch per step)",
+        "roofline": {"bound": "hbm", "kernel": ("growth_tiles_kernel" if args.mode == 0 else "growth_kernel") + " (persistent, one launch per step)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
                      "algorithmic_bytes_per_launch": alg_bytes,
-                     "note": "latency-bound by design: the path is a chain of dependent BFS levels, not a stream"},
+                     "note": "latency-bound by design: the path is a chain of dependent hops (BFS depth x hop latency), not a stream; "
+                             "see bfs_depth_per_update and us_per_bfs_level"},
     }
 
     if rank == 0 and world == 1 and not args.no_secondary:
@@ -261,8 +291,8 @@ def run_b200(args, rank: int, world: int):
         out["secondary"] = {"workload": sc.name + ", equilibrated variant", "value": sec["flipped"] / (ms * 1e-3), "unit": UNIT,
                             "updates_per_s": sec["updates"] / (ms * 1e-3), "ms_per_step": ms / args.steps,
                             "updates_per_step": args.secondary_updates, "mean_cluster": sec["flipped"] / sec["updates"],
-                            "levels_per_update": sec["levels"] / sec["updates"],
-                            "us_per_level": sum(sec["growth_ms"]) * 1e3 / max(sec["levels"], 1)}
+                            "bfs_depth_per_update": sec["levels"] / sec["updates"],
+                            "us_per_bfs_level": sum(sec["growth_ms"]) * 1e3 / max(sec["levels"], 1)}
         sec["h"].close()
         lit = {}
         for name in (args.workload, args.secondary):
@@ -340,6 +370,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--reference-updates", type=int, default=3)
     ap.add_argument("--mode", type=int, default=0, help="growth kernel: 0 = default (shared-memory-resident), 4 = level-synchronous tiers")
+    ap.add_argument("--no-depth", action="store_true", help="skip the untimed BFS-depth replay of the timed updates")
     ap.add_argument("--no-secondary", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
