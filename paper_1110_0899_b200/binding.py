@@ -19,7 +19,7 @@ WOLFF_OK, WOLFF_EINVAL, WOLFF_ENOMEM, WOLFF_ECUDA, WOLFF_EINTERNAL = 0, -1, -2, 
 NSTATS = 16
 STAT_NAMES = ("updates", "flipped", "levels_cta", "levels_cluster", "levels_grid", "cluster_wakeups",
               "levels_rebalanced", "claim_attempts", "widest_frontier", "monitor_polls",
-              "s10", "messages", "ring_pushes", "warp_passes", "spills", "s15")
+              "inline_passes", "messages", "ring_pushes", "warp_passes", "spills", "fill_chunks")
 
 # every symbol include/wolff.h declares (tests/test_abi.py checks the header against this table)
 _SIGNATURES = {

@@ -62,7 +62,9 @@ struct wolff_ctx {
     // shared-memory-resident kernel (growth_tiles.cu): knobs, plan, and the device state that goes with the plan
     int tile_log_opt = 0;           // 0 = auto
     int tile_ctas_opt = 0;          // 0 = one CTA per SM
-    uint32_t ring_cap = 8192;
+    uint32_t ring_cap = 2048;
+    int fill_mode = 1;              // bond tables: 0 off, 1 adaptive, 2 always
+    uint64_t fill_min_us = 30;
     uint64_t watchdog_ms = 20000;
     uint32_t idle_ns = 1000;
     size_t smem_optin = 0;          // shared memory one CTA may use
@@ -73,6 +75,7 @@ struct wolff_ctx {
     unsigned long long *tile_inbox = nullptr;
     unsigned long long *tile_ctr = nullptr;     // gtail[G], gdone[G], gspill[G], added
     uint32_t *tile_spill = nullptr;
+    uint32_t *tile_fill = nullptr;
 };
 
 namespace {
@@ -149,6 +152,7 @@ void free_tile_state(wolff_ctx *h)
     cudaFree(h->tile_inbox); h->tile_inbox = nullptr;
     cudaFree(h->tile_ctr); h->tile_ctr = nullptr;
     cudaFree(h->tile_spill); h->tile_spill = nullptr;
+    cudaFree(h->tile_fill); h->tile_fill = nullptr;
 }
 
 uint32_t ceil_log2(uint64_t v) { uint32_t l = 0; while ((1ull << l) < v) ++l; return l; }
@@ -173,7 +177,11 @@ int refresh_plan(wolff_ctx *h)
     if (h->tile_ctas_opt > 0 && (uint32_t)h->tile_ctas_opt < G) G = (uint32_t)h->tile_ctas_opt;
     if (ntiles < G) G = (uint32_t)ntiles;
     const uint32_t slots = (uint32_t)((ntiles + G - 1) / G);
-    const size_t smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap);
+    if (slots > 0xFFFFu || G > 0xFFFFu) return WOLFF_OK;
+    // bond tables (growth_tiles.cu) when they fit beside the lattice; a tile must hold at least one 32-bit word of bonds
+    bool tables = h->fill_mode != 0 && dim * b >= 5u;
+    size_t smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap, tables);
+    if (tables && smem + 256 > h->smem_optin) { tables = false; smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap, false); }
     if (smem + 256 > h->smem_optin) return WOLFF_OK;
     int per_sm = 0;
     cudaError_t e = tiles_prepare(h->dim, smem, &per_sm);
@@ -198,6 +206,9 @@ int refresh_plan(wolff_ctx *h)
     tp.ring_cap = h->ring_cap;
     tp.watchdog_ns = h->watchdog_ms * 1000000ull;
     tp.idle_ns = h->idle_ns;
+    tp.tables = tables ? 1u : 0u;
+    tp.fill_mode = tables ? (uint32_t)h->fill_mode : 0u;
+    tp.fill_min_ns = h->fill_min_us * 1000ull;
     tp.thr32 = (uint32_t)h->thr;
     tp.thr_all = (h->thr >> 32) != 0 ? 1u : 0u;
     h->tile_smem = smem;
@@ -206,7 +217,7 @@ int refresh_plan(wolff_ctx *h)
     const size_t ctr_bytes = (3 * (size_t)G + 1) * sizeof(unsigned long long);
     const size_t spill_bytes = ((size_t)G << tp.spill_log) * sizeof(uint32_t);
     if (cudaMalloc(&h->tile_inbox, inbox_bytes) != cudaSuccess || cudaMalloc(&h->tile_ctr, ctr_bytes) != cudaSuccess ||
-        cudaMalloc(&h->tile_spill, spill_bytes) != cudaSuccess) {
+        cudaMalloc(&h->tile_spill, spill_bytes) != cudaSuccess || cudaMalloc(&h->tile_fill, (size_t)G * sizeof(uint32_t)) != cudaSuccess) {
         cudaGetLastError();
         free_tile_state(h);
         return WOLFF_OK;      // not enough memory for the tiled kernel's queues: the level-synchronous kernel needs none
@@ -214,12 +225,14 @@ int refresh_plan(wolff_ctx *h)
     CHECK_CUDA(h, cudaMemset(h->tile_inbox, 0, inbox_bytes), "clear inboxes");
     CHECK_CUDA(h, cudaMemset(h->tile_ctr, 0, ctr_bytes), "clear counters");
     CHECK_CUDA(h, cudaMemset(h->tile_spill, 0, spill_bytes), "clear spill lists");
+    CHECK_CUDA(h, cudaMemset(h->tile_fill, 0, (size_t)G * sizeof(uint32_t)), "clear fill flags");
     tp.inbox = h->tile_inbox;
     tp.gtail = h->tile_ctr;
     tp.gdone = h->tile_ctr + G;
     tp.gspill = h->tile_ctr + 2 * (size_t)G;
     tp.added = h->tile_ctr + 3 * (size_t)G;
     tp.spill = h->tile_spill;
+    tp.gfill = h->tile_fill;
     h->plan_ok = true;
     return WOLFF_OK;
 }
@@ -476,6 +489,14 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
     } else if (!strcmp(key, "watchdog_ms")) {
         if (value < 1 || value > 3600000) { set_error("watchdog_ms must be in [1, 3600000]"); return WOLFF_EINVAL; }
         h->watchdog_ms = (uint64_t)value;
+        h->plan_dirty = true;
+    } else if (!strcmp(key, "fill")) {
+        if (value < 0 || value > 2) { set_error("fill must be 0 (never), 1 (adaptive) or 2 (always)"); return WOLFF_EINVAL; }
+        h->fill_mode = (int)value;
+        h->plan_dirty = true;
+    } else if (!strcmp(key, "fill_min_us")) {
+        if (value < 0 || value > 1000000) { set_error("fill_min_us must be in [0, 1000000]"); return WOLFF_EINVAL; }
+        h->fill_min_us = (uint64_t)value;
         h->plan_dirty = true;
     } else if (!strcmp(key, "idle_ns")) {
         if (value < 0 || value > 1000000) { set_error("idle_ns must be in [0, 1000000]"); return WOLFF_EINVAL; }

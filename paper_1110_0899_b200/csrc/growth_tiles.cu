@@ -10,16 +10,29 @@
 //   - for the length of one launch the int8 lattice LIVES IN SHARED MEMORY.  It is cut into tiles of
 //     B^dim sites; tile t belongs to CTA (t*A mod ntiles) mod G, one CTA per SM, so every BASELINE
 //     lattice (<= 16 MiB) fits the 148 x 227 KiB of the chip.  Claim-and-flip (A4) is the same single
-//     idempotent atomic as in growth.cu, but on shared memory: the dependent chain of one hop is
-//     LDS gather || Philox -> ATOMS -> ballot, a few hundred cycles instead of two L2 round trips;
-//   - a site is always expanded by the CTA that owns its tile.  A warp that claims neighbours keeps up to
-//     32 of them in registers and expands them in its next pass; the rest goes to a shared-memory ring that
-//     the other warps of the CTA drain (overflow: a per-CTA global spill list);
-//   - an active bond that leaves the CTA's territory becomes a MESSAGE "claim site j" in the owner's inbox
-//     (global memory, one L2 atomicAdd for the slot + one 8-byte store); the owner's receiver warp polls its
-//     inbox, makes the claim on its own shared memory and feeds its ring.  Bond variables are a function of
-//     (seed, update, bond), so the cluster is the connected component of the seed
-//     site whatever the order of expansion: no BFS levels, no barrier (A6 becomes a work hand-over);
+//     idempotent atomic as in growth.cu, but on shared memory;
+//   - inside a CTA a site is its LOCAL ADDRESS a = slot * B^dim + (within-tile index): a neighbour in the
+//     same tile is a +- stride, a neighbour across a tile border comes from a small per-slot table
+//     (owner CTA, slot) built in the prologue.  Global site ids are only rebuilt where a Philox counter
+//     needs one;
+//   - ONE LANE PER BOND: a warp holds up to 32 / (2 dim) sites per pass and lane (q, k) tests the bond
+//     from site q to its neighbour k.  The frontier inside one CTA is a handful of sites wide, so lanes
+//     are cheap; what an update waits for is the dependent instruction chain of a pass;
+//   - BOND TABLES: the bond variables of update v are a pure function of (seed, v, bond) -- they do not
+//     depend on the spins -- so warps with nothing to expand evaluate Philox4x32-10 for the tiles of
+//     their CTA AHEAD of time (update v, then v + 1, double-buffered bit planes in shared memory, one
+//     bit per bond).  A worker then reads one bit instead of running ten Philox rounds on its critical
+//     path; where a tile's table is not ready (or the bond belongs to a site of another CTA) the lane
+//     evaluates the same Philox block inline.  Both give the same bit, so the result cannot depend on
+//     which one ran;
+//   - a warp that claims neighbours keeps up to S of them in registers for its next pass; the rest goes
+//     to a shared-memory ring that the other warps of the CTA drain (overflow: a per-CTA global spill list);
+//   - an active bond that leaves the CTA's territory becomes a MESSAGE "claim the site at your local
+//     address a" in the owner's inbox (global memory, one L2 atomicAdd for the slot + one 8-byte
+//     store); the owner's receiver warp polls its inbox, makes the claim on its own shared memory and
+//     feeds its ring.  Bond variables are a function of (seed, update, bond), so
+//     the cluster is the connected component of the seed site whatever the order of expansion: no BFS
+//     levels, no barrier (A6 becomes a work hand-over);
 //   - termination of an update: every CTA publishes gdone[c] = "inbox messages consumed, with their whole
 //     local progeny expanded" whenever it runs dry; a monitor warp in CTA 0 reads every gdone[], then every
 //     gtail[] (messages ever pushed).  Both only grow, a message is counted in gtail before anything it
@@ -38,7 +51,8 @@ namespace {
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;
 constexpr int kT = kTileThreads;
 constexpr int kWarps = kT / 32;
-constexpr int kStage = 32;                         // winners one warp can produce in one pass (one per lane)
+constexpr int kStage = 64;                         // two buffers of 32 winners per warp (one winner per lane and pass)
+constexpr uint32_t kBusy = 0x80000000u;            // bond-table state: a warp is filling this tile
 
 // message = [kind:2 | lap:1 | k:29] [site:31 | s0<0:1]
 enum Kind : unsigned int { kKindNone = 0, kKindClaim = 1, kKindSeed = 2, kKindExit = 3 };
@@ -79,23 +93,6 @@ __device__ __forceinline__ uint32_t selp_u32(uint32_t a, uint32_t b, bool pick_a
     asm("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n selp.u32 %0, %1, %2, p;\n}" : "=r"(r) : "r"(a), "r"(b), "r"((unsigned int)pick_a));
     return r;
 }
-// Claim on shared memory: OR (s0 = +1) or AND (s0 = -1) on the word at shared address saddr, when `go`; returns the old word.
-__device__ __forceinline__ unsigned int atoms_claim(uint32_t saddr, unsigned int mask_or, bool go_or, bool go_and)
-{
-    unsigned int old = 0;
-    asm volatile("{\n .reg .pred p, q;\n .reg .b32 m;\n setp.ne.u32 p, %3, 0;\n setp.ne.u32 q, %4, 0;\n not.b32 m, %2;\n"
-                 " @p atom.shared.or.b32 %0, [%1], %2;\n @q atom.shared.and.b32 %0, [%1], m;\n}"
-                 : "+r"(old) : "r"(saddr), "r"(mask_or), "r"((unsigned int)go_or), "r"((unsigned int)go_and) : "memory");
-    return old;
-}
-__device__ __forceinline__ unsigned long long atomg_inc_if(unsigned long long *p, bool go)
-{
-    unsigned long long old = 0;
-    asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %2, 0;\n @p atom.global.add.u64 %0, [%1], 1;\n}"
-                 : "+l"(old) : "l"(p), "r"((unsigned int)go) : "memory");
-    return old;
-}
-
 // Per-CTA shared state.
 struct alignas(16) TShared {
     unsigned int head, tail;            // ring: entries [head, tail) wait for a worker warp (one aligned 64-bit word)
@@ -105,6 +102,9 @@ struct alignas(16) TShared {
     unsigned int pub_lock;              // publishers of this CTA take turns
     int s0;                             // seed spin of the running update
     uint32_t u_lo, u_hi;                // its index
+    unsigned int krel;                  // ... relative to the first update of the launch
+    unsigned int fill_on;               // idle warps fill bond tables (adaptive: off when updates are too short to pay for it)
+    unsigned int pad;
     unsigned long long ihead;           // inbox messages consumed (written by the receiver warp only)
     unsigned long long spill_head, spill_tail;   // running positions in the CTA's global spill list (kept across launches)
 };
@@ -115,26 +115,28 @@ struct Tally {
     unsigned int ring_pushes = 0;       // sites handed to the ring (per lane)
     unsigned int spills = 0;            // sites spilled to global memory (per lane)
     unsigned int passes = 0;            // warp passes (lane 0)
+    unsigned int inline_passes = 0;     // ... of which at least one lane ran Philox inline (lane 0)
+    unsigned int chunks = 0;            // bond-table chunks filled: 32 sites each (lane 0)
 #ifdef WOLFF_PROFILE
     unsigned long long cyc_pass = 0;    // cycles inside passes (lane 0)
     unsigned long long lanes = 0;       // sites expanded (lane 0)
-    unsigned long long cyc1 = 0, n1 = 0, cyc1r = 0, cyc2 = 0, cyc3 = 0, cyc23c = 0, n23c = 0;
 #endif
 };
 
 // ------------------------------------------------------------------------------------------ geometry of the tiling
 // Site i = x + L*y (+ L*L*z), L a power of two.  Tile coordinates (x >> b, ...), tile index t = tx + ntx*ty (+ ...),
 // p = (t * A) mod ntiles (A odd: a bijection), owner = p mod G, slot = p div G.  Inside a tile sites are
-// row-major again: w = (x & m) + B*(y & m) (+ B*B*(z & m)); shared-memory byte address = slot*B^dim + w.
+// row-major again: w = (x & m) + B*(y & m) (+ B*B*(z & m)); local address a = slot * B^dim + w.
 template <int DIM>
 struct Tiling {
-    uint32_t b, m, nt_log, nt_mask, ntiles_mask, A, G, logL, Lmask;
+    uint32_t b, m, nt_log, nt_mask, ntiles_mask, A, G, logL, Lmask, ts_log, ts_mask;
     unsigned long long magic;
 
     __device__ __forceinline__ explicit Tiling(const TileParams &tp)
         : b(tp.tile_log), m((1u << tp.tile_log) - 1u), nt_log(tp.g.geo.logL - tp.tile_log),
           nt_mask((1u << (tp.g.geo.logL - tp.tile_log)) - 1u), ntiles_mask(tp.ntiles - 1u), A(tp.permA), G(tp.G),
-          logL(tp.g.geo.logL), Lmask(tp.g.geo.L - 1u), magic(tp.magicG) {}
+          logL(tp.g.geo.logL), Lmask(tp.g.geo.L - 1u), ts_log(DIM * tp.tile_log), ts_mask((1u << (DIM * tp.tile_log)) - 1u),
+          magic(tp.magicG) {}
 
     __device__ __forceinline__ void coords(uint32_t i, uint32_t &x, uint32_t &y, uint32_t &z) const
     {
@@ -161,7 +163,64 @@ struct Tiling {
         slot = (uint32_t)(((unsigned long long)p * magic) >> 40);
         owner = p - slot * G;
     }
+    // global site id of a within-tile index, relative to the tile's origin
+    __device__ __forceinline__ uint32_t spread(uint32_t w) const
+    {
+        uint32_t g = (w & m) | (((w >> b) & m) << logL);
+        if (DIM == 3) g |= (w >> (2u * b)) << (2u * logL);
+        return g;
+    }
+    // (owner CTA, local address there) of global site i
+    __device__ __forceinline__ void locate(uint32_t i, uint32_t &owner, uint32_t &addr) const
+    {
+        uint32_t x, y, z, slot;
+        coords(i, x, y, z);
+        place(tile_of(x, y, z), owner, slot);
+        addr = (slot << ts_log) | within(x, y, z);
+    }
 };
+
+// Shared-memory layout of one CTA (offsets follow tiles_smem_bytes()).
+struct Layout {
+    int8_t *lat;           // slots * B^dim spins
+    uint32_t *bond;        // [buf 2][d DIM][slot][B^dim / 32] bond bits (only when tp.tables)
+    uint32_t *state;       // [buf 2][slot]: k + 1 when the tile's bits of update k (relative to the launch) are complete
+    uint32_t *nbrtab;      // [slot][2 DIM]: (owner << 16) | slot of the neighbouring tile
+    uint32_t *origin;      // [slot]: global id of the tile's first site
+    uint32_t *ring;        // ring_cap entries
+    uint32_t *stage;       // kWarps * kStage
+    uint32_t wpt;          // bond words per tile and plane
+    uint32_t plane;        // bond words per plane (slots * wpt)
+    uint32_t myslots;      // slots this CTA really owns
+
+    template <int DIM>
+    static __device__ __forceinline__ Layout make(const TileParams &tp, unsigned char *base, unsigned int c)
+    {
+        Layout l;
+        l.init<DIM>(tp, base, c);
+        return l;
+    }
+    template <int DIM>
+    __device__ __forceinline__ void init(const TileParams &tp, unsigned char *base, unsigned int c)
+    {
+        const uint32_t ts_log = DIM * tp.tile_log;
+        const uint32_t lat_bytes = ((tp.slots << ts_log) + 15u) & ~15u;
+        lat = reinterpret_cast<int8_t *>(base);
+        uint32_t *q = reinterpret_cast<uint32_t *>(base + lat_bytes);
+        wpt = tp.tables ? (1u << (ts_log - 5u)) : 0u;
+        plane = tp.slots * wpt;
+        bond = q;   q += 2u * DIM * plane;
+        state = q;  q += 2u * tp.slots;
+        nbrtab = q; q += 2u * DIM * tp.slots;
+        origin = q; q += tp.slots;
+        ring = q;   q += tp.ring_cap;
+        stage = q;
+        myslots = c < tp.ntiles ? (tp.ntiles - c + tp.G - 1u) / tp.G : 0u;
+    }
+};
+
+template <typename T>
+__device__ __forceinline__ T vol(const T *p) { return *reinterpret_cast<const volatile T *>(p); }
 
 // ------------------------------------------------------------------------------------------ queues
 // Reserve n consecutive ring entries; false when the ring cannot take them.
@@ -187,7 +246,7 @@ __device__ __forceinline__ void ring_put(uint32_t *slot, uint32_t v)
 // before (or the zero the list starts with) never looks valid and nothing has to be cleared.
 __device__ __forceinline__ uint32_t spill_tag(unsigned long long pos, uint32_t cap_log) { return (uint32_t)((pos >> cap_log) + 1ull) & 1u; }
 
-// Hand n sites (stage[0..n), warp-collective) to the other warps of the CTA: the ring, or the spill list when
+// Hand n sites (items[0..n), warp-collective) to the other warps of the CTA: the ring, or the spill list when
 // the ring is full.  The caller has already counted them in sh.pending.
 __device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uint32_t *ring, const uint32_t *items, unsigned int n,
                                           unsigned int c, Tally &tl)
@@ -235,203 +294,320 @@ __device__ __forceinline__ void publish(const TileParams &tp, TShared &sh, unsig
 
 __device__ __forceinline__ void raise_abort(Control *ctl, unsigned int code) { st_relaxed_u32(&ctl->error, code); }
 
-// ------------------------------------------------------------------------------------------ worker warp
-// Expands sites owned by this CTA until the launch is over (A2-A5 on shared memory).
-//
-// One LANE PER BOND: a warp holds up to S = 32 / (2*DIM) sites per pass (8 in 2D, 5 in 3D) and lane (q, k) tests the
-// bond from site q to its neighbour k (k = 2d: +d, k = 2d + 1: -d).  The frontier inside one CTA is a handful of
-// sites wide, so lanes are cheap and the dependent instruction chain of a pass is what an update waits for: per lane
-// one neighbour address, one Philox block (the bond owner's), one LDS, one ATOMS, one ballot for the whole warp.
+// ------------------------------------------------------------------------------------------ bond tables
+// State a warp keeps about the tile it is filling (warp-uniform registers).
+struct Filler {
+    unsigned int active = 0, buf = 0, slot = 0, chunk = 0, v = 0;
+};
+
+// One step of table filling by an idle warp (warp-collective): claim a tile that has no bits for the running update
+// or the next one, or evaluate 32 more sites of the claimed tile.  Returns false when there is nothing to do.
+// A tile is written by the one warp that holds its kBusy claim, so a warp that is called away to expand sites simply
+// continues later; a claim that has become useless (the update is over) is dropped.
 template <int DIM>
-__device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, int8_t *lat, uint32_t *ring, uint32_t *stage,
-                                            unsigned int c, Tally &tl)
+__device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, const Layout &ly, const Tiling<DIM> &tg, Filler &f, Tally &tl)
+{
+    const GrowthParams &p = tp.g;
+    const unsigned int lane = threadIdx.x & 31u;
+    const unsigned int cur = ld_vol(&sh.krel);
+    if (!f.active) {
+        if (ld_vol(&sh.fill_on) == 0u) return false;
+        for (unsigned int t = 0; t < 2u; ++t) {
+            const unsigned int v = cur + t;
+            if ((unsigned long long)v >= p.n_updates) break;
+            const unsigned int buf = v & 1u, tag = v + 1u;
+            for (unsigned int base = 0; base < ly.myslots; base += 32u) {
+                const unsigned int sl = base + lane;
+                const unsigned int st = sl < ly.myslots ? vol(ly.state + buf * tp.slots + sl) : tag;
+                const unsigned int cand = __ballot_sync(kFullMask, st != tag && (st & kBusy) == 0u);
+                if (cand == 0u) continue;
+                const unsigned int pick = (unsigned int)__ffs((int)cand) - 1u;
+                const unsigned int seen = __shfl_sync(kFullMask, st, pick);
+                unsigned int ok = 0;
+                if (lane == 0) ok = atomicCAS(ly.state + buf * tp.slots + base + pick, seen, kBusy | tag) == seen ? 1u : 0u;
+                ok = __shfl_sync(kFullMask, ok, 0);
+                if (ok) { f.active = 1u; f.buf = buf; f.slot = base + pick; f.chunk = 0u; f.v = v; }
+                return true;       // claimed, or lost the race: either way something is going on
+            }
+        }
+        return false;
+    }
+    if (f.v < cur || f.v > cur + 1u) {         // the update these bits were for is over
+        if (lane == 0) st_vol(ly.state + f.buf * tp.slots + f.slot, 0u);
+        f.active = 0u;
+        return true;
+    }
+    const unsigned long long u = p.u0 + (unsigned long long)f.v;
+    const uint32_t w = f.chunk * 32u + lane;
+    const uint32_t gid = vol(ly.origin + f.slot) + tg.spread(w);
+    const uint4 blk = philox4x32_10(gid, kDomainBond, (uint32_t)u, (uint32_t)(u >> 32), p.key0, p.key1);
+    const bool all = tp.thr_all != 0u;
+    const unsigned int b0 = __ballot_sync(kFullMask, all || blk.x < tp.thr32);
+    const unsigned int b1 = __ballot_sync(kFullMask, all || blk.y < tp.thr32);
+    const unsigned int b2 = DIM == 3 ? __ballot_sync(kFullMask, all || blk.z < tp.thr32) : 0u;
+    if (lane < (unsigned int)DIM)
+        ly.bond[(f.buf * DIM + lane) * ly.plane + f.slot * ly.wpt + f.chunk] = lane == 0u ? b0 : (lane == 1u ? b1 : b2);
+    if (lane == 0) ++tl.chunks;
+    if (++f.chunk == ly.wpt) {
+        __syncwarp();
+        if (lane == 0) { __threadfence_block(); st_vol(ly.state + f.buf * tp.slots + f.slot, f.v + 1u); }
+        f.active = 0u;
+    }
+    return true;
+}
+
+// ------------------------------------------------------------------------------------------ worker warp
+// Expands sites owned by this CTA until the launch is over (A2-A5 on shared memory), one lane per bond: a warp
+// holds up to S = 32 / (2*DIM) sites per pass (8 in 2D, 5 in 3D) and lane (q, k) tests the bond from site q to its
+// neighbour k (k = 2d: +d, k = 2d + 1: -d).  Per lane and pass: one neighbour address, one bond bit (table, else one
+// Philox block), one LDS of the neighbour's spin, one ATOMS.  A pass that adds exactly one site -- a path being
+// followed, the common case on the critical chain -- hands it to the next pass with two warp reductions and touches
+// no queue, counter or barrier.
+struct WorkerState {
+    uint32_t a = 0;              // local address of this lane's site
+    unsigned int nsites = 0;     // sites held by the warp (warp-uniform); lanes of group q < nsites work
+    int s0 = 1;
+    uint32_t u_lo = 0, u_hi = 0, krel = 0;
+    unsigned int mywon = 0;      // spins this lane claimed since the warp last ran dry
+    unsigned int sbuf = 0;       // which half of stage[] the next general pass writes
+};
+
+// Passes until the warp holds no site.  POS: the seed spin s0 of the running update is +1 (claim = OR), else -1 (AND).
+template <int DIM, bool POS>
+__device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, const Layout &ly, const Tiling<DIM> &tg, uint32_t *stage,
+                                           unsigned int c, WorkerState &ws, Tally &tl)
+{
+    constexpr unsigned int ND = 2u * DIM, S = 32u / ND;
+    const GrowthParams &p = tp.g;
+    const unsigned int lane = threadIdx.x & 31u;
+    const unsigned int lt = (1u << lane) - 1u;
+    const unsigned int q = lane / ND, k = lane - q * ND, d = k >> 1, sgn = k & 1u;
+    const uint32_t db = d * tg.b;
+    const uint32_t edge = sgn ? 0u : tg.m;                                   // within-tile coordinate at which the neighbour is in the next tile
+    const uint32_t step_in = sgn ? 0u - (1u << db) : (1u << db);             // a -> neighbour in the same tile
+    const uint32_t step_out = sgn ? (tg.m << db) : 0u - (tg.m << db);        // w -> within-tile index in the neighbouring tile
+    const uint32_t sh_d = d * tg.logL, fmask = tg.Lmask << sh_d, delta = sgn ? 0xFFFFFFFFu : 1u;
+    const uint32_t in_mask = tp.in_cap - 1u;
+    unsigned int *const words = reinterpret_cast<unsigned int *>(ly.lat);
+    const uint32_t *const nbr_k = ly.nbrtab + k;
+    const bool tables = tp.tables != 0u;
+    const uint32_t *const bond_d = ly.bond + ((ws.krel & 1u) * DIM + d) * ly.plane;     // plane (krel & 1, d)
+    const uint32_t *const state_b = ly.state + (ws.krel & 1u) * tp.slots;
+    const uint32_t tag = ws.krel + 1u;
+    const unsigned int s0w = POS ? 0x01010101u : 0xFFFFFFFFu;                // the seed spin in every byte
+    const uint32_t cself = c << 16;
+    const uint32_t u_lo = ws.u_lo, u_hi = ws.u_hi, krel = ws.krel;
+    uint32_t a = ws.a;
+    unsigned int nsites = ws.nsites, mywon = ws.mywon, sbuf = ws.sbuf;
+    unsigned long long msg_pos = 0;      // a message whose inbox slot is on its way back from L2
+    uint32_t msg_own = 0, msg_na = 0;
+    bool msg_valid = false;
+
+    do {
+#ifdef WOLFF_PROFILE
+        const long long tp0 = clock64();
+#endif
+        const bool have = q < nsites;        // lanes 30, 31 in 3D: q = S >= nsites
+        // ---- A2: this lane's neighbour: same tile (a +- stride) or across a tile border (table of neighbouring tiles)
+        const uint32_t w = a & tg.ts_mask;
+        const bool inside = ((w >> db) & tg.m) != edge;
+        uint32_t nt = cself;
+        if (have && !inside) nt = vol(nbr_k + (a >> tg.ts_log) * ND);
+        const uint32_t na = inside ? a + step_in : (((nt & 0xFFFFu) << tg.ts_log) | (w + step_out));
+        const uint32_t own = nt >> 16;
+        const bool local = own == c;
+        // ---- A3, table: the bond to the +d neighbour is owned by this site, the bond to the -d neighbour by that neighbour
+        const uint32_t oa = sgn ? na : a;
+        const bool known = have && tables && (sgn == 0u || local);
+        unsigned int st = 0, bw = 0, spw = 0;
+        if (known) { st = vol(state_b + (oa >> tg.ts_log)); bw = vol(bond_d + (oa >> 5)); }     // state first: see fill_step()
+        if (have && local) spw = vol(words + (na >> 2));                                        // gather
+        const unsigned int bytemask = 0xFFu << ((na & 3u) * 8u);
+        const bool tabled = known && st == tag;
+        bool bit = tabled && (bw & (1u << (oa & 31u))) != 0u;
+        // ---- A3, inline: the same Philox block the table would hold
+        const bool need_inline = have && !tabled;
+        if (__any_sync(kFullMask, need_inline)) {
+            if (need_inline) {
+                const uint32_t gs = vol(ly.origin + (a >> tg.ts_log)) + tg.spread(w);
+                const uint32_t gn = (gs & ~fmask) | ((((gs >> sh_d) + delta) & tg.Lmask) << sh_d);
+                const uint4 blk = philox4x32_10(sgn ? gn : gs, kDomainBond, u_lo, u_hi, p.key0, p.key1);
+                const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
+                bit = r < tp.thr32 || tp.thr_all != 0u;
+            }
+            if (lane == 0) ++tl.inline_passes;
+        }
+        const bool cand_l = bit && local && ((spw ^ s0w) & bytemask) == 0u;
+        const bool cand_r = bit && !local;
+
+        // ---- A4 across the territory border: a message to the owner (slot by one L2 atomic, then one 8-byte store).
+        // The store waits for the atomic's round trip, so it is issued one pass later (or before this warp next
+        // accounts for its sites, whichever comes first): a message always leaves before the pass that caused it
+        // can stop being pending.
+        if (__any_sync(kFullMask, cand_r || msg_valid)) {
+            if (msg_valid) {
+                st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
+                               pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
+                msg_valid = false;
+            }
+            if (cand_r) {
+                msg_pos = atomicAdd(tp.gtail + own, 1ull);
+                msg_own = own;
+                msg_na = na;
+                msg_valid = true;
+                ++tl.messages;
+            }
+        }
+        // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
+        unsigned int old = ~s0w;
+        if (cand_l) {
+            old = POS ? atomicOr(words + (na >> 2), 0xFEFEFEFEu & bytemask) : atomicAnd(words + (na >> 2), ~(0xFEFEFEFEu & bytemask));
+            ++tl.attempts;
+        }
+        const bool won = ((old ^ s0w) & bytemask) == 0u;
+        mywon += won ? 1u : 0u;
+        if (lane == 0) ++tl.passes;
+
+        // ---- A5: compact the winners; the first S are this warp's next pass
+        const unsigned int wb = __ballot_sync(kFullMask, won);
+        const unsigned int total = __popc(wb);
+        const unsigned int expanded = nsites;
+        uint32_t *const st_out = stage + sbuf;
+        sbuf ^= 32u;
+        if (won) st_out[__popc(wb & lt)] = na;
+        __syncwarp();
+        if (total != expanded) {
+            // accounting: the new sites are counted before any of them can be seen by another warp; a site stops
+            // being pending only after the messages it caused have left
+            if (total < expanded && __any_sync(kFullMask, msg_valid)) {
+                if (msg_valid) {
+                    st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
+                                   pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
+                    msg_valid = false;
+                }
+                __syncwarp();
+            }
+            if (total == 0u) {
+                // the warp runs dry: its claims become visible to the publisher before its sites stop being pending
+                const unsigned int wsum = __reduce_add_sync(kFullMask, mywon);
+                mywon = 0;
+                if (lane == 0) {
+                    if (wsum) atomicAdd(&sh.claimed, wsum);
+                    __threadfence_block();
+                    const unsigned int before = atomicSub(&sh.pending, expanded);
+                    if (before == expanded) publish(tp, sh, c);
+                }
+            } else if (lane == 0) {
+                atomicAdd(&sh.pending, total - expanded);
+            }
+        }
+        nsites = total < S ? total : S;
+        if (q < nsites) a = st_out[q];
+        if (total > S) hand_over(tp, sh, ly.ring, st_out + S, total - S, c, tl);
+#ifdef WOLFF_PROFILE
+        tl.cyc_pass += (unsigned long long)(clock64() - tp0);
+        tl.lanes += expanded;
+#endif
+    } while (nsites != 0u);
+    ws.a = a; ws.nsites = 0u; ws.mywon = mywon; ws.sbuf = sbuf;
+}
+
+template <int DIM>
+__device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, const Layout &ly, uint32_t *stage, unsigned int c, Tally &tl)
 {
     constexpr unsigned int ND = 2u * DIM, S = 32u / ND;
     const GrowthParams &p = tp.g;
     const Tiling<DIM> tg(tp);
     const unsigned int lane = threadIdx.x & 31u;
-    const unsigned int bit = 1u << lane, lt = bit - 1u;
-    const unsigned int q = lane / ND, k = lane - q * ND, d = k >> 1, sgn = k & 1u;
-    const bool alive = q < S;
-    const uint32_t sh_d = d * tg.logL, fmask = tg.Lmask << sh_d, delta = sgn ? 0xFFFFFFFFu : 1u;
+    const unsigned int q = lane / ND;
     const uint32_t rmask = tp.ring_cap - 1u;
-    const uint32_t tile_sites_log = DIM * tp.tile_log;
-    const uint32_t in_mask = tp.in_cap - 1u;
-    const uint32_t lat_s = (uint32_t)__cvta_generic_to_shared(lat);
-    uint32_t site = 0;
-    unsigned int nsites = 0;     // sites held by the warp (warp-uniform); lanes of group q < nsites work
-    int s0 = 1;
-    unsigned int s0_byte = 1u;
-    uint32_t u_lo = 0, u_hi = 0, krel = 0;
-    unsigned int mywon = 0;      // spins this lane claimed since the warp last ran dry
+    const bool tables = tp.tables != 0u;
+    WorkerState ws;
+    unsigned int idle = 0;
+    Filler fl;
 
     for (;;) {
-        if (nsites == 0u) {
-            // ---- take up to S sites from the ring, else from the spill list
-            unsigned int n = 0, h = 0, from_spill = 0;
-            unsigned long long sh_pos = 0;
-            if (lane == 0) {
-                unsigned int idle = 0;
-                for (;;) {
-                    // one 64-bit load: a consistent (head, tail) pair; the three loads of an idle poll are independent
-                    const unsigned long long ht = ld_vol64(reinterpret_cast<const unsigned long long *>(&sh.head));
-                    sh_pos = ld_vol64(&sh.spill_head);
-                    const unsigned long long st = ld_vol64(&sh.spill_tail);
-                    const unsigned int stop = ld_vol(&sh.stop);
-                    h = (unsigned int)ht;
-                    const unsigned int t = (unsigned int)(ht >> 32);
-                    if (t != h) {
-                        n = t - h < S ? t - h : S;
-                        if (atomicCAS(&sh.head, h, h + n) == h) break;
-                        n = 0;
-                        continue;
-                    }
-                    if (st != sh_pos) {
-                        n = st - sh_pos < (unsigned long long)S ? (unsigned int)(st - sh_pos) : S;
-                        if (atomicCAS(&sh.spill_head, sh_pos, sh_pos + n) == sh_pos) { from_spill = 1; break; }
-                        n = 0;
-                        continue;
-                    }
-                    if (stop) break;
-                    // idle warps share the SM's load/store pipe with the working ones: back off (the warps of a CTA are
-                    // staggered by their idle counts, so one of them polls every few tens of nanoseconds)
-                    ++idle;
-                    if (idle > 2u) __nanosleep(idle < 8u ? 64u : (idle < 16u ? 256u : tp.idle_ns));
-                }
+        // ---- take up to S sites from the ring, else from the spill list; with neither, fill bond tables or sleep
+        unsigned int n = 0, h = 0, from_spill = 0, stop = 0;
+        unsigned long long sh_pos = 0;
+        if (lane == 0) {
+            // one 64-bit load: a consistent (head, tail) pair; the loads of a poll are independent
+            const unsigned long long ht = ld_vol64(reinterpret_cast<const unsigned long long *>(&sh.head));
+            sh_pos = ld_vol64(&sh.spill_head);
+            const unsigned long long st = ld_vol64(&sh.spill_tail);
+            stop = ld_vol(&sh.stop);
+            h = (unsigned int)ht;
+            const unsigned int t = (unsigned int)(ht >> 32);
+            if (t != h) {
+                n = t - h < S ? t - h : S;
+                if (atomicCAS(&sh.head, h, h + n) != h) { n = 0; stop = 0; }
+            } else if (st != sh_pos) {
+                n = st - sh_pos < (unsigned long long)S ? (unsigned int)(st - sh_pos) : S;
+                if (atomicCAS(&sh.spill_head, sh_pos, sh_pos + n) == sh_pos) from_spill = 1; else { n = 0; stop = 0; }
             }
-            n = __shfl_sync(kFullMask, n, 0);
-            h = __shfl_sync(kFullMask, h, 0);
-            from_spill = __shfl_sync(kFullMask, from_spill, 0);
-            sh_pos = __shfl_sync(kFullMask, sh_pos, 0);
-            if (n == 0u) break;                                  // launch over
-            uint32_t ent = 0;
-            if (lane < n) {
-                unsigned int spins = 0;
-                if (!from_spill) {
-                    uint32_t *slot = ring + ((h + lane) & rmask);
-                    do {
-                        ent = atomicExch(slot, kEmpty);          // the producer reserved it; its store is on the way
-                        if (ent == kEmpty && ++spins > (1u << 26)) { raise_abort(p.ctl, 4u); ent = 0u; }
-                    } while (ent == kEmpty);
-                } else {
-                    const unsigned long long pos = sh_pos + (unsigned long long)lane;
-                    const uint32_t *slot = tp.spill + ((size_t)c << tp.spill_log) + ((uint32_t)pos & ((1u << tp.spill_log) - 1u));
-                    const uint32_t tag = spill_tag(pos, tp.spill_log);
-                    uint32_t v;
-                    do {
-                        v = ld_relaxed_u32(slot);
-                        if ((v & 1u) != tag && ++spins > (1u << 24)) { raise_abort(p.ctl, 5u); v = tag; }
-                    } while ((v & 1u) != tag);
-                    ent = v >> 1;
-                }
+        }
+        n = __shfl_sync(kFullMask, n, 0);
+        if (n == 0u) {
+            if (__shfl_sync(kFullMask, stop, 0)) break;                // launch over
+            if (tables && fill_step<DIM>(tp, sh, ly, tg, fl, tl)) { idle = 0; continue; }
+            // idle warps share the SM's issue slots and load/store pipe with the working ones: back off
+            ++idle;
+            if (idle > 2u) __nanosleep(idle < 8u ? 64u : (idle < 16u ? 256u : tp.idle_ns));
+            continue;
+        }
+        idle = 0;
+        h = __shfl_sync(kFullMask, h, 0);
+        from_spill = __shfl_sync(kFullMask, from_spill, 0);
+        sh_pos = __shfl_sync(kFullMask, sh_pos, 0);
+        uint32_t ent = 0;
+        if (lane < n) {
+            unsigned int spins = 0;
+            if (!from_spill) {
+                uint32_t *slot = ly.ring + ((h + lane) & rmask);
+                do {
+                    ent = atomicExch(slot, kEmpty);          // the producer reserved it; its store is on the way
+                    if (ent == kEmpty && ++spins > (1u << 26)) { raise_abort(p.ctl, 4u); ent = 0u; }
+                } while (ent == kEmpty);
+            } else {
+                const unsigned long long pos = sh_pos + (unsigned long long)lane;
+                const uint32_t *slot = tp.spill + ((size_t)c << tp.spill_log) + ((uint32_t)pos & ((1u << tp.spill_log) - 1u));
+                const uint32_t tag = spill_tag(pos, tp.spill_log);
+                uint32_t v;
+                do {
+                    v = ld_relaxed_u32(slot);
+                    if ((v & 1u) != tag && ++spins > (1u << 24)) { raise_abort(p.ctl, 5u); v = tag; }
+                } while ((v & 1u) != tag);
+                ent = v >> 1;
             }
-            site = __shfl_sync(kFullMask, ent, q);
-            nsites = n;
-            // the update these sites belong to (written by the receiver before it fed the ring)
-            s0 = *reinterpret_cast<volatile int *>(&sh.s0);
-            s0_byte = (unsigned int)s0 & 0xFFu;
-            u_lo = ld_vol(&sh.u_lo);
-            u_hi = ld_vol(&sh.u_hi);
-            krel = (uint32_t)((((unsigned long long)u_hi << 32) | u_lo) - p.u0);
         }
-#ifdef WOLFF_PROFILE
-        const long long tp0 = clock64();
-#endif
-        const unsigned int expanded = nsites;
-        const bool have = alive && q < nsites;
-
-        // ---- A2: this lane's neighbour; is it in this CTA's shared memory, and where
-        const uint32_t nid = (site & ~fmask) | ((((site >> sh_d) + delta) & tg.Lmask) << sh_d);
-        uint32_t nx, ny, nz, own, slot;
-        tg.coords(nid, nx, ny, nz);
-        tg.place(tg.tile_of(nx, ny, nz), own, slot);
-        const uint32_t addr = (slot << tile_sites_log) + tg.within(nx, ny, nz);
-        const bool local = own == c;
-        const unsigned int shift = (addr & 3u) * 8u;
-        // gather (LDS), in flight while the Philox rounds execute
-        const uint32_t saddr = lat_s + (addr & ~3u);
-        unsigned int spw = 0;
-        if (have && local) asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(spw) : "r"(saddr));
-        // ---- A3: the bond to the +d neighbour is owned by this site, the bond to the -d neighbour by that neighbour
-        const uint4 blk = philox4x32_10(sgn ? nid : site, kDomainBond, u_lo, u_hi, p.key0, p.key1);
-        const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
-        const bool active = have && (r < tp.thr32 || tp.thr_all != 0u);
-        const bool cand_l = active && local && (((spw >> shift) & 0xFFu) == s0_byte);
-        const bool cand_r = active && !local;
-
-        // ---- A4 across the territory border: a message to the owner (slot by one L2 atomic, then one 8-byte store)
-        const unsigned long long pos = atomg_inc_if(tp.gtail + own, cand_r);
-        // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
-        const unsigned int old = atoms_claim(saddr, 0xFEu << shift, cand_l && s0 > 0, cand_l && s0 < 0);
-        const bool won = cand_l && (((old >> shift) & 0xFFu) == s0_byte);
-        tl.attempts += cand_l ? 1u : 0u;
-        mywon += won ? 1u : 0u;
-        if (lane == 0) ++tl.passes;
-#ifdef WOLFF_PROFILE
-        const long long tp1 = clock64();
-        const bool anyr = __any_sync(kFullMask, cand_r);
-        if (anyr) tl.cyc1r += (unsigned long long)(tp1 - tp0); else { tl.cyc1 += (unsigned long long)(tp1 - tp0); ++tl.n1; }
-#endif
-
-        // ---- A5: compact the winners; the first S are this warp's next pass
-        const unsigned int wb = __ballot_sync(kFullMask, won);
-        const unsigned int total = __popc(wb);
-        if (won) stage[__popc(wb & lt)] = nid;
-        // messages leave before this pass is accounted for
-        if (cand_r) {
-            const unsigned int lap = (unsigned int)(pos >> tp.in_log) & 1u;
-            st_relaxed_u64(tp.inbox + ((size_t)own << tp.in_log) + ((uint32_t)pos & in_mask), pack_msg(kKindClaim, lap, krel, nid, s0));
-            ++tl.messages;
-        }
-        __syncwarp();
-#ifdef WOLFF_PROFILE
-        const long long tp2 = clock64();
-        tl.cyc2 += (unsigned long long)(tp2 - tp1);
-#endif
-        // ---- accounting: the new sites are counted before any of them can be seen by another warp
-        if (total == 0u) {
-            // the warp runs dry: its claims become visible to the publisher before its sites stop being pending
-            const unsigned int w = __reduce_add_sync(kFullMask, mywon);
-            mywon = 0;
-            if (lane == 0) {
-                if (w) atomicAdd(&sh.claimed, w);
-                __threadfence_block();
-                const unsigned int before = atomicSub(&sh.pending, expanded);
-                if (before == expanded) publish(tp, sh, c);
-            }
-        } else if (total != expanded) {
-            if (lane == 0) atomicAdd(&sh.pending, total - expanded);
-        }
-        nsites = total < S ? total : S;
-        if (alive && q < nsites) site = stage[q];
-        if (total > S) hand_over(tp, sh, ring, stage + S, total - S, c, tl);
-        __syncwarp();      // stage[] is rewritten in the next pass
-#ifdef WOLFF_PROFILE
-        const long long tp3 = clock64();
-        tl.cyc_pass += (unsigned long long)(tp3 - tp0);
-        tl.cyc3 += (unsigned long long)(tp3 - tp2);
-        if (total != 0u && total <= S && !anyr) { tl.cyc23c += (unsigned long long)(tp3 - tp1); ++tl.n23c; }
-        tl.lanes += expanded;
-#endif
+        ws.a = __shfl_sync(kFullMask, ent, q);
+        ws.nsites = n;
+        // the update these sites belong to (written by the receiver before it fed the ring)
+        ws.s0 = *reinterpret_cast<volatile int *>(&sh.s0);
+        ws.u_lo = ld_vol(&sh.u_lo);
+        ws.u_hi = ld_vol(&sh.u_hi);
+        ws.krel = ld_vol(&sh.krel);
+        if (ws.s0 > 0) run_passes<DIM, true>(tp, sh, ly, tg, stage, c, ws, tl);
+        else run_passes<DIM, false>(tp, sh, ly, tg, stage, c, ws, tl);
     }
 }
 
 // ------------------------------------------------------------------------------------------ receiver warp
 // Polls the CTA's inbox; makes the claims other CTAs (and the monitor: the seed site, A1) ask for, on its own
-// shared memory; feeds the ring.
+// shared memory; feeds the ring.  A message names the site by its local address in THIS CTA.
 template <int DIM>
-__device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh, int8_t *lat, uint32_t *ring, uint32_t *stage,
-                                              unsigned int c, Tally &tl)
+__device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh, const Layout &ly, uint32_t *stage, unsigned int c, Tally &tl)
 {
     const GrowthParams &p = tp.g;
-    const Tiling<DIM> tg(tp);
     const unsigned int lane = threadIdx.x & 31u;
-    const unsigned int bit = 1u << lane, lt = bit - 1u;
+    const unsigned int lt = (1u << lane) - 1u;
     const uint32_t in_mask = tp.in_cap - 1u;
-    const uint32_t tile_sites_log = DIM * tp.tile_log;
     const unsigned long long *const box = tp.inbox + ((size_t)c << tp.in_log);
     unsigned long long ih = ld_vol64(&sh.ihead);
     unsigned int polls = 0;
+    // adaptive table filling: mean time per update between two updates this CTA hears of
+    unsigned long long last_t = globaltimer_ns();
+    unsigned int last_k = 0;
     for (;;) {
         const unsigned long long pos = ih + (unsigned long long)lane;
         const unsigned long long v = ld_relaxed_u64(box + ((uint32_t)pos & in_mask));
@@ -451,16 +627,12 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
             if (lane == 0) { st_vol64(&sh.ihead, ih); atomicMax(tp.gdone + c, ih); }
             break;
         }
-        const uint32_t site = lo >> 1;
+        const uint32_t addr = lo >> 1;
         int s0 = (lo & 1u) ? -1 : 1;
         bool win = false;
         if (mine) {
-            uint32_t x, y, z, own, slot;
-            tg.coords(site, x, y, z);
-            tg.place(tg.tile_of(x, y, z), own, slot);
-            const uint32_t addr = (slot << tile_sites_log) + tg.within(x, y, z);
-            if (kind == kKindSeed) s0 = (int)*reinterpret_cast<volatile signed char *>(lat + addr);   // A1: the seed spin
-            win = claim_and_flip(lat, addr, s0);
+            if (kind == kKindSeed) s0 = (int)vol(reinterpret_cast<const signed char *>(ly.lat) + addr);   // A1: the seed spin
+            win = claim_and_flip(ly.lat, addr, s0);
             ++tl.attempts;
         }
         const unsigned int wb = __ballot_sync(kFullMask, win);
@@ -473,19 +645,26 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
             *reinterpret_cast<volatile int *>(&sh.s0) = s0u;
             st_vol(&sh.u_lo, (uint32_t)u);
             st_vol(&sh.u_hi, (uint32_t)(u >> 32));
+            st_vol(&sh.krel, krel);
             atomicAdd(&sh.pending, w + 1u);            // the winners, and a token that keeps the CTA busy until they are queued
             if (w) atomicAdd(&sh.claimed, w);
             __threadfence_block();
             st_vol64(&sh.ihead, ih);                   // after pending: see publish()
             __threadfence_block();
         }
-        if (win) stage[__popc(wb & lt)] = site;
+        if (win) stage[__popc(wb & lt)] = addr;
         __syncwarp();
-        if (w) hand_over(tp, sh, ring, stage, w, c, tl);
+        if (w) hand_over(tp, sh, ly.ring, stage, w, c, tl);
         __syncwarp();
         if (lane == 0) {
             const unsigned int before = atomicSub(&sh.pending, 1u);
             if (before == 1u) publish(tp, sh, c);
+            if (tp.fill_mode == 1u && krel != last_k) {
+                const unsigned long long now = globaltimer_ns();
+                st_vol(&sh.fill_on, now - last_t > (unsigned long long)(krel - last_k) * tp.fill_min_ns ? 1u : 0u);
+                last_t = now;
+                last_k = krel;
+            }
         }
     }
     __syncwarp();
@@ -513,12 +692,11 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
             const uint4 xr = philox4x32_10(0u, kDomainSite, (uint32_t)u, (uint32_t)(u >> 32), p.key0, p.key1);
             const unsigned long long rr = (unsigned long long)xr.x | ((unsigned long long)xr.y << 32);
             const uint32_t i0 = (uint32_t)__umul64hi(rr, (unsigned long long)p.geo.N);
-            uint32_t x, y, z, own, slot;
-            tg.coords(i0, x, y, z);
-            tg.place(tg.tile_of(x, y, z), own, slot);
+            uint32_t own, addr;
+            tg.locate(i0, own, addr);
             const unsigned long long pos = atomicAdd(tp.gtail + own, 1ull);
             st_relaxed_u64(tp.inbox + ((size_t)own << tp.in_log) + ((uint32_t)pos & in_mask),
-                           pack_msg(kKindSeed, (unsigned int)(pos >> tp.in_log) & 1u, (unsigned int)k, i0, 1));
+                           pack_msg(kKindSeed, (unsigned int)(pos >> tp.in_log) & 1u, (unsigned int)k, addr, 1));
             ++tl.messages;
         }
         const unsigned long long t0 = globaltimer_ns();
@@ -560,9 +738,7 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
     if (lane == 0) {
         ctl->stats[0] += p.n_updates;
         ctl->stats[1] += flipped;
-#ifndef WOLFF_PROFILE
         ctl->stats[9] += polls_total;
-#endif
     }
 }
 
@@ -596,20 +772,48 @@ __device__ __forceinline__ void copy_tiles(const TileParams &tp, int8_t *lat, un
     }
 }
 
+// Per-slot tables of CTA c: origin of the tile, and (owner, slot) of its 2*DIM neighbouring tiles.
+template <int DIM>
+__device__ __forceinline__ void build_tables(const TileParams &tp, const Layout &ly, unsigned int c)
+{
+    constexpr unsigned int ND = 2u * DIM;
+    const Tiling<DIM> tg(tp);
+    for (uint32_t i = threadIdx.x; i < tp.slots * ND; i += kT) {
+        const uint32_t slot = i / ND, k = i - slot * ND, d = k >> 1;
+        const uint32_t pidx = slot * tp.G + c;
+        uint32_t entry = c << 16;
+        if (pidx < tp.ntiles) {
+            const uint32_t t = (pidx * tp.permAinv) & tg.ntiles_mask;
+            const uint32_t tc = (t >> (d * tg.nt_log)) & tg.nt_mask;
+            const uint32_t tn = (t & ~(tg.nt_mask << (d * tg.nt_log))) | ((((k & 1u) ? tc - 1u : tc + 1u) & tg.nt_mask) << (d * tg.nt_log));
+            uint32_t own, ns;
+            tg.place(tn, own, ns);
+            entry = (own << 16) | ns;
+            if (k == 0u) {
+                uint32_t o = (t & tg.nt_mask) << tg.b;
+                o |= (((t >> tg.nt_log) & tg.nt_mask) << tg.b) << tg.logL;
+                if (DIM == 3) o |= ((t >> (2u * tg.nt_log)) << tg.b) << (2u * tg.logL);
+                ly.origin[slot] = o;
+            }
+        } else if (k == 0u) {
+            ly.origin[slot] = 0u;
+        }
+        ly.nbrtab[i] = entry;
+    }
+    for (uint32_t i = threadIdx.x; i < 2u * tp.slots; i += kT) ly.state[i] = 0u;
+}
+
 template <int DIM>
 __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp)
 {
     extern __shared__ __align__(16) unsigned char smem_t[];
     __shared__ TShared sh;
-    const uint32_t lat_bytes = tp.slots << (DIM * tp.tile_log);
-    int8_t *const lat = reinterpret_cast<int8_t *>(smem_t);
-    uint32_t *const ring = reinterpret_cast<uint32_t *>(smem_t + lat_bytes);
-    uint32_t *const stage_all = ring + tp.ring_cap;
     const unsigned int tid = threadIdx.x, warp = tid >> 5;
     const unsigned int c = blockIdx.x;
+    const Layout ly = Layout::make<DIM>(tp, smem_t, c);
     Tally tl;
 
-    for (unsigned int i = tid; i < tp.ring_cap; i += kT) ring[i] = kEmpty;
+    for (unsigned int i = tid; i < tp.ring_cap; i += kT) ly.ring[i] = kEmpty;
     if (tid == 0) {
         sh.head = sh.tail = 0u;
         sh.pending = sh.claimed = 0u;
@@ -617,19 +821,25 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         sh.pub_lock = 0u;
         sh.s0 = 1;
         sh.u_lo = sh.u_hi = 0u;
+        sh.krel = 0u;
+        sh.fill_on = tp.fill_mode == 0u ? 0u : (tp.fill_mode == 2u ? 1u : tp.gfill[c]);
         sh.ihead = ld_relaxed_u64(tp.gdone + c);          // everything ever sent to this CTA was consumed by the last launch
         sh.spill_head = sh.spill_tail = ld_relaxed_u64(tp.gspill + c);
     }
-    copy_tiles<DIM, true>(tp, lat, c);
+    build_tables<DIM>(tp, ly, c);
+    copy_tiles<DIM, true>(tp, ly.lat, c);
     __syncthreads();
 
-    if (warp == 0u) receiver_warp<DIM>(tp, sh, lat, ring, stage_all, c, tl);
+    if (warp == 0u) receiver_warp<DIM>(tp, sh, ly, ly.stage, c, tl);
     else if (warp == 1u && c == 0u) monitor_warp<DIM>(tp, tl);
-    else worker_warp<DIM>(tp, sh, lat, ring, stage_all + warp * kStage, c, tl);
+    else worker_warp<DIM>(tp, sh, ly, ly.stage + warp * kStage, c, tl);
     __syncthreads();
 
-    copy_tiles<DIM, false>(tp, lat, c);
-    if (tid == 0) tp.gspill[c] = ld_vol64(&sh.spill_tail);
+    copy_tiles<DIM, false>(tp, ly.lat, c);
+    if (tid == 0) {
+        tp.gspill[c] = ld_vol64(&sh.spill_tail);
+        tp.gfill[c] = ld_vol(&sh.fill_on);
+    }
     // tallies
     Control *ctl = tp.g.ctl;
     const unsigned int a = __reduce_add_sync(kFullMask, tl.attempts);
@@ -638,20 +848,15 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
     const unsigned int sp = __reduce_add_sync(kFullMask, tl.spills);
     if ((tid & 31u) == 0u) {
         if (a) atomicAdd(&ctl->stats[7], (unsigned long long)a);
+        if (tl.inline_passes) atomicAdd(&ctl->stats[10], (unsigned long long)tl.inline_passes);
         if (ms) atomicAdd(&ctl->stats[11], (unsigned long long)ms);
         if (rp) atomicAdd(&ctl->stats[12], (unsigned long long)rp);
         if (tl.passes) atomicAdd(&ctl->stats[13], (unsigned long long)tl.passes);
         if (sp) atomicAdd(&ctl->stats[14], (unsigned long long)sp);
+        if (tl.chunks) atomicAdd(&ctl->stats[15], (unsigned long long)tl.chunks);
 #ifdef WOLFF_PROFILE
-        if (tl.cyc_pass) atomicAdd(&ctl->stats[15], tl.cyc_pass);
-        if (tl.lanes) atomicAdd(&ctl->stats[10], tl.lanes);
-        if (tl.cyc1) atomicAdd(&ctl->stats[2], tl.cyc1);
-        if (tl.n1) atomicAdd(&ctl->stats[3], tl.n1);
-        if (tl.cyc1r) atomicAdd(&ctl->stats[4], tl.cyc1r);
-        if (tl.cyc2) atomicAdd(&ctl->stats[5], tl.cyc2);
-        if (tl.cyc3) atomicAdd(&ctl->stats[6], tl.cyc3);
-        if (tl.cyc23c) atomicAdd(&ctl->stats[8], tl.cyc23c);
-        if (tl.n23c) atomicAdd(&ctl->stats[9], tl.n23c);
+        if (tl.cyc_pass) atomicAdd(&ctl->stats[2], tl.cyc_pass);
+        if (tl.lanes) atomicAdd(&ctl->stats[3], tl.lanes);
 #endif
     }
 }
@@ -675,9 +880,15 @@ cudaError_t prepare_one(size_t smem_bytes, int *ctas_per_sm)
 
 }  // namespace
 
-size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap)
+size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, bool tables)
 {
-    return ((size_t)slots << ((uint32_t)dim * tile_log)) + ((size_t)ring_cap + (size_t)kWarps * kStage) * sizeof(uint32_t);
+    const uint32_t ts_log = (uint32_t)dim * tile_log;
+    size_t bytes = (((size_t)slots << ts_log) + 15u) & ~(size_t)15u;                       // lattice
+    size_t words = 0;
+    if (tables) words += 2u * (size_t)dim * slots * ((size_t)1 << (ts_log - 5u));           // bond planes, two buffers
+    words += 2u * (size_t)slots + 2u * (size_t)dim * slots + slots;                         // state, nbrtab, origin
+    words += (size_t)ring_cap + (size_t)kWarps * kStage;                                    // ring, stage
+    return bytes + words * sizeof(uint32_t);
 }
 
 cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm)

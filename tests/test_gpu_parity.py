@@ -18,7 +18,13 @@ MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 3},
          {"mode": 1, "grid_ctas": 3, "cluster_ctas": 1},
          {"mode": 0, "up_threshold": 2, "down_threshold": 1, "cluster_ctas": 4, "balance_min": 0},
          {"mode": 3, "cluster_ctas": 8, "cluster_up_threshold": 100, "grid_down_threshold": 100, "grid_ctas": 16},
-         {"mode": 3, "cluster_ctas": 2, "balance_min": 1000000, "cooperative": 0}]
+         {"mode": 3, "cluster_ctas": 2, "balance_min": 1000000, "cooperative": 0},
+         # shared-memory-resident kernel (mode 0): tiny tiles on few CTAs (every hop crosses a border), a ring so small
+         # that sites spill to global memory, bond tables never / always filled
+         {"mode": 0, "tile_log": 2, "tile_ctas": 3, "fill": 2},
+         {"mode": 0, "tile_log": 3, "ring_cap": 32, "fill": 2, "idle_ns": 0},
+         {"mode": 0, "fill": 0},
+         {"mode": 0, "fill": 2, "tile_ctas": 5, "tile_log": 4}]
 
 
 # ------------------------------------------------------------------ BASELINE config C1, exactly as written
@@ -102,7 +108,7 @@ def test_seeds_and_large_update_index():
 
 
 # ------------------------------------------------------------------ medium sizes: several tiles, ragged tails
-@pytest.mark.parametrize("options", [{"mode": 0}, {"mode": 1}, {"mode": 3}])
+@pytest.mark.parametrize("options", [{"mode": 0}, {"mode": 1}, {"mode": 3}, {"mode": 0, "fill": 2}, {"mode": 0, "fill": 0}])
 @pytest.mark.parametrize("name,n", [("C2", 40), ("C4", 40)])
 def test_medium_configs_equilibrated_variant(name, n, options):
     c = wl.CONFIGS[name]
@@ -119,11 +125,12 @@ def test_medium_configs_literal_random_start(name):
 
 
 # ------------------------------------------------------------------ BASELINE full sizes in the bench's launch configuration
+@pytest.mark.parametrize("options", [{}, {"fill": 2}])
 @pytest.mark.parametrize("name,batches", [("C3", [1, 5]), ("C5a", [1, 8]), ("C5b", [2, 30])])
-def test_full_size_configs_equilibrated_variant(name, batches):
+def test_full_size_configs_equilibrated_variant(name, batches, options):
     # cold start (the bench's 'equilibrated' variant): the first clusters span the lattice, then shrink towards T_c sizes
     c = wl.CONFIGS[name]
-    gpu, ref = make_pair(*c.create_args(), start=wl.cold(c.N))
+    gpu, ref = make_pair(*c.create_args(), start=wl.cold(c.N), options=options)
     compare_batched(gpu, ref, batches)
 
 
