@@ -93,6 +93,20 @@ __device__ __forceinline__ uint32_t selp_u32(uint32_t a, uint32_t b, bool pick_a
     asm("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n selp.u32 %0, %1, %2, p;\n}" : "=r"(r) : "r"(a), "r"(b), "r"((unsigned int)pick_a));
     return r;
 }
+// Shared-memory atomics by ONE lane of a warp, as plain PTX: nvcc would otherwise wrap them in warp aggregation
+// (a vote, a reduction, a prefix scan) that costs more than the atomic.
+__device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void red_shared_add(uint32_t saddr, unsigned int v)
+{
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned int atom_shared_add(uint32_t saddr, unsigned int v)
+{
+    unsigned int old;
+    asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(saddr), "r"(v) : "memory");
+    return old;
+}
+
 // Per-CTA shared state.
 struct alignas(16) TShared {
     unsigned int head, tail;            // ring: entries [head, tail) wait for a worker warp (one aligned 64-bit word)
@@ -183,7 +197,9 @@ struct Tiling {
 // Shared-memory layout of one CTA (offsets follow tiles_smem_bytes()).
 struct Layout {
     int8_t *lat;           // slots * B^dim spins
-    uint32_t *bond;        // [buf 2][d DIM][slot][B^dim / 32] bond bits (only when tp.tables)
+    uint32_t *bond;        // [buf 2][d DIM][slot][B^dim / 32] bond bits (only when tp.tables): bit w of (d, slot) = bond (site w, d)
+    uint32_t *halo;        // [buf 2][d DIM][slot][fw] bits of the bonds that enter the tile through its low-d face: bit i of
+                           // (d, slot) = bond (n, d), n the -d neighbour (another tile's site) of face site i
     uint32_t *state;       // [buf 2][slot]: k + 1 when the tile's bits of update k (relative to the launch) are complete
     uint32_t *nbrtab;      // [slot][2 DIM]: (owner << 16) | slot of the neighbouring tile
     uint32_t *origin;      // [slot]: global id of the tile's first site
@@ -191,6 +207,7 @@ struct Layout {
     uint32_t *stage;       // kWarps * kStage
     uint32_t wpt;          // bond words per tile and plane
     uint32_t plane;        // bond words per plane (slots * wpt)
+    uint32_t fw;           // halo words per tile and direction: max(1, B^(dim-1) / 32)
     uint32_t myslots;      // slots this CTA really owns
 
     template <int DIM>
@@ -210,6 +227,9 @@ struct Layout {
         wpt = tp.tables ? (1u << (ts_log - 5u)) : 0u;
         plane = tp.slots * wpt;
         bond = q;   q += 2u * DIM * plane;
+        const uint32_t face_log = (DIM - 1) * tp.tile_log;
+        fw = tp.tables ? (face_log > 5u ? 1u << (face_log - 5u) : 1u) : 0u;
+        halo = q;   q += 2u * DIM * tp.slots * fw;
         state = q;  q += 2u * tp.slots;
         nbrtab = q; q += 2u * DIM * tp.slots;
         origin = q; q += tp.slots;
@@ -338,17 +358,32 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
         return true;
     }
     const unsigned long long u = p.u0 + (unsigned long long)f.v;
-    const uint32_t w = f.chunk * 32u + lane;
-    const uint32_t gid = vol(ly.origin + f.slot) + tg.spread(w);
-    const uint4 blk = philox4x32_10(gid, kDomainBond, (uint32_t)u, (uint32_t)(u >> 32), p.key0, p.key1);
     const bool all = tp.thr_all != 0u;
-    const unsigned int b0 = __ballot_sync(kFullMask, all || blk.x < tp.thr32);
-    const unsigned int b1 = __ballot_sync(kFullMask, all || blk.y < tp.thr32);
-    const unsigned int b2 = DIM == 3 ? __ballot_sync(kFullMask, all || blk.z < tp.thr32) : 0u;
-    if (lane < (unsigned int)DIM)
-        ly.bond[(f.buf * DIM + lane) * ly.plane + f.slot * ly.wpt + f.chunk] = lane == 0u ? b0 : (lane == 1u ? b1 : b2);
+    if (f.chunk < ly.wpt) {
+        // 32 sites of the tile: all their forward bonds
+        const uint32_t w = f.chunk * 32u + lane;
+        const uint32_t gid = vol(ly.origin + f.slot) + tg.spread(w);
+        const uint4 blk = philox4x32_10(gid, kDomainBond, (uint32_t)u, (uint32_t)(u >> 32), p.key0, p.key1);
+        const unsigned int b0 = __ballot_sync(kFullMask, all || blk.x < tp.thr32);
+        const unsigned int b1 = __ballot_sync(kFullMask, all || blk.y < tp.thr32);
+        const unsigned int b2 = DIM == 3 ? __ballot_sync(kFullMask, all || blk.z < tp.thr32) : 0u;
+        if (lane < (unsigned int)DIM)
+            ly.bond[(f.buf * DIM + lane) * ly.plane + f.slot * ly.wpt + f.chunk] = lane == 0u ? b0 : (lane == 1u ? b1 : b2);
+    } else {
+        // 32 sites of the low-d face: the bond each of them has with its -d neighbour (owned by that neighbour)
+        const uint32_t j = f.chunk - ly.wpt, d = j / ly.fw, i = (j - d * ly.fw) * 32u + lane;
+        const uint32_t db = d * tg.b, sh_d = d * tg.logL;
+        const uint32_t w = (i & ((1u << db) - 1u)) | ((i >> db) << (db + tg.b));          // face site: coordinate d = 0
+        const bool valid = i < (1u << ((DIM - 1) * tg.b));
+        const uint32_t gs = vol(ly.origin + f.slot) + tg.spread(valid ? w : 0u);
+        const uint32_t gn = (gs & ~(tg.Lmask << sh_d)) | ((((gs >> sh_d) - 1u) & tg.Lmask) << sh_d);
+        const uint4 blk = philox4x32_10(gn, kDomainBond, (uint32_t)u, (uint32_t)(u >> 32), p.key0, p.key1);
+        const uint32_t r = d == 0u ? blk.x : (d == 1u ? blk.y : blk.z);
+        const unsigned int bb = __ballot_sync(kFullMask, valid && (all || r < tp.thr32));
+        if (lane == 0) ly.halo[((f.buf * DIM + d) * tp.slots + f.slot) * ly.fw + (j - d * ly.fw)] = bb;
+    }
     if (lane == 0) ++tl.chunks;
-    if (++f.chunk == ly.wpt) {
+    if (++f.chunk == ly.wpt + DIM * ly.fw) {
         __syncwarp();
         if (lane == 0) { __threadfence_block(); st_vol(ly.state + f.buf * tp.slots + f.slot, f.v + 1u); }
         f.active = 0u;
@@ -356,24 +391,42 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
     return true;
 }
 
+// True when every tile of this CTA has its complete bond table of the update with tag `tag` (warp-collective).
+__device__ __forceinline__ bool tables_ready(const TileParams &tp, const Layout &ly, unsigned int buf, unsigned int tag)
+{
+    const unsigned int lane = threadIdx.x & 31u;
+    bool ok = true;
+    for (unsigned int base = 0; base < ly.myslots; base += 32u) {
+        const unsigned int sl = base + lane;
+        if (sl < ly.myslots && vol(ly.state + buf * tp.slots + sl) != tag) ok = false;
+    }
+    return __all_sync(kFullMask, ok);
+}
+
 // ------------------------------------------------------------------------------------------ worker warp
 // Expands sites owned by this CTA until the launch is over (A2-A5 on shared memory), one lane per bond: a warp
 // holds up to S = 32 / (2*DIM) sites per pass (8 in 2D, 5 in 3D) and lane (q, k) tests the bond from site q to its
 // neighbour k (k = 2d: +d, k = 2d + 1: -d).  Per lane and pass: one neighbour address, one bond bit (table, else one
-// Philox block), one LDS of the neighbour's spin, one ATOMS.  A pass that adds exactly one site -- a path being
-// followed, the common case on the critical chain -- hands it to the next pass with two warp reductions and touches
-// no queue, counter or barrier.
+// Philox block), one LDS of the neighbour's spin, one ATOMS; per warp one ballot and one hand-over of the winners
+// through its private stage.  An update waits for the dependent chain of these passes (one per BFS level the CTA
+// takes part in), so the loop is written for instruction count, not for lane utilisation.
+//
+// Accounting (sh.pending): a warp that took n sites from the ring holds n units until it runs dry, whatever its
+// private frontier does in between; only the sites it hands to other warps are added.
 struct WorkerState {
     uint32_t a = 0;              // local address of this lane's site
     unsigned int nsites = 0;     // sites held by the warp (warp-uniform); lanes of group q < nsites work
+    unsigned int units = 0;      // what the warp owes sh.pending when it runs dry
     int s0 = 1;
     uint32_t u_lo = 0, u_hi = 0, krel = 0;
     unsigned int mywon = 0;      // spins this lane claimed since the warp last ran dry
-    unsigned int sbuf = 0;       // which half of stage[] the next general pass writes
+    unsigned int sbuf = 0;       // which half of stage[] the next pass writes
 };
 
-// Passes until the warp holds no site.  POS: the seed spin s0 of the running update is +1 (claim = OR), else -1 (AND).
-template <int DIM, bool POS>
+// Passes until the warp holds no site (READY) or for at most 32 passes (!READY: the caller looks again whether the
+// tables have become complete).  POS: the seed spin s0 of the running update is +1 (claim = OR), else -1 (AND).
+// READY: every tile of this CTA has its bond table of this update, so no state is checked and no Philox runs here.
+template <int DIM, bool POS, bool READY>
 __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, const Layout &ly, const Tiling<DIM> &tg, uint32_t *stage,
                                            unsigned int c, WorkerState &ws, Tally &tl)
 {
@@ -382,68 +435,89 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned int lt = (1u << lane) - 1u;
     const unsigned int q = lane / ND, k = lane - q * ND, d = k >> 1, sgn = k & 1u;
-    const uint32_t db = d * tg.b;
+    const uint32_t db = d * tg.b, lowmask = (1u << db) - 1u;
     const uint32_t edge = sgn ? 0u : tg.m;                                   // within-tile coordinate at which the neighbour is in the next tile
     const uint32_t step_in = sgn ? 0u - (1u << db) : (1u << db);             // a -> neighbour in the same tile
     const uint32_t step_out = sgn ? (tg.m << db) : 0u - (tg.m << db);        // w -> within-tile index in the neighbouring tile
     const uint32_t sh_d = d * tg.logL, fmask = tg.Lmask << sh_d, delta = sgn ? 0xFFFFFFFFu : 1u;
     const uint32_t in_mask = tp.in_cap - 1u;
     unsigned int *const words = reinterpret_cast<unsigned int *>(ly.lat);
+    const uint32_t lat_s = smem_addr(ly.lat), pend_s = smem_addr(&sh.pending), claimed_s = smem_addr(&sh.claimed);
     const uint32_t *const nbr_k = ly.nbrtab + k;
     const bool tables = tp.tables != 0u;
-    const uint32_t *const bond_d = ly.bond + ((ws.krel & 1u) * DIM + d) * ly.plane;     // plane (krel & 1, d)
-    const uint32_t *const state_b = ly.state + (ws.krel & 1u) * tp.slots;
-    const uint32_t tag = ws.krel + 1u;
+    const uint32_t krel = ws.krel, u_lo = ws.u_lo, u_hi = ws.u_hi;
+    const uint32_t *const bond_d = ly.bond + ((krel & 1u) * DIM + d) * ly.plane;             // plane (krel & 1, d)
+    const uint32_t *const halo_d = ly.halo + ((krel & 1u) * DIM + d) * tp.slots * ly.fw;
+    const uint32_t *const state_b = ly.state + (krel & 1u) * tp.slots;
+    const uint32_t tag = krel + 1u;
     const unsigned int s0w = POS ? 0x01010101u : 0xFFFFFFFFu;                // the seed spin in every byte
     const uint32_t cself = c << 16;
-    const uint32_t u_lo = ws.u_lo, u_hi = ws.u_hi, krel = ws.krel;
     uint32_t a = ws.a;
     unsigned int nsites = ws.nsites, mywon = ws.mywon, sbuf = ws.sbuf;
     unsigned long long msg_pos = 0;      // a message whose inbox slot is on its way back from L2
     uint32_t msg_own = 0, msg_na = 0;
     bool msg_valid = false;
+    unsigned int budget = 32u;
 
-    do {
+    for (;;) {
 #ifdef WOLFF_PROFILE
         const long long tp0 = clock64();
+        tl.lanes += nsites;
 #endif
         const bool have = q < nsites;        // lanes 30, 31 in 3D: q = S >= nsites
         // ---- A2: this lane's neighbour: same tile (a +- stride) or across a tile border (table of neighbouring tiles)
-        const uint32_t w = a & tg.ts_mask;
+        const uint32_t w = a & tg.ts_mask, slot = a >> tg.ts_log;
         const bool inside = ((w >> db) & tg.m) != edge;
         uint32_t nt = cself;
-        if (have && !inside) nt = vol(nbr_k + (a >> tg.ts_log) * ND);
+        if (have && !inside) nt = vol(nbr_k + slot * ND);
         const uint32_t na = inside ? a + step_in : (((nt & 0xFFFFu) << tg.ts_log) | (w + step_out));
         const uint32_t own = nt >> 16;
         const bool local = own == c;
-        // ---- A3, table: the bond to the +d neighbour is owned by this site, the bond to the -d neighbour by that neighbour
-        const uint32_t oa = sgn ? na : a;
-        const bool known = have && tables && (sgn == 0u || local);
-        unsigned int st = 0, bw = 0, spw = 0;
-        if (known) { st = vol(state_b + (oa >> tg.ts_log)); bw = vol(bond_d + (oa >> 5)); }     // state first: see fill_step()
-        if (have && local) spw = vol(words + (na >> 2));                                        // gather
+        // ---- A3, table.  The bond to the +d neighbour is owned by this site (bit a of plane d); the bond to the -d
+        // neighbour is owned by that neighbour: bit na of plane d when it is in the same tile, else the halo bit of
+        // this site's place on the tile's low-d face.
+        const bool use_halo = sgn != 0u && !inside;
+        const uint32_t fidx = (w & lowmask) | ((w >> (db + tg.b)) << db);
+        const uint32_t bi = use_halo ? fidx : (sgn ? na : a);
+        const uint32_t *const bptr = use_halo ? halo_d + slot * ly.fw : bond_d;
+        unsigned int st = tag, bw = 0, spw = 0;
+        if (READY) {
+            if (have) bw = vol(bptr + (bi >> 5));
+        } else if (tables) {
+            if (have) { st = vol(state_b + slot); bw = vol(bptr + (bi >> 5)); }      // state first: see fill_step()
+        }
+        if (have && local) spw = vol(words + (na >> 2));                              // gather
         const unsigned int bytemask = 0xFFu << ((na & 3u) * 8u);
-        const bool tabled = known && st == tag;
-        bool bit = tabled && (bw & (1u << (oa & 31u))) != 0u;
-        // ---- A3, inline: the same Philox block the table would hold
-        const bool need_inline = have && !tabled;
-        if (__any_sync(kFullMask, need_inline)) {
-            if (need_inline) {
-                const uint32_t gs = vol(ly.origin + (a >> tg.ts_log)) + tg.spread(w);
-                const uint32_t gn = (gs & ~fmask) | ((((gs >> sh_d) + delta) & tg.Lmask) << sh_d);
-                const uint4 blk = philox4x32_10(sgn ? gn : gs, kDomainBond, u_lo, u_hi, p.key0, p.key1);
-                const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
-                bit = r < tp.thr32 || tp.thr_all != 0u;
+        bool bit = have && (bw & (1u << (bi & 31u))) != 0u;
+        if (!READY) {
+            // ---- A3, inline: the same Philox block the table would hold
+            const bool tabled = tables && st == tag;
+            bit = bit && tabled;
+            const bool need_inline = have && !tabled;
+            if (__any_sync(kFullMask, need_inline)) {
+                if (need_inline) {
+                    const uint32_t gs = vol(ly.origin + slot) + tg.spread(w);
+                    const uint32_t gn = (gs & ~fmask) | ((((gs >> sh_d) + delta) & tg.Lmask) << sh_d);
+                    const uint4 blk = philox4x32_10(sgn ? gn : gs, kDomainBond, u_lo, u_hi, p.key0, p.key1);
+                    const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
+                    bit = r < tp.thr32 || tp.thr_all != 0u;
+                }
+                if (lane == 0) ++tl.inline_passes;
             }
-            if (lane == 0) ++tl.inline_passes;
         }
         const bool cand_l = bit && local && ((spw ^ s0w) & bytemask) == 0u;
         const bool cand_r = bit && !local;
 
+        // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
+        unsigned int old = ~s0w;
+        if (POS) asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.shared.or.b32 %0, [%1], %2;\n}"
+                              : "+r"(old) : "r"(lat_s + (na & ~3u)), "r"(0xFEFEFEFEu & bytemask), "r"((unsigned int)cand_l) : "memory");
+        else     asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.shared.and.b32 %0, [%1], %2;\n}"
+                              : "+r"(old) : "r"(lat_s + (na & ~3u)), "r"(~(0xFEFEFEFEu & bytemask)), "r"((unsigned int)cand_l) : "memory");
+        tl.attempts += cand_l ? 1u : 0u;
         // ---- A4 across the territory border: a message to the owner (slot by one L2 atomic, then one 8-byte store).
-        // The store waits for the atomic's round trip, so it is issued one pass later (or before this warp next
-        // accounts for its sites, whichever comes first): a message always leaves before the pass that caused it
-        // can stop being pending.
+        // The store waits for the atomic's round trip, so it is issued one pass later (or when the warp runs dry):
+        // the slot is counted in gtail -- the atomic has returned -- before the pass that caused it stops being pending.
         if (__any_sync(kFullMask, cand_r || msg_valid)) {
             if (msg_valid) {
                 st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
@@ -458,58 +532,50 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
                 ++tl.messages;
             }
         }
-        // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
-        unsigned int old = ~s0w;
-        if (cand_l) {
-            old = POS ? atomicOr(words + (na >> 2), 0xFEFEFEFEu & bytemask) : atomicAnd(words + (na >> 2), ~(0xFEFEFEFEu & bytemask));
-            ++tl.attempts;
-        }
         const bool won = ((old ^ s0w) & bytemask) == 0u;
         mywon += won ? 1u : 0u;
+#ifdef WOLFF_PROFILE
         if (lane == 0) ++tl.passes;
+#endif
 
-        // ---- A5: compact the winners; the first S are this warp's next pass
+        // ---- A5: compact the winners; the first S are this warp's next pass, the rest goes to the ring
         const unsigned int wb = __ballot_sync(kFullMask, won);
+        if (wb == 0u) break;                                     // the warp runs dry
         const unsigned int total = __popc(wb);
-        const unsigned int expanded = nsites;
         uint32_t *const st_out = stage + sbuf;
         sbuf ^= 32u;
         if (won) st_out[__popc(wb & lt)] = na;
         __syncwarp();
-        if (total != expanded) {
-            // accounting: the new sites are counted before any of them can be seen by another warp; a site stops
-            // being pending only after the messages it caused have left
-            if (total < expanded && __any_sync(kFullMask, msg_valid)) {
-                if (msg_valid) {
-                    st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
-                                   pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
-                    msg_valid = false;
-                }
-                __syncwarp();
-            }
-            if (total == 0u) {
-                // the warp runs dry: its claims become visible to the publisher before its sites stop being pending
-                const unsigned int wsum = __reduce_add_sync(kFullMask, mywon);
-                mywon = 0;
-                if (lane == 0) {
-                    if (wsum) atomicAdd(&sh.claimed, wsum);
-                    __threadfence_block();
-                    const unsigned int before = atomicSub(&sh.pending, expanded);
-                    if (before == expanded) publish(tp, sh, c);
-                }
-            } else if (lane == 0) {
-                atomicAdd(&sh.pending, total - expanded);
-            }
-        }
         nsites = total < S ? total : S;
         if (q < nsites) a = st_out[q];
-        if (total > S) hand_over(tp, sh, ly.ring, st_out + S, total - S, c, tl);
+        if (total > S) {
+            if (lane == 0) red_shared_add(pend_s, total - S);    // counted before another warp can see them
+            hand_over(tp, sh, ly.ring, st_out + S, total - S, c, tl);
+        }
 #ifdef WOLFF_PROFILE
         tl.cyc_pass += (unsigned long long)(clock64() - tp0);
-        tl.lanes += expanded;
 #endif
-    } while (nsites != 0u);
-    ws.a = a; ws.nsites = 0u; ws.mywon = mywon; ws.sbuf = sbuf;
+        if (!READY && --budget == 0u) {
+            // back to the caller: have the tables become complete?  (messages in flight leave first)
+            if (msg_valid)
+                st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
+                               pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
+            ws.a = a; ws.nsites = nsites; ws.mywon = mywon; ws.sbuf = sbuf;
+            return;
+        }
+    }
+    // ---- dry: the messages leave, the claims become visible to the publisher, then the warp's units stop being pending
+    if (msg_valid)
+        st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
+                       pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
+    const unsigned int wsum = __reduce_add_sync(kFullMask, mywon);
+    if (lane == 0) {
+        if (wsum) red_shared_add(claimed_s, wsum);
+        __threadfence_block();
+        const unsigned int before = atom_shared_add(pend_s, 0u - ws.units);
+        if (before == ws.units) publish(tp, sh, c);
+    }
+    ws.a = a; ws.nsites = 0u; ws.mywon = 0u; ws.sbuf = sbuf;
 }
 
 template <int DIM>
@@ -582,13 +648,22 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         }
         ws.a = __shfl_sync(kFullMask, ent, q);
         ws.nsites = n;
+        ws.units = n;
         // the update these sites belong to (written by the receiver before it fed the ring)
         ws.s0 = *reinterpret_cast<volatile int *>(&sh.s0);
         ws.u_lo = ld_vol(&sh.u_lo);
         ws.u_hi = ld_vol(&sh.u_hi);
         ws.krel = ld_vol(&sh.krel);
-        if (ws.s0 > 0) run_passes<DIM, true>(tp, sh, ly, tg, stage, c, ws, tl);
-        else run_passes<DIM, false>(tp, sh, ly, tg, stage, c, ws, tl);
+        while (ws.nsites != 0u) {
+            const bool ready = tables && tables_ready(tp, ly, ws.krel & 1u, ws.krel + 1u);
+            if (ws.s0 > 0) {
+                if (ready) run_passes<DIM, true, true>(tp, sh, ly, tg, stage, c, ws, tl);
+                else run_passes<DIM, true, false>(tp, sh, ly, tg, stage, c, ws, tl);
+            } else {
+                if (ready) run_passes<DIM, false, true>(tp, sh, ly, tg, stage, c, ws, tl);
+                else run_passes<DIM, false, false>(tp, sh, ly, tg, stage, c, ws, tl);
+            }
+        }
     }
 }
 
@@ -885,7 +960,11 @@ size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t rin
     const uint32_t ts_log = (uint32_t)dim * tile_log;
     size_t bytes = (((size_t)slots << ts_log) + 15u) & ~(size_t)15u;                       // lattice
     size_t words = 0;
-    if (tables) words += 2u * (size_t)dim * slots * ((size_t)1 << (ts_log - 5u));           // bond planes, two buffers
+    if (tables) {
+        const uint32_t face_log = (uint32_t)(dim - 1) * tile_log;
+        words += 2u * (size_t)dim * slots * ((size_t)1 << (ts_log - 5u));                   // bond planes, two buffers
+        words += 2u * (size_t)dim * slots * (face_log > 5u ? (size_t)1 << (face_log - 5u) : 1u);   // halo planes
+    }
     words += 2u * (size_t)slots + 2u * (size_t)dim * slots + slots;                         // state, nbrtab, origin
     words += (size_t)ring_cap + (size_t)kWarps * kStage;                                    // ring, stage
     return bytes + words * sizeof(uint32_t);
