@@ -96,6 +96,16 @@ __device__ __forceinline__ uint32_t selp_u32(uint32_t a, uint32_t b, bool pick_a
 // Shared-memory atomics by ONE lane of a warp, as plain PTX: nvcc would otherwise wrap them in warp aggregation
 // (a vote, a reduction, a prefix scan) that costs more than the atomic.
 __device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned int lds_u32(uint32_t saddr)
+{
+    unsigned int v;
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_u32(uint32_t saddr, unsigned int v)
+{
+    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+}
 __device__ __forceinline__ void red_shared_add(uint32_t saddr, unsigned int v)
 {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
@@ -118,6 +128,7 @@ struct alignas(16) TShared {
     uint32_t u_lo, u_hi;                // its index
     unsigned int krel;                  // ... relative to the first update of the launch
     unsigned int fill_on;               // idle warps fill bond tables (adaptive: off when updates are too short to pay for it)
+    unsigned int ready_tag[2];          // k + 1 when EVERY tile of the CTA has its bits of update k in buffer k & 1
     unsigned int pad;
     unsigned long long ihead;           // inbox messages consumed (written by the receiver warp only)
     unsigned long long spill_head, spill_tail;   // running positions in the CTA's global spill list (kept across launches)
@@ -320,6 +331,18 @@ struct Filler {
     unsigned int active = 0, buf = 0, slot = 0, chunk = 0, v = 0;
 };
 
+// True when every tile of this CTA has its complete bond table of the update with tag `tag` (warp-collective).
+__device__ __forceinline__ bool tables_ready(const TileParams &tp, const Layout &ly, unsigned int buf, unsigned int tag)
+{
+    const unsigned int lane = threadIdx.x & 31u;
+    bool ok = true;
+    for (unsigned int base = 0; base < ly.myslots; base += 32u) {
+        const unsigned int sl = base + lane;
+        if (sl < ly.myslots && vol(ly.state + buf * tp.slots + sl) != tag) ok = false;
+    }
+    return __all_sync(kFullMask, ok);
+}
+
 // One step of table filling by an idle warp (warp-collective): claim a tile that has no bits for the running update
 // or the next one, or evaluate 32 more sites of the claimed tile.  Returns false when there is nothing to do.
 // A tile is written by the one warp that holds its kBusy claim, so a warp that is called away to expand sites simply
@@ -387,20 +410,10 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
         __syncwarp();
         if (lane == 0) { __threadfence_block(); st_vol(ly.state + f.buf * tp.slots + f.slot, f.v + 1u); }
         f.active = 0u;
+        __syncwarp();
+        if (tables_ready(tp, ly, f.buf, f.v + 1u) && lane == 0) st_vol(&sh.ready_tag[f.buf], f.v + 1u);
     }
     return true;
-}
-
-// True when every tile of this CTA has its complete bond table of the update with tag `tag` (warp-collective).
-__device__ __forceinline__ bool tables_ready(const TileParams &tp, const Layout &ly, unsigned int buf, unsigned int tag)
-{
-    const unsigned int lane = threadIdx.x & 31u;
-    bool ok = true;
-    for (unsigned int base = 0; base < ly.myslots; base += 32u) {
-        const unsigned int sl = base + lane;
-        if (sl < ly.myslots && vol(ly.state + buf * tp.slots + sl) != tag) ok = false;
-    }
-    return __all_sync(kFullMask, ok);
 }
 
 // ------------------------------------------------------------------------------------------ worker warp
@@ -441,14 +454,15 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     const uint32_t step_out = sgn ? (tg.m << db) : 0u - (tg.m << db);        // w -> within-tile index in the neighbouring tile
     const uint32_t sh_d = d * tg.logL, fmask = tg.Lmask << sh_d, delta = sgn ? 0xFFFFFFFFu : 1u;
     const uint32_t in_mask = tp.in_cap - 1u;
-    unsigned int *const words = reinterpret_cast<unsigned int *>(ly.lat);
+    // shared-window addresses: every shared-memory access of the loop is a plain ld/st/atom.shared on one of these
     const uint32_t lat_s = smem_addr(ly.lat), pend_s = smem_addr(&sh.pending), claimed_s = smem_addr(&sh.claimed);
-    const uint32_t *const nbr_k = ly.nbrtab + k;
+    const uint32_t nbr_s = smem_addr(ly.nbrtab + k), origin_s = smem_addr(ly.origin), stage_s = smem_addr(stage);
     const bool tables = tp.tables != 0u;
     const uint32_t krel = ws.krel, u_lo = ws.u_lo, u_hi = ws.u_hi;
-    const uint32_t *const bond_d = ly.bond + ((krel & 1u) * DIM + d) * ly.plane;             // plane (krel & 1, d)
-    const uint32_t *const halo_d = ly.halo + ((krel & 1u) * DIM + d) * tp.slots * ly.fw;
-    const uint32_t *const state_b = ly.state + (krel & 1u) * tp.slots;
+    const uint32_t bond_s = smem_addr(ly.bond + ((krel & 1u) * DIM + d) * ly.plane);          // plane (krel & 1, d)
+    const uint32_t halo_s = smem_addr(ly.halo + ((krel & 1u) * DIM + d) * tp.slots * ly.fw);
+    const uint32_t state_s = smem_addr(ly.state + (krel & 1u) * tp.slots);
+    const uint32_t fw4 = ly.fw * 4u;
     const uint32_t tag = krel + 1u;
     const unsigned int s0w = POS ? 0x01010101u : 0xFFFFFFFFu;                // the seed spin in every byte
     const uint32_t cself = c << 16;
@@ -469,7 +483,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         const uint32_t w = a & tg.ts_mask, slot = a >> tg.ts_log;
         const bool inside = ((w >> db) & tg.m) != edge;
         uint32_t nt = cself;
-        if (have && !inside) nt = vol(nbr_k + slot * ND);
+        if (have && !inside) nt = lds_u32(nbr_s + slot * (ND * 4u));
         const uint32_t na = inside ? a + step_in : (((nt & 0xFFFFu) << tg.ts_log) | (w + step_out));
         const uint32_t own = nt >> 16;
         const bool local = own == c;
@@ -479,14 +493,14 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         const bool use_halo = sgn != 0u && !inside;
         const uint32_t fidx = (w & lowmask) | ((w >> (db + tg.b)) << db);
         const uint32_t bi = use_halo ? fidx : (sgn ? na : a);
-        const uint32_t *const bptr = use_halo ? halo_d + slot * ly.fw : bond_d;
+        const uint32_t baddr = (use_halo ? halo_s + slot * fw4 : bond_s) + ((bi >> 5) << 2);
         unsigned int st = tag, bw = 0, spw = 0;
         if (READY) {
-            if (have) bw = vol(bptr + (bi >> 5));
+            if (have) bw = lds_u32(baddr);
         } else if (tables) {
-            if (have) { st = vol(state_b + slot); bw = vol(bptr + (bi >> 5)); }      // state first: see fill_step()
+            if (have) { st = lds_u32(state_s + slot * 4u); bw = lds_u32(baddr); }     // state first: see fill_step()
         }
-        if (have && local) spw = vol(words + (na >> 2));                              // gather
+        if (have && local) spw = lds_u32(lat_s + (na & ~3u));                         // gather
         const unsigned int bytemask = 0xFFu << ((na & 3u) * 8u);
         bool bit = have && (bw & (1u << (bi & 31u))) != 0u;
         if (!READY) {
@@ -496,7 +510,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
             const bool need_inline = have && !tabled;
             if (__any_sync(kFullMask, need_inline)) {
                 if (need_inline) {
-                    const uint32_t gs = vol(ly.origin + slot) + tg.spread(w);
+                    const uint32_t gs = lds_u32(origin_s + slot * 4u) + tg.spread(w);
                     const uint32_t gn = (gs & ~fmask) | ((((gs >> sh_d) + delta) & tg.Lmask) << sh_d);
                     const uint4 blk = philox4x32_10(sgn ? gn : gs, kDomainBond, u_lo, u_hi, p.key0, p.key1);
                     const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
@@ -543,11 +557,12 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         if (wb == 0u) break;                                     // the warp runs dry
         const unsigned int total = __popc(wb);
         uint32_t *const st_out = stage + sbuf;
+        const uint32_t out_s = stage_s + sbuf * 4u;
         sbuf ^= 32u;
-        if (won) st_out[__popc(wb & lt)] = na;
+        if (won) sts_u32(out_s + __popc(wb & lt) * 4u, na);
         __syncwarp();
         nsites = total < S ? total : S;
-        if (q < nsites) a = st_out[q];
+        if (q < nsites) a = lds_u32(out_s + q * 4u);
         if (total > S) {
             if (lane == 0) red_shared_add(pend_s, total - S);    // counted before another warp can see them
             hand_over(tp, sh, ly.ring, st_out + S, total - S, c, tl);
@@ -588,6 +603,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
     const unsigned int q = lane / ND;
     const uint32_t rmask = tp.ring_cap - 1u;
     const bool tables = tp.tables != 0u;
+    const bool hot = (threadIdx.x >> 5) == (c == 0u ? 2u : 1u);
     WorkerState ws;
     unsigned int idle = 0;
     Filler fl;
@@ -615,6 +631,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         n = __shfl_sync(kFullMask, n, 0);
         if (n == 0u) {
             if (__shfl_sync(kFullMask, stop, 0)) break;                // launch over
+            if (hot) continue;       // one warp per CTA does nothing but watch the ring: what the receiver hands over starts at once
             if (tables && fill_step<DIM>(tp, sh, ly, tg, fl, tl)) { idle = 0; continue; }
             // idle warps share the SM's issue slots and load/store pipe with the working ones: back off
             ++idle;
@@ -655,7 +672,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         ws.u_hi = ld_vol(&sh.u_hi);
         ws.krel = ld_vol(&sh.krel);
         while (ws.nsites != 0u) {
-            const bool ready = tables && tables_ready(tp, ly, ws.krel & 1u, ws.krel + 1u);
+            const bool ready = tables && ld_vol(&sh.ready_tag[ws.krel & 1u]) == ws.krel + 1u;
             if (ws.s0 > 0) {
                 if (ready) run_passes<DIM, true, true>(tp, sh, ly, tg, stage, c, ws, tl);
                 else run_passes<DIM, true, false>(tp, sh, ly, tg, stage, c, ws, tl);
@@ -897,6 +914,7 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         sh.s0 = 1;
         sh.u_lo = sh.u_hi = 0u;
         sh.krel = 0u;
+        sh.ready_tag[0] = sh.ready_tag[1] = 0u;
         sh.fill_on = tp.fill_mode == 0u ? 0u : (tp.fill_mode == 2u ? 1u : tp.gfill[c]);
         sh.ihead = ld_relaxed_u64(tp.gdone + c);          // everything ever sent to this CTA was consumed by the last launch
         sh.spill_head = sh.spill_tail = ld_relaxed_u64(tp.gspill + c);
