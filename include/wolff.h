@@ -92,11 +92,25 @@ WOLFF_API int wolff_get_state(wolff_handle h, uint64_t *update_index, uint64_t *
 /* Set the update index (to resume a chain: lattice + index + seed is the whole state). */
 WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
 
-/* Tuning / test knobs; never change the result.  The growth kernel runs each BFS level in one of
- * three tiers by frontier width n: one CTA (n <= up), one thread-block cluster (n <= cluster_up), the
- * whole grid (above).  Keys:
- *   "mode"                 0 = auto (default), 1 = every level grid-wide, 2 = one CTA whenever the frontier
- *                          fits its shared-memory queue, 3 = the cluster whenever it fits
+/* Tuning / test knobs; never change the result.  Two growth kernels implement wolff_run:
+ *  - the shared-memory-resident, barrier-free kernel (lattice tiles live in the CTAs' shared memory for the
+ *    launch, claims across CTAs travel as messages, bond variables come from tables filled ahead of time):
+ *    used whenever L is a power of two >= 4 and the lattice fits the chip's shared memory;
+ *  - the level-synchronous kernel, which runs each BFS level in one of three tiers by frontier width n: one
+ *    CTA (n <= up), one thread-block cluster (n <= cluster_up), the whole grid (above): used otherwise.
+ * Keys:
+ *   "mode"                 0 = shared-memory-resident kernel where it applies, else level-synchronous tiers
+ *                          (default); level-synchronous kernel only: 4 = tiers by frontier width, 1 = every level
+ *                          grid-wide, 2 = one CTA whenever the frontier fits its shared-memory queue, 3 = the
+ *                          cluster whenever it fits
+ *   "tile_log"             shared-memory-resident kernel: log2 of the tile side (0 = auto: 6 in 2D, 4 in 3D)
+ *   "tile_ctas"            ... CTAs that share the lattice (0 = one per SM)
+ *   "ring_cap"             ... entries of a CTA's shared-memory work ring (power of two; overflow spills to global memory)
+ *   "fill"                 ... bond tables: 0 = never (Philox inline), 1 = filled by idle warps when updates are long
+ *                          enough to pay for it (default), 2 = always
+ *   "fill_min_us"          ... fill = 1: mean time per update above which tables are filled (default 30)
+ *   "idle_ns"              ... longest sleep of an idle worker warp between two polls of the ring
+ *   "watchdog_ms"          ... an update that takes longer aborts the launch (WOLFF_EINTERNAL at the next call)
  *   "up_threshold"         frontier width above which growth leaves one-CTA mode and wakes the cluster
  *   "down_threshold"       frontier width at or below which cluster growth returns to one CTA
  *   "cluster_up_threshold" frontier width above which growth leaves cluster mode for a grid phase
@@ -113,7 +127,12 @@ WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);
 /* Counters of the most recent wolff_run, for the latency roofline (host pointer, WOLFF_NSTATS values):
  *   [0] updates            [1] flipped spins        [2] one-CTA levels       [3] cluster levels
  *   [4] grid-wide levels   [5] cluster wake-ups     [6] rebalanced cluster levels
- *   [7] claim attempts (atomics)                    [8] widest frontier seen [9] reserved
+ *   [7] claim attempts (atomics)                    [8] widest frontier seen
+ * shared-memory-resident kernel ([2]-[6], [8] stay 0):
+ *   [9] termination polls of the monitor            [10] passes with a Philox block evaluated inline
+ *   [11] messages between CTAs                      [12] sites handed over through the ring
+ *   [13] warp passes (profiling builds)             [14] sites spilled to global memory
+ *   [15] bond-table chunks filled (32 sites each)
  * Blocks until the run has finished. */
 #define WOLFF_NSTATS 16
 WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
