@@ -279,7 +279,7 @@ __device__ __forceinline__ uint32_t spill_tag(unsigned long long pos, uint32_t c
 
 // Hand n sites (items[0..n), warp-collective) to the other warps of the CTA: the ring, or the spill list when
 // the ring is full.  The caller has already counted them in sh.pending.
-__device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uint32_t *ring, const uint32_t *items, unsigned int n,
+__device__ __noinline__ void hand_over(const TileParams &tp, TShared &sh, uint32_t *ring, const uint32_t *items, unsigned int n,
                                           unsigned int c, Tally &tl)
 {
     const unsigned int lane = threadIdx.x & 31u;
@@ -308,7 +308,7 @@ __device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uin
 // nothing being expanded.  ihead is read BEFORE pending is looked at again, and the receiver raises pending before
 // it moves ihead, so pending == 0 here means every message below I is done with all its local progeny.  Publishers
 // of one CTA take turns (pub_lock): the claims of an earlier one reach `added` before a later one moves gdone.
-__device__ __forceinline__ void publish(const TileParams &tp, TShared &sh, unsigned int c)
+__device__ __noinline__ void publish(const TileParams &tp, TShared &sh, unsigned int c)
 {
     while (atomicCAS(&sh.pub_lock, 0u, 1u) != 0u) { }
     const unsigned long long I = ld_vol64(&sh.ihead);
@@ -483,7 +483,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         const uint32_t w = a & tg.ts_mask, slot = a >> tg.ts_log;
         const bool inside = ((w >> db) & tg.m) != edge;
         uint32_t nt = cself;
-        if (have && !inside) nt = lds_u32(nbr_s + slot * (ND * 4u));
+        if (!inside) nt = lds_u32(nbr_s + slot * (ND * 4u));       // lanes without a site hold a stale (valid) address: their loads are harmless
         const uint32_t na = inside ? a + step_in : (((nt & 0xFFFFu) << tg.ts_log) | (w + step_out));
         const uint32_t own = nt >> 16;
         const bool local = own == c;
@@ -496,11 +496,12 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         const uint32_t baddr = (use_halo ? halo_s + slot * fw4 : bond_s) + ((bi >> 5) << 2);
         unsigned int st = tag, bw = 0, spw = 0;
         if (READY) {
-            if (have) bw = lds_u32(baddr);
+            bw = lds_u32(baddr);
         } else if (tables) {
-            if (have) { st = lds_u32(state_s + slot * 4u); bw = lds_u32(baddr); }     // state first: see fill_step()
+            st = lds_u32(state_s + slot * 4u);                                        // state first: see fill_step()
+            bw = lds_u32(baddr);
         }
-        if (have && local) spw = lds_u32(lat_s + (na & ~3u));                         // gather
+        if (local) spw = lds_u32(lat_s + (na & ~3u));                                 // gather
         const unsigned int bytemask = 0xFFu << ((na & 3u) * 8u);
         bool bit = have && (bw & (1u << (bi & 31u))) != 0u;
         if (!READY) {

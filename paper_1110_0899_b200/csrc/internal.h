@@ -97,7 +97,7 @@ struct GrowthLaunch {
 };
 
 constexpr int kGrowthThreads = 512;
-constexpr int kTileThreads = 512;
+constexpr int kTileThreads = 384;
 
 // launchers (defined next to their kernels)
 cudaError_t launch_growth(const GrowthParams &p, int dim, const GrowthLaunch &l, cudaStream_t stream);
