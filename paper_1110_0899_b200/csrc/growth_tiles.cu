@@ -117,6 +117,13 @@ __device__ __forceinline__ unsigned int atom_shared_add(uint32_t saddr, unsigned
     return old;
 }
 
+__device__ __forceinline__ unsigned long long atom_global_inc_u64(unsigned long long *p)
+{
+    unsigned long long old;
+    asm volatile("atom.global.add.u64 %0, [%1], 1;" : "=l"(old) : "l"(p) : "memory");
+    return old;
+}
+
 // Per-CTA shared state.
 struct alignas(16) TShared {
     unsigned int head, tail;            // ring: entries [head, tail) wait for a worker warp (one aligned 64-bit word)
@@ -137,8 +144,6 @@ struct alignas(16) TShared {
 struct Tally {
     unsigned int attempts = 0;          // claim atomics on shared memory (per lane)
     unsigned int messages = 0;          // messages pushed (per lane)
-    unsigned int ring_pushes = 0;       // sites handed to the ring (per lane)
-    unsigned int spills = 0;            // sites spilled to global memory (per lane)
     unsigned int passes = 0;            // warp passes (lane 0)
     unsigned int inline_passes = 0;     // ... of which at least one lane ran Philox inline (lane 0)
     unsigned int chunks = 0;            // bond-table chunks filled: 32 sites each (lane 0)
@@ -280,7 +285,7 @@ __device__ __forceinline__ uint32_t spill_tag(unsigned long long pos, uint32_t c
 // Hand n sites (items[0..n), warp-collective) to the other warps of the CTA: the ring, or the spill list when
 // the ring is full.  The caller has already counted them in sh.pending.
 __device__ __noinline__ void hand_over(const TileParams &tp, TShared &sh, uint32_t *ring, const uint32_t *items, unsigned int n,
-                                          unsigned int c, Tally &tl)
+                                       unsigned int c)
 {
     const unsigned int lane = threadIdx.x & 31u;
     const uint32_t rmask = tp.ring_cap - 1u;
@@ -289,7 +294,8 @@ __device__ __noinline__ void hand_over(const TileParams &tp, TShared &sh, uint32
     ok = __shfl_sync(kFullMask, ok, 0);
     base = __shfl_sync(kFullMask, base, 0);
     if (ok) {
-        for (unsigned int j = lane; j < n; j += 32u) { ring_put(ring + ((base + j) & rmask), items[j]); ++tl.ring_pushes; }
+        for (unsigned int j = lane; j < n; j += 32u) ring_put(ring + ((base + j) & rmask), items[j]);
+        if (lane == 0) atomicAdd(&tp.g.ctl->stats[12], (unsigned long long)n);
     } else {
         unsigned long long sbase = 0;
         if (lane == 0) sbase = atomicAdd(&sh.spill_tail, (unsigned long long)n);
@@ -299,8 +305,8 @@ __device__ __noinline__ void hand_over(const TileParams &tp, TShared &sh, uint32
         for (unsigned int j = lane; j < n; j += 32u) {
             const unsigned long long pos = sbase + (unsigned long long)j;
             st_relaxed_u32(seg + ((uint32_t)pos & smask), (items[j] << 1) | spill_tag(pos, tp.spill_log));
-            ++tl.spills;
         }
+        if (lane == 0) atomicAdd(&tp.g.ctl->stats[14], (unsigned long long)n);
     }
 }
 
@@ -540,7 +546,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
                 msg_valid = false;
             }
             if (cand_r) {
-                msg_pos = atomicAdd(tp.gtail + own, 1ull);
+                msg_pos = atom_global_inc_u64(tp.gtail + own);
                 msg_own = own;
                 msg_na = na;
                 msg_valid = true;
@@ -566,7 +572,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         if (q < nsites) a = lds_u32(out_s + q * 4u);
         if (total > S) {
             if (lane == 0) red_shared_add(pend_s, total - S);    // counted before another warp can see them
-            hand_over(tp, sh, ly.ring, st_out + S, total - S, c, tl);
+            hand_over(tp, sh, ly.ring, st_out + S, total - S, c);
         }
 #ifdef WOLFF_PROFILE
         tl.cyc_pass += (unsigned long long)(clock64() - tp0);
@@ -747,7 +753,7 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
         }
         if (win) stage[__popc(wb & lt)] = addr;
         __syncwarp();
-        if (w) hand_over(tp, sh, ly.ring, stage, w, c, tl);
+        if (w) hand_over(tp, sh, ly.ring, stage, w, c);
         __syncwarp();
         if (lane == 0) {
             const unsigned int before = atomicSub(&sh.pending, 1u);
@@ -938,15 +944,11 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
     Control *ctl = tp.g.ctl;
     const unsigned int a = __reduce_add_sync(kFullMask, tl.attempts);
     const unsigned int ms = __reduce_add_sync(kFullMask, tl.messages);
-    const unsigned int rp = __reduce_add_sync(kFullMask, tl.ring_pushes);
-    const unsigned int sp = __reduce_add_sync(kFullMask, tl.spills);
     if ((tid & 31u) == 0u) {
         if (a) atomicAdd(&ctl->stats[7], (unsigned long long)a);
         if (tl.inline_passes) atomicAdd(&ctl->stats[10], (unsigned long long)tl.inline_passes);
         if (ms) atomicAdd(&ctl->stats[11], (unsigned long long)ms);
-        if (rp) atomicAdd(&ctl->stats[12], (unsigned long long)rp);
         if (tl.passes) atomicAdd(&ctl->stats[13], (unsigned long long)tl.passes);
-        if (sp) atomicAdd(&ctl->stats[14], (unsigned long long)sp);
         if (tl.chunks) atomicAdd(&ctl->stats[15], (unsigned long long)tl.chunks);
 #ifdef WOLFF_PROFILE
         if (tl.cyc_pass) atomicAdd(&ctl->stats[2], tl.cyc_pass);
