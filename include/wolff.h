@@ -103,6 +103,9 @@ WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
  *                          (default); level-synchronous kernel only: 4 = tiers by frontier width, 1 = every level
  *                          grid-wide, 2 = one CTA whenever the frontier fits its shared-memory queue, 3 = the
  *                          cluster whenever it fits
+ *   "small_cluster"        mode 0: when the last finished run (seen at the caller's next synchronising call) had a mean
+ *                          cluster below this size, the next run uses the level-synchronous kernel, whose fixed
+ *                          cost per update is lower (default 16; 0 = never)
  *   "tile_log"             shared-memory-resident kernel: log2 of the tile side (0 = auto: 6 in 2D, 4 in 3D)
  *   "tile_ctas"            ... CTAs that share the lattice (0 = one per SM)
  *   "ring_cap"             ... entries of a CTA's shared-memory work ring (power of two; overflow spills to global memory)

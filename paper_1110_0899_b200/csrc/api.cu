@@ -76,6 +76,10 @@ struct wolff_ctx {
     unsigned long long *tile_ctr = nullptr;     // gtail[G], gdone[G], gspill[G], added
     uint32_t *tile_spill = nullptr;
     uint32_t *tile_fill = nullptr;
+    // kernel choice in mode 0: mean cluster size of the last finished run (read when the caller next synchronises)
+    uint64_t small_cluster = 16;    // below this mean size the level-synchronous kernel runs (its fixed cost per update is lower); 0 = never
+    bool have_mean = false;
+    double mean_cluster = 0.0;
 };
 
 namespace {
@@ -241,13 +245,16 @@ int sync_and_check(wolff_ctx *h)
 {
     CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
     if (h->ran) {
-        unsigned int err = 0;
-        CHECK_CUDA(h, cudaMemcpy(&err, &h->ctl->error, sizeof(err), cudaMemcpyDeviceToHost), "read error flag");
-        if (err != 0) {
-            set_error("device watchdog: a grid barrier did not complete (error flag %u)", err);
+        // error flag and the first two counters (updates, flipped spins) of the last run: 8 + 16 bytes behind one another
+        struct { unsigned int error, pad; unsigned long long updates, flipped; } head;
+        static_assert(offsetof(Control, stats) == offsetof(Control, error) + 8, "Control layout");
+        CHECK_CUDA(h, cudaMemcpy(&head, &h->ctl->error, sizeof(head), cudaMemcpyDeviceToHost), "read error flag");
+        if (head.error != 0) {
+            set_error("device watchdog: a grid barrier did not complete (error flag %u)", head.error);
             h->cuda_failed = true;
             return WOLFF_EINTERNAL;
         }
+        if (head.updates > 0) { h->have_mean = true; h->mean_cluster = (double)head.flipped / (double)head.updates; }
     }
     return WOLFF_OK;
 }
@@ -375,7 +382,8 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
         rc = refresh_plan(h);
         if (rc) return rc;
     }
-    if (h->mode == 0 && h->plan_ok) {
+    const bool small = h->small_cluster > 0 && h->have_mean && h->mean_cluster < (double)h->small_cluster;
+    if (h->mode == 0 && h->plan_ok && !small) {
         // shared-memory-resident kernel; a message carries the update index relative to the launch in 29 bits
         const uint64_t chunk = (1ull << 29) - 1;
         for (uint64_t done = 0; done < n_updates; done += chunk) {
@@ -452,6 +460,7 @@ int wolff_set_spins(wolff_handle h, const int8_t *src)
     CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     if (invalid) { set_error("set_spins: every byte must be +1 or -1"); return WOLFF_EINVAL; }
     CHECK_CUDA(h, cudaMemcpyAsync(h->spins, staging, (size_t)h->N, cudaMemcpyDeviceToDevice, s), "commit lattice");
+    h->have_mean = false;           // a new lattice: nothing is known about its clusters
     CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     return WOLFF_OK;
 }
@@ -490,6 +499,9 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
         if (value < 1 || value > 3600000) { set_error("watchdog_ms must be in [1, 3600000]"); return WOLFF_EINVAL; }
         h->watchdog_ms = (uint64_t)value;
         h->plan_dirty = true;
+    } else if (!strcmp(key, "small_cluster")) {
+        if (value < 0 || value > (int64_t)0x7FFFFFFF) { set_error("small_cluster must be in [0, 2^31)"); return WOLFF_EINVAL; }
+        h->small_cluster = (uint64_t)value;
     } else if (!strcmp(key, "fill")) {
         if (value < 0 || value > 2) { set_error("fill must be 0 (never), 1 (adaptive) or 2 (always)"); return WOLFF_EINVAL; }
         h->fill_mode = (int)value;

@@ -21,10 +21,11 @@ MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 3},
          {"mode": 3, "cluster_ctas": 2, "balance_min": 1000000, "cooperative": 0},
          # shared-memory-resident kernel (mode 0): tiny tiles on few CTAs (every hop crosses a border), a ring so small
          # that sites spill to global memory, bond tables never / always filled
-         {"mode": 0, "tile_log": 2, "tile_ctas": 3, "fill": 2},
-         {"mode": 0, "tile_log": 3, "ring_cap": 32, "fill": 2, "idle_ns": 0},
-         {"mode": 0, "fill": 0},
-         {"mode": 0, "fill": 2, "tile_ctas": 5, "tile_log": 4}]
+         {"mode": 0, "tile_log": 2, "tile_ctas": 3, "fill": 2, "small_cluster": 0},
+         {"mode": 0, "tile_log": 3, "ring_cap": 32, "fill": 2, "idle_ns": 0, "small_cluster": 0},
+         {"mode": 0, "fill": 0, "small_cluster": 0},
+         {"mode": 0, "fill": 2, "tile_ctas": 5, "tile_log": 4, "small_cluster": 0},
+         {"mode": 0, "small_cluster": 1000000}]
 
 
 # ------------------------------------------------------------------ BASELINE config C1, exactly as written
