@@ -99,12 +99,12 @@ __device__ __forceinline__ uint32_t smem_addr(const void *p) { return (uint32_t)
 __device__ __forceinline__ unsigned int lds_u32(uint32_t saddr)
 {
     unsigned int v;
-    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
     return v;
 }
 __device__ __forceinline__ void sts_u32(uint32_t saddr, unsigned int v)
 {
-    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
 }
 __device__ __forceinline__ void red_shared_add(uint32_t saddr, unsigned int v)
 {
@@ -479,7 +479,8 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     bool msg_valid = false;
     unsigned int budget = 32u;
 
-    for (;;) {
+    // one pass; 0: go on, 1: the warp ran dry, 2: back to the caller (!READY only)
+    auto pass = [&]() -> int {
 #ifdef WOLFF_PROFILE
         const long long tp0 = clock64();
         tl.lanes += nsites;
@@ -561,7 +562,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
 
         // ---- A5: compact the winners; the first S are this warp's next pass, the rest goes to the ring
         const unsigned int wb = __ballot_sync(kFullMask, won);
-        if (wb == 0u) break;                                     // the warp runs dry
+        if (wb == 0u) return 1;                                  // the warp runs dry
         const unsigned int total = __popc(wb);
         uint32_t *const st_out = stage + sbuf;
         const uint32_t out_s = stage_s + sbuf * 4u;
@@ -583,9 +584,19 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
                 st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
                                pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
             ws.a = a; ws.nsites = nsites; ws.mywon = mywon; ws.sbuf = sbuf;
-            return;
+            return 2;
         }
+        return 0;
+    };
+    // two passes per trip: the loop-back (and the YIELD ptxas puts at the head of such loops) costs about 50 cycles
+    int status;
+    for (;;) {
+        status = pass();
+        if (status != 0) break;
+        status = pass();
+        if (status != 0) break;
     }
+    if (status == 2) return;
     // ---- dry: the messages leave, the claims become visible to the publisher, then the warp's units stop being pending
     if (msg_valid)
         st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
