@@ -65,6 +65,7 @@ struct wolff_ctx {
     uint32_t ring_cap = 2048;
     int fill_mode = 1;              // bond tables: 0 off, 1 adaptive, 2 always
     uint64_t fill_min_us = 30;
+    int fill_bufs = 0;              // 0 = two buffers when they fit, else one; 1 = one
     uint64_t watchdog_ms = 20000;
     uint32_t idle_ns = 1000;
     size_t smem_optin = 0;          // shared memory one CTA may use
@@ -183,10 +184,11 @@ int refresh_plan(wolff_ctx *h)
     const uint32_t slots = (uint32_t)((ntiles + G - 1) / G);
     if (slots > 0xFFFFu || G > 0xFFFFu) return WOLFF_OK;
     // bond tables (growth_tiles.cu) when they fit beside the lattice; a tile must hold at least one 32-bit word of bonds
-    bool tables = h->fill_mode != 0 && dim * b >= 5u;
-    size_t smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap, tables);
-    if (tables && smem + 256 > h->smem_optin) { tables = false; smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap, false); }
+    uint32_t nbuf = (h->fill_mode != 0 && dim * b >= 5u) ? (h->fill_bufs == 1 ? 1u : 2u) : 0u;
+    size_t smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap, nbuf);
+    while (nbuf > 0 && smem + 256 > h->smem_optin) { --nbuf; smem = tiles_smem_bytes(h->dim, b, slots, h->ring_cap, nbuf); }
     if (smem + 256 > h->smem_optin) return WOLFF_OK;
+    const bool tables = nbuf != 0;
     int per_sm = 0;
     cudaError_t e = tiles_prepare(h->dim, smem, &per_sm);
     if (e != cudaSuccess || per_sm < 1) { cudaGetLastError(); return WOLFF_OK; }
@@ -211,6 +213,7 @@ int refresh_plan(wolff_ctx *h)
     tp.watchdog_ns = h->watchdog_ms * 1000000ull;
     tp.idle_ns = h->idle_ns;
     tp.tables = tables ? 1u : 0u;
+    tp.nbuf = nbuf;
     tp.fill_mode = tables ? (uint32_t)h->fill_mode : 0u;
     tp.fill_min_ns = h->fill_min_us * 1000ull;
     tp.thr32 = (uint32_t)h->thr;
@@ -505,6 +508,10 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
     } else if (!strcmp(key, "fill")) {
         if (value < 0 || value > 2) { set_error("fill must be 0 (never), 1 (adaptive) or 2 (always)"); return WOLFF_EINVAL; }
         h->fill_mode = (int)value;
+        h->plan_dirty = true;
+    } else if (!strcmp(key, "fill_bufs")) {
+        if (value < 0 || value > 2) { set_error("fill_bufs must be 0 (auto), 1 or 2"); return WOLFF_EINVAL; }
+        h->fill_bufs = (int)value;
         h->plan_dirty = true;
     } else if (!strcmp(key, "fill_min_us")) {
         if (value < 0 || value > 1000000) { set_error("fill_min_us must be in [0, 1000000]"); return WOLFF_EINVAL; }

@@ -135,6 +135,7 @@ struct alignas(16) TShared {
     uint32_t u_lo, u_hi;                // its index
     unsigned int krel;                  // ... relative to the first update of the launch
     unsigned int fill_on;               // idle warps fill bond tables (adaptive: off when updates are too short to pay for it)
+    unsigned int watcher;               // 1 while some idle worker warp holds the watch (polls the ring without backing off)
     unsigned int ready_tag[2];          // k + 1 when EVERY tile of the CTA has its bits of update k in buffer k & 1
     unsigned int pad;
     unsigned long long ihead;           // inbox messages consumed (written by the receiver warp only)
@@ -242,10 +243,10 @@ struct Layout {
         uint32_t *q = reinterpret_cast<uint32_t *>(base + lat_bytes);
         wpt = tp.tables ? (1u << (ts_log - 5u)) : 0u;
         plane = tp.slots * wpt;
-        bond = q;   q += 2u * DIM * plane;
+        bond = q;   q += tp.nbuf * DIM * plane;
         const uint32_t face_log = (DIM - 1) * tp.tile_log;
         fw = tp.tables ? (face_log > 5u ? 1u << (face_log - 5u) : 1u) : 0u;
-        halo = q;   q += 2u * DIM * tp.slots * fw;
+        halo = q;   q += tp.nbuf * DIM * tp.slots * fw;
         state = q;  q += 2u * tp.slots;
         nbrtab = q; q += 2u * DIM * tp.slots;
         origin = q; q += tp.slots;
@@ -361,10 +362,10 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
     const unsigned int cur = ld_vol(&sh.krel);
     if (!f.active) {
         if (ld_vol(&sh.fill_on) == 0u) return false;
-        for (unsigned int t = 0; t < 2u; ++t) {
+        for (unsigned int t = 0; t < tp.nbuf; ++t) {
             const unsigned int v = cur + t;
             if ((unsigned long long)v >= p.n_updates) break;
-            const unsigned int buf = v & 1u, tag = v + 1u;
+            const unsigned int buf = v & (tp.nbuf - 1u), tag = v + 1u;
             for (unsigned int base = 0; base < ly.myslots; base += 32u) {
                 const unsigned int sl = base + lane;
                 const unsigned int st = sl < ly.myslots ? vol(ly.state + buf * tp.slots + sl) : tag;
@@ -381,7 +382,7 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
         }
         return false;
     }
-    if (f.v < cur || f.v > cur + 1u) {         // the update these bits were for is over
+    if (f.v < cur || f.v >= cur + tp.nbuf) {   // the update these bits were for is over
         if (lane == 0) st_vol(ly.state + f.buf * tp.slots + f.slot, 0u);
         f.active = 0u;
         return true;
@@ -465,9 +466,9 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     const uint32_t nbr_s = smem_addr(ly.nbrtab + k), origin_s = smem_addr(ly.origin), stage_s = smem_addr(stage);
     const bool tables = tp.tables != 0u;
     const uint32_t krel = ws.krel, u_lo = ws.u_lo, u_hi = ws.u_hi;
-    const uint32_t bond_s = smem_addr(ly.bond + ((krel & 1u) * DIM + d) * ly.plane);          // plane (krel & 1, d)
-    const uint32_t halo_s = smem_addr(ly.halo + ((krel & 1u) * DIM + d) * tp.slots * ly.fw);
-    const uint32_t state_s = smem_addr(ly.state + (krel & 1u) * tp.slots);
+    const uint32_t bond_s = smem_addr(ly.bond + ((krel & (tp.nbuf - 1u)) * DIM + d) * ly.plane);    // plane (buffer of krel, d)
+    const uint32_t halo_s = smem_addr(ly.halo + ((krel & (tp.nbuf - 1u)) * DIM + d) * tp.slots * ly.fw);
+    const uint32_t state_s = smem_addr(ly.state + (krel & (tp.nbuf - 1u)) * tp.slots);
     const uint32_t fw4 = ly.fw * 4u;
     const uint32_t tag = krel + 1u;
     const unsigned int s0w = POS ? 0x01010101u : 0xFFFFFFFFu;                // the seed spin in every byte
@@ -621,7 +622,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
     const unsigned int q = lane / ND;
     const uint32_t rmask = tp.ring_cap - 1u;
     const bool tables = tp.tables != 0u;
-    const bool hot = (threadIdx.x >> 5) == (c == 0u ? 2u : 1u);
+    bool watcher = false;        // this warp holds the CTA's watch: it polls the ring without sleeping or filling
     WorkerState ws;
     unsigned int idle = 0;
     Filler fl;
@@ -649,7 +650,14 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         n = __shfl_sync(kFullMask, n, 0);
         if (n == 0u) {
             if (__shfl_sync(kFullMask, stop, 0)) break;                // launch over
-            if (hot) continue;       // one warp per CTA does nothing but watch the ring: what the receiver hands over starts at once
+            // one idle warp per CTA holds the watch: it does nothing but poll the ring, so what the receiver (or a warp
+            // with more winners than it can keep) hands over starts at once; the watch passes on when its holder finds work
+            if (!watcher) {
+                unsigned int got = 0;
+                if (lane == 0) got = atomicCAS(&sh.watcher, 0u, 1u) == 0u ? 1u : 0u;
+                watcher = __shfl_sync(kFullMask, got, 0) != 0u;
+            }
+            if (watcher) continue;
             if (tables && fill_step<DIM>(tp, sh, ly, tg, fl, tl)) { idle = 0; continue; }
             // idle warps share the SM's issue slots and load/store pipe with the working ones: back off
             ++idle;
@@ -657,6 +665,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
             continue;
         }
         idle = 0;
+        if (watcher) { watcher = false; if (lane == 0) st_vol(&sh.watcher, 0u); }
         h = __shfl_sync(kFullMask, h, 0);
         from_spill = __shfl_sync(kFullMask, from_spill, 0);
         sh_pos = __shfl_sync(kFullMask, sh_pos, 0);
@@ -690,7 +699,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         ws.u_hi = ld_vol(&sh.u_hi);
         ws.krel = ld_vol(&sh.krel);
         while (ws.nsites != 0u) {
-            const bool ready = tables && ld_vol(&sh.ready_tag[ws.krel & 1u]) == ws.krel + 1u;
+            const bool ready = tables && ld_vol(&sh.ready_tag[ws.krel & (tp.nbuf - 1u)]) == ws.krel + 1u;
             if (ws.s0 > 0) {
                 if (ready) run_passes<DIM, true, true>(tp, sh, ly, tg, stage, c, ws, tl);
                 else run_passes<DIM, true, false>(tp, sh, ly, tg, stage, c, ws, tl);
@@ -933,6 +942,7 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         sh.u_lo = sh.u_hi = 0u;
         sh.krel = 0u;
         sh.ready_tag[0] = sh.ready_tag[1] = 0u;
+        sh.watcher = 0u;
         sh.fill_on = tp.fill_mode == 0u ? 0u : (tp.fill_mode == 2u ? 1u : tp.gfill[c]);
         sh.ihead = ld_relaxed_u64(tp.gdone + c);          // everything ever sent to this CTA was consumed by the last launch
         sh.spill_head = sh.spill_tail = ld_relaxed_u64(tp.gspill + c);
@@ -987,15 +997,15 @@ cudaError_t prepare_one(size_t smem_bytes, int *ctas_per_sm)
 
 }  // namespace
 
-size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, bool tables)
+size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, uint32_t nbuf)
 {
     const uint32_t ts_log = (uint32_t)dim * tile_log;
     size_t bytes = (((size_t)slots << ts_log) + 15u) & ~(size_t)15u;                       // lattice
     size_t words = 0;
-    if (tables) {
+    if (nbuf) {
         const uint32_t face_log = (uint32_t)(dim - 1) * tile_log;
-        words += 2u * (size_t)dim * slots * ((size_t)1 << (ts_log - 5u));                   // bond planes, two buffers
-        words += 2u * (size_t)dim * slots * (face_log > 5u ? (size_t)1 << (face_log - 5u) : 1u);   // halo planes
+        words += (size_t)nbuf * dim * slots * ((size_t)1 << (ts_log - 5u));                  // bond planes
+        words += (size_t)nbuf * dim * slots * (face_log > 5u ? (size_t)1 << (face_log - 5u) : 1u);   // halo planes
     }
     words += 2u * (size_t)slots + 2u * (size_t)dim * slots + slots;                         // state, nbrtab, origin
     words += (size_t)ring_cap + (size_t)kWarps * kStage;                                    // ring, stage

@@ -79,7 +79,8 @@ struct TileParams {
     uint32_t spill_log;              // spill entries per CTA (at least the sites the CTA owns)
     uint32_t ring_cap;               // entries of the shared-memory ring (power of two)
     unsigned long long watchdog_ns;  // an update longer than this aborts the launch
-    uint32_t tables;                 // 1: bond tables (two buffers of dim bit planes per tile) are part of the shared-memory layout
+    uint32_t tables;                 // 1: bond tables (nbuf buffers of dim bit planes per tile) are part of the shared-memory layout
+    uint32_t nbuf;                   // 2: the tables of the running update and the next one; 1: the running update only (0 without tables)
     uint32_t fill_mode;              // idle warps fill bond tables: 0 never, 1 when updates are long enough to pay for it, 2 always
     unsigned long long fill_min_ns;  // fill_mode 1: mean time per update above which tables are filled
     uint32_t *gfill;                 // [G] fill_on of CTA c at the end of the last launch
@@ -104,7 +105,7 @@ cudaError_t launch_growth(const GrowthParams &p, int dim, const GrowthLaunch &l,
 // sets the kernel's attributes for this launch shape and reports how many clusters can be co-resident
 cudaError_t growth_max_clusters(int dim, bool pow2, const GrowthLaunch &l, int *max_clusters);
 // shared-memory-resident kernel: shared memory needed, attributes + co-resident CTAs per SM, cooperative launch of tp.G CTAs
-size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, bool tables);
+size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, uint32_t nbuf);
 cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm);
 cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, cudaStream_t stream);
