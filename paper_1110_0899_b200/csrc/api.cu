@@ -80,6 +80,7 @@ struct wolff_ctx {
     // kernel choice in mode 0: mean cluster size of the last finished run (read when the caller next synchronises)
     uint64_t small_cluster = 16;    // below this mean size the level-synchronous kernel runs (its fixed cost per update is lower); 0 = never
     bool have_mean = false;
+    bool run_since_set = false;     // a run has been queued since the lattice was last loaded: its counters describe this lattice
     double mean_cluster = 0.0;
 };
 
@@ -257,7 +258,7 @@ int sync_and_check(wolff_ctx *h)
             h->cuda_failed = true;
             return WOLFF_EINTERNAL;
         }
-        if (head.updates > 0) { h->have_mean = true; h->mean_cluster = (double)head.flipped / (double)head.updates; }
+        if (head.updates > 0 && h->run_since_set) { h->have_mean = true; h->mean_cluster = (double)head.flipped / (double)head.updates; }
     }
     return WOLFF_OK;
 }
@@ -411,6 +412,7 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     h->last_n = n_updates;
     h->last_stream = stream;
     h->ran = true;
+    h->run_since_set = true;
     return WOLFF_OK;
 }
 
@@ -418,18 +420,52 @@ int wolff_observables(wolff_handle h, int64_t *E, int64_t *M, uint32_t *cluster_
 {
     int rc = check_handle(h);
     if (rc) return rc;
-    rc = sync_and_check(h);
-    if (rc) return rc;
     cudaStream_t s = h->last_stream;
-    if (E || M) {
-        CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, h->num_sms, s), "launch E/M reduction");
-        if (E) CHECK_CUDA(h, cudaMemcpyAsync(E, &h->ctl->E, sizeof(int64_t), cudaMemcpyDefault, s), "copy E");
-        if (M) CHECK_CUDA(h, cudaMemcpyAsync(M, &h->ctl->M, sizeof(int64_t), cudaMemcpyDefault, s), "copy M");
-    }
+    // Everything is queued behind the last run on its stream; ONE small device-to-host copy then brings the error
+    // flag, the run's first counters and E, M (they sit within 296 bytes of the control block), and one
+    // synchronise ends the call.
+    if (E || M) CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, h->num_sms, s), "launch E/M reduction");
     if (cluster_sizes && h->last_n > 0)
         CHECK_CUDA(h, cudaMemcpyAsync(cluster_sizes, h->sizes, (size_t)h->last_n * sizeof(uint32_t), cudaMemcpyDefault, s),
                    "copy cluster sizes");
+    constexpr size_t span = offsetof(Control, M) + sizeof(long long) - offsetof(Control, error);
+    unsigned char head[span];
+    CHECK_CUDA(h, cudaMemcpyAsync(head, &h->ctl->error, span, cudaMemcpyDeviceToHost, s), "read control block");
     CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    unsigned int err = 0;
+    unsigned long long updates = 0, flipped = 0;
+    long long Ev = 0, Mv = 0;
+    memcpy(&err, head, sizeof(err));
+    memcpy(&updates, head + (offsetof(Control, stats) - offsetof(Control, error)), sizeof(updates));
+    memcpy(&flipped, head + (offsetof(Control, stats) - offsetof(Control, error)) + 8, sizeof(flipped));
+    memcpy(&Ev, head + (offsetof(Control, E) - offsetof(Control, error)), sizeof(Ev));
+    memcpy(&Mv, head + (offsetof(Control, M) - offsetof(Control, error)), sizeof(Mv));
+    if (h->ran) {
+        if (err != 0) {
+            set_error("device watchdog: an update or a grid barrier did not complete (error flag %u)", err);
+            h->cuda_failed = true;
+            return WOLFF_EINTERNAL;
+        }
+        if (updates > 0 && h->run_since_set) { h->have_mean = true; h->mean_cluster = (double)flipped / (double)updates; }
+    }
+    // E and M go to host or device memory, whichever the caller passed
+    int64_t *const dst[2] = {E, M};
+    const long long val[2] = {Ev, Mv};
+    const long long *const src[2] = {&h->ctl->E, &h->ctl->M};
+    bool queued = false;
+    for (int k = 0; k < 2; ++k) {
+        if (!dst[k]) continue;
+        cudaPointerAttributes attr{};
+        const cudaError_t e = cudaPointerGetAttributes(&attr, dst[k]);
+        if (e != cudaSuccess) cudaGetLastError();
+        if (e == cudaSuccess && (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged)) {
+            CHECK_CUDA(h, cudaMemcpyAsync(dst[k], src[k], sizeof(int64_t), cudaMemcpyDeviceToDevice, s), "copy E/M");
+            queued = true;
+        } else {
+            *dst[k] = (int64_t)val[k];
+        }
+    }
+    if (queued) CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     return WOLFF_OK;
 }
 
@@ -464,6 +500,7 @@ int wolff_set_spins(wolff_handle h, const int8_t *src)
     if (invalid) { set_error("set_spins: every byte must be +1 or -1"); return WOLFF_EINVAL; }
     CHECK_CUDA(h, cudaMemcpyAsync(h->spins, staging, (size_t)h->N, cudaMemcpyDeviceToDevice, s), "commit lattice");
     h->have_mean = false;           // a new lattice: nothing is known about its clusters
+    h->run_since_set = false;
     CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     return WOLFF_OK;
 }

@@ -863,32 +863,40 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
 
 // ------------------------------------------------------------------------------------------ the kernel
 // Copy the tiles of CTA c between the global lattice and shared memory, one 32-bit word (4 sites along x) at a time.
-template <int DIM, bool LOAD>
-__device__ __forceinline__ void copy_tiles(const TileParams &tp, int8_t *lat, unsigned int c)
+template <int DIM, bool LOAD, typename V>
+__device__ __forceinline__ void copy_tiles_vec(const TileParams &tp, const Layout &ly)
 {
-    const uint32_t b = tp.tile_log, m = (1u << b) - 1u;
-    const uint32_t nt_log = tp.g.geo.logL - b, nt_mask = (1u << nt_log) - 1u;
-    const uint32_t ts_log = DIM * b;
-    const uint32_t words_per_tile = 1u << (ts_log - 2u);
-    const uint32_t logL = tp.g.geo.logL;
-    unsigned int *const glob = reinterpret_cast<unsigned int *>(tp.g.spins);
-    unsigned int *const loc = reinterpret_cast<unsigned int *>(lat);
-    for (uint32_t slot = 0; slot < tp.slots; ++slot) {
-        const uint32_t pidx = slot * tp.G + c;
-        if (pidx >= tp.ntiles) break;
-        const uint32_t t = (pidx * tp.permAinv) & (tp.ntiles - 1u);
-        const uint32_t ox = (t & nt_mask) << b;
-        const uint32_t oy = ((t >> nt_log) & nt_mask) << b;
-        const uint32_t oz = (DIM == 3) ? ((t >> (2u * nt_log)) << b) : 0u;
-        for (uint32_t w4 = threadIdx.x; w4 < words_per_tile; w4 += kT) {
-            const uint32_t w = w4 << 2;
-            const uint32_t wx = w & m, wy = (w >> b) & m, wz = (DIM == 3) ? (w >> (2u * b)) : 0u;
-            uint32_t gi = (ox + wx) + ((oy + wy) << logL);
-            if (DIM == 3) gi += (oz + wz) << (2u * logL);
-            if (LOAD) loc[(slot << (ts_log - 2u)) + w4] = __ldcg(glob + (gi >> 2));
-            else glob[gi >> 2] = loc[(slot << (ts_log - 2u)) + w4];
+    // V = uint4 (16 sites along x) when a tile row holds at least 16 sites, else unsigned int (4 sites).  The local
+    // lattice is linear in (slot, within-tile index); U loads are in flight per thread before the first store.
+    constexpr uint32_t VB = sizeof(V), U = 4;
+    const Tiling<DIM> tg(tp);
+    const uint32_t total = (ly.myslots << tg.ts_log) / VB;           // vectors this CTA owns
+    V *const loc = reinterpret_cast<V *>(ly.lat);
+    for (uint32_t base = threadIdx.x; base < total; base += kT * U) {
+        V v[U];
+        V *gp[U];
+#pragma unroll
+        for (uint32_t u = 0; u < U; ++u) {
+            const uint32_t idx = base + u * kT;
+            const uint32_t a = (idx < total ? idx : 0u) * VB;
+            const uint32_t gi = ly.origin[a >> tg.ts_log] + tg.spread(a & tg.ts_mask);
+            gp[u] = reinterpret_cast<V *>(tp.g.spins + gi);
+            if (idx < total) v[u] = LOAD ? __ldcg(gp[u]) : loc[idx];
+        }
+#pragma unroll
+        for (uint32_t u = 0; u < U; ++u) {
+            const uint32_t idx = base + u * kT;
+            if (idx < total) { if (LOAD) loc[idx] = v[u]; else *gp[u] = v[u]; }
         }
     }
+}
+
+// Copy the tiles of CTA c between the global lattice and shared memory (after build_tables(): uses origin[]).
+template <int DIM, bool LOAD>
+__device__ __forceinline__ void copy_tiles(const TileParams &tp, const Layout &ly)
+{
+    if (tp.tile_log >= 4u) copy_tiles_vec<DIM, LOAD, uint4>(tp, ly);
+    else copy_tiles_vec<DIM, LOAD, unsigned int>(tp, ly);
 }
 
 // Per-slot tables of CTA c: origin of the tile, and (owner, slot) of its 2*DIM neighbouring tiles.
@@ -948,7 +956,8 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         sh.spill_head = sh.spill_tail = ld_relaxed_u64(tp.gspill + c);
     }
     build_tables<DIM>(tp, ly, c);
-    copy_tiles<DIM, true>(tp, ly.lat, c);
+    __syncthreads();
+    copy_tiles<DIM, true>(tp, ly);
     __syncthreads();
 
     if (warp == 0u) receiver_warp<DIM>(tp, sh, ly, ly.stage, c, tl);
@@ -956,7 +965,7 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
     else worker_warp<DIM>(tp, sh, ly, ly.stage + warp * kStage, c, tl);
     __syncthreads();
 
-    copy_tiles<DIM, false>(tp, ly.lat, c);
+    copy_tiles<DIM, false>(tp, ly);
     if (tid == 0) {
         tp.gspill[c] = ld_vol64(&sh.spill_tail);
         tp.gfill[c] = ld_vol(&sh.fill_on);
