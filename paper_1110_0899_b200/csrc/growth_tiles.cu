@@ -48,10 +48,14 @@
 namespace wolff {
 namespace {
 
+#ifndef WOLFF_WIDE
+#define WOLFF_WIDE 1
+#endif
+constexpr unsigned int kWide = WOLFF_WIDE;         // sites per lane group and pass: a warp holds up to kWide * 32 / (2 dim) sites
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;
 constexpr int kT = kTileThreads;
 constexpr int kWarps = kT / 32;
-constexpr int kStage = 64;                         // two buffers of 32 winners per warp (one winner per lane and pass)
+constexpr int kStage = 64 * WOLFF_WIDE;            // two buffers of 32 * kWide winners per warp (kWide winners per lane and pass)
 constexpr uint32_t kBusy = 0x80000000u;            // bond-table state: a warp is filling this tile
 
 // message = [kind:2 | lap:1 | k:29] [site:31 | s0<0:1]
@@ -434,7 +438,7 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
 // Accounting (sh.pending): a warp that took n sites from the ring holds n units until it runs dry, whatever its
 // private frontier does in between; only the sites it hands to other warps are added.
 struct WorkerState {
-    uint32_t a = 0;              // local address of this lane's site
+    uint32_t a[kWide] = {};      // local addresses of this lane's sites
     unsigned int nsites = 0;     // sites held by the warp (warp-uniform); lanes of group q < nsites work
     unsigned int units = 0;      // what the warp owes sh.pending when it runs dry
     int s0 = 1;
@@ -450,7 +454,7 @@ template <int DIM, bool POS, bool READY>
 __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, const Layout &ly, const Tiling<DIM> &tg, uint32_t *stage,
                                            unsigned int c, WorkerState &ws, Tally &tl)
 {
-    constexpr unsigned int ND = 2u * DIM, S = 32u / ND;
+    constexpr unsigned int ND = 2u * DIM, S = 32u / ND, W = kWide;
     const GrowthParams &p = tp.g;
     const unsigned int lane = threadIdx.x & 31u;
     const unsigned int lt = (1u << lane) - 1u;
@@ -473,118 +477,164 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     const uint32_t tag = krel + 1u;
     const unsigned int s0w = POS ? 0x01010101u : 0xFFFFFFFFu;                // the seed spin in every byte
     const uint32_t cself = c << 16;
-    uint32_t a = ws.a;
+    uint32_t a[W];
+#pragma unroll
+    for (unsigned int j = 0; j < W; ++j) a[j] = ws.a[j];
     unsigned int nsites = ws.nsites, mywon = ws.mywon, sbuf = ws.sbuf;
-    unsigned long long msg_pos = 0;      // a message whose inbox slot is on its way back from L2
-    uint32_t msg_own = 0, msg_na = 0;
-    bool msg_valid = false;
+    unsigned long long msg_pos[W];       // messages whose inbox slots are on their way back from L2
+    uint32_t msg_own[W], msg_na[W];
+    bool msg_valid[W];
+#pragma unroll
+    for (unsigned int j = 0; j < W; ++j) { msg_pos[j] = 0; msg_own[j] = msg_na[j] = 0; msg_valid[j] = false; }
     unsigned int budget = 32u;
 
-    // one pass; 0: go on, 1: the warp ran dry, 2: back to the caller (!READY only)
+    auto send = [&](unsigned int j) {
+        st_relaxed_u64(tp.inbox + ((size_t)msg_own[j] << tp.in_log) + ((uint32_t)msg_pos[j] & in_mask),
+                       pack_msg(kKindClaim, (unsigned int)(msg_pos[j] >> tp.in_log) & 1u, krel, msg_na[j], POS ? 1 : -1));
+        msg_valid[j] = false;
+    };
+
+    // one pass; 0: go on, 1: the warp ran dry, 2: back to the caller (!READY only).  Lane (q, k) works on the sites
+    // q, q + S, ... (W of them): W independent dependent-chains side by side, so a pass over W*S sites takes little
+    // longer than a pass over S.
     auto pass = [&]() -> int {
 #ifdef WOLFF_PROFILE
         const long long tp0 = clock64();
         tl.lanes += nsites;
 #endif
-        const bool have = q < nsites;        // lanes 30, 31 in 3D: q = S >= nsites
-        // ---- A2: this lane's neighbour: same tile (a +- stride) or across a tile border (table of neighbouring tiles)
-        const uint32_t w = a & tg.ts_mask, slot = a >> tg.ts_log;
-        const bool inside = ((w >> db) & tg.m) != edge;
-        uint32_t nt = cself;
-        if (!inside) nt = lds_u32(nbr_s + slot * (ND * 4u));       // lanes without a site hold a stale (valid) address: their loads are harmless
-        const uint32_t na = inside ? a + step_in : (((nt & 0xFFFFu) << tg.ts_log) | (w + step_out));
-        const uint32_t own = nt >> 16;
-        const bool local = own == c;
-        // ---- A3, table.  The bond to the +d neighbour is owned by this site (bit a of plane d); the bond to the -d
-        // neighbour is owned by that neighbour: bit na of plane d when it is in the same tile, else the halo bit of
-        // this site's place on the tile's low-d face.
-        const bool use_halo = sgn != 0u && !inside;
-        const uint32_t fidx = (w & lowmask) | ((w >> (db + tg.b)) << db);
-        const uint32_t bi = use_halo ? fidx : (sgn ? na : a);
-        const uint32_t baddr = (use_halo ? halo_s + slot * fw4 : bond_s) + ((bi >> 5) << 2);
-        unsigned int st = tag, bw = 0, spw = 0;
-        if (READY) {
-            bw = lds_u32(baddr);
-        } else if (tables) {
-            st = lds_u32(state_s + slot * 4u);                                        // state first: see fill_step()
-            bw = lds_u32(baddr);
+        bool have[W], local[W], bit[W];
+        uint32_t w[W], slot[W], na[W], own[W], bi[W];
+        unsigned int st[W], bw[W], spw[W], bytemask[W], old[W];
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j) {
+            have[j] = q < S && q + j * S < nsites;       // lanes 30, 31 in 3D (q = S) never hold a site
+            // ---- A2: this lane's neighbour: same tile (a +- stride) or across a tile border (table of neighbouring tiles)
+            w[j] = a[j] & tg.ts_mask;
+            slot[j] = a[j] >> tg.ts_log;
+            const bool inside = ((w[j] >> db) & tg.m) != edge;
+            uint32_t nt = cself;
+            if (!inside) nt = lds_u32(nbr_s + slot[j] * (ND * 4u));   // lanes without a site hold a stale (valid) address: their loads are harmless
+            na[j] = inside ? a[j] + step_in : (((nt & 0xFFFFu) << tg.ts_log) | (w[j] + step_out));
+            own[j] = nt >> 16;
+            local[j] = own[j] == c;
+            // ---- A3, table.  The bond to the +d neighbour is owned by this site (bit a of plane d); the bond to the -d
+            // neighbour is owned by that neighbour: bit na of plane d when it is in the same tile, else the halo bit of
+            // this site's place on the tile's low-d face.
+            const bool use_halo = sgn != 0u && !inside;
+            const uint32_t fidx = (w[j] & lowmask) | ((w[j] >> (db + tg.b)) << db);
+            bi[j] = use_halo ? fidx : (sgn ? na[j] : a[j]);
+            const uint32_t baddr = (use_halo ? halo_s + slot[j] * fw4 : bond_s) + ((bi[j] >> 5) << 2);
+            st[j] = tag; bw[j] = 0; spw[j] = 0;
+            if (READY) {
+                bw[j] = lds_u32(baddr);
+            } else if (tables) {
+                st[j] = lds_u32(state_s + slot[j] * 4u);                              // state first: see fill_step()
+                bw[j] = lds_u32(baddr);
+            }
+            if (local[j]) spw[j] = lds_u32(lat_s + (na[j] & ~3u));                    // gather
+            bytemask[j] = 0xFFu << ((na[j] & 3u) * 8u);
         }
-        if (local) spw = lds_u32(lat_s + (na & ~3u));                                 // gather
-        const unsigned int bytemask = 0xFFu << ((na & 3u) * 8u);
-        bool bit = have && (bw & (1u << (bi & 31u))) != 0u;
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j) bit[j] = have[j] && (bw[j] & (1u << (bi[j] & 31u))) != 0u;
         if (!READY) {
             // ---- A3, inline: the same Philox block the table would hold
-            const bool tabled = tables && st == tag;
-            bit = bit && tabled;
-            const bool need_inline = have && !tabled;
-            if (__any_sync(kFullMask, need_inline)) {
-                if (need_inline) {
-                    const uint32_t gs = lds_u32(origin_s + slot * 4u) + tg.spread(w);
-                    const uint32_t gn = (gs & ~fmask) | ((((gs >> sh_d) + delta) & tg.Lmask) << sh_d);
-                    const uint4 blk = philox4x32_10(sgn ? gn : gs, kDomainBond, u_lo, u_hi, p.key0, p.key1);
-                    const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
-                    bit = r < tp.thr32 || tp.thr_all != 0u;
+            bool need_inline[W];
+            bool any = false;
+#pragma unroll
+            for (unsigned int j = 0; j < W; ++j) {
+                const bool tabled = tables && st[j] == tag;
+                bit[j] = bit[j] && tabled;
+                need_inline[j] = have[j] && !tabled;
+                any = any || need_inline[j];
+            }
+            if (__any_sync(kFullMask, any)) {
+#pragma unroll
+                for (unsigned int j = 0; j < W; ++j) {
+                    if (need_inline[j]) {
+                        const uint32_t gs = lds_u32(origin_s + slot[j] * 4u) + tg.spread(w[j]);
+                        const uint32_t gn = (gs & ~fmask) | ((((gs >> sh_d) + delta) & tg.Lmask) << sh_d);
+                        const uint4 blk = philox4x32_10(sgn ? gn : gs, kDomainBond, u_lo, u_hi, p.key0, p.key1);
+                        const uint32_t r = selp_u32(blk.x, selp_u32(blk.y, blk.z, d == 1u), d == 0u);
+                        bit[j] = r < tp.thr32 || tp.thr_all != 0u;
+                    }
                 }
                 if (lane == 0) ++tl.inline_passes;
             }
         }
-        const bool cand_l = bit && local && ((spw ^ s0w) & bytemask) == 0u;
-        const bool cand_r = bit && !local;
-
-        // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
-        unsigned int old = ~s0w;
-        if (POS) asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.shared.or.b32 %0, [%1], %2;\n}"
-                              : "+r"(old) : "r"(lat_s + (na & ~3u)), "r"(0xFEFEFEFEu & bytemask), "r"((unsigned int)cand_l) : "memory");
-        else     asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.shared.and.b32 %0, [%1], %2;\n}"
-                              : "+r"(old) : "r"(lat_s + (na & ~3u)), "r"(~(0xFEFEFEFEu & bytemask)), "r"((unsigned int)cand_l) : "memory");
-        tl.attempts += cand_l ? 1u : 0u;
+        bool cand_r[W];
+        bool any_r = false;
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j) {
+            const bool cand_l = bit[j] && local[j] && ((spw[j] ^ s0w) & bytemask[j]) == 0u;
+            cand_r[j] = bit[j] && !local[j];
+            any_r = any_r || cand_r[j] || msg_valid[j];
+            // ---- A4 inside the territory: the same idempotent atomic as claim_and_flip(), on shared memory
+            old[j] = ~s0w;
+            if (POS) asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.shared.or.b32 %0, [%1], %2;\n}"
+                                  : "+r"(old[j]) : "r"(lat_s + (na[j] & ~3u)), "r"(0xFEFEFEFEu & bytemask[j]), "r"((unsigned int)cand_l) : "memory");
+            else     asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.shared.and.b32 %0, [%1], %2;\n}"
+                                  : "+r"(old[j]) : "r"(lat_s + (na[j] & ~3u)), "r"(~(0xFEFEFEFEu & bytemask[j])), "r"((unsigned int)cand_l) : "memory");
+            tl.attempts += cand_l ? 1u : 0u;
+        }
         // ---- A4 across the territory border: a message to the owner (slot by one L2 atomic, then one 8-byte store).
         // The store waits for the atomic's round trip, so it is issued one pass later (or when the warp runs dry):
         // the slot is counted in gtail -- the atomic has returned -- before the pass that caused it stops being pending.
-        if (__any_sync(kFullMask, cand_r || msg_valid)) {
-            if (msg_valid) {
-                st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
-                               pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
-                msg_valid = false;
-            }
-            if (cand_r) {
-                msg_pos = atom_global_inc_u64(tp.gtail + own);
-                msg_own = own;
-                msg_na = na;
-                msg_valid = true;
-                ++tl.messages;
+        if (__any_sync(kFullMask, any_r)) {
+#pragma unroll
+            for (unsigned int j = 0; j < W; ++j) {
+                if (msg_valid[j]) send(j);
+                if (cand_r[j]) {
+                    msg_pos[j] = atom_global_inc_u64(tp.gtail + own[j]);
+                    msg_own[j] = own[j];
+                    msg_na[j] = na[j];
+                    msg_valid[j] = true;
+                    ++tl.messages;
+                }
             }
         }
-        const bool won = ((old ^ s0w) & bytemask) == 0u;
-        mywon += won ? 1u : 0u;
+        bool won[W];
+        unsigned int wb[W];
+        unsigned int total = 0;
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j) {
+            won[j] = ((old[j] ^ s0w) & bytemask[j]) == 0u;
+            mywon += won[j] ? 1u : 0u;
+        }
 #ifdef WOLFF_PROFILE
         if (lane == 0) ++tl.passes;
 #endif
-
-        // ---- A5: compact the winners; the first S are this warp's next pass, the rest goes to the ring
-        const unsigned int wb = __ballot_sync(kFullMask, won);
-        if (wb == 0u) return 1;                                  // the warp runs dry
-        const unsigned int total = __popc(wb);
+        // ---- A5: compact the winners; the first W*S are this warp's next pass, the rest goes to the ring
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j) { wb[j] = __ballot_sync(kFullMask, won[j]); total += __popc(wb[j]); }
+        if (total == 0u) return 1;                               // the warp runs dry
         uint32_t *const st_out = stage + sbuf;
         const uint32_t out_s = stage_s + sbuf * 4u;
-        sbuf ^= 32u;
-        if (won) sts_u32(out_s + __popc(wb & lt) * 4u, na);
+        sbuf ^= 32u * W;
+        unsigned int before = 0;
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j) {
+            if (won[j]) sts_u32(out_s + (before + __popc(wb[j] & lt)) * 4u, na[j]);
+            before += __popc(wb[j]);
+        }
         __syncwarp();
-        nsites = total < S ? total : S;
-        if (q < nsites) a = lds_u32(out_s + q * 4u);
-        if (total > S) {
-            if (lane == 0) red_shared_add(pend_s, total - S);    // counted before another warp can see them
-            hand_over(tp, sh, ly.ring, st_out + S, total - S, c);
+        nsites = total < W * S ? total : W * S;
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j)
+            if (q < S && q + j * S < nsites) a[j] = lds_u32(out_s + (q + j * S) * 4u);
+        if (total > W * S) {
+            if (lane == 0) red_shared_add(pend_s, total - W * S);    // counted before another warp can see them
+            hand_over(tp, sh, ly.ring, st_out + W * S, total - W * S, c);
         }
 #ifdef WOLFF_PROFILE
         tl.cyc_pass += (unsigned long long)(clock64() - tp0);
 #endif
         if (!READY && --budget == 0u) {
             // back to the caller: have the tables become complete?  (messages in flight leave first)
-            if (msg_valid)
-                st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
-                               pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
-            ws.a = a; ws.nsites = nsites; ws.mywon = mywon; ws.sbuf = sbuf;
+#pragma unroll
+            for (unsigned int j = 0; j < W; ++j) if (msg_valid[j]) send(j);
+            ws.nsites = nsites; ws.mywon = mywon; ws.sbuf = sbuf;
+#pragma unroll
+            for (unsigned int j = 0; j < W; ++j) ws.a[j] = a[j];
             return 2;
         }
         return 0;
@@ -599,9 +649,8 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     }
     if (status == 2) return;
     // ---- dry: the messages leave, the claims become visible to the publisher, then the warp's units stop being pending
-    if (msg_valid)
-        st_relaxed_u64(tp.inbox + ((size_t)msg_own << tp.in_log) + ((uint32_t)msg_pos & in_mask),
-                       pack_msg(kKindClaim, (unsigned int)(msg_pos >> tp.in_log) & 1u, krel, msg_na, POS ? 1 : -1));
+#pragma unroll
+    for (unsigned int j = 0; j < W; ++j) if (msg_valid[j]) send(j);
     const unsigned int wsum = __reduce_add_sync(kFullMask, mywon);
     if (lane == 0) {
         if (wsum) red_shared_add(claimed_s, wsum);
@@ -609,13 +658,13 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         const unsigned int before = atom_shared_add(pend_s, 0u - ws.units);
         if (before == ws.units) publish(tp, sh, c);
     }
-    ws.a = a; ws.nsites = 0u; ws.mywon = 0u; ws.sbuf = sbuf;
+    ws.nsites = 0u; ws.mywon = 0u; ws.sbuf = sbuf;
 }
 
 template <int DIM>
 __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, const Layout &ly, uint32_t *stage, unsigned int c, Tally &tl)
 {
-    constexpr unsigned int ND = 2u * DIM, S = 32u / ND;
+    constexpr unsigned int ND = 2u * DIM, S = 32u / ND, W = kWide;
     const GrowthParams &p = tp.g;
     const Tiling<DIM> tg(tp);
     const unsigned int lane = threadIdx.x & 31u;
@@ -640,10 +689,10 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
             h = (unsigned int)ht;
             const unsigned int t = (unsigned int)(ht >> 32);
             if (t != h) {
-                n = t - h < S ? t - h : S;
+                n = t - h < W * S ? t - h : W * S;
                 if (atomicCAS(&sh.head, h, h + n) != h) { n = 0; stop = 0; }
             } else if (st != sh_pos) {
-                n = st - sh_pos < (unsigned long long)S ? (unsigned int)(st - sh_pos) : S;
+                n = st - sh_pos < (unsigned long long)(W * S) ? (unsigned int)(st - sh_pos) : W * S;
                 if (atomicCAS(&sh.spill_head, sh_pos, sh_pos + n) == sh_pos) from_spill = 1; else { n = 0; stop = 0; }
             }
         }
@@ -690,7 +739,8 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
                 ent = v >> 1;
             }
         }
-        ws.a = __shfl_sync(kFullMask, ent, q);
+#pragma unroll
+        for (unsigned int j = 0; j < W; ++j) ws.a[j] = __shfl_sync(kFullMask, ent, (q + j * S) & 31u);
         ws.nsites = n;
         ws.units = n;
         // the update these sites belong to (written by the receiver before it fed the ring)
