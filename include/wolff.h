@@ -111,6 +111,8 @@ WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
  *   "ring_cap"             ... entries of a CTA's shared-memory work ring (power of two; overflow spills to global memory)
  *   "fill"                 ... bond tables: 0 = never (Philox inline), 1 = filled by idle warps when updates are long
  *                          enough to pay for it (default), 2 = always
+ *   "fill_bufs"            ... bond-table buffers: 0 = two (the running update and the next one) when they fit beside the
+ *                          lattice, else one (default); 1 = one
  *   "fill_min_us"          ... fill = 1: mean time per update above which tables are filled (default 30)
  *   "idle_ns"              ... longest sleep of an idle worker warp between two polls of the ring
  *   "watchdog_ms"          ... an update that takes longer aborts the launch (WOLFF_EINTERNAL at the next call)

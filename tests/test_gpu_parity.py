@@ -84,6 +84,25 @@ def test_crafted_start_lattices(dim, L, T, maker):
     compare_batched(gpu, ref, [1, 2, 17, 80])
 
 
+@pytest.mark.parametrize("case_seed", range(4))
+def test_randomised_knobs_shared_memory_resident_kernel(case_seed):
+    # 25 short chains per seed with random lattice, temperature, start and every knob of the tiled kernel (tile size,
+    # CTAs, ring size, bond tables never / adaptive / always, one or two buffers): the knobs never change the result
+    import random
+    rng = random.Random(1000 + case_seed)
+    for _ in range(25):
+        dim = rng.choice([2, 3])
+        L = rng.choice([8, 16, 32, 64] if dim == 2 else [4, 8, 16])
+        T = rng.choice([wl.TC_2D, 1.8, 3.0] if dim == 2 else [wl.TC_3D, 4.0, 5.0])
+        opts = {"mode": 0, "small_cluster": 0, "tile_log": rng.choice([2, 3, 4, 5, 6]), "tile_ctas": rng.choice([0, 1, 2, 3, 7, 16, 64]),
+                "fill": rng.choice([0, 1, 2, 2]), "ring_cap": rng.choice([32, 64, 2048]), "idle_ns": rng.choice([0, 100, 1000]),
+                "fill_bufs": rng.choice([0, 1]), "fill_min_us": rng.choice([0, 30])}
+        start = rng.choice([None, wl.cold(L ** dim), wl.blobs(dim, L, seed=rng.randrange(1000))])
+        gpu, ref = make_pair(dim, L, 1.0, T, seed=rng.randrange(1 << 40), start=start, options=opts)
+        compare_batched(gpu, ref, [rng.choice([1, 2, 5]), rng.choice([50, 300]), rng.choice([1, 500])])
+        gpu.close()
+
+
 def test_split_run_equivalence_and_resume():
     c = wl.CONFIGS["C1"]
     a, ref = make_pair(*c.create_args())
