@@ -1,5 +1,5 @@
-// expand.cuh -- expansion of one cluster site per lane, shared by the
-// level-synchronous kernel (growth.cu) and the barrier-free kernel (growth_async.cu).
+// expand.cuh -- expansion of one cluster site per lane for the level-synchronous
+// kernel (growth.cu).  growth_tiles.cu includes it for kFullMask only: its pass is written per bond, not per site.
 //
 // PAPER.md:45-46 (steps ii/iii): every neighbour of a newly added spin that is parallel to the seed
 // spin and not yet a member joins with probability p = 1 - exp(-2J/T).  Here the random number of a
