@@ -125,6 +125,8 @@ WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
  *   "cluster_ctas"         CTAs per thread-block cluster: 1, 2, 4, 8 or 16 (default 16)
  *   "grid_ctas"            total CTAs of the persistent kernel (0 = as many clusters as can be co-resident)
  *   "cooperative"          1 (default) = cooperative launch, 0 = plain launch of a grid sized to be co-resident
+ *   "speculative"          level-synchronous kernel: 1 = no neighbour gather, the claim atomic is issued for every active
+ *                          bond and its returned byte says whether the neighbour was parallel (default 0)
  * Thresholds are clamped to what the shared-memory queues can hold.  Unknown key or out-of-range
  * value: WOLFF_EINVAL. */
 WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);

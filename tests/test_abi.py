@@ -63,3 +63,14 @@ def test_product_path_does_not_touch_the_oracle():
         if f.endswith((".py", ".c", ".h")):
             assert "paper_1110_0899_b200" not in open(os.path.join(ROOT, "oracle", f)).read().replace(
                 "``paper_1110_0899_b200``", "").replace("paper_1110_0899_b200/csrc/", ""), f
+
+
+def test_header_documents_every_option_key_the_library_accepts():
+    import re
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    api = open(os.path.join(root, "paper_1110_0899_b200", "csrc", "api.cu")).read()
+    header = open(os.path.join(root, "include", "wolff.h")).read()
+    keys = set(re.findall(r'!strcmp\(key, "([a-z_]+)"\)', api))
+    assert len(keys) >= 15
+    missing = sorted(k for k in keys if '"%s"' % k not in header)
+    assert not missing, "option keys accepted by wolff_set_option but not documented in include/wolff.h: %s" % missing

@@ -25,7 +25,8 @@ MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 3},
          {"mode": 0, "tile_log": 3, "ring_cap": 32, "fill": 2, "idle_ns": 0, "small_cluster": 0},
          {"mode": 0, "fill": 0, "small_cluster": 0},
          {"mode": 0, "fill": 2, "tile_ctas": 5, "tile_log": 4, "small_cluster": 0},
-         {"mode": 0, "small_cluster": 1000000}]
+         {"mode": 0, "small_cluster": 1000000},
+         {"mode": 4, "speculative": 1, "up_threshold": 8, "down_threshold": 3, "cluster_up_threshold": 40, "grid_down_threshold": 20}]
 
 
 # ------------------------------------------------------------------ BASELINE config C1, exactly as written
