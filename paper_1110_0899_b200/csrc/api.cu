@@ -235,7 +235,7 @@ int refresh_plan(wolff_ctx *h)
     CHECK_CUDA(h, cudaMemset(h->tile_spill, 0, spill_bytes), "clear spill lists");
     CHECK_CUDA(h, cudaMemset(h->tile_fill, 0, (size_t)G * sizeof(uint32_t)), "clear fill flags");
     tp.inbox = h->tile_inbox;
-    tp.gtail = h->tile_ctr;
+    tp.gtail = reinterpret_cast<unsigned int *>(h->tile_ctr);      // G 32-bit counters in the first G 64-bit words
     tp.gdone = h->tile_ctr + G;
     tp.gspill = h->tile_ctr + 2 * (size_t)G;
     tp.added = h->tile_ctr + 3 * (size_t)G;

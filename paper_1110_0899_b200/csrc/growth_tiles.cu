@@ -121,13 +121,6 @@ __device__ __forceinline__ unsigned int atom_shared_add(uint32_t saddr, unsigned
     return old;
 }
 
-__device__ __forceinline__ unsigned long long atom_global_inc_u64(unsigned long long *p)
-{
-    unsigned long long old;
-    asm volatile("atom.global.add.u64 %0, [%1], 1;" : "=l"(old) : "l"(p) : "memory");
-    return old;
-}
-
 // Per-CTA shared state.
 struct alignas(16) TShared {
     unsigned int head, tail;            // ring: entries [head, tail) wait for a worker warp (one aligned 64-bit word)
@@ -481,7 +474,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
 #pragma unroll
     for (unsigned int j = 0; j < W; ++j) a[j] = ws.a[j];
     unsigned int nsites = ws.nsites, mywon = ws.mywon, sbuf = ws.sbuf;
-    unsigned long long msg_pos[W];       // messages whose inbox slots are on their way back from L2
+    unsigned int msg_pos[W];           // messages whose inbox slots are on their way back from L2
     uint32_t msg_own[W], msg_na[W];
     bool msg_valid[W];
 #pragma unroll
@@ -489,8 +482,8 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     unsigned int budget = 32u;
 
     auto send = [&](unsigned int j) {
-        st_relaxed_u64(tp.inbox + ((size_t)msg_own[j] << tp.in_log) + ((uint32_t)msg_pos[j] & in_mask),
-                       pack_msg(kKindClaim, (unsigned int)(msg_pos[j] >> tp.in_log) & 1u, krel, msg_na[j], POS ? 1 : -1));
+        st_relaxed_u64(tp.inbox + ((size_t)msg_own[j] << tp.in_log) + (msg_pos[j] & in_mask),
+                       pack_msg(kKindClaim, (msg_pos[j] >> tp.in_log) & 1u, krel, msg_na[j], POS ? 1 : -1));
         msg_valid[j] = false;
     };
 
@@ -583,8 +576,11 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
 #pragma unroll
             for (unsigned int j = 0; j < W; ++j) {
                 if (msg_valid[j]) send(j);
+                // the atomic writes the loop-carried register itself (an in-out operand, 32 bits: a 64-bit result needs an
+                // aligned register pair, which ptxas then copies out of -- and a copy waits for the L2 round trip here)
+                asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %2, 0;\n @p atom.global.add.u32 %0, [%1], 1;\n}"
+                             : "+r"(msg_pos[j]) : "l"(tp.gtail + own[j]), "r"((unsigned int)cand_r[j]) : "memory");
                 if (cand_r[j]) {
-                    msg_pos[j] = atom_global_inc_u64(tp.gtail + own[j]);
                     msg_own[j] = own[j];
                     msg_na[j] = na[j];
                     msg_valid[j] = true;
@@ -863,20 +859,21 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
             const uint32_t i0 = (uint32_t)__umul64hi(rr, (unsigned long long)p.geo.N);
             uint32_t own, addr;
             tg.locate(i0, own, addr);
-            const unsigned long long pos = atomicAdd(tp.gtail + own, 1ull);
-            st_relaxed_u64(tp.inbox + ((size_t)own << tp.in_log) + ((uint32_t)pos & in_mask),
-                           pack_msg(kKindSeed, (unsigned int)(pos >> tp.in_log) & 1u, (unsigned int)k, addr, 1));
+            const unsigned int pos = atomicAdd(tp.gtail + own, 1u);
+            st_relaxed_u64(tp.inbox + ((size_t)own << tp.in_log) + (pos & in_mask),
+                           pack_msg(kKindSeed, (pos >> tp.in_log) & 1u, (unsigned int)k, addr, 1));
             ++tl.messages;
         }
         const unsigned long long t0 = globaltimer_ns();
         unsigned int passes = 0;
         for (;;) {
-            unsigned long long d = 0, t = 0;
-            for (unsigned int cc = lane; cc < G; cc += 32u) d += ld_relaxed_u64(tp.gdone + cc);
+            // sums modulo 2^32: gtail[] are 32-bit running counters, and what is in flight is far below 2^32 messages
+            unsigned int d = 0, t = 0;
+            for (unsigned int cc = lane; cc < G; cc += 32u) d += (unsigned int)ld_relaxed_u64(tp.gdone + cc);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) d += __shfl_xor_sync(kFullMask, d, o);
             fence_acq_rel_gpu();      // every gtail (and `added`) is read after every gdone
-            for (unsigned int cc = lane; cc < G; cc += 32u) t += ld_relaxed_u64(tp.gtail + cc);
+            for (unsigned int cc = lane; cc < G; cc += 32u) t += ld_relaxed_u32(tp.gtail + cc);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(kFullMask, t, o);
             ++passes;
@@ -900,9 +897,9 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
     }
     // everybody leaves (also after an abort: receivers poll the error flag, but an exit message is quicker)
     for (unsigned int cc = lane; cc < G; cc += 32u) {
-        const unsigned long long pos = atomicAdd(tp.gtail + cc, 1ull);
-        st_relaxed_u64(tp.inbox + ((size_t)cc << tp.in_log) + ((uint32_t)pos & in_mask),
-                       pack_msg(kKindExit, (unsigned int)(pos >> tp.in_log) & 1u, 0u, 0u, 1));
+        const unsigned int pos = atomicAdd(tp.gtail + cc, 1u);
+        st_relaxed_u64(tp.inbox + ((size_t)cc << tp.in_log) + (pos & in_mask),
+                       pack_msg(kKindExit, (pos >> tp.in_log) & 1u, 0u, 0u, 1));
     }
     if (lane == 0) {
         ctl->stats[0] += p.n_updates;

@@ -64,7 +64,7 @@ struct GrowthParams {
 struct TileParams {
     GrowthParams g;
     unsigned long long *inbox;       // G segments of in_cap messages; slot validity by lap parity, never cleared
-    unsigned long long *gtail;       // [G] messages ever pushed into CTA c's inbox
+    unsigned int *gtail;             // [G] messages ever pushed into CTA c's inbox, modulo 2^32 (its low bits are the inbox slot)
     unsigned long long *gdone;       // [G] of those, how many are consumed with their whole local progeny expanded
     unsigned long long *gspill;      // [G] running position of CTA c's spill list
     unsigned long long *added;       // spins ever claimed (sum over CTAs, published with gdone)
