@@ -46,7 +46,7 @@ def measured_peak_hbm():
 # ncu `--set full` DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of one launch of the growth kernel,
 # bytes: profiles/r1_growth_tiles_C3.md (a 10-update C3 launch: the 16 MiB lattice is read once in the prologue; the
 # write-back and all queue traffic stay in L2).  It does not grow with the updates per launch.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 22598912 + 1883136
+NCU_TRAFFIC_BYTES_PER_LAUNCH = 22624256 + 493056
 
 
 class ClockSampler:

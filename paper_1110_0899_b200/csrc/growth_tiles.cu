@@ -282,7 +282,7 @@ __device__ __forceinline__ uint32_t spill_tag(unsigned long long pos, uint32_t c
 
 // Hand n sites (items[0..n), warp-collective) to the other warps of the CTA: the ring, or the spill list when
 // the ring is full.  The caller has already counted them in sh.pending.
-__device__ __noinline__ void hand_over(const TileParams &tp, TShared &sh, uint32_t *ring, const uint32_t *items, unsigned int n,
+__device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uint32_t *ring, const uint32_t *items, unsigned int n,
                                        unsigned int c)
 {
     const unsigned int lane = threadIdx.x & 31u;
