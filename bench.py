@@ -321,6 +321,16 @@ def run_b200(args, rank: int, world: int):
                              "see bfs_depth_per_update and us_per_bfs_level"},
     }
 
+    if rank == 0 and world == 1 and not args.no_depth and args.mode == 0:
+        # latency roofline: T_update >= BFS depth x t_pass, t_pass floor from wolff_microbench [7]
+        micro = binding.microbench()
+        depth = primary["levels"] / primary["updates"]
+        floor_ms = depth * micro["smem_pass_floor_ns"] * 1e-6
+        achieved_ms = sum(primary["growth_ms"]) / primary["updates"]
+        out["latency_roofline"] = {"bfs_depth_per_update": depth, "t_pass_floor_ns": micro["smem_pass_floor_ns"],
+                                   "bound_ms_per_update": floor_ms, "achieved_ms_per_update": achieved_ms,
+                                   "frac": floor_ms / achieved_ms if achieved_ms else None,
+                                   "microbench_ns": {k: v for k, v in micro.items()}}
     if rank == 0 and world == 1 and not args.no_secondary:
         out.update(measurement_legs(primary["h"], c, 50))
         primary["h"].close()

@@ -151,8 +151,12 @@ WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
  *   [1] dependent L2 load, one warp, 32 scattered lines   [2] dependent atom.or with return, one lane
  *   [3] dependent atom.or, one warp, 32 scattered words   [4] __syncthreads at 512 threads
  *   [5] three Philox4x32-10 blocks, one warp              [6] the library's grid barrier, one CTA per SM
+ *   [7] one pass of the minimal dependent chain of the shared-memory-resident kernel, one warp alone on an SM:
+ *       ld.shared (spin, bond bit) -> atom.shared (claim) -> ballot/popc -> st.shared -> __syncwarp -> ld.shared;
+ *       this is the floor of t_pass in the latency roofline T_update >= depth x t_pass
+ *   [8] fraction of lanes that won their claim in [7] (1.0 when the chain ran as intended; not a time)
  * Not part of the measured path. */
-#define WOLFF_NMICRO 7
+#define WOLFF_NMICRO 9
 WOLFF_API int wolff_microbench(double *out_ns, int n_out);
 
 /* Free everything.  NULL is allowed. */

@@ -90,7 +90,7 @@ def _stream_handle(stream):
 
 
 MICRO_NAMES = ("l2_load_lane_ns", "l2_load_warp_ns", "l2_atomic_lane_ns", "l2_atomic_warp_ns", "syncthreads_ns",
-               "philox_x3_ns", "grid_barrier_ns")
+               "philox_x3_ns", "grid_barrier_ns", "smem_pass_floor_ns", "smem_pass_win_fraction")
 
 
 def microbench() -> dict:

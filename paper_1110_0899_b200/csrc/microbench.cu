@@ -122,6 +122,46 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) grid_barrier_kernel(Control
     if (threadIdx.x == 0 && blockIdx.x == 0) out[6] = (double)(globaltimer_ns() - t0) / iters;
 }
 
+// out[7] = ns per pass of the minimal dependent chain of the shared-memory-resident kernel (growth_tiles.cu), one warp
+// alone on an SM: site address -> ld.shared of the neighbour's spin word and of a bond word -> compare ->
+// atom.shared (claim) -> compare -> ballot, popc -> st.shared (stage) -> __syncwarp -> ld.shared (next site).
+// Every lane wins every pass (fresh bytes; the seed spin flips sign after each sweep of the 64 KiB region), so
+// this is the floor of one pass: no Philox, no messages, no queue.
+__global__ void __launch_bounds__(32, 1) smem_pass_kernel(int iters, double *out)
+{
+    extern __shared__ __align__(16) unsigned int dyn[];
+    constexpr unsigned int kBytes = 64u << 10, kStep = 132u, kSweep = (kBytes - 128u) / kStep;
+    unsigned int *const lat = dyn;                         // kBytes of spins, 0x01 = +1, 0xFF = -1
+    unsigned int *const bond = dyn + kBytes / 4u;          // one bit per site
+    unsigned int *const stage = bond + kBytes / 32u;
+    const unsigned int lane = threadIdx.x, lt = (1u << lane) - 1u;
+    for (unsigned int i = lane; i < kBytes / 4u; i += 32u) lat[i] = 0x01010101u;
+    for (unsigned int i = lane; i < kBytes / 32u; i += 32u) bond[i] = 0xFFFFFFFFu;
+    __syncwarp();
+    unsigned int a = lane * 4u, won_total = 0;
+    const unsigned long long t0 = globaltimer_ns();
+    for (int k = 0; k < iters; ++k) {
+        const unsigned int step = (unsigned int)k % kSweep;
+        const bool pos = (((unsigned int)k / kSweep) & 1u) == 0u;
+        const unsigned int s0w = pos ? 0x01010101u : 0xFFFFFFFFu;
+        const unsigned int na = step == 0u ? lane * 4u + (a & 3u) : a + kStep;      // depends on the staged site
+        const unsigned int spw = *reinterpret_cast<volatile unsigned int *>(lat + (na >> 2));
+        const unsigned int bw = *reinterpret_cast<volatile unsigned int *>(bond + (na >> 5));
+        const unsigned int bytemask = 0xFFu << ((na & 3u) * 8u);
+        const bool cand = ((bw >> (na & 31u)) & 1u) != 0u && ((spw ^ s0w) & bytemask) == 0u;
+        unsigned int old = ~s0w;
+        if (cand) old = pos ? atomicOr(lat + (na >> 2), 0xFEFEFEFEu & bytemask) : atomicAnd(lat + (na >> 2), ~(0xFEFEFEFEu & bytemask));
+        const bool won = ((old ^ s0w) & bytemask) == 0u;
+        const unsigned int wb = __ballot_sync(0xFFFFFFFFu, won);
+        if (won) *reinterpret_cast<volatile unsigned int *>(stage + __popc(wb & lt)) = na;
+        __syncwarp();
+        won_total += __popc(wb);
+        a = *reinterpret_cast<volatile unsigned int *>(stage + ((lane + 1u) & 31u));
+    }
+    const unsigned long long t1 = globaltimer_ns();
+    if (lane == 0) { out[7] = (double)(t1 - t0) / iters; out[8] = (double)won_total / (32.0 * iters); }
+}
+
 }  // namespace
 }  // namespace wolff
 
@@ -151,6 +191,11 @@ extern "C" WOLFF_API int wolff_microbench(double *out_host, int n_out)
     void *args[] = { &ctl, const_cast<int *>(&iters), &out };
     cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(&grid_barrier_kernel), dim3(grid),
                                                 dim3(kGrowthThreads), args, 0, nullptr);
+    if (e == cudaSuccess) {
+        const size_t smem = (64u << 10) + (64u << 10) / 8u + 32u * sizeof(unsigned int);
+        e = cudaFuncSetAttribute(smem_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) smem_pass_kernel<<<1, 32, smem>>>(4 * 496, out);
+    }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e == cudaSuccess) e = cudaMemcpy(out_host, out, sizeof(double) * WOLFF_NMICRO, cudaMemcpyDeviceToHost);
     if (e != cudaSuccess) rc = WOLFF_ECUDA;

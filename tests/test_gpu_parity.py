@@ -161,3 +161,13 @@ def test_full_size_configs_literal_random_start(name):
     gpu, ref = make_pair(*c.create_args())
     assert_same_state(gpu, ref, "start lattice")
     compare_batched(gpu, ref, [1000, 2000])
+
+
+def test_microbench_pass_floor_runs_as_intended():
+    # the latency-roofline floor (wolff_microbench [7]): every lane must have won every claim, else the chain timed is not
+    # the one DESIGN.md section 6 describes
+    from paper_1110_0899_b200 import binding
+    m = binding.microbench()
+    assert m["smem_pass_win_fraction"] == 1.0
+    assert 20.0 < m["smem_pass_floor_ns"] < 2000.0
+    assert m["l2_load_lane_ns"] > m["smem_pass_floor_ns"] / 10.0
