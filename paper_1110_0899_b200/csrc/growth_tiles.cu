@@ -27,6 +27,7 @@
 //     which one ran;
 //   - a warp that claims neighbours keeps up to S of them in registers for its next pass; the rest goes
 //     to a shared-memory ring that the other warps of the CTA drain (overflow: a per-CTA global spill list);
+//     one idle warp per CTA holds the "watch" and polls the ring without backing off;
 //   - an active bond that leaves the CTA's territory becomes a MESSAGE "claim the site at your local
 //     address a" in the owner's inbox (global memory, one L2 atomicAdd for the slot + one 8-byte
 //     store); the owner's receiver warp polls its inbox, makes the claim on its own shared memory and
@@ -35,7 +36,8 @@
 //     levels, no barrier (A6 becomes a work hand-over);
 //   - termination of an update: every CTA publishes gdone[c] = "inbox messages consumed, with their whole
 //     local progeny expanded" whenever it runs dry; a monitor warp in CTA 0 reads every gdone[], then every
-//     gtail[] (messages ever pushed).  Both only grow, a message is counted in gtail before anything it
+//     gtail[] (messages ever pushed; 32-bit running counters, sums compared modulo 2^32 -- what is in flight is far
+//     below 2^32).  Both only grow, a message is counted in gtail before anything it
 //     causes can be counted in gdone, so equal sums mean: at the instant between the two passes nothing was
 //     queued, in flight or being expanded anywhere.  The monitor then logs the size (A7) and sends the seed
 //     message of the next update (A1) to the owner of the seed site.
