@@ -133,6 +133,12 @@ def aggregate_replicas(flipped: int, updates: int, total_ms: float, world: int, 
 def run_b200(args, rank: int, world: int):
     import numpy as np
     import torch
+    from paper_1110_0899_b200 import build as cuda_build
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        cuda_build.build()              # no-op when libwolff_b200.so is up to date; the .so is not in the history
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
     from paper_1110_0899_b200 import binding, workloads as wl
 
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
