@@ -897,11 +897,21 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
             prev = a;
         }
     }
-    // everybody leaves (also after an abort: receivers poll the error flag, but an exit message is quicker)
-    for (unsigned int cc = lane; cc < G; cc += 32u) {
-        const unsigned int pos = atomicAdd(tp.gtail + cc, 1u);
-        st_relaxed_u64(tp.inbox + ((size_t)cc << tp.in_log) + (pos & in_mask),
-                       pack_msg(kKindExit, (pos >> tp.in_log) & 1u, 0u, 0u, 1));
+    // everybody leaves (also after an abort: receivers poll the error flag, but an exit message is quicker).  Eight slot
+    // atomics per lane are in flight before the first message is stored.
+    for (unsigned int base = 0; base < G; base += 256u) {
+        unsigned int pos[8];
+#pragma unroll
+        for (unsigned int i = 0; i < 8u; ++i) {
+            const unsigned int cc = base + i * 32u + lane;
+            pos[i] = cc < G ? atomicAdd(tp.gtail + cc, 1u) : 0u;
+        }
+#pragma unroll
+        for (unsigned int i = 0; i < 8u; ++i) {
+            const unsigned int cc = base + i * 32u + lane;
+            if (cc < G)
+                st_relaxed_u64(tp.inbox + ((size_t)cc << tp.in_log) + (pos[i] & in_mask), pack_msg(kKindExit, (pos[i] >> tp.in_log) & 1u, 0u, 0u, 1));
+        }
     }
     if (lane == 0) {
         ctl->stats[0] += p.n_updates;
