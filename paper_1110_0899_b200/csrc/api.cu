@@ -234,6 +234,9 @@ int refresh_plan(wolff_ctx *h)
     CHECK_CUDA(h, cudaMemset(h->tile_ctr, 0, ctr_bytes), "clear counters");
     CHECK_CUDA(h, cudaMemset(h->tile_spill, 0, spill_bytes), "clear spill lists");
     CHECK_CUDA(h, cudaMemset(h->tile_fill, 0, (size_t)G * sizeof(uint32_t)), "clear fill flags");
+    // The memsets above run on the legacy default stream; the kernel that uses these buffers may be launched on a
+    // non-blocking stream, which does not wait for it: finish them here (a plan is made once per knob change).
+    CHECK_CUDA(h, cudaDeviceSynchronize(), "cudaDeviceSynchronize");
     tp.inbox = h->tile_inbox;
     tp.gtail = reinterpret_cast<unsigned int *>(h->tile_ctr);      // G 32-bit counters in the first G 64-bit words
     tp.gdone = h->tile_ctr + G;

@@ -1014,17 +1014,32 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         sh.ihead = ld_relaxed_u64(tp.gdone + c);          // everything ever sent to this CTA was consumed by the last launch
         sh.spill_head = sh.spill_tail = ld_relaxed_u64(tp.gspill + c);
     }
+#ifdef WOLFF_PROFILE
+    const unsigned long long tk0 = globaltimer_ns();
+#endif
     build_tables<DIM>(tp, ly, c);
     __syncthreads();
     copy_tiles<DIM, true>(tp, ly);
     __syncthreads();
+#ifdef WOLFF_PROFILE
+    const unsigned long long tk1 = globaltimer_ns();
+#endif
 
     if (warp == 0u) receiver_warp<DIM>(tp, sh, ly, ly.stage, c, tl);
     else if (warp == 1u && c == 0u) monitor_warp<DIM>(tp, tl);
     else worker_warp<DIM>(tp, sh, ly, ly.stage + warp * kStage, c, tl);
     __syncthreads();
 
+#ifdef WOLFF_PROFILE
+    const unsigned long long tk2 = globaltimer_ns();
+#endif
     copy_tiles<DIM, false>(tp, ly);
+#ifdef WOLFF_PROFILE
+    __syncthreads();
+    if (tid == 0 && c == 0) {
+        tp.g.ctl->stats[4] = tk1 - tk0; tp.g.ctl->stats[5] = tk2 - tk1; tp.g.ctl->stats[6] = globaltimer_ns() - tk2;
+    }
+#endif
     if (tid == 0) {
         tp.gspill[c] = ld_vol64(&sh.spill_tail);
         tp.gfill[c] = ld_vol(&sh.fill_on);

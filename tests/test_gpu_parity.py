@@ -171,3 +171,20 @@ def test_microbench_pass_floor_runs_as_intended():
     assert m["smem_pass_win_fraction"] == 1.0
     assert 20.0 < m["smem_pass_floor_ns"] < 2000.0
     assert m["l2_load_lane_ns"] > m["smem_pass_floor_ns"] / 10.0
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C4"])
+def test_first_run_on_a_fresh_non_blocking_stream(name):
+    # the very first wolff_run of a handle allocates and clears the tiled kernel's queues; a kernel launched on a
+    # non-blocking stream must not start before that clearing has finished (regression: lost messages, watchdog abort)
+    import torch
+    c = wl.CONFIGS[name]
+    for seed in range(3):
+        gpu, ref = make_pair(c.dim, c.L, c.J, c.T, seed=100 + seed, options={"small_cluster": 0, "watchdog_ms": 5000})
+        stream = torch.cuda.Stream()
+        gpu.run(10, stream=stream)
+        E, M, sz = gpu.observables(sizes=True)
+        assert np.array_equal(sz, ref.run(10))
+        assert (E, M) == ref.observables()
+        assert_same_state(gpu, ref)
+        gpu.close()
