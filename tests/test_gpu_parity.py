@@ -188,3 +188,51 @@ def test_first_run_on_a_fresh_non_blocking_stream(name):
         assert (E, M) == ref.observables()
         assert_same_state(gpu, ref)
         gpu.close()
+
+
+@pytest.mark.parametrize("case_seed", range(3))
+def test_random_api_sequences(case_seed):
+    # 40 chains per seed of randomly interleaved calls: runs on the default and on non-blocking streams, knob changes in
+    # the middle of a chain (kernel, tiling, tables), lattices loaded and read back through device and host buffers,
+    # update index jumps -- compared with the oracle after every step that returns something
+    import random
+    import torch
+    rng = random.Random(2000 + case_seed)
+    streams = [None, torch.cuda.Stream(), torch.cuda.Stream()]
+    knobs = {"mode": [0, 0, 4, 1, 3], "small_cluster": [0, 16, 100000], "tile_log": [0, 2, 3, 4, 5], "tile_ctas": [0, 1, 3, 16],
+             "fill": [0, 1, 2], "fill_bufs": [0, 1], "ring_cap": [32, 2048], "idle_ns": [0, 1000], "fill_min_us": [0, 30]}
+    for _ in range(40):
+        dim = rng.choice([2, 3])
+        L = rng.choice([8, 16, 32, 64] if dim == 2 else [4, 8, 16])
+        gpu, ref = make_pair(dim, L, 1.0, rng.choice([wl.TC_2D, 1.9] if dim == 2 else [wl.TC_3D, 4.0]), seed=rng.randrange(1 << 40))
+        for _step in range(rng.randrange(4, 12)):
+            op = rng.choice(["run", "run", "run", "opt", "set", "obs_dev", "get_dev", "idx"])
+            if op == "run":
+                k = rng.choice([1, 2, 7, 60, 400])
+                gpu.run(k, stream=rng.choice(streams))
+                rs = ref.run(k)
+                if rng.random() < 0.6:
+                    E, M, sz = gpu.observables(sizes=True)
+                    assert np.array_equal(sz, rs) and (E, M) == ref.observables()
+            elif op == "opt":
+                key = rng.choice(list(knobs))
+                gpu.set_option(key, rng.choice(knobs[key]))
+            elif op == "set":
+                start = rng.choice([wl.cold(L ** dim), wl.blobs(dim, L, seed=rng.randrange(99)), wl.checkerboard(dim, L)])
+                gpu.set_spins(start)
+                ref.set_spins(start)
+            elif op == "obs_dev":
+                E = torch.zeros(1, dtype=torch.int64, device="cuda")
+                M = torch.zeros(1, dtype=torch.int64, device="cuda")
+                gpu.observables_into(E, M, None)
+                assert (int(E.item()), int(M.item())) == ref.observables()
+            elif op == "get_dev":
+                d = torch.empty(L ** dim, dtype=torch.int8, device="cuda")
+                gpu.get_spins_into(d)
+                assert np.array_equal(d.cpu().numpy(), ref.get_spins())
+            else:
+                u = rng.randrange(1 << 45)
+                gpu.update_index = u
+                ref.update_index = u
+        assert_same_state(gpu, ref, "end of a random call sequence")
+        gpu.close()
