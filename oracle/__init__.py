@@ -79,6 +79,10 @@ def lib() -> ctypes.CDLL:
         L.oracle_run.restype = i32
         L.oracle_run_logged.argtypes = [vp, u64, vp, vp, vp]
         L.oracle_run_logged.restype = i32
+        L.oracle_moments.argtypes = [u64, vp, vp, vp, vp]
+        L.oracle_moments.restype = None
+        L.oracle_binder.argtypes = [vp]
+        L.oracle_binder.restype = dbl
         L.ising_enum_joint_dos.argtypes = [i32, i32, vp]
         L.ising_enum_joint_dos.restype = i32
         _lib = L
@@ -174,6 +178,34 @@ class OracleWolff:
         if a.size != self.N or not np.all(np.abs(a) == 1):
             raise ValueError("need N spins of +/-1")
         self._L.oracle_set_spins(self._h, a.ctypes.data)
+
+
+MOMENT_NAMES = ("n", "sum_E", "sum_absM", "sum_E2", "sum_M2", "sum_M4")
+
+
+def moments_raw(E, M, acc=None) -> np.ndarray:
+    """oracle_moments: the ten 64-bit words (layout in wolff_oracle.c) over the series (E_k, M_k), continuing `acc`."""
+    E = np.ascontiguousarray(E, dtype=np.int64)
+    M = np.ascontiguousarray(M, dtype=np.int64)
+    assert E.shape == M.shape and E.ndim == 1
+    out = np.zeros(10, dtype=np.uint64)
+    a = None if acc is None else np.ascontiguousarray(acc, dtype=np.uint64)
+    lib().oracle_moments(E.size, E.ctypes.data, M.ctypes.data, None if a is None else a.ctypes.data, out.ctypes.data)
+    return out
+
+
+def moments_dict(raw) -> dict:
+    """The ten words as exact Python integers."""
+    w = [int(x) for x in raw]
+    sum_E = w[1] - (1 << 64) if w[1] >> 63 else w[1]
+    return {"n": w[0], "sum_E": sum_E, "sum_absM": w[2], "sum_E2": w[3] | (w[4] << 64),
+            "sum_M2": w[5] | (w[6] << 64), "sum_M4": w[7] | (w[8] << 64)}
+
+
+def binder(raw) -> float:
+    """oracle_binder: Eq. 3 of the paper from the accumulated sums."""
+    a = np.ascontiguousarray(raw, dtype=np.uint64)
+    return float(lib().oracle_binder(a.ctypes.data))
 
 
 def joint_density_of_states(dim: int, L: int) -> np.ndarray:

@@ -32,6 +32,9 @@
  *                          within 3 standard errors; <|C|> = <M^2>/N;
  *                          Kaufman's exact finite-torus energy; Onsager band
  *   observables .......... closed forms (cold lattice, checkerboard, stripes)
+ *   moments / binder ..... hand-computed series, Python big integers past 2^64,
+ *                          |M| = N gives U = 2/3, Gaussian M gives U -> 0, exact
+ *                          4x4 / 3x3x3 enumeration (U = 0.61719932 at 2D T_c)
  * No function in this file is "parity unpinned".
  *
  * Precision: everything is integer except the threshold, which is IEEE
@@ -273,4 +276,60 @@ int oracle_run_logged(oracle_ctx *h, uint64_t n_updates, uint32_t *sizes,
         oracle_observables(h, E_log ? &E_log[k] : NULL, M_log ? &M_log[k] : NULL);
     }
     return 0;
+}
+
+/* ----------------------------------------------------------------- moments */
+
+/* Accumulated moments of a measured series and the Binder ratio.
+ * PAPER.md:126 ("the measurement of energy and magnetization" after every
+ * update; the "+ measurement" columns of Tables 1-2) and
+ * PAPER.md:159-164 Eq. 3:  U(T) = 1 - <M^4> / (3 <M^2>^2),  averages over the
+ * measured updates (the updates after the discarded ones).
+ *
+ * Definition, written out: over the n samples (E_k, M_k)
+ *   out[0] = n              out[1] = sum E_k (two's complement)
+ *   out[2] = sum |M_k|      out[3..4] = sum E_k^2  (low, high 64 bits)
+ *   out[5..6] = sum M_k^2   out[7..8] = sum M_k^4  out[9] = 0 (reserved)
+ * All sums are exact integers: M^4 reaches 2^96 at N = 2^24 spins, so the
+ * second and fourth moments are kept in 128 bits.  `acc` continues an earlier
+ * accumulation (acc may equal out; NULL starts from zero). */
+void oracle_moments(uint64_t n, const int64_t *E, const int64_t *M, const uint64_t *acc, uint64_t out[10])
+{
+    uint64_t cnt = 0, sum_absM = 0;
+    int64_t sum_E = 0;
+    unsigned __int128 sum_E2 = 0, sum_M2 = 0, sum_M4 = 0;
+    if (acc) {
+        cnt = acc[0]; sum_E = (int64_t)acc[1]; sum_absM = acc[2];
+        sum_E2 = ((unsigned __int128)acc[4] << 64) | acc[3];
+        sum_M2 = ((unsigned __int128)acc[6] << 64) | acc[5];
+        sum_M4 = ((unsigned __int128)acc[8] << 64) | acc[7];
+    }
+    for (uint64_t k = 0; k < n; ++k) {
+        uint64_t absM = (uint64_t)(M[k] < 0 ? -M[k] : M[k]);
+        uint64_t absE = (uint64_t)(E[k] < 0 ? -E[k] : E[k]);
+        unsigned __int128 m2 = (unsigned __int128)absM * absM;
+        cnt += 1;
+        sum_E += E[k];
+        sum_absM += absM;
+        sum_E2 += (unsigned __int128)absE * absE;
+        sum_M2 += m2;
+        sum_M4 += m2 * m2;
+    }
+    out[0] = cnt; out[1] = (uint64_t)sum_E; out[2] = sum_absM;
+    out[3] = (uint64_t)sum_E2; out[4] = (uint64_t)(sum_E2 >> 64);
+    out[5] = (uint64_t)sum_M2; out[6] = (uint64_t)(sum_M2 >> 64);
+    out[7] = (uint64_t)sum_M4; out[8] = (uint64_t)(sum_M4 >> 64);
+    out[9] = 0;
+}
+
+/* Eq. 3 from the accumulated sums:
+ * U = 1 - (S4/n) / (3 (S2/n)^2) = 1 - n S4 / (3 S2^2), in long double.
+ * Returns NaN when no sample or S2 = 0. */
+double oracle_binder(const uint64_t moments[10])
+{
+    long double n = (long double)moments[0];
+    long double s2 = (long double)moments[6] * 18446744073709551616.0L + (long double)moments[5];
+    long double s4 = (long double)moments[8] * 18446744073709551616.0L + (long double)moments[7];
+    if (moments[0] == 0 || s2 == 0.0L) return (double)NAN;
+    return (double)(1.0L - (n * s4) / (3.0L * s2 * s2));
 }
