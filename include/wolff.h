@@ -26,6 +26,10 @@
  *   - Every call returns 0 (WOLFF_OK) or a negative error code; the reason is kept in
  *     a thread-local string returned by wolff_last_error().  Nothing aborts, throws or
  *     prints.  A CUDA error is sticky on the handle (later calls return WOLFF_ECUDA).
+ *     A device-side watchdog abort is sticky on the device: launches queued behind the
+ *     aborted one do nothing, and the next synchronising call returns WOLFF_EINTERNAL.
+ *   - Calls make the handle's device current for their own duration and restore the
+ *     caller's current device before they return.
  *   - A handle is not thread-safe; distinct handles are independent.
  *   - There is no CPU fallback: without a usable CUDA device wolff_create fails.
  */
@@ -92,6 +96,31 @@ WOLFF_API int wolff_get_state(wolff_handle h, uint64_t *update_index, uint64_t *
 /* Set the update index (to resume a chain: lattice + index + seed is the whole state). */
 WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
 
+/* In-kernel measurement -- the paper's "+ measurement" columns ("the time for only spin-update and that
+ * including the measurement of energy and magnetization"; Tables 1-2) and its Binder ratio (Eq. 3,
+ * PAPER.md:159-164).  With wolff_set_option(h, "measure", 1) every wolff_run evaluates E and M after EVERY update
+ * without leaving the persistent kernel, logs them on the device, and adds them to exact integer accumulators:
+ *   - shared-memory-resident kernel: after each update every CTA sums the tiles it holds (the low faces of the tiles are
+ *     exchanged through global memory); cost per update independent of the cluster, a few microseconds;
+ *   - level-synchronous kernel: M changes by -2 s0 |C|; E by 2 * sum over the cluster's boundary bonds (member i,
+ *     non-member j) of s0 s_j, counted in a pass over the update's member list while every member still carries a mark
+ *     in bit 1 of its byte (the role of the flag the paper packs into the spin word); cost
+ *     proportional to the cluster.
+ * Both give exactly the values wolff_observables would return after each update.
+ *
+ * wolff_get_series: the per-update series of the MOST RECENT wolff_run, n_updates entries each: E and M after each
+ * update (needs "measure" = 1 during that run, else WOLFF_EINVAL) and the duration of each update in nanoseconds as
+ * the kernel saw it (always recorded; saturates at 2^32 - 1).  Any pointer may be NULL; host or device.  Blocks. */
+WOLFF_API int wolff_get_series(wolff_handle h, int64_t *E_series, int64_t *M_series, uint32_t *update_ns);
+
+/* Accumulated over all measured updates since creation or the last reset, ten 64-bit words (host pointer):
+ *   [0] n   [1] sum E (two's complement)   [2] sum |M|   [3],[4] sum E^2 (low, high word)
+ *   [5],[6] sum M^2   [7],[8] sum M^4   [9] 0
+ * exact integers (M^4 reaches 2^96 at 2^24 spins, hence 128 bits), and the Binder ratio of PAPER.md Eq. 3,
+ * U = 1 - <M^4> / (3 <M^2>^2), from them (NaN without samples).  Either pointer may be NULL.  Blocks. */
+WOLFF_API int wolff_get_moments(wolff_handle h, uint64_t *moments, double *binder);
+WOLFF_API int wolff_reset_moments(wolff_handle h);
+
 /* Tuning / test knobs; never change the result.  Two growth kernels implement wolff_run:
  *  - the shared-memory-resident, barrier-free kernel (lattice tiles live in the CTAs' shared memory for the
  *    launch, claims across CTAs travel as messages, bond variables come from tables filled ahead of time):
@@ -103,12 +132,16 @@ WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
  *                          (default); level-synchronous kernel only: 4 = tiers by frontier width, 1 = every level
  *                          grid-wide, 2 = one CTA whenever the frontier fits its shared-memory queue, 3 = the
  *                          cluster whenever it fits
+ *   "measure"              1 = E and M after every update inside the kernel (see wolff_get_series); default 0
  *   "small_cluster"        mode 0: when the last finished run (seen at the caller's next synchronising call) had a mean
  *                          cluster below this size, the next run uses the level-synchronous kernel, whose fixed
  *                          cost per update is lower (default 16; 0 = never)
  *   "tile_log"             shared-memory-resident kernel: log2 of the tile side (0 = auto: 6 in 2D, 4 in 3D)
  *   "tile_ctas"            ... CTAs that share the lattice (0 = one per SM)
  *   "ring_cap"             ... entries of a CTA's shared-memory work ring (power of two; overflow spills to global memory)
+ *   "inbox_log"            ... log2 of the entries of a CTA's inbox, the global-memory queue of claims other CTAs send it
+ *                          (0 = auto: what one update can send at most, capped at 12; 5..24).  A sender that finds an
+ *                          inbox full waits for its receiver, which never waits for anybody
  *   "fill"                 ... bond tables: 0 = never (Philox inline), 1 = filled by idle warps when updates are long
  *                          enough to pay for it (default), 2 = always
  *   "fill_bufs"            ... bond-table buffers: 0 = two (the running update and the next one) when they fit beside the

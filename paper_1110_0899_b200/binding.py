@@ -31,6 +31,9 @@ _SIGNATURES = {
     "wolff_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]),
     "wolff_set_update_index": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_uint64]),
     "wolff_set_option": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_char_p, ctypes.c_int64]),
+    "wolff_get_series": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_get_moments": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_double)]),
+    "wolff_reset_moments": (ctypes.c_int, [ctypes.c_void_p]),
     "wolff_get_stats": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]),
     "wolff_microbench": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.c_int]),
     "wolff_destroy": (ctypes.c_int, [ctypes.c_void_p]),
@@ -189,6 +192,36 @@ class Wolff:
 
     def set_option(self, key: str, value: int):
         self._check(self._lib.wolff_set_option(self._h, key.encode(), int(value)))
+
+    # -- in-kernel measurement (set_option("measure", 1))
+    def series_into(self, E=None, M=None, update_ns=None):
+        """wolff_get_series with caller-owned buffers (host or device)."""
+        self._check(self._lib.wolff_get_series(self._h, _ptr(E), _ptr(M), _ptr(update_ns)))
+
+    def series(self):
+        """(E, M) after every update of the most recent (measured) run, numpy int64 arrays on the host."""
+        E = np.empty(self.last_n, dtype=np.int64)
+        M = np.empty(self.last_n, dtype=np.int64)
+        if self.last_n:
+            self.series_into(E, M, None)
+        return E, M
+
+    def update_ns(self) -> np.ndarray:
+        """Duration of every update of the most recent run in nanoseconds, as the kernel saw it."""
+        ns = np.empty(self.last_n, dtype=np.uint32)
+        if self.last_n:
+            self.series_into(None, None, ns)
+        return ns
+
+    def moments(self):
+        """(ten raw 64-bit words, Binder ratio): wolff_get_moments."""
+        buf = (ctypes.c_uint64 * 10)()
+        U = ctypes.c_double()
+        self._check(self._lib.wolff_get_moments(self._h, buf, ctypes.byref(U)))
+        return np.array([int(x) for x in buf], dtype=np.uint64), float(U.value)
+
+    def reset_moments(self):
+        self._check(self._lib.wolff_reset_moments(self._h))
 
     def stats(self) -> dict:
         buf = (ctypes.c_uint64 * NSTATS)()

@@ -13,12 +13,13 @@ LIB_NAME = "libwolff_b200.so"
 LIB_PATH = os.path.join(HERE, LIB_NAME)
 SOURCES = ["api.cu", "growth.cu", "growth_tiles.cu", "measure.cu", "microbench.cu"]
 HEADERS = ["internal.h", "device_common.cuh", "expand.cuh", os.path.join(ROOT, "include", "wolff.h")]
-NVCC_FLAGS = [
+NVCC_COMPILE_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-Xcompiler", "-fPIC,-fvisibility=hidden,-Wall",
-    "--shared", "-cudart", "static",
 ]
+NVCC_LINK_FLAGS = ["--shared", "-cudart", "static", "-gencode", "arch=compute_100a,code=sm_100a"]
+OBJ_DIR = os.path.join(HERE, "build")
 
 
 def nvcc_path() -> str:
@@ -28,26 +29,55 @@ def nvcc_path() -> str:
     raise RuntimeError("nvcc not found: libwolff_b200.so cannot be built (there is no CPU fallback)")
 
 
+def _header_paths():
+    return [h if os.path.isabs(h) else os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
+
+
 def needs_build() -> bool:
     if not os.path.exists(LIB_PATH):
         return True
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + [h if os.path.isabs(h) else os.path.join(CSRC, h) for h in HEADERS]
-    deps.append(os.path.abspath(__file__))
+    deps = [os.path.join(CSRC, s) for s in SOURCES] + _header_paths()
     return os.path.getmtime(LIB_PATH) < max(os.path.getmtime(d) for d in deps)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """One nvcc per source file, side by side (the files share no device code, so there is no device link), then one
+    link.  Objects are kept under paper_1110_0899_b200/build/ (git-ignored) and reused while they are newer than
+    their source and every header."""
     if not force and not needs_build():
         return LIB_PATH
-    tmp = LIB_PATH + ".tmp.%d" % os.getpid()
+    nvcc = nvcc_path()
     extra = os.environ.get("WOLFF_NVCC_EXTRA", "").split()      # e.g. -DWOLFF_PROFILE (per-section cycle counters)
-    cmd = [nvcc_path()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    tag = ("_" + "".join(c if c.isalnum() else "_" for c in " ".join(extra))) if extra else ""
+    newest_header = max(os.path.getmtime(h) for h in _header_paths())
+    jobs = []
+    objs = []
+    for src in SOURCES:
+        path = os.path.join(CSRC, src)
+        obj = os.path.join(OBJ_DIR, os.path.splitext(src)[0] + tag + ".o")
+        objs.append(obj)
+        fresh = os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(path), newest_header)
+        if fresh and not force:
+            continue
+        cmd = [nvcc] + NVCC_COMPILE_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj + ".tmp", path]
+        jobs.append((cmd, obj, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)))
+    failed = []
+    for cmd, obj, proc in jobs:
+        _, err = proc.communicate()
+        if proc.returncode != 0:
+            failed.append("%s\n%s" % (" ".join(cmd), err))
+        else:
+            os.replace(obj + ".tmp", obj)
+            if verbose:
+                sys.stderr.write(err)
+    if failed:
+        raise RuntimeError("nvcc failed:\n" + "\n".join(failed))
+    tmp = LIB_PATH + ".tmp.%d" % os.getpid()
+    cmd = [nvcc] + NVCC_LINK_FLAGS + ["-o", tmp] + objs
     proc = subprocess.run(cmd, capture_output=True, text=True)
     if proc.returncode != 0:
-        raise RuntimeError("nvcc failed:\n%s\n%s" % (" ".join(cmd), proc.stderr))
-    if verbose:
-        sys.stderr.write(proc.stderr)
+        raise RuntimeError("link failed:\n%s\n%s" % (" ".join(cmd), proc.stderr))
     os.replace(tmp, LIB_PATH)
     return LIB_PATH
 

@@ -39,7 +39,12 @@ struct wolff_ctx {
     int8_t *spins = nullptr;
     uint32_t *clist = nullptr;
     uint32_t *sizes = nullptr;
-    uint64_t sizes_cap = 0;         // entries allocated
+    uint32_t *ns_log = nullptr;     // per-update duration of the most recent run
+    long long *E_log = nullptr;     // per-update E, M of the most recent run ("measure" = 1)
+    long long *M_log = nullptr;
+    uint64_t sizes_cap = 0;         // entries allocated in each of the four logs
+    int measure = 0;                // in-kernel measurement after every update
+    bool last_measured = false;     // the most recent run was a measured one
     uint64_t last_n = 0;            // updates in the most recent wolff_run
     Control *ctl = nullptr;
     cudaStream_t last_stream = nullptr;
@@ -63,6 +68,7 @@ struct wolff_ctx {
     int tile_log_opt = 0;           // 0 = auto
     int tile_ctas_opt = 0;          // 0 = one CTA per SM
     uint32_t ring_cap = 2048;
+    int inbox_log_opt = 0;          // 0 = auto (at most 2^12 entries per CTA)
     int fill_mode = 1;              // bond tables: 0 off, 1 adaptive, 2 always
     uint64_t fill_min_us = 30;
     int fill_bufs = 0;              // 0 = two buffers when they fit, else one; 1 = one
@@ -77,6 +83,7 @@ struct wolff_ctx {
     unsigned long long *tile_ctr = nullptr;     // gtail[G], gdone[G], gspill[G], added
     uint32_t *tile_spill = nullptr;
     uint32_t *tile_fill = nullptr;
+    int8_t *tile_faces = nullptr;   // in-kernel measurement: the low faces of every tile
     // kernel choice in mode 0: mean cluster size of the last finished run (read when the caller next synchronises)
     uint64_t small_cluster = 16;    // below this mean size the level-synchronous kernel runs (its fixed cost per update is lower); 0 = never
     bool have_mean = false;
@@ -99,12 +106,28 @@ int fail_cuda(wolff_ctx *h, cudaError_t e, const char *what)
         if (e_ != cudaSuccess) return fail_cuda((h), e_, (what));   \
     } while (0)
 
+// Makes the handle's device current for the length of one API call and puts the caller's device back afterwards
+// (work the caller issues next on this thread must not land on another GPU).
+class DeviceScope {
+public:
+    explicit DeviceScope(const wolff_ctx *h)
+    {
+        if (!h) return;
+        if (cudaGetDevice(&prev_) != cudaSuccess) { cudaGetLastError(); prev_ = -1; }
+        if (prev_ != h->device) { cudaSetDevice(h->device); switched_ = true; }
+    }
+    ~DeviceScope() { if (switched_ && prev_ >= 0) cudaSetDevice(prev_); }
+    DeviceScope(const DeviceScope &) = delete;
+    DeviceScope &operator=(const DeviceScope &) = delete;
+private:
+    int prev_ = -1;
+    bool switched_ = false;
+};
+
 int check_handle(wolff_ctx *h)
 {
     if (!h) { set_error("null handle"); return WOLFF_EINVAL; }
     if (h->cuda_failed) { set_error("handle is in a failed CUDA state"); return WOLFF_ECUDA; }
-    cudaError_t e = cudaSetDevice(h->device);
-    if (e != cudaSuccess) return fail_cuda(h, e, "cudaSetDevice");
     return WOLFF_OK;
 }
 
@@ -159,6 +182,7 @@ void free_tile_state(wolff_ctx *h)
     cudaFree(h->tile_ctr); h->tile_ctr = nullptr;
     cudaFree(h->tile_spill); h->tile_spill = nullptr;
     cudaFree(h->tile_fill); h->tile_fill = nullptr;
+    cudaFree(h->tile_faces); h->tile_faces = nullptr;
 }
 
 uint32_t ceil_log2(uint64_t v) { uint32_t l = 0; while ((1ull << l) < v) ++l; return l; }
@@ -166,7 +190,7 @@ uint32_t ceil_log2(uint64_t v) { uint32_t l = 0; while ((1ull << l) < v) ++l; re
 // (Re)derive the tiling of growth_tiles.cu from the knobs and allocate its inboxes, spill lists and counters.
 // plan_ok == false (L not a power of two, L < 4, or the lattice does not fit the chip's shared memory) is not an
 // error: wolff_run then uses the level-synchronous kernel of growth.cu.
-int refresh_plan(wolff_ctx *h)
+int refresh_plan(wolff_ctx *h, cudaStream_t stream)
 {
     if (!h->plan_dirty) return WOLFF_OK;
     if (h->ran) CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
@@ -205,9 +229,14 @@ int refresh_plan(wolff_ctx *h)
     tp.G = G;
     tp.magicG = ((1ull << 40) + G - 1) / G;
     tp.slots = slots;
-    // messages one update can send to one CTA: every bond across the surface of its tiles once, the seed, the exit
+    // Inbox of a CTA: never more entries than one update can send it (every bond across the surface of its tiles once,
+    // the seed, the exit), and by default at most 2^12 -- a sender that finds the inbox full waits for the receiver
+    // (which never waits for anybody), and a small inbox stays in L2 lines that were touched a moment ago.
     const uint64_t surface = (uint64_t)slots * 2ull * dim * (1ull << ((dim - 1) * b));
     tp.in_log = ceil_log2(surface + 4);
+    const uint32_t in_log_max = h->inbox_log_opt > 0 ? (uint32_t)h->inbox_log_opt : 12u;
+    if (tp.in_log > in_log_max) tp.in_log = in_log_max;
+    if (tp.in_log < 5u) tp.in_log = 5u;              // the receiver looks at 32 slots at a time
     tp.in_cap = 1u << tp.in_log;
     tp.spill_log = ceil_log2((uint64_t)slots << (dim * b));
     tp.ring_cap = h->ring_cap;
@@ -222,48 +251,65 @@ int refresh_plan(wolff_ctx *h)
     h->tile_smem = smem;
 
     const size_t inbox_bytes = ((size_t)G << tp.in_log) * sizeof(unsigned long long);
-    const size_t ctr_bytes = (3 * (size_t)G + 1) * sizeof(unsigned long long);
+    const size_t ctr_bytes = (4 * (size_t)G + 1) * sizeof(unsigned long long);
     const size_t spill_bytes = ((size_t)G << tp.spill_log) * sizeof(uint32_t);
+    // one byte per site of the dim low faces of every tile (indexed by slot * G + owner: slots * G tiles at most)
+    const size_t faces_bytes = (size_t)slots * G * dim * ((size_t)1 << ((dim - 1) * b)) + 16;
     if (cudaMalloc(&h->tile_inbox, inbox_bytes) != cudaSuccess || cudaMalloc(&h->tile_ctr, ctr_bytes) != cudaSuccess ||
-        cudaMalloc(&h->tile_spill, spill_bytes) != cudaSuccess || cudaMalloc(&h->tile_fill, (size_t)G * sizeof(uint32_t)) != cudaSuccess) {
+        cudaMalloc(&h->tile_spill, spill_bytes) != cudaSuccess || cudaMalloc(&h->tile_fill, (size_t)G * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&h->tile_faces, faces_bytes) != cudaSuccess) {
         cudaGetLastError();
         free_tile_state(h);
         return WOLFF_OK;      // not enough memory for the tiled kernel's queues: the level-synchronous kernel needs none
     }
-    CHECK_CUDA(h, cudaMemset(h->tile_inbox, 0, inbox_bytes), "clear inboxes");
-    CHECK_CUDA(h, cudaMemset(h->tile_ctr, 0, ctr_bytes), "clear counters");
-    CHECK_CUDA(h, cudaMemset(h->tile_spill, 0, spill_bytes), "clear spill lists");
-    CHECK_CUDA(h, cudaMemset(h->tile_fill, 0, (size_t)G * sizeof(uint32_t)), "clear fill flags");
-    // The memsets above run on the legacy default stream; the kernel that uses these buffers may be launched on a
-    // non-blocking stream, which does not wait for it: finish them here (a plan is made once per knob change).
-    CHECK_CUDA(h, cudaDeviceSynchronize(), "cudaDeviceSynchronize");
+    // cleared on the stream the kernel is about to be launched on: nothing else on the device has to wait
+    CHECK_CUDA(h, cudaMemsetAsync(h->tile_inbox, 0, inbox_bytes, stream), "clear inboxes");
+    CHECK_CUDA(h, cudaMemsetAsync(h->tile_ctr, 0, ctr_bytes, stream), "clear counters");
+    CHECK_CUDA(h, cudaMemsetAsync(h->tile_spill, 0, spill_bytes, stream), "clear spill lists");
+    CHECK_CUDA(h, cudaMemsetAsync(h->tile_fill, 0, (size_t)G * sizeof(uint32_t), stream), "clear fill flags");
     tp.inbox = h->tile_inbox;
     tp.gtail = reinterpret_cast<unsigned int *>(h->tile_ctr);      // G 32-bit counters in the first G 64-bit words
     tp.gdone = h->tile_ctr + G;
     tp.gspill = h->tile_ctr + 2 * (size_t)G;
-    tp.added = h->tile_ctr + 3 * (size_t)G;
+    tp.gihead = reinterpret_cast<unsigned int *>(h->tile_ctr + 3 * (size_t)G);   // G 32-bit words
+    tp.added = h->tile_ctr + 4 * (size_t)G;
     tp.spill = h->tile_spill;
     tp.gfill = h->tile_fill;
+    tp.faces = h->tile_faces;
     h->plan_ok = true;
+    return WOLFF_OK;
+}
+
+// What the host needs from the control block after a run, read in one copy.
+int read_control(wolff_ctx *h, Control *host, cudaStream_t s)
+{
+    CHECK_CUDA(h, cudaMemcpyAsync(host, h->ctl, sizeof(Control), cudaMemcpyDeviceToHost, s), "read control block");
+    CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+// After a synchronise: the sticky device error flag and the counters of the last run.
+int digest_control(wolff_ctx *h, const Control &c)
+{
+    if (!h->ran) return WOLFF_OK;
+    if (c.error != 0) {
+        set_error("device watchdog: an update or a grid barrier did not complete (error flag %u)", c.error);
+        h->cuda_failed = true;
+        return WOLFF_EINTERNAL;
+    }
+    if (c.stats[0] > 0 && h->run_since_set) { h->have_mean = true; h->mean_cluster = (double)c.stats[1] / (double)c.stats[0]; }
     return WOLFF_OK;
 }
 
 int sync_and_check(wolff_ctx *h)
 {
-    CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
-    if (h->ran) {
-        // error flag and the first two counters (updates, flipped spins) of the last run: 8 + 16 bytes behind one another
-        struct { unsigned int error, pad; unsigned long long updates, flipped; } head;
-        static_assert(offsetof(Control, stats) == offsetof(Control, error) + 8, "Control layout");
-        CHECK_CUDA(h, cudaMemcpy(&head, &h->ctl->error, sizeof(head), cudaMemcpyDeviceToHost), "read error flag");
-        if (head.error != 0) {
-            set_error("device watchdog: a grid barrier did not complete (error flag %u)", head.error);
-            h->cuda_failed = true;
-            return WOLFF_EINTERNAL;
-        }
-        if (head.updates > 0 && h->run_since_set) { h->have_mean = true; h->mean_cluster = (double)head.flipped / (double)head.updates; }
+    if (!h->ran) {
+        CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+        return WOLFF_OK;
     }
-    return WOLFF_OK;
+    Control c;
+    const int rc = read_control(h, &c, h->last_stream);
+    return rc ? rc : digest_control(h, c);
 }
 
 }  // namespace
@@ -330,7 +376,7 @@ wolff_handle wolff_create(int dim, int L, double J, double T, uint64_t seed)
     }
     e = cudaMemset(h->ctl, 0, sizeof(Control));
     if (e == cudaSuccess) e = cudaMemset(h->spins, 0, lattice_bytes);
-    if (e == cudaSuccess) e = launch_init_lattice(h->spins, h->geo.N, seed, nullptr);
+    if (e == cudaSuccess) e = launch_init_lattice(h->spins, h->geo.N, seed, h->num_sms, nullptr);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) {
         set_error("lattice initialisation failed: %s", cudaGetErrorString(e));
@@ -343,11 +389,14 @@ wolff_handle wolff_create(int dim, int L, double J, double T, uint64_t seed)
 int wolff_destroy(wolff_handle h)
 {
     if (!h) return WOLFF_OK;
-    cudaSetDevice(h->device);
+    DeviceScope scope(h);
     if (h->last_stream || h->ran) cudaStreamSynchronize(h->last_stream);
     cudaFree(h->spins);
     cudaFree(h->clist);
     cudaFree(h->sizes);
+    cudaFree(h->ns_log);
+    cudaFree(h->E_log);
+    cudaFree(h->M_log);
     cudaFree(h->ctl);
     free_tile_state(h);
     delete h;
@@ -357,6 +406,7 @@ int wolff_destroy(wolff_handle h)
 int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
 {
     int rc = check_handle(h);
+    DeviceScope scope(h);
     if (rc) return rc;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if (n_updates == 0) return WOLFF_OK;
@@ -369,39 +419,69 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
         if (h->ran) CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
         uint64_t cap = h->sizes_cap ? h->sizes_cap : 1024;
         while (cap < n_updates) cap *= 2;
-        uint32_t *fresh = nullptr;
-        if (cudaMalloc(&fresh, (size_t)cap * sizeof(uint32_t)) != cudaSuccess) {
+        uint32_t *fresh = nullptr, *fresh_ns = nullptr;
+        long long *fresh_E = nullptr, *fresh_M = nullptr;
+        if (cudaMalloc(&fresh, (size_t)cap * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&fresh_ns, (size_t)cap * sizeof(uint32_t)) != cudaSuccess ||
+            cudaMalloc(&fresh_E, (size_t)cap * sizeof(long long)) != cudaSuccess || cudaMalloc(&fresh_M, (size_t)cap * sizeof(long long)) != cudaSuccess) {
             cudaGetLastError();
-            set_error("cannot allocate the cluster-size log for %llu updates", (unsigned long long)n_updates);
+            cudaFree(fresh); cudaFree(fresh_ns); cudaFree(fresh_E); cudaFree(fresh_M);
+            set_error("cannot allocate the per-update logs for %llu updates", (unsigned long long)n_updates);
             return WOLFF_ENOMEM;
         }
-        cudaFree(h->sizes);
-        h->sizes = fresh;
+        cudaFree(h->sizes); cudaFree(h->ns_log); cudaFree(h->E_log); cudaFree(h->M_log);
+        h->sizes = fresh; h->ns_log = fresh_ns; h->E_log = fresh_E; h->M_log = fresh_M;
         h->sizes_cap = cap;
     }
     GrowthParams p{};
     p.spins = h->spins; p.clist = h->clist; p.sizes = h->sizes; p.ctl = h->ctl; p.geo = h->geo;
     p.key0 = (uint32_t)h->seed; p.key1 = (uint32_t)(h->seed >> 32);
     p.thr = h->thr; p.u0 = h->u; p.n_updates = n_updates; p.qcap = h->qcap;
-    // control words of the growth kernels start from zero at every launch (generation 0, no error, no stats)
-    CHECK_CUDA(h, cudaMemsetAsync(h->ctl, 0, offsetof(Control, acc_unequal), stream), "cudaMemsetAsync(control)");
+    p.measure = h->measure ? 1u : 0u;
+    p.claim_bits = 0xFEu;
+    p.E_log = h->E_log; p.M_log = h->M_log; p.ns_log = h->ns_log;
+    // control words of the growth kernels start from zero at every launch (generation 0, no stats); the error flag
+    // is not among them: it is sticky until the host has read it
+    CHECK_CUDA(h, cudaMemsetAsync(h->ctl, 0, kControlClearBytes, stream), "cudaMemsetAsync(control)");
     if (h->mode == 0) {
-        rc = refresh_plan(h);
+        rc = refresh_plan(h, stream);
         if (rc) return rc;
     }
     const bool small = h->small_cluster > 0 && h->have_mean && h->mean_cluster < (double)h->small_cluster;
-    if (h->mode == 0 && h->plan_ok && !small) {
+    bool tiled = h->mode == 0 && h->plan_ok && !small;
+    if (tiled) {
         // shared-memory-resident kernel; a message carries the update index relative to the launch in 29 bits
         const uint64_t chunk = (1ull << 29) - 1;
-        for (uint64_t done = 0; done < n_updates; done += chunk) {
+        for (uint64_t done = 0; done < n_updates && tiled; done += chunk) {
             TileParams tp = h->tp;
             tp.g = p;
             tp.g.u0 = h->u + done;
             tp.g.n_updates = n_updates - done < chunk ? n_updates - done : chunk;
             tp.g.sizes = h->sizes + done;
-            CHECK_CUDA(h, launch_growth_tiles(tp, h->dim, h->tile_smem, stream), "launch tiled growth kernel");
+            tp.g.ns_log = h->ns_log + done;
+            tp.g.E_log = h->E_log + done;
+            tp.g.M_log = h->M_log + done;
+            if (h->measure && tp.idle_ns > 200u) tp.idle_ns = 200u;     // every warp of every CTA is waited for after each update
+            if (done != 0)        // the measurement's arrival counters count from zero in every launch
+                CHECK_CUDA(h, cudaMemsetAsync(&h->ctl->meas_arrive_a, 0, offsetof(Control, error) - offsetof(Control, meas_arrive_a), stream),
+                           "cudaMemsetAsync(measurement counters)");
+            const cudaError_t e = launch_growth_tiles(tp, h->dim, h->tile_smem, stream);
+            if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorLaunchOutOfResources || e == cudaErrorInvalidConfiguration) {
+                // the SMs cannot all be had right now (another context holds some): not a fault of the handle.
+                // Nothing has run when the first launch is refused, so the level-synchronous kernel takes the call.
+                cudaGetLastError();
+                if (done == 0) { tiled = false; break; }
+            }
+            CHECK_CUDA(h, e, "launch tiled growth kernel");
         }
-    } else {
+    }
+    if (!tiled) {
+        if (h->measure) {
+            // the level-synchronous kernel keeps running E and M: it starts from a whole-lattice evaluation (into the
+            // control block) and marks the members of the running cluster in the spin bytes (claim_with_bits)
+            p.claim_bits = 0xFCu;
+            CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, nullptr, nullptr, h->num_sms, stream),
+                       "launch E/M reduction");
+        }
         effective_thresholds(h, &p);
         rc = refresh_shape(h);
         if (rc) return rc;
@@ -413,6 +493,7 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     }
     h->u += n_updates;
     h->last_n = n_updates;
+    h->last_measured = h->measure != 0;
     h->last_stream = stream;
     h->ran = true;
     h->run_since_set = true;
@@ -422,59 +503,42 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
 int wolff_observables(wolff_handle h, int64_t *E, int64_t *M, uint32_t *cluster_sizes)
 {
     int rc = check_handle(h);
+    DeviceScope scope(h);
     if (rc) return rc;
     cudaStream_t s = h->last_stream;
-    // Everything is queued behind the last run on its stream; ONE small device-to-host copy then brings the error
-    // flag, the run's first counters and E, M (they sit within 296 bytes of the control block), and one
-    // synchronise ends the call.
-    if (E || M) CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, h->num_sms, s), "launch E/M reduction");
-    if (cluster_sizes && h->last_n > 0)
-        CHECK_CUDA(h, cudaMemcpyAsync(cluster_sizes, h->sizes, (size_t)h->last_n * sizeof(uint32_t), cudaMemcpyDefault, s),
-                   "copy cluster sizes");
-    constexpr size_t span = offsetof(Control, M) + sizeof(long long) - offsetof(Control, error);
-    unsigned char head[span];
-    CHECK_CUDA(h, cudaMemcpyAsync(head, &h->ctl->error, span, cudaMemcpyDeviceToHost, s), "read control block");
-    CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
-    unsigned int err = 0;
-    unsigned long long updates = 0, flipped = 0;
-    long long Ev = 0, Mv = 0;
-    memcpy(&err, head, sizeof(err));
-    memcpy(&updates, head + (offsetof(Control, stats) - offsetof(Control, error)), sizeof(updates));
-    memcpy(&flipped, head + (offsetof(Control, stats) - offsetof(Control, error)) + 8, sizeof(flipped));
-    memcpy(&Ev, head + (offsetof(Control, E) - offsetof(Control, error)), sizeof(Ev));
-    memcpy(&Mv, head + (offsetof(Control, M) - offsetof(Control, error)), sizeof(Mv));
-    if (h->ran) {
-        if (err != 0) {
-            set_error("device watchdog: an update or a grid barrier did not complete (error flag %u)", err);
-            h->cuda_failed = true;
-            return WOLFF_EINTERNAL;
-        }
-        if (updates > 0 && h->run_since_set) { h->have_mean = true; h->mean_cluster = (double)flipped / (double)updates; }
-    }
-    // E and M go to host or device memory, whichever the caller passed
+    // Everything is queued behind the last run on its stream.  E and M: a destination in device memory is written by
+    // the reduction kernel itself (its last CTA); a host destination is filled from the ONE small device-to-host copy
+    // that also brings the error flag and the run's counters.  One synchronise ends the call.
+    long long *dev_dst[2] = {nullptr, nullptr};
     int64_t *const dst[2] = {E, M};
-    const long long val[2] = {Ev, Mv};
-    const long long *const src[2] = {&h->ctl->E, &h->ctl->M};
-    bool queued = false;
     for (int k = 0; k < 2; ++k) {
         if (!dst[k]) continue;
         cudaPointerAttributes attr{};
         const cudaError_t e = cudaPointerGetAttributes(&attr, dst[k]);
         if (e != cudaSuccess) cudaGetLastError();
-        if (e == cudaSuccess && (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged)) {
-            CHECK_CUDA(h, cudaMemcpyAsync(dst[k], src[k], sizeof(int64_t), cudaMemcpyDeviceToDevice, s), "copy E/M");
-            queued = true;
-        } else {
-            *dst[k] = (int64_t)val[k];
-        }
+        if (e == cudaSuccess && (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged))
+            dev_dst[k] = reinterpret_cast<long long *>(dst[k]);
     }
-    if (queued) CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    if (E || M)
+        CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, dev_dst[0], dev_dst[1], h->num_sms, s),
+                   "launch E/M reduction");
+    if (cluster_sizes && h->last_n > 0)
+        CHECK_CUDA(h, cudaMemcpyAsync(cluster_sizes, h->sizes, (size_t)h->last_n * sizeof(uint32_t), cudaMemcpyDefault, s),
+                   "copy cluster sizes");
+    Control c;
+    rc = read_control(h, &c, s);
+    if (rc) return rc;
+    rc = digest_control(h, c);
+    if (rc) return rc;
+    for (int k = 0; k < 2; ++k)
+        if (dst[k] && !dev_dst[k]) *dst[k] = (int64_t)(k == 0 ? c.E : c.M);
     return WOLFF_OK;
 }
 
 int wolff_get_spins(wolff_handle h, int8_t *dst)
 {
     int rc = check_handle(h);
+    DeviceScope scope(h);
     if (rc) return rc;
     if (!dst) { set_error("dst is NULL"); return WOLFF_EINVAL; }
     rc = sync_and_check(h);
@@ -487,6 +551,7 @@ int wolff_get_spins(wolff_handle h, int8_t *dst)
 int wolff_set_spins(wolff_handle h, const int8_t *src)
 {
     int rc = check_handle(h);
+    DeviceScope scope(h);
     if (rc) return rc;
     if (!src) { set_error("src is NULL"); return WOLFF_EINVAL; }
     rc = sync_and_check(h);
@@ -496,7 +561,7 @@ int wolff_set_spins(wolff_handle h, const int8_t *src)
     int8_t *staging = reinterpret_cast<int8_t *>(h->clist);
     CHECK_CUDA(h, cudaMemcpyAsync(staging, src, (size_t)h->N, cudaMemcpyDefault, s), "copy lattice in");
     CHECK_CUDA(h, cudaMemsetAsync(&h->ctl->invalid, 0, sizeof(unsigned int), s), "reset validation flag");
-    CHECK_CUDA(h, launch_validate(staging, h->geo.N, h->ctl, s), "launch validation");
+    CHECK_CUDA(h, launch_validate(staging, h->geo.N, h->ctl, h->num_sms, s), "launch validation");
     unsigned int invalid = 0;
     CHECK_CUDA(h, cudaMemcpyAsync(&invalid, &h->ctl->invalid, sizeof(invalid), cudaMemcpyDeviceToHost, s), "read validation flag");
     CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
@@ -526,6 +591,7 @@ int wolff_set_update_index(wolff_handle h, uint64_t update_index)
 int wolff_set_option(wolff_handle h, const char *key, int64_t value)
 {
     if (!h || !key) { set_error("null handle or key"); return WOLFF_EINVAL; }
+    DeviceScope scope(h);
     const uint32_t up_max = cta_capacity(h);
     if (!strcmp(key, "mode")) {
         if (value < 0 || value > 4) { set_error("mode must be 0, 1, 2, 3 or 4"); return WOLFF_EINVAL; }
@@ -565,6 +631,13 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
         if (value < 32 || value > 32768 || (value & (value - 1)) != 0) { set_error("ring_cap must be a power of two in [32, 32768]"); return WOLFF_EINVAL; }
         h->ring_cap = (uint32_t)value;
         h->plan_dirty = true;
+    } else if (!strcmp(key, "measure")) {
+        if (value != 0 && value != 1) { set_error("measure must be 0 or 1"); return WOLFF_EINVAL; }
+        h->measure = (int)value;
+    } else if (!strcmp(key, "inbox_log")) {
+        if (value != 0 && (value < 5 || value > 24)) { set_error("inbox_log must be 0 (auto) or in [5, 24]"); return WOLFF_EINVAL; }
+        h->inbox_log_opt = (int)value;
+        h->plan_dirty = true;
     } else if (!strcmp(key, "up_threshold")) {
         if (value < 0 || value > (int64_t)up_max) { set_error("up_threshold must be in [0, %u]", up_max); return WOLFF_EINVAL; }
         h->up = (uint32_t)value;
@@ -591,7 +664,7 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
         const int before = h->cluster_ctas;
         h->cluster_ctas = (int)value;
         h->shape_dirty = true;
-        if (check_handle(h) != WOLFF_OK || refresh_shape(h) != WOLFF_OK) {
+        if (refresh_shape(h) != WOLFF_OK) {
             h->cluster_ctas = before;
             h->shape_dirty = true;
             return WOLFF_EINVAL;
@@ -600,7 +673,7 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
         if (value != 0 && value != 1) { set_error("speculative must be 0 or 1"); return WOLFF_EINVAL; }
         h->spec = (int)value;
         h->shape_dirty = true;
-        if (check_handle(h) != WOLFF_OK || refresh_shape(h) != WOLFF_OK) return WOLFF_EINVAL;
+        if (refresh_shape(h) != WOLFF_OK) return WOLFF_EINVAL;
     } else if (!strcmp(key, "cooperative")) {
         if (value != 0 && value != 1) { set_error("cooperative must be 0 or 1"); return WOLFF_EINVAL; }
         h->cooperative = (int)value;
@@ -611,15 +684,73 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
     return WOLFF_OK;
 }
 
+int wolff_get_series(wolff_handle h, int64_t *E_series, int64_t *M_series, uint32_t *update_ns)
+{
+    int rc = check_handle(h);
+    DeviceScope scope(h);
+    if (rc) return rc;
+    if ((E_series || M_series) && h->ran && !h->last_measured) {
+        set_error("the most recent wolff_run was not a measured one (wolff_set_option \"measure\" = 1)");
+        return WOLFF_EINVAL;
+    }
+    cudaStream_t s = h->last_stream;
+    const size_t n = h->ran ? (size_t)h->last_n : 0;
+    if (n) {
+        if (E_series) CHECK_CUDA(h, cudaMemcpyAsync(E_series, h->E_log, n * sizeof(int64_t), cudaMemcpyDefault, s), "copy E series");
+        if (M_series) CHECK_CUDA(h, cudaMemcpyAsync(M_series, h->M_log, n * sizeof(int64_t), cudaMemcpyDefault, s), "copy M series");
+        if (update_ns) CHECK_CUDA(h, cudaMemcpyAsync(update_ns, h->ns_log, n * sizeof(uint32_t), cudaMemcpyDefault, s), "copy update times");
+    }
+    return sync_and_check(h);
+}
+
+int wolff_get_moments(wolff_handle h, uint64_t *moments, double *binder)
+{
+    int rc = check_handle(h);
+    DeviceScope scope(h);
+    if (rc) return rc;
+    Control c;
+    rc = read_control(h, &c, h->last_stream);
+    if (rc) return rc;
+    rc = digest_control(h, c);
+    if (rc) return rc;
+    if (moments) memcpy(moments, c.moments, sizeof(c.moments));
+    if (binder) {
+        // Eq. 3: U = 1 - <M^4> / (3 <M^2>^2) = 1 - n S4 / (3 S2^2)
+        const long double two64 = 18446744073709551616.0L;
+        const long double n = (long double)c.moments[0];
+        const long double s2 = (long double)c.moments[6] * two64 + (long double)c.moments[5];
+        const long double s4 = (long double)c.moments[8] * two64 + (long double)c.moments[7];
+        *binder = (c.moments[0] == 0 || s2 == 0.0L) ? std::nan("") : (double)(1.0L - (n * s4) / (3.0L * s2 * s2));
+    }
+    return WOLFF_OK;
+}
+
+int wolff_reset_moments(wolff_handle h)
+{
+    int rc = check_handle(h);
+    DeviceScope scope(h);
+    if (rc) return rc;
+    rc = sync_and_check(h);
+    if (rc) return rc;
+    CHECK_CUDA(h, cudaMemsetAsync(h->ctl->moments, 0, sizeof(h->ctl->moments), h->last_stream), "clear moments");
+    CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
 int wolff_get_stats(wolff_handle h, uint64_t *stats)
 {
     int rc = check_handle(h);
+    DeviceScope scope(h);
     if (rc) return rc;
     if (!stats) { set_error("stats is NULL"); return WOLFF_EINVAL; }
-    rc = sync_and_check(h);
-    if (rc) return rc;
     if (!h->ran) { memset(stats, 0, WOLFF_NSTATS * sizeof(uint64_t)); return WOLFF_OK; }
-    CHECK_CUDA(h, cudaMemcpy(stats, h->ctl->stats, WOLFF_NSTATS * sizeof(uint64_t), cudaMemcpyDeviceToHost), "read stats");
+    Control c;
+    rc = read_control(h, &c, h->last_stream);
+    if (rc) return rc;
+    rc = digest_control(h, c);
+    if (rc) return rc;
+    static_assert(sizeof(c.stats) == WOLFF_NSTATS * sizeof(uint64_t), "stats layout");
+    memcpy(stats, c.stats, sizeof(c.stats));
     return WOLFF_OK;
 }
 

@@ -139,6 +139,59 @@ __device__ __forceinline__ bool claim_and_flip(int8_t *spins, uint32_t j, int s0
     return ((old >> shift) & 0xFFu) == ((unsigned int)s0 & 0xFFu);
 }
 
+// Claim with an explicit bit pattern (in-kernel measurement, growth.cu / growth_batch.cu): claim_bits = 0xFE is
+// claim_and_flip(); claim_bits = 0xFC leaves bit 1 as it was, so a spin claimed in the RUNNING update reads 0xFD
+// (was +1, now -1) or 0x03 (was -1, now +1): its sign (bit 7) is already the new one, and bit 1 != bit 7 marks it as
+// a member of the running cluster -- the role of the flag the paper packs into the spin word -- until
+// the update's post-pass has counted the cluster's boundary bonds and stored the plain value.
+__device__ __forceinline__ bool claim_with_bits(int8_t *spins, uint32_t j, int s0, unsigned int claim_bits)
+{
+    unsigned int *word = reinterpret_cast<unsigned int *>(spins) + (j >> 2);
+    const unsigned int shift = (j & 3u) * 8u;
+    unsigned int old;
+    if (s0 > 0) old = atomicOr(word, claim_bits << shift);
+    else        old = atomicAnd(word, ~(claim_bits << shift));
+    return ((old >> shift) & 0xFFu) == ((unsigned int)s0 & 0xFFu);
+}
+__device__ __forceinline__ bool is_marked_member(unsigned int byte) { return (((byte >> 1) ^ (byte >> 7)) & 1u) != 0u; }
+
+// ---------------------------------------------------------------- measurement (Eq. 3)
+// Accumulated sums of the measured series, ten 64-bit words (layout of wolff_get_moments):
+// [0] n  [1] sum E  [2] sum |M|  [3..4] sum E^2  [5..6] sum M^2  [7..8] sum M^4 (low, high)  [9] reserved.
+// M^4 reaches 2^96 at N = 2^24, so the even moments are exact 128-bit integers.
+struct Moments {
+    unsigned long long n = 0, sum_absM = 0;
+    long long sum_E = 0;
+    unsigned __int128 sum_E2 = 0, sum_M2 = 0, sum_M4 = 0;
+
+    __device__ __forceinline__ void load(const unsigned long long *w)
+    {
+        n = w[0]; sum_E = (long long)w[1]; sum_absM = w[2];
+        sum_E2 = ((unsigned __int128)w[4] << 64) | w[3];
+        sum_M2 = ((unsigned __int128)w[6] << 64) | w[5];
+        sum_M4 = ((unsigned __int128)w[8] << 64) | w[7];
+    }
+    __device__ __forceinline__ void store(unsigned long long *w) const
+    {
+        w[0] = n; w[1] = (unsigned long long)sum_E; w[2] = sum_absM;
+        w[3] = (unsigned long long)sum_E2; w[4] = (unsigned long long)(sum_E2 >> 64);
+        w[5] = (unsigned long long)sum_M2; w[6] = (unsigned long long)(sum_M2 >> 64);
+        w[7] = (unsigned long long)sum_M4; w[8] = (unsigned long long)(sum_M4 >> 64);
+        w[9] = 0ull;
+    }
+    __device__ __forceinline__ void add(long long E, long long M)
+    {
+        const unsigned long long aM = (unsigned long long)(M < 0 ? -M : M), aE = (unsigned long long)(E < 0 ? -E : E);
+        const unsigned __int128 m2 = (unsigned __int128)aM * aM;
+        n += 1ull;
+        sum_E += E;
+        sum_absM += aM;
+        sum_E2 += (unsigned __int128)aE * aE;
+        sum_M2 += m2;
+        sum_M4 += m2 * m2;
+    }
+};
+
 // ---------------------------------------------------------------- inter-CTA synchronisation words
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long *p)
 {
@@ -160,6 +213,12 @@ __device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long
 {
     unsigned long long v;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int *p)
+{
+    unsigned int v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void fence_acq_rel_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }

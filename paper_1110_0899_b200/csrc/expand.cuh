@@ -103,11 +103,11 @@ __device__ __forceinline__ void claim_neighbours(const GrowthParams &p, int s0, 
     if (s0 > 0) {   // uniform for the whole update
 #pragma unroll
         for (int k = 0; k < 2 * DIM; ++k)
-            if (cand[k]) old[k] = atomicOr(words + (nbr[k] >> 2), 0xFEu << ((nbr[k] & 3u) * 8u));
+            if (cand[k]) old[k] = atomicOr(words + (nbr[k] >> 2), p.claim_bits << ((nbr[k] & 3u) * 8u));
     } else {
 #pragma unroll
         for (int k = 0; k < 2 * DIM; ++k)
-            if (cand[k]) old[k] = atomicAnd(words + (nbr[k] >> 2), ~(0xFEu << ((nbr[k] & 3u) * 8u)));
+            if (cand[k]) old[k] = atomicAnd(words + (nbr[k] >> 2), ~(p.claim_bits << ((nbr[k] & 3u) * 8u)));
     }
     const unsigned int s0_byte = (unsigned int)s0 & 0xFFu;
 #pragma unroll
@@ -116,6 +116,32 @@ __device__ __forceinline__ void claim_neighbours(const GrowthParams &p, int s0, 
         attempts += cand[k] ? 1u : 0u;
         won |= w ? (1u << k) : 0u;
     }
+}
+
+// Post-pass of a measured update (in-kernel measurement, growth.cu / growth_batch.cu): this thread's share of
+//   sum over members i, over the 2*DIM bonds (i, j) with j NOT a member, of (+1 if s_j == s0 else -1)
+// for the members list[first], list[first + step], ... below `size`.  Flipping the cluster changes exactly the
+// bonds between a member and a non-member, from -s0*s_j to +s0*s_j, so dE = 2 * (that sum) in units of J.  Called
+// after the cluster is complete and before the marks are removed: members read 0xFD / 0x03 (claim_with_bits).
+template <int DIM, bool POW2>
+__device__ __forceinline__ int boundary_partial(const Geometry &geo, const int8_t *spins, const uint32_t *list, int s0,
+                                                uint32_t size, uint32_t first, uint32_t step)
+{
+    int acc = 0;
+    const unsigned int want_negative = s0 < 0 ? 1u : 0u;
+    for (uint32_t e = first; e < size; e += step) {
+        const uint32_t i = __ldcg(list + e);
+        uint32_t x, y, z, nbr[2 * DIM];
+        site_coords<DIM, POW2>(geo, i, x, y, z);
+        neighbours_at<DIM>(geo, i, x, y, z, nbr);
+        unsigned int b[2 * DIM];
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k) b[k] = (unsigned int)__ldcg(reinterpret_cast<const unsigned char *>(spins) + nbr[k]);
+#pragma unroll
+        for (int k = 0; k < 2 * DIM; ++k)
+            if (!is_marked_member(b[k])) acc += ((b[k] >> 7) == want_negative) ? 1 : -1;
+    }
+    return acc;
 }
 
 // A2-A5 for one site per lane: claim_neighbours, then append the winners to dst[] with ONE atomic per

@@ -29,6 +29,12 @@ namespace {
 
 constexpr int kMaxClusterCtas = 16;
 
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 __device__ __forceinline__ unsigned long long pack_bar(unsigned int gen, unsigned int phase, unsigned int hi)
 {
     return ((unsigned long long)(gen & 0xFFFFFFu) << 40) | ((unsigned long long)(phase & 0xFFu) << 32) |
@@ -115,6 +121,7 @@ struct Command {
     int s0;                    // seed spin of the current update
     unsigned int u_lo, u_hi;   // update index
     unsigned int n;            // entries the master holds in its buffer `par`
+    unsigned int size0;        // members of the cluster so far (measured runs: the member log clist[0, size0) ends with those n)
 };
 
 // Per-CTA shared state.
@@ -126,6 +133,7 @@ struct SharedState {
     unsigned int lcnt[3];      // one-CTA mode: rotating level counters
     Command cmd;
     unsigned long long word;   // broadcast: grid barrier word
+    unsigned long long post_acc;   // measured runs: boundary-bond sum of the post-pass (two's complement)
 };
 
 enum CommandOp : unsigned int { kCmdCluster = 1, kCmdExit = 2 };
@@ -212,7 +220,7 @@ enum Outcome : unsigned int { kOutDone = 0, kOutToCta = 1, kOutAbort = 2 };
 template <int DIM, bool POW2, bool SPEC>
 __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, SharedState &sh, uint32_t *q0, uint32_t *q1,
                                                        unsigned int R, unsigned int r, int s0, uint32_t u_lo, uint32_t u_hi,
-                                                       unsigned int par, unsigned long long &added, Counters &c)
+                                                       unsigned int par, uint32_t size0, unsigned long long &added, Counters &c)
 {
     constexpr int T = kGrowthThreads;
     const unsigned int tid = threadIdx.x;
@@ -235,12 +243,20 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
             n += cq[q];
             maxq = cq[q] > maxq ? cq[q] : maxq;
         }
-        if (!first) added += n;
+        uint32_t *const cur = par ? q1 : q0;
+        uint32_t *const nxt = par ? q0 : q1;
+        if (!first) {
+            added += n;
+            // measured runs: the member log (clist) takes this level's sites; whoever hands a frontier to this loop
+            // has logged it already
+            if (p.measure) {
+                const uint32_t base = size0 + (uint32_t)(added - n) + before;
+                for (unsigned int e = tid; e < mine; e += T) p.clist[base + e] = cur[e];
+            }
+        }
         first = false;
         if (n == 0u) return kOutDone;
         if (n > c.widest) c.widest = n;
-        uint32_t *const cur = par ? q1 : q0;
-        uint32_t *const nxt = par ? q0 : q1;
         const uint32_t sh_cur = par ? sh_q1 : sh_q0;
 
         if (n <= p.down) {
@@ -264,21 +280,25 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
         const bool fits_local = maxq * (2u * DIM) <= p.qcap;
         const bool fits_shared = per * (2u * DIM) <= p.qcap;
         if (n > p.cl_up || !fits_shared) {
-            // ---- grid phase: spill the queues into the window [0, n) of the global list
-            for (unsigned int e = tid; e < mine; e += T) p.clist[before + e] = cur[e];
+            // ---- grid phase over a window of the global list: [0, n), filled from the queues now -- or, in a measured
+            // run, the end of the member log, where this frontier already sits: [S - n, S), S = members so far
+            const uint32_t S = size0 + (uint32_t)added;
+            const uint32_t lo0 = p.measure ? S - n : 0u, hi0 = p.measure ? S : n;
+            if (!p.measure)
+                for (unsigned int e = tid; e < mine; e += T) p.clist[before + e] = cur[e];
             if (r == 0u && tid == 0) {
-                st_relaxed_u32(&ctl->tail, n);
-                st_relaxed_u32(&ctl->lo, 0u);
+                st_relaxed_u32(&ctl->tail, hi0);
+                st_relaxed_u32(&ctl->lo, lo0);
                 st_relaxed_u32(reinterpret_cast<unsigned int *>(&ctl->s0), (unsigned int)s0);
                 ctl->u = ((unsigned long long)u_hi << 32) | u_lo;
             }
             __threadfence();
             cluster_sync();
-            if (r == 0u && tid == 0) st_release_u64(&ctl->bar, pack_bar(c.gen + 1u, kPhaseGrid, n));
+            if (r == 0u && tid == 0) st_release_u64(&ctl->bar, pack_bar(c.gen + 1u, kPhaseGrid, hi0));
             ++c.gen;
-            uint32_t lo = 0u, hi = n;
+            uint32_t lo = lo0, hi = hi0;
             const unsigned int out = grid_levels<DIM, POW2, SPEC>(p, sh, s0, u_lo, u_hi, lo, hi, c);
-            added += (unsigned long long)(hi - n);
+            added += (unsigned long long)(hi - hi0);
             if (out == kPhaseAbort) return kOutAbort;
             if (out == kPhaseDone) return kOutDone;
             // ---- frontier narrowed: window [lo, hi) goes back into the cluster's queues, equal shares
@@ -353,7 +373,7 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
 
 // Store the command block into CTA `target` of the cluster (called by the master, one lane per target).
 __device__ __forceinline__ void send_command(SharedState &sh, unsigned int target, unsigned int op, unsigned int par, int s0,
-                                             uint32_t u_lo, uint32_t u_hi, unsigned int n)
+                                             uint32_t u_lo, uint32_t u_hi, unsigned int n, unsigned int size0)
 {
     const uint32_t cb = map_to_rank(smem_addr(&sh.cmd), target);
     st_dsmem_u32(cb + (uint32_t)offsetof(Command, op), op);
@@ -362,6 +382,7 @@ __device__ __forceinline__ void send_command(SharedState &sh, unsigned int targe
     st_dsmem_u32(cb + (uint32_t)offsetof(Command, u_lo), u_lo);
     st_dsmem_u32(cb + (uint32_t)offsetof(Command, u_hi), u_hi);
     st_dsmem_u32(cb + (uint32_t)offsetof(Command, n), n);
+    st_dsmem_u32(cb + (uint32_t)offsetof(Command, size0), size0);
 }
 
 // Entry into a cluster phase, run by every CTA of cluster 0 after the barrier that delivered the
@@ -387,6 +408,8 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
     const bool in_cluster0 = cluster_id_x() == 0u;
     Control *ctl = p.ctl;
     Counters c;
+    // sticky error flag: an earlier launch of this handle was aborted and the host has not yet looked
+    if (ld_relaxed_u32(&ctl->error) != 0u) return;
 
     if (!in_cluster0) {
         // ---------------------------------------------------------------- worker CTAs: grid phases only
@@ -397,7 +420,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
             __syncthreads();
             ++c.gen;
             if (bar_phase(w) != kPhaseGrid) break;   // exit or abort
-            uint32_t lo = 0u, hi = bar_hi(w);
+            uint32_t lo = ld_relaxed_u32(&ctl->lo), hi = bar_hi(w);
             const int s0 = (int)ld_relaxed_u32(reinterpret_cast<unsigned int *>(&ctl->s0));
             const unsigned long long u = __ldcg(&ctl->u);
             const unsigned int out = grid_levels<DIM, POW2, SPEC>(p, sh, s0, (uint32_t)u, (uint32_t)(u >> 32), lo, hi, c);
@@ -418,7 +441,7 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
             const uint32_t u_lo = sh.cmd.u_lo, u_hi = sh.cmd.u_hi;
             begin_cluster_phase(sh, par, sh.cmd.n);
             unsigned long long added = 0;
-            const unsigned int out = cluster_levels<DIM, POW2, SPEC>(p, sh, q0, q1, R, r, s0, u_lo, u_hi, par, added, c);
+            const unsigned int out = cluster_levels<DIM, POW2, SPEC>(p, sh, q0, q1, R, r, s0, u_lo, u_hi, par, sh.cmd.size0, added, c);
             if (out == kOutAbort) break;
         }
         if (c.attempts) atomicAdd(&ctl->stats[7], (unsigned long long)c.attempts);
@@ -428,16 +451,23 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
     // -------------------------------------------------------------------- master CTA: the update loop
     unsigned long long flipped = 0, levels_cta = 0, to_cluster = 0;
     bool aborted = false;
+    // measured runs (thread 0): running E and M, from the whole-lattice reduction the host queued before this launch
+    long long runE = 0, runM = 0;
+    Moments mom;
+    if (p.measure && tid == 0) { runE = ctl->E; runM = ctl->M; mom.load(ctl->moments); }
     for (unsigned long long k = 0; k < p.n_updates && !aborted; ++k) {
         const unsigned long long u = p.u0 + k;
         const uint32_t u_lo = (uint32_t)u, u_hi = (uint32_t)(u >> 32);
+        unsigned long long t_start = 0;
         // A1: seed draw (reading R8) and initial flip
         if (tid == 0) {
+            t_start = globaltimer_ns();
             const uint4 x = philox4x32_10(0u, kDomainSite, u_lo, u_hi, p.key0, p.key1);
             const unsigned long long rr = (unsigned long long)x.x | ((unsigned long long)x.y << 32);
             const uint32_t i0 = (uint32_t)__umul64hi(rr, (unsigned long long)p.geo.N);
             const int s = load_spin_l2(p.spins, i0);
-            claim_and_flip(p.spins, i0, s);
+            claim_with_bits(p.spins, i0, s, p.claim_bits);
+            if (p.measure) p.clist[0] = i0;
             q0[0] = i0;
             sh.lcnt[0] = 1u;
             sh.lcnt[1] = 0u;
@@ -457,11 +487,11 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
                 ++to_cluster;
                 const unsigned int par = (cur == q1) ? 1u : 0u;
                 __syncthreads();                                      // everybody has read lcnt/cmd of this level
-                if (tid < R) send_command(sh, tid, kCmdCluster, par, s0, u_lo, u_hi, n);
+                if (tid < R) send_command(sh, tid, kCmdCluster, par, s0, u_lo, u_hi, n, (unsigned int)size);
                 cluster_sync();
                 begin_cluster_phase(sh, par, n);
                 unsigned long long added = 0;
-                const unsigned int out = cluster_levels<DIM, POW2, SPEC>(p, sh, q0, q1, R, 0u, s0, u_lo, u_hi, par, added, c);
+                const unsigned int out = cluster_levels<DIM, POW2, SPEC>(p, sh, q0, q1, R, 0u, s0, u_lo, u_hi, par, (uint32_t)size, added, c);
                 size += added;
                 if (out == kOutAbort) { aborted = true; break; }
                 if (out == kOutDone) break;
@@ -480,18 +510,45 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
                 expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, &sh.lcnt[lvl1], c.attempts);
             }
             __syncthreads();
-            size += sh.lcnt[lvl1];
+            const unsigned int n1 = sh.lcnt[lvl1];
+            if (p.measure)                                            // member log of a measured run
+                for (unsigned int e = tid; e < n1; e += T) p.clist[(uint32_t)size + e] = nxt[e];
+            size += n1;
             lvl = lvl1;
             uint32_t *t = cur; cur = nxt; nxt = t;
         }
+        if (p.measure && !aborted) {
+            // ---- post-pass of a measured update: dE from the cluster's boundary bonds (every member still carries its
+            // mark), then the marks go: members get their plain value -s0.  M changes by -2 s0 |C|.
+            if (tid == 0) sh.post_acc = 0ull;
+            __syncthreads();
+            int part = boundary_partial<DIM, POW2>(p.geo, p.spins, p.clist, s0, (uint32_t)size, tid, (uint32_t)T);
+            part = __reduce_add_sync(kFullMask, part);
+            if ((tid & 31u) == 0u && part != 0) atomicAdd(&sh.post_acc, (unsigned long long)(long long)part);
+            __syncthreads();
+            const int8_t plain = (int8_t)(-s0);
+            for (uint32_t e = tid; e < (uint32_t)size; e += T) p.spins[__ldcg(p.clist + e)] = plain;
+            if (tid == 0) {
+                runE += 2ll * (long long)sh.post_acc;
+                runM -= 2ll * (long long)s0 * (long long)size;
+                p.E_log[k] = runE;
+                p.M_log[k] = runM;
+                mom.add(runE, runM);
+            }
+        }
         // A7: epilogue
-        if (tid == 0) p.sizes[k] = (uint32_t)size;
+        if (tid == 0) {
+            p.sizes[k] = (uint32_t)size;
+            const unsigned long long dt = globaltimer_ns() - t_start;
+            p.ns_log[k] = dt > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)dt;
+        }
         flipped += size;
         __syncthreads();
     }
+    if (p.measure && tid == 0) { ctl->E = runE; ctl->M = runM; mom.store(ctl->moments); }
     if (!aborted) {
         if (tid == 0) st_release_u64(&ctl->bar, pack_bar(c.gen + 1u, kPhaseExit, 0u));   // workers leave
-        if (tid < R) send_command(sh, tid, kCmdExit, 0u, 0, 0u, 0u, 0u);                 // helpers leave
+        if (tid < R) send_command(sh, tid, kCmdExit, 0u, 0, 0u, 0u, 0u, 0u);                 // helpers leave
         cluster_sync();
     }
     if (tid == 0) {
@@ -508,26 +565,6 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
 #endif
     }
     if (c.attempts) atomicAdd(&ctl->stats[7], (unsigned long long)c.attempts);
-}
-
-template <int DIM, bool POW2, bool SPEC>
-cudaError_t launch_one(const GrowthParams &p, const GrowthLaunch &l, cudaStream_t stream)
-{
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned int)l.grid_ctas);
-    cfg.blockDim = dim3(kGrowthThreads);
-    cfg.dynamicSmemBytes = l.smem_bytes;
-    cfg.stream = stream;
-    cudaLaunchAttribute attrs[2];
-    attrs[0].id = cudaLaunchAttributeClusterDimension;
-    attrs[0].val.clusterDim.x = (unsigned int)l.cluster_ctas;
-    attrs[0].val.clusterDim.y = 1;
-    attrs[0].val.clusterDim.z = 1;
-    attrs[1].id = cudaLaunchAttributeCooperative;     // all CTAs co-resident: the grid barrier needs it
-    attrs[1].val.cooperative = 1;
-    cfg.attrs = attrs;
-    cfg.numAttrs = l.cooperative ? 2 : 1;
-    return cudaLaunchKernelEx(&cfg, growth_kernel<DIM, POW2, SPEC>, p);
 }
 
 template <int DIM, bool POW2, bool SPEC>
@@ -555,6 +592,29 @@ cudaError_t prepare_one(const GrowthLaunch &l, int *max_clusters)
         e = cudaOccupancyMaxActiveClusters(max_clusters, growth_kernel<DIM, POW2, SPEC>, &cfg);
     }
     return e;
+}
+
+template <int DIM, bool POW2, bool SPEC>
+cudaError_t launch_one(const GrowthParams &p, const GrowthLaunch &l, cudaStream_t stream)
+{
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned int)l.grid_ctas);
+    cfg.blockDim = dim3(kGrowthThreads);
+    cfg.dynamicSmemBytes = l.smem_bytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attrs[2];
+    attrs[0].id = cudaLaunchAttributeClusterDimension;
+    attrs[0].val.clusterDim.x = (unsigned int)l.cluster_ctas;
+    attrs[0].val.clusterDim.y = 1;
+    attrs[0].val.clusterDim.z = 1;
+    attrs[1].id = cudaLaunchAttributeCooperative;     // all CTAs co-resident: the grid barrier needs it
+    attrs[1].val.cooperative = 1;
+    cfg.attrs = attrs;
+    cfg.numAttrs = l.cooperative ? 2 : 1;
+    // per-process kernel attributes may have been changed by another handle since this one derived its shape
+    const cudaError_t ea = prepare_one<DIM, POW2, SPEC>(l, nullptr);
+    if (ea != cudaSuccess) return ea;
+    return cudaLaunchKernelEx(&cfg, growth_kernel<DIM, POW2, SPEC>, p);
 }
 
 }  // namespace

@@ -53,6 +53,9 @@ namespace {
 #ifndef WOLFF_WIDE
 #define WOLFF_WIDE 1
 #endif
+#ifndef WOLFF_BACKPRESSURE
+#define WOLFF_BACKPRESSURE 1      // 0: probe builds without the inbox capacity check (the host must then size the inboxes for the worst case)
+#endif
 constexpr unsigned int kWide = WOLFF_WIDE;         // sites per lane group and pass: a warp holds up to kWide * 32 / (2 dim) sites
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;
 constexpr int kT = kTileThreads;
@@ -136,7 +139,8 @@ struct alignas(16) TShared {
     unsigned int fill_on;               // idle warps fill bond tables (adaptive: off when updates are too short to pay for it)
     unsigned int watcher;               // 1 while some idle worker warp holds the watch (polls the ring without backing off)
     unsigned int ready_tag[2];          // k + 1 when EVERY tile of the CTA has its bits of update k in buffer k & 1
-    unsigned int pad;
+    unsigned int meas_req;              // k + 1 once the monitor has asked for the measurement after update k (in-kernel measurement)
+    unsigned long long meas_un, meas_ng;   // ... this CTA's sums of one evaluation: unequal forward bonds, negative spins
     unsigned long long ihead;           // inbox messages consumed (written by the receiver warp only)
     unsigned long long spill_head, spill_tail;   // running positions in the CTA's global spill list (kept across launches)
 };
@@ -147,6 +151,8 @@ struct Tally {
     unsigned int passes = 0;            // warp passes (lane 0)
     unsigned int inline_passes = 0;     // ... of which at least one lane ran Philox inline (lane 0)
     unsigned int chunks = 0;            // bond-table chunks filled: 32 sites each (lane 0)
+    unsigned int ring_pushes = 0;       // sites handed to other warps through the ring (lane 0)
+    unsigned int spills = 0;            // ... through the global spill list (lane 0)
 #ifdef WOLFF_PROFILE
     unsigned long long cyc_pass = 0;    // cycles inside passes (lane 0)
     unsigned long long lanes = 0;       // sites expanded (lane 0)
@@ -285,7 +291,7 @@ __device__ __forceinline__ uint32_t spill_tag(unsigned long long pos, uint32_t c
 // Hand n sites (items[0..n), warp-collective) to the other warps of the CTA: the ring, or the spill list when
 // the ring is full.  The caller has already counted them in sh.pending.
 __device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uint32_t *ring, const uint32_t *items, unsigned int n,
-                                       unsigned int c)
+                                       unsigned int c, Tally &tl)
 {
     const unsigned int lane = threadIdx.x & 31u;
     const uint32_t rmask = tp.ring_cap - 1u;
@@ -295,7 +301,7 @@ __device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uin
     base = __shfl_sync(kFullMask, base, 0);
     if (ok) {
         for (unsigned int j = lane; j < n; j += 32u) ring_put(ring + ((base + j) & rmask), items[j]);
-        if (lane == 0) atomicAdd(&tp.g.ctl->stats[12], (unsigned long long)n);
+        if (lane == 0) tl.ring_pushes += n;
     } else {
         unsigned long long sbase = 0;
         if (lane == 0) sbase = atomicAdd(&sh.spill_tail, (unsigned long long)n);
@@ -306,7 +312,7 @@ __device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uin
             const unsigned long long pos = sbase + (unsigned long long)j;
             st_relaxed_u32(seg + ((uint32_t)pos & smask), (items[j] << 1) | spill_tag(pos, tp.spill_log));
         }
-        if (lane == 0) atomicAdd(&tp.g.ctl->stats[14], (unsigned long long)n);
+        if (lane == 0) tl.spills += n;
     }
 }
 
@@ -330,6 +336,19 @@ __device__ __noinline__ void publish(const TileParams &tp, TShared &sh, unsigned
 }
 
 __device__ __forceinline__ void raise_abort(Control *ctl, unsigned int code) { st_relaxed_u32(&ctl->error, code); }
+
+// Back-pressure of the inboxes.  Slot pos of CTA `own` may be written once its receiver has taken message
+// pos - in_cap out of it: pos - gihead[own] < in_cap (32-bit running counters; gihead only grows, so a value read
+// earlier is a safe lower bound).  Rare: the sender has usually read a recent gihead next to its slot atomic.  The
+// receiver never waits for a sender (it only claims, and feeds its ring or spill list), so this wait always ends.
+__device__ __noinline__ void wait_inbox(const TileParams &tp, uint32_t own, unsigned int pos)
+{
+    unsigned int polls = 0;
+    while (pos - ld_relaxed_u32(tp.gihead + own) >= tp.in_cap) {
+        if ((++polls & 0x3FFu) == 0u && ld_relaxed_u32(&tp.g.ctl->error) != 0u) return;     // the launch is being aborted
+        __nanosleep(64);
+    }
+}
 
 // ------------------------------------------------------------------------------------------ bond tables
 // State a warp keeps about the tile it is filling (warp-uniform registers).
@@ -422,6 +441,127 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
     return true;
 }
 
+// ------------------------------------------------------------------------------------------ in-kernel measurement
+// "+ measurement": E and M of the whole lattice after an update, evaluated where the lattice
+// is -- in the CTAs' shared memory -- without leaving the persistent kernel.  The forward bonds (+d) of a tile's
+// high-d face end in the low-d face of the next tile, which lives in another CTA: every CTA first copies the low
+// faces of its tiles to global memory (tp.faces), all CTAs meet at an arrival counter, then every CTA sums its own
+// tiles (16 sites per load; sign-bit XOR + popc as in measure.cu) and adds its two counts to the control block.
+// Called by every warp of the CTA but the monitor, between two updates (nothing is queued or in flight).
+__device__ __forceinline__ void bar_sync_named(unsigned int id, unsigned int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ unsigned int popc_sign4(const uint4 &v)
+{
+    return __popc(v.x & 0x80808080u) + __popc(v.y & 0x80808080u) + __popc(v.z & 0x80808080u) + __popc(v.w & 0x80808080u);
+}
+__device__ __forceinline__ unsigned int unequal4(const uint4 &a, const uint4 &b)
+{
+    return __popc((a.x ^ b.x) & 0x80808080u) + __popc((a.y ^ b.y) & 0x80808080u) + __popc((a.z ^ b.z) & 0x80808080u) +
+           __popc((a.w ^ b.w) & 0x80808080u);
+}
+
+template <int DIM>
+__device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, const Layout &ly, unsigned int c, unsigned int ptid,
+                                          unsigned int P, unsigned int krel)
+{
+    constexpr unsigned int ND = 2u * DIM;
+    const Tiling<DIM> tg(tp);
+    Control *ctl = tp.g.ctl;
+    const uint32_t b = tg.b, B = 1u << b, m = tg.m, TS = 1u << tg.ts_log;
+    const uint32_t F = 1u << ((DIM - 1) * b), F4 = F >> 2;             // bytes / words of one face (B >= 4: F >= 4)
+    const unsigned char *const lat = reinterpret_cast<const unsigned char *>(ly.lat);
+    const unsigned char *const faces = reinterpret_cast<const unsigned char *>(tp.faces);
+    // ---- 1. the low faces of my tiles -> global memory, four sites per store
+    {
+        unsigned int *const fout = reinterpret_cast<unsigned int *>(tp.faces);
+        const uint32_t nwords = ly.myslots * DIM * F4;
+        for (uint32_t idx = ptid; idx < nwords; idx += P) {
+            const uint32_t slot = idx / (DIM * F4), rem = idx - slot * (DIM * F4), d = rem / F4, f0 = (rem - d * F4) << 2;
+            const uint32_t low = (1u << (d * b)) - 1u;
+            uint32_t word = 0;
+#pragma unroll
+            for (uint32_t j = 0; j < 4u; ++j) {
+                const uint32_t f = f0 + j;
+                const uint32_t w = (f & low) | ((f >> (d * b)) << ((d + 1u) * b));     // coordinate d = 0
+                word |= (uint32_t)lat[(slot << tg.ts_log) + w] << (8u * j);
+            }
+            fout[((slot * tp.G + c) * DIM + d) * F4 + (f0 >> 2)] = word;
+        }
+    }
+    __threadfence();
+    bar_sync_named(1u, P);
+    if (ptid == 0u) {
+        atomicAdd(&ctl->meas_arrive_a, 1u);
+        const unsigned int target = (krel + 1u) * tp.G;
+        unsigned int polls = 0;
+        while (ld_acquire_u32(&ctl->meas_arrive_a) != target)
+            if ((++polls & 0xFFu) == 0u && ld_relaxed_u32(&ctl->error) != 0u) break;
+    }
+    bar_sync_named(1u, P);
+    // ---- 2. my tiles: negative spins and unequal forward bonds
+    unsigned int un = 0, ng = 0;
+    auto face_of = [&](uint32_t slot, uint32_t d) -> const unsigned char * {
+        const uint32_t nt = ly.nbrtab[slot * ND + 2u * d];                  // (owner << 16) | slot of the +d neighbouring tile
+        return faces + (size_t)(((nt & 0xFFFFu) * tp.G + (nt >> 16)) * DIM + d) * F;
+    };
+    if (b >= 4u) {
+        const uint32_t cpt_log = tg.ts_log - 4u, total = ly.myslots << cpt_log;
+        for (uint32_t ch = ptid; ch < total; ch += P) {
+            const uint32_t slot = ch >> cpt_log, w0 = (ch & ((1u << cpt_log) - 1u)) << 4;
+            const uint32_t x0 = w0 & m, y = (w0 >> b) & m, z = DIM == 3 ? (w0 >> (2u * b)) : 0u;
+            const unsigned char *const at = lat + (slot << tg.ts_log) + w0;
+            const uint4 a = *reinterpret_cast<const uint4 *>(at);
+            ng += popc_sign4(a);
+            // +x: the 16 sites shifted by one byte; the 17th is the next site of the row, or the +x tile's low-x face
+            const uint32_t nb = x0 + 16u < B ? (uint32_t)at[16] : (uint32_t)__ldcg(face_of(slot, 0u) + (w0 >> b));
+            un += __popc((a.x ^ __funnelshift_r(a.x, a.y, 8)) & 0x80808080u) + __popc((a.y ^ __funnelshift_r(a.y, a.z, 8)) & 0x80808080u) +
+                  __popc((a.z ^ __funnelshift_r(a.z, a.w, 8)) & 0x80808080u) + __popc((a.w ^ __funnelshift_r(a.w, nb, 8)) & 0x80808080u);
+            const uint4 by = y + 1u < B ? *reinterpret_cast<const uint4 *>(at + B)
+                                        : __ldcg(reinterpret_cast<const uint4 *>(face_of(slot, 1u) + (x0 | (z << b))));
+            un += unequal4(a, by);
+            if (DIM == 3) {
+                const uint4 bz = z + 1u < B ? *reinterpret_cast<const uint4 *>(at + (B << b))
+                                            : __ldcg(reinterpret_cast<const uint4 *>(face_of(slot, 2u) + (x0 | (y << b))));
+                un += unequal4(a, bz);
+            }
+        }
+    } else {
+        // tiles narrower than a 16-byte load (test configurations): one site at a time
+        const uint32_t total = ly.myslots << tg.ts_log;
+        for (uint32_t idx = ptid; idx < total; idx += P) {
+            const uint32_t slot = idx >> tg.ts_log, w = idx & tg.ts_mask;
+            const uint32_t s = lat[idx];
+            ng += s >> 7;
+#pragma unroll
+            for (uint32_t d = 0; d < (uint32_t)DIM; ++d) {
+                const uint32_t low = (1u << (d * b)) - 1u;
+                uint32_t nbv;
+                if (((w >> (d * b)) & m) != m) nbv = lat[idx + (1u << (d * b))];
+                else nbv = __ldcg(face_of(slot, d) + ((w & low) | ((w >> ((d + 1u) * b)) << (d * b))));
+                un += ((s ^ nbv) >> 7) & 1u;
+            }
+        }
+    }
+    un = __reduce_add_sync(kFullMask, un);
+    ng = __reduce_add_sync(kFullMask, ng);
+    if ((threadIdx.x & 31u) == 0u) {
+        if (un) atomicAdd(&sh.meas_un, (unsigned long long)un);
+        if (ng) atomicAdd(&sh.meas_ng, (unsigned long long)ng);
+    }
+    bar_sync_named(1u, P);
+    if (ptid == 0u) {
+        const unsigned long long tun = ld_vol64(&sh.meas_un), tng = ld_vol64(&sh.meas_ng);
+        st_vol64(&sh.meas_un, 0ull);
+        st_vol64(&sh.meas_ng, 0ull);
+        if (tun) atomicAdd(&ctl->meas_unequal, tun);
+        if (tng) atomicAdd(&ctl->meas_negative, tng);
+        __threadfence();
+        atomicAdd(&ctl->meas_arrive_b, 1u);
+    }
+}
+
 // ------------------------------------------------------------------------------------------ worker warp
 // Expands sites owned by this CTA until the launch is over (A2-A5 on shared memory), one lane per bond: a warp
 // holds up to S = 32 / (2*DIM) sites per pass (8 in 2D, 5 in 3D) and lane (q, k) tests the bond from site q to its
@@ -477,13 +617,17 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     for (unsigned int j = 0; j < W; ++j) a[j] = ws.a[j];
     unsigned int nsites = ws.nsites, mywon = ws.mywon, sbuf = ws.sbuf;
     unsigned int msg_pos[W];           // messages whose inbox slots are on their way back from L2
+    unsigned int msg_seen[W];          // ... and what the owner's receiver had consumed at about that time (back-pressure)
     uint32_t msg_own[W], msg_na[W];
     bool msg_valid[W];
 #pragma unroll
-    for (unsigned int j = 0; j < W; ++j) { msg_pos[j] = 0; msg_own[j] = msg_na[j] = 0; msg_valid[j] = false; }
+    for (unsigned int j = 0; j < W; ++j) { msg_pos[j] = msg_seen[j] = 0; msg_own[j] = msg_na[j] = 0; msg_valid[j] = false; }
     unsigned int budget = 32u;
 
     auto send = [&](unsigned int j) {
+#if WOLFF_BACKPRESSURE
+        if (msg_pos[j] - msg_seen[j] >= tp.in_cap) wait_inbox(tp, msg_own[j], msg_pos[j]);
+#endif
         st_relaxed_u64(tp.inbox + ((size_t)msg_own[j] << tp.in_log) + (msg_pos[j] & in_mask),
                        pack_msg(kKindClaim, (msg_pos[j] >> tp.in_log) & 1u, krel, msg_na[j], POS ? 1 : -1));
         msg_valid[j] = false;
@@ -580,8 +724,15 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
                 if (msg_valid[j]) send(j);
                 // the atomic writes the loop-carried register itself (an in-out operand, 32 bits: a 64-bit result needs an
                 // aligned register pair, which ptxas then copies out of -- and a copy waits for the L2 round trip here)
+#if WOLFF_BACKPRESSURE
+                asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.global.add.u32 %0, [%2], 1;\n"
+                             " @p ld.relaxed.gpu.global.u32 %1, [%4];\n}"
+                             : "+r"(msg_pos[j]), "+r"(msg_seen[j]) : "l"(tp.gtail + own[j]), "r"((unsigned int)cand_r[j]), "l"(tp.gihead + own[j])
+                             : "memory");
+#else
                 asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %2, 0;\n @p atom.global.add.u32 %0, [%1], 1;\n}"
                              : "+r"(msg_pos[j]) : "l"(tp.gtail + own[j]), "r"((unsigned int)cand_r[j]) : "memory");
+#endif
                 if (cand_r[j]) {
                     msg_own[j] = own[j];
                     msg_na[j] = na[j];
@@ -621,7 +772,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
             if (q < S && q + j * S < nsites) a[j] = lds_u32(out_s + (q + j * S) * 4u);
         if (total > W * S) {
             if (lane == 0) red_shared_add(pend_s, total - W * S);    // counted before another warp can see them
-            hand_over(tp, sh, ly.ring, st_out + W * S, total - W * S, c);
+            hand_over(tp, sh, ly.ring, st_out + W * S, total - W * S, c, tl);
         }
 #ifdef WOLFF_PROFILE
         tl.cyc_pass += (unsigned long long)(clock64() - tp0);
@@ -673,10 +824,14 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
     WorkerState ws;
     unsigned int idle = 0;
     Filler fl;
+    // in-kernel measurement: every warp of the CTA but the monitor takes part
+    const unsigned int warp = threadIdx.x >> 5;
+    const unsigned int P = c == 0u ? kT - 32u : kT, ptid = c == 0u ? (warp - 1u) * 32u + lane : threadIdx.x;
+    unsigned int meas_done = 0;
 
     for (;;) {
         // ---- take up to S sites from the ring, else from the spill list; with neither, fill bond tables or sleep
-        unsigned int n = 0, h = 0, from_spill = 0, stop = 0;
+        unsigned int n = 0, h = 0, from_spill = 0, stop = 0, mreq = 0;
         unsigned long long sh_pos = 0;
         if (lane == 0) {
             // one 64-bit load: a consistent (head, tail) pair; the loads of a poll are independent
@@ -684,6 +839,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
             sh_pos = ld_vol64(&sh.spill_head);
             const unsigned long long st = ld_vol64(&sh.spill_tail);
             stop = ld_vol(&sh.stop);
+            mreq = ld_vol(&sh.meas_req);
             h = (unsigned int)ht;
             const unsigned int t = (unsigned int)(ht >> 32);
             if (t != h) {
@@ -696,6 +852,12 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         }
         n = __shfl_sync(kFullMask, n, 0);
         if (n == 0u) {
+            mreq = __shfl_sync(kFullMask, mreq, 0);
+            if (mreq != meas_done) {                                   // the update is over everywhere: measure (see measure_phase)
+                measure_phase<DIM>(tp, sh, ly, c, ptid, P, mreq - 1u);
+                meas_done = mreq;
+                continue;
+            }
             if (__shfl_sync(kFullMask, stop, 0)) break;                // launch over
             // one idle warp per CTA holds the watch: it does nothing but poll the ring, so what the receiver (or a warp
             // with more winners than it can keep) hands over starts at once; the watch passes on when its holder finds work
@@ -788,10 +950,20 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
             continue;
         }
         const bool mine = lane < k;
-        if (__any_sync(kFullMask, mine && kind == kKindExit)) {
-            // sent by the monitor after the last update is complete: nothing is queued anywhere
+        const unsigned int ctlb = __ballot_sync(kFullMask, mine && kind == kKindExit);
+        if (ctlb != 0u) {
+            // sent by the monitor when an update is complete and nothing is queued anywhere: leave (site field 0),
+            // or take part in the measurement after update krel (site field 1)
+            const unsigned int src = (unsigned int)__ffs((int)ctlb) - 1u;
+            const unsigned int what = __shfl_sync(kFullMask, lo >> 1, src), krel_m = __shfl_sync(kFullMask, hi & (kMaxK - 1u), src);
             ih += (unsigned long long)k;
-            if (lane == 0) { st_vol64(&sh.ihead, ih); atomicMax(tp.gdone + c, ih); }
+            if (lane == 0) { st_vol64(&sh.ihead, ih); st_relaxed_u32(tp.gihead + c, (unsigned int)ih); atomicMax(tp.gdone + c, ih); }
+            if (what == 1u) {
+                if (lane == 0) { __threadfence_block(); st_vol(&sh.meas_req, krel_m + 1u); }
+                __syncwarp();
+                measure_phase<DIM>(tp, sh, ly, c, lane, c == 0u ? kT - 32u : kT, krel_m);
+                continue;
+            }
             break;
         }
         const uint32_t addr = lo >> 1;
@@ -808,6 +980,7 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
         const unsigned int krel = __shfl_sync(kFullMask, hi & (kMaxK - 1u), 0);
         ih += (unsigned long long)k;
         if (lane == 0) {
+            st_relaxed_u32(tp.gihead + c, (unsigned int)ih);     // these slots may be written again (back-pressure)
             const unsigned long long u = p.u0 + (unsigned long long)krel;
             *reinterpret_cast<volatile int *>(&sh.s0) = s0u;
             st_vol(&sh.u_lo, (uint32_t)u);
@@ -821,7 +994,7 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
         }
         if (win) stage[__popc(wb & lt)] = addr;
         __syncwarp();
-        if (w) hand_over(tp, sh, ly.ring, stage, w, c);
+        if (w) hand_over(tp, sh, ly.ring, stage, w, c, tl);
         __syncwarp();
         if (lane == 0) {
             const unsigned int before = atomicSub(&sh.pending, 1u);
@@ -853,6 +1026,9 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
     unsigned long long prev = ld_relaxed_u64(tp.added);
     unsigned long long flipped = 0, polls_total = 0;
     bool aborted = false;
+    Moments mom;
+    long long lastE = 0, lastM = 0;
+    if (p.measure && lane == 0) mom.load(ctl->moments);
     for (unsigned long long k = 0; k < p.n_updates && !aborted; ++k) {
         if (lane == 0) {
             const unsigned long long u = p.u0 + k;
@@ -862,6 +1038,7 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
             uint32_t own, addr;
             tg.locate(i0, own, addr);
             const unsigned int pos = atomicAdd(tp.gtail + own, 1u);
+            wait_inbox(tp, own, pos);
             st_relaxed_u64(tp.inbox + ((size_t)own << tp.in_log) + (pos & in_mask),
                            pack_msg(kKindSeed, (pos >> tp.in_log) & 1u, (unsigned int)k, addr, 1));
             ++tl.messages;
@@ -893,10 +1070,53 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
         if (!aborted && lane == 0) {
             const unsigned long long a = ld_relaxed_u64(tp.added);
             p.sizes[k] = (uint32_t)(a - prev);      // A7
+            const unsigned long long dt = globaltimer_ns() - t0;
+            p.ns_log[k] = dt > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)dt;
             flipped += a - prev;
             prev = a;
         }
+        if (p.measure && !aborted) {
+            // "+ measurement": every CTA evaluates its tiles (measure_phase); the request travels like the exit message
+            for (unsigned int base = 0; base < G; base += 256u) {
+                unsigned int pos[8];
+#pragma unroll
+                for (unsigned int i = 0; i < 8u; ++i) {
+                    const unsigned int cc = base + i * 32u + lane;
+                    pos[i] = cc < G ? atomicAdd(tp.gtail + cc, 1u) : 0u;
+                }
+#pragma unroll
+                for (unsigned int i = 0; i < 8u; ++i) {
+                    const unsigned int cc = base + i * 32u + lane;
+                    if (cc < G) {
+                        wait_inbox(tp, cc, pos[i]);
+                        st_relaxed_u64(tp.inbox + ((size_t)cc << tp.in_log) + (pos[i] & in_mask),
+                                       pack_msg(kKindExit, (pos[i] >> tp.in_log) & 1u, (unsigned int)k, 1u, 1));
+                    }
+                }
+            }
+            unsigned int bad = 0;
+            if (lane == 0) {
+                const unsigned int target = ((unsigned int)k + 1u) * G;
+                unsigned int polls = 0;
+                while (ld_acquire_u32(&ctl->meas_arrive_b) != target) {
+                    if ((++polls & 0xFFu) == 0u) {
+                        if (ld_relaxed_u32(&ctl->error) != 0u) { bad = 1; break; }
+                        if (globaltimer_ns() - t0 > tp.watchdog_ns) { raise_abort(ctl, 6u); bad = 1; break; }
+                    }
+                }
+                if (!bad) {
+                    const unsigned long long un = atomicExch(&ctl->meas_unequal, 0ull), ng = atomicExch(&ctl->meas_negative, 0ull);
+                    lastE = 2ll * (long long)un - (long long)DIM * (long long)p.geo.N;
+                    lastM = (long long)p.geo.N - 2ll * (long long)ng;
+                    p.E_log[k] = lastE;
+                    p.M_log[k] = lastM;
+                    mom.add(lastE, lastM);
+                }
+            }
+            if (__shfl_sync(kFullMask, bad, 0)) aborted = true;
+        }
     }
+    if (p.measure && lane == 0 && !aborted && p.n_updates > 0) { ctl->E = lastE; ctl->M = lastM; mom.store(ctl->moments); }
     // everybody leaves (also after an abort: receivers poll the error flag, but an exit message is quicker).  Eight slot
     // atomics per lane are in flight before the first message is stored.
     for (unsigned int base = 0; base < G; base += 256u) {
@@ -909,8 +1129,10 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
 #pragma unroll
         for (unsigned int i = 0; i < 8u; ++i) {
             const unsigned int cc = base + i * 32u + lane;
-            if (cc < G)
+            if (cc < G) {
+                wait_inbox(tp, cc, pos[i]);
                 st_relaxed_u64(tp.inbox + ((size_t)cc << tp.in_log) + (pos[i] & in_mask), pack_msg(kKindExit, (pos[i] >> tp.in_log) & 1u, 0u, 0u, 1));
+            }
         }
     }
     if (lane == 0) {
@@ -998,6 +1220,9 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
     const unsigned int c = blockIdx.x;
     const Layout ly = Layout::make<DIM>(tp, smem_t, c);
     Tally tl;
+    // the error flag is sticky: an earlier launch of this handle was aborted and the host has not yet looked (the
+    // queues are not in a state to continue from; the host marks the handle failed at its next synchronising call)
+    if (ld_relaxed_u32(&tp.g.ctl->error) != 0u) return;
 
     for (unsigned int i = tid; i < tp.ring_cap; i += kT) ly.ring[i] = kEmpty;
     if (tid == 0) {
@@ -1010,6 +1235,8 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         sh.krel = 0u;
         sh.ready_tag[0] = sh.ready_tag[1] = 0u;
         sh.watcher = 0u;
+        sh.meas_req = 0u;
+        sh.meas_un = sh.meas_ng = 0ull;
         sh.fill_on = tp.fill_mode == 0u ? 0u : (tp.fill_mode == 2u ? 1u : tp.gfill[c]);
         sh.ihead = ld_relaxed_u64(tp.gdone + c);          // everything ever sent to this CTA was consumed by the last launch
         sh.spill_head = sh.spill_tail = ld_relaxed_u64(tp.gspill + c);
@@ -1054,6 +1281,8 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
         if (ms) atomicAdd(&ctl->stats[11], (unsigned long long)ms);
         if (tl.passes) atomicAdd(&ctl->stats[13], (unsigned long long)tl.passes);
         if (tl.chunks) atomicAdd(&ctl->stats[15], (unsigned long long)tl.chunks);
+        if (tl.ring_pushes) atomicAdd(&ctl->stats[12], (unsigned long long)tl.ring_pushes);
+        if (tl.spills) atomicAdd(&ctl->stats[14], (unsigned long long)tl.spills);
 #ifdef WOLFF_PROFILE
         if (tl.cyc_pass) atomicAdd(&ctl->stats[2], tl.cyc_pass);
         if (tl.lanes) atomicAdd(&ctl->stats[3], tl.lanes);
@@ -1064,6 +1293,11 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp
 template <int DIM>
 cudaError_t launch_one(const TileParams &tp, size_t smem_bytes, cudaStream_t stream)
 {
+    // the attribute belongs to the kernel function, i.e. to the process: another live handle of the same dim may have
+    // made its plan (and set a smaller value) since this handle made its own
+    const void *fn = reinterpret_cast<const void *>(&growth_tiles_kernel<DIM>);
+    const cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    if (ea != cudaSuccess) return ea;
     void *args[] = { const_cast<TileParams *>(&tp) };
     return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(&growth_tiles_kernel<DIM>), dim3(tp.G), dim3(kT), args,
                                        smem_bytes, stream);

@@ -1,5 +1,6 @@
 // internal.h -- host/device shared declarations of libwolff_b200 (not part of the public ABI).
 #pragma once
+#include <cstddef>
 #include <cstdint>
 #include <cuda_runtime.h>
 
@@ -17,7 +18,9 @@ enum Phase : unsigned int {
 };
 
 // Global-memory control block of one handle.  Every hot word sits in its own 128-byte line.
-// The words before acc_unequal are zeroed at every launch of a growth kernel.
+// The words before `error` are zeroed at every launch of a growth kernel (kControlClearBytes); what follows is
+// never cleared by a launch: the error flag is STICKY (a kernel that finds it set leaves at once; the host reads it
+// at its next synchronising call and marks the handle failed), and the measurement state runs on across launches.
 struct alignas(128) Control {
     // [gen:24 | phase:8 | hi:32]; polled by every CTA, written by the last arriver / by CTA 0.
     alignas(128) unsigned long long bar;
@@ -27,17 +30,25 @@ struct alignas(128) Control {
     alignas(128) unsigned int lo;
     int s0;
     unsigned long long u;
-    alignas(128) unsigned int error;           // nonzero: a barrier / phase timed out
-    unsigned int pad4;
-    unsigned long long stats[16];              // see WOLFF_NSTATS in wolff.h
-    // E/M reduction scratch
-    alignas(128) unsigned long long acc_unequal;
+    alignas(128) unsigned long long stats[16]; // see WOLFF_NSTATS in wolff.h
+    // in-kernel measurement of the shared-memory-resident kernel: arrival counters (modulo 2^32: G per measured
+    // update) and the sums of one whole-lattice evaluation
+    alignas(128) unsigned int meas_arrive_a;   // CTAs whose tile faces of the finished update are in global memory
+    alignas(128) unsigned int meas_arrive_b;   // CTAs whose partial sums are in meas_unequal / meas_negative
+    alignas(128) unsigned long long meas_unequal;
+    unsigned long long meas_negative;
+    // ---------------------------------------------------------------- not cleared by a launch
+    alignas(128) unsigned int error;           // nonzero: a barrier / an update timed out (sticky)
+    unsigned int invalid;                      // set_spins validation
+    unsigned int ticket;                       // E/M reduction: CTAs done
+    unsigned int pad0;
+    unsigned long long acc_unequal;            // E/M reduction scratch
     unsigned long long acc_negative;
-    unsigned int ticket;
-    unsigned int invalid;         // set_spins validation
-    long long E;
-    long long M;
+    long long E;                               // result of the last reduction; with in-kernel measurement: the
+    long long M;                               // running values after the last measured update
+    unsigned long long moments[10];            // in-kernel measurement: accumulated sums (layout: wolff_get_moments)
 };
+constexpr size_t kControlClearBytes = offsetof(Control, error);
 
 struct GrowthParams {
     int8_t *spins;
@@ -55,6 +66,12 @@ struct GrowthParams {
     uint32_t grid_down;     // return from a grid phase to cluster mode when the frontier is at most this wide
     uint32_t bal_min;       // cluster mode: a CTA holding more than max(bal_min, 2 x fair share) triggers rebalancing
     uint32_t qcap;          // entries per shared-memory queue buffer
+    // in-kernel measurement (wolff_set_option "measure"): E and M after every update, accumulated moments
+    uint32_t measure;       // 1: on
+    uint32_t claim_bits;    // 0xFE, or 0xFC when measuring in the level-synchronous kernel (membership mark, device_common.cuh)
+    long long *E_log;       // per-update E, M of this launch (n_updates entries each) when measure
+    long long *M_log;
+    uint32_t *ns_log;       // per-update duration in nanoseconds (always written; saturates at 2^32 - 1)
 };
 
 // Shared-memory-resident barrier-free kernel (growth_tiles.cu).  The lattice (L a power of two) is cut into tiles of
@@ -67,6 +84,8 @@ struct TileParams {
     unsigned int *gtail;             // [G] messages ever pushed into CTA c's inbox, modulo 2^32 (its low bits are the inbox slot)
     unsigned long long *gdone;       // [G] of those, how many are consumed with their whole local progeny expanded
     unsigned long long *gspill;      // [G] running position of CTA c's spill list
+    unsigned int *gihead;            // [G] messages CTA c's receiver has taken out of its inbox, modulo 2^32: a sender may write
+                                     // slot pos only while pos - gihead[c] < in_cap (back-pressure)
     unsigned long long *added;       // spins ever claimed (sum over CTAs, published with gdone)
     uint32_t *spill;                 // G segments of 2^spill_log entries: overflow of the shared-memory ring
     unsigned long long magicG;       // ceil(2^40 / G)
@@ -75,7 +94,7 @@ struct TileParams {
     uint32_t permA, permAinv;        // odd multiplier and its inverse mod ntiles
     uint32_t G;                      // CTAs (one per SM, all co-resident)
     uint32_t slots;                  // tiles per CTA (upper bound)
-    uint32_t in_log, in_cap;         // inbox entries per CTA (a power of two above the messages one update can send it)
+    uint32_t in_log, in_cap;         // inbox entries per CTA (a power of two, at least 32)
     uint32_t spill_log;              // spill entries per CTA (at least the sites the CTA owns)
     uint32_t ring_cap;               // entries of the shared-memory ring (power of two)
     unsigned long long watchdog_ns;  // an update longer than this aborts the launch
@@ -86,6 +105,10 @@ struct TileParams {
     uint32_t *gfill;                 // [G] fill_on of CTA c at the end of the last launch
     uint32_t thr32, thr_all;         // low word of the bond threshold; thr_all = 1 when thr = 2^32 (every bond active)
     uint32_t idle_ns;                // longest sleep of an idle worker warp between two polls of the ring
+    // in-kernel measurement: the low faces of every tile (the sites with coordinate d = 0 inside the tile), written by
+    // the tile's owner after each measured update and read by the owner of the tile next to it in direction -d:
+    // faces[((slot * G + owner) * dim + d) * B^(dim-1) + f], one byte per site
+    int8_t *faces;
 };
 
 // Launch shape of the persistent kernel.
@@ -108,9 +131,10 @@ cudaError_t growth_max_clusters(int dim, bool pow2, const GrowthLaunch &l, int *
 size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, uint32_t nbuf);
 cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm);
 cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes, cudaStream_t stream);
-cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, cudaStream_t stream);
-cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, cudaStream_t stream);
+cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, int num_sms, cudaStream_t stream);
+cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, int num_sms, cudaStream_t stream);
+// E and M of the lattice into ctl->E, ctl->M and, when not null, into the DEVICE words E_dst, M_dst
 cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo, int dim, Control *ctl,
-                                        int num_sms, cudaStream_t stream);
+                                        long long *E_dst, long long *M_dst, int num_sms, cudaStream_t stream);
 
 }  // namespace wolff

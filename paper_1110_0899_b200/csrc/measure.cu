@@ -50,19 +50,34 @@ __global__ void __launch_bounds__(kThreads) init_lattice_kernel(int8_t *spins, u
 }
 
 // ---------------------------------------------------------------- set_spins validation
+// A word of four spins is valid when every byte is 0x01 or 0xFF: with s = the four sign bits, the only valid word
+// is 0x01010101 | s * 0xFE.  16 bytes per load (the staging buffer is 16-byte aligned and padded), bytes beyond N
+// are not looked at.
+__device__ __forceinline__ bool word_valid(uint32_t w)
+{
+    const uint32_t s = (w >> 7) & 0x01010101u;
+    return w == (0x01010101u | (s * 0xFEu));
+}
+
 __global__ void __launch_bounds__(kThreads) validate_kernel(const int8_t *spins, uint32_t N, Control *ctl)
 {
     bool bad = false;
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
-        const int8_t s = spins[i];
-        bad |= (s != 1 && s != -1);
+    const uint32_t chunks = N / 16u;
+    const uint4 *const v = reinterpret_cast<const uint4 *>(spins);
+    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < chunks; c += gridDim.x * blockDim.x) {
+        const uint4 a = v[c];
+        bad |= !(word_valid(a.x) && word_valid(a.y) && word_valid(a.z) && word_valid(a.w));
+    }
+    if (blockIdx.x == 0 && threadIdx.x < (N & 15u)) {            // ragged tail, at most 15 bytes
+        const int8_t b = spins[chunks * 16u + threadIdx.x];
+        bad |= (b != 1 && b != -1);
     }
     if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(&ctl->invalid, 1u);
 }
 
 // ---------------------------------------------------------------- E / M reduction
 __device__ __forceinline__ void block_accumulate(unsigned long long unequal, unsigned long long negative, Control *ctl,
-                                                 uint32_t N, int dim)
+                                                 uint32_t N, int dim, long long *E_dst, long long *M_dst)
 {
     __shared__ unsigned long long s_un[kThreads / 32], s_ng[kThreads / 32];
     __shared__ bool last;
@@ -87,8 +102,12 @@ __device__ __forceinline__ void block_accumulate(unsigned long long unequal, uns
             __threadfence();
             const unsigned long long tun = atomicAdd(&ctl->acc_unequal, 0ull);
             const unsigned long long tng = atomicAdd(&ctl->acc_negative, 0ull);
-            ctl->E = 2ll * (long long)tun - (long long)dim * (long long)N;
-            ctl->M = (long long)N - 2ll * (long long)tng;
+            const long long Ev = 2ll * (long long)tun - (long long)dim * (long long)N;
+            const long long Mv = (long long)N - 2ll * (long long)tng;
+            ctl->E = Ev;
+            ctl->M = Mv;
+            if (E_dst) *E_dst = Ev;          // the caller's device words: no bounce through the host
+            if (M_dst) *M_dst = Mv;
             ctl->acc_unequal = 0ull;
             ctl->acc_negative = 0ull;
             ctl->ticket = 0u;
@@ -96,49 +115,67 @@ __device__ __forceinline__ void block_accumulate(unsigned long long unequal, uns
     }
 }
 
-// Vector path: L is a multiple of 16, so a 16-byte chunk never straddles a row.
+// Vector path: L is a multiple of 16, so a 16-byte chunk never straddles a row.  A thread takes kU chunks per
+// iteration and issues all their loads (the chunk, its +y and +z neighbours, the byte that follows it) before it
+// uses any: the kernel is a few microseconds long, so what it needs is bytes in flight.
+constexpr int kU = 4;
+
 template <int DIM>
-__global__ void __launch_bounds__(kThreads) energy_magnetisation_vec16(const int8_t *__restrict__ spins, Geometry g, Control *ctl)
+__global__ void __launch_bounds__(kThreads) energy_magnetisation_vec16(const int8_t *__restrict__ spins, Geometry g, Control *ctl,
+                                                                       long long *E_dst, long long *M_dst)
 {
     const uint32_t chunks = g.N / 16u;
     const uint32_t chunks_per_row = g.L / 16u;
+    const uint32_t stride = gridDim.x * blockDim.x;
     unsigned long long unequal = 0, negative = 0;
-    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < chunks; c += gridDim.x * blockDim.x) {
-        const uint32_t i = c * 16u;
-        const uint32_t row = c / chunks_per_row;          // y + L*z
-        const uint32_t cx = c - row * chunks_per_row;     // chunk index along x
-        const uint32_t y = (DIM == 3) ? row % g.L : row;
-        const uint4 a = *reinterpret_cast<const uint4 *>(spins + i);
-        // +x: the 16 sites shifted by one byte; the 17th byte is the first site of the next chunk (wrapping)
-        const uint32_t inext = (cx + 1u == chunks_per_row) ? i + 16u - g.L : i + 16u;
-        const uint32_t nb = (uint32_t)(uint8_t)spins[inext];
-        uint32_t acc = 0, neg = 0;
-        acc += __popc((a.x ^ __funnelshift_r(a.x, a.y, 8)) & kSignMask);
-        acc += __popc((a.y ^ __funnelshift_r(a.y, a.z, 8)) & kSignMask);
-        acc += __popc((a.z ^ __funnelshift_r(a.z, a.w, 8)) & kSignMask);
-        acc += __popc((a.w ^ __funnelshift_r(a.w, nb, 8)) & kSignMask);
-        neg += __popc(a.x & kSignMask) + __popc(a.y & kSignMask) + __popc(a.z & kSignMask) + __popc(a.w & kSignMask);
-        // +y
-        const uint32_t iy = (y + 1u == g.L) ? i - (g.LL - g.L) : i + g.L;
-        const uint4 by = *reinterpret_cast<const uint4 *>(spins + iy);
-        acc += __popc((a.x ^ by.x) & kSignMask) + __popc((a.y ^ by.y) & kSignMask) +
-               __popc((a.z ^ by.z) & kSignMask) + __popc((a.w ^ by.w) & kSignMask);
-        if (DIM == 3) {
-            const uint32_t z = row / g.L;
-            const uint32_t iz = (z + 1u == g.L) ? i - (g.N - g.LL) : i + g.LL;
-            const uint4 bz = *reinterpret_cast<const uint4 *>(spins + iz);
-            acc += __popc((a.x ^ bz.x) & kSignMask) + __popc((a.y ^ bz.y) & kSignMask) +
-                   __popc((a.z ^ bz.z) & kSignMask) + __popc((a.w ^ bz.w) & kSignMask);
+    for (uint32_t c0 = blockIdx.x * blockDim.x + threadIdx.x; c0 < chunks; c0 += stride * kU) {
+        uint4 a[kU], by[kU], bz[kU];
+        uint32_t nb[kU];
+        bool on[kU];
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            const uint32_t c = c0 + (uint32_t)u * stride;
+            on[u] = c < chunks;
+            const uint32_t cc = on[u] ? c : 0u;
+            const uint32_t i = cc * 16u;
+            const uint32_t row = cc / chunks_per_row;          // y + L*z
+            const uint32_t cx = cc - row * chunks_per_row;     // chunk index along x
+            const uint32_t y = (DIM == 3) ? row % g.L : row;
+            a[u] = *reinterpret_cast<const uint4 *>(spins + i);
+            // +x: the 16 sites shifted by one byte; the 17th byte is the first site of the next chunk (wrapping)
+            const uint32_t inext = (cx + 1u == chunks_per_row) ? i + 16u - g.L : i + 16u;
+            nb[u] = (uint32_t)(uint8_t)spins[inext];
+            const uint32_t iy = (y + 1u == g.L) ? i - (g.LL - g.L) : i + g.L;
+            by[u] = *reinterpret_cast<const uint4 *>(spins + iy);
+            if (DIM == 3) {
+                const uint32_t z = row / g.L;
+                const uint32_t iz = (z + 1u == g.L) ? i - (g.N - g.LL) : i + g.LL;
+                bz[u] = *reinterpret_cast<const uint4 *>(spins + iz);
+            }
         }
-        unequal += acc;
-        negative += neg;
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+            uint32_t acc = 0, neg = 0;
+            acc += __popc((a[u].x ^ __funnelshift_r(a[u].x, a[u].y, 8)) & kSignMask);
+            acc += __popc((a[u].y ^ __funnelshift_r(a[u].y, a[u].z, 8)) & kSignMask);
+            acc += __popc((a[u].z ^ __funnelshift_r(a[u].z, a[u].w, 8)) & kSignMask);
+            acc += __popc((a[u].w ^ __funnelshift_r(a[u].w, nb[u], 8)) & kSignMask);
+            neg += __popc(a[u].x & kSignMask) + __popc(a[u].y & kSignMask) + __popc(a[u].z & kSignMask) + __popc(a[u].w & kSignMask);
+            acc += __popc((a[u].x ^ by[u].x) & kSignMask) + __popc((a[u].y ^ by[u].y) & kSignMask) +
+                   __popc((a[u].z ^ by[u].z) & kSignMask) + __popc((a[u].w ^ by[u].w) & kSignMask);
+            if (DIM == 3)
+                acc += __popc((a[u].x ^ bz[u].x) & kSignMask) + __popc((a[u].y ^ bz[u].y) & kSignMask) +
+                       __popc((a[u].z ^ bz[u].z) & kSignMask) + __popc((a[u].w ^ bz[u].w) & kSignMask);
+            if (on[u]) { unequal += acc; negative += neg; }
+        }
     }
-    block_accumulate(unequal, negative, ctl, g.N, DIM);
+    block_accumulate(unequal, negative, ctl, g.N, DIM, E_dst, M_dst);
 }
 
 // Generic path: any L >= 2, one site per thread iteration.
 template <int DIM>
-__global__ void __launch_bounds__(kThreads) energy_magnetisation_scalar(const int8_t *__restrict__ spins, Geometry g, Control *ctl)
+__global__ void __launch_bounds__(kThreads) energy_magnetisation_scalar(const int8_t *__restrict__ spins, Geometry g, Control *ctl,
+                                                                        long long *E_dst, long long *M_dst)
 {
     unsigned long long unequal = 0, negative = 0;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < g.N; i += gridDim.x * blockDim.x) {
@@ -149,7 +186,7 @@ __global__ void __launch_bounds__(kThreads) energy_magnetisation_scalar(const in
 #pragma unroll
         for (int d = 0; d < DIM; ++d) unequal += (spins[nbr[2 * d]] != s);
     }
-    block_accumulate(unequal, negative, ctl, g.N, DIM);
+    block_accumulate(unequal, negative, ctl, g.N, DIM, E_dst, M_dst);
 }
 
 inline int grid_for(uint64_t items, int num_sms, int per_sm)
@@ -163,32 +200,32 @@ inline int grid_for(uint64_t items, int num_sms, int per_sm)
 
 }  // namespace
 
-cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, cudaStream_t stream)
+cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, int num_sms, cudaStream_t stream)
 {
-    const int grid = grid_for((N + 15u) / 16u, 148, 8);
+    const int grid = grid_for((N + 15u) / 16u, num_sms, 8);
     init_lattice_kernel<<<grid, kThreads, 0, stream>>>(spins, N, (uint32_t)seed, (uint32_t)(seed >> 32));
     return cudaGetLastError();
 }
 
-cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, cudaStream_t stream)
+cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, int num_sms, cudaStream_t stream)
 {
-    const int grid = grid_for(N, 148, 8);
+    const int grid = grid_for((N + 15u) / 16u, num_sms, 8);
     validate_kernel<<<grid, kThreads, 0, stream>>>(spins, N, ctl);
     return cudaGetLastError();
 }
 
-cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo, int dim, Control *ctl, int num_sms,
-                                        cudaStream_t stream)
+cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo, int dim, Control *ctl,
+                                        long long *E_dst, long long *M_dst, int num_sms, cudaStream_t stream)
 {
     if (geo.L % 16u == 0u) {
-        // one wave: every SM holds up to 8 CTAs of 256 threads
-        const int grid = grid_for(geo.N / 16u, num_sms, 8);
-        if (dim == 2) energy_magnetisation_vec16<2><<<grid, kThreads, 0, stream>>>(spins, geo, ctl);
-        else          energy_magnetisation_vec16<3><<<grid, kThreads, 0, stream>>>(spins, geo, ctl);
+        // one wave, kU chunks per thread: 4 CTAs of 256 threads per SM at 16 MiB
+        const int grid = grid_for((geo.N / 16u + kU - 1) / kU, num_sms, 8);
+        if (dim == 2) energy_magnetisation_vec16<2><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
+        else          energy_magnetisation_vec16<3><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
     } else {
         const int grid = grid_for(geo.N, num_sms, 8);
-        if (dim == 2) energy_magnetisation_scalar<2><<<grid, kThreads, 0, stream>>>(spins, geo, ctl);
-        else          energy_magnetisation_scalar<3><<<grid, kThreads, 0, stream>>>(spins, geo, ctl);
+        if (dim == 2) energy_magnetisation_scalar<2><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
+        else          energy_magnetisation_scalar<3><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
     }
     return cudaGetLastError();
 }

@@ -1,0 +1,134 @@
+"""In-kernel measurement ("measure" = 1) against the oracle: E and M after EVERY update, bit-exact.
+
+PAPER.md:126, 138, 147 (the "+ measurement" columns) and Eq. 3.  The CUDA path evaluates E and M
+inside the persistent kernel (growth_tiles.cu: every CTA sums the tiles it holds; growth.cu: running values from the
+cluster's boundary bonds); the oracle sums the whole lattice after every update (oracle_run_logged) and accumulates the
+moments by their definition (oracle_moments).  Everything is integer: tolerance none, except the Binder ratio, a
+double computed from identical integers on both sides (1e-12).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import protocol_farm as farm
+from paper_1110_0899_b200 import binding, workloads as wl
+from parity_util import assert_same_state, make_pair
+from test_gpu_parity import MODES
+
+pytestmark = pytest.mark.gpu
+
+
+def compare_measured(gpu, ref, batches, acc=None):
+    """run(n) with in-kernel measurement; sizes, E and M series, accumulated moments, lattice -- all against the oracle."""
+    for n in batches:
+        gpu.run(n)
+        E, M = gpu.series()
+        _, _, sz = gpu.observables(sizes=True)
+        rs, rE, rM = ref.run_logged(n)
+        assert np.array_equal(sz, rs), "cluster sizes differ"
+        if not np.array_equal(E, rE):
+            k = int(np.nonzero(E != rE)[0][0])
+            raise AssertionError("E differs at update %d of %d: gpu %d oracle %d (size %d)" % (k, n, E[k], rE[k], rs[k]))
+        if not np.array_equal(M, rM):
+            k = int(np.nonzero(M != rM)[0][0])
+            raise AssertionError("M differs at update %d of %d: gpu %d oracle %d" % (k, n, M[k], rM[k]))
+        acc = oracle.moments_raw(rE, rM, acc=acc)
+        raw, U = gpu.moments()
+        assert np.array_equal(raw, acc), (oracle.moments_dict(raw), oracle.moments_dict(acc))
+        Uo = oracle.binder(acc)
+        assert (np.isnan(U) and np.isnan(Uo)) or abs(U - Uo) < 1e-12
+        assert_same_state(gpu, ref, "after a measured batch of %d" % n)
+    return acc
+
+
+MEASURE_MODES = [dict(o, measure=1) for o in MODES]
+
+
+@pytest.mark.parametrize("options", [{"mode": 0, "small_cluster": 0}, {"mode": 0}, {"mode": 4}, {"mode": 1},
+                                      {"mode": 0, "small_cluster": 0, "fill": 2, "tile_log": 4}])
+def test_config_c1_measured_every_update(options):
+    c = wl.CONFIGS["C1"]
+    gpu, ref = make_pair(*c.create_args(), options=dict(options, measure=1))
+    compare_measured(gpu, ref, [c.n_meas])
+    gpu.close()
+
+
+SMALL = [(2, 2, 2.0), (2, 3, 2.0), (2, 4, wl.TC_2D), (2, 6, 1.8), (3, 2, 4.0), (3, 3, wl.TC_3D), (3, 4, wl.TC_3D),
+         (2, 16, wl.TC_2D), (3, 8, wl.TC_3D), (2, 48, 2.1), (3, 12, 4.2), (2, 64, 2.0), (3, 16, 4.3)]
+
+
+@pytest.mark.parametrize("options", MEASURE_MODES)
+@pytest.mark.parametrize("dim,L,T", SMALL)
+def test_small_lattices_measured(dim, L, T, options):
+    gpu, ref = make_pair(dim, L, 1.0, T, seed=70 + L, options=options)
+    compare_measured(gpu, ref, [1, 2, 60])
+    gpu.close()
+
+
+@pytest.mark.parametrize("options", MEASURE_MODES)
+@pytest.mark.parametrize("dim,L", [(2, 64), (2, 100), (3, 16), (3, 20)])
+def test_p_one_cold_start_measured(dim, L, options):
+    # every spin in one cluster: the member log of the level-synchronous kernel runs through every tier, the post-pass
+    # sees a cluster without boundary; then ragged blobs (large boundaries)
+    N = L ** dim
+    gpu, ref = make_pair(dim, L, 1.0, 0.04, seed=3, start=wl.cold(N), options=options)
+    compare_measured(gpu, ref, [1, 1, 3])
+    gpu.set_spins(wl.blobs(dim, L, seed=5))
+    ref.set_spins(wl.blobs(dim, L, seed=5))
+    compare_measured(gpu, ref, [1] * 4, acc=gpu.moments()[0])
+    gpu.close()
+
+
+@pytest.mark.parametrize("options", [{"mode": 0, "small_cluster": 0}, {"mode": 4}, {"mode": 3}, {"mode": 1}])
+@pytest.mark.parametrize("name,n", [("C2", 150), ("C4", 100)])
+def test_medium_configs_measured(name, n, options):
+    c = wl.CONFIGS[name]
+    gpu, ref = make_pair(*c.create_args(), start=wl.cold(c.N), options=dict(options, measure=1))
+    compare_measured(gpu, ref, [3, n])
+    gpu.close()
+
+
+def test_moments_run_on_across_runs_and_reset():
+    c = wl.CONFIGS["C1"]
+    gpu, ref = make_pair(*c.create_args(), options={"measure": 1})
+    acc = compare_measured(gpu, ref, [10, 40])
+    gpu.set_option("measure", 0)                       # an unmeasured run leaves the accumulators alone
+    gpu.run(25); ref.run(25)
+    with pytest.raises(binding.WolffError):
+        gpu.series()
+    ns = gpu.update_ns()                               # durations are always recorded
+    assert ns.shape == (25,) and np.all(ns > 0)
+    assert np.array_equal(gpu.moments()[0], acc)
+    gpu.set_option("measure", 1)
+    acc = compare_measured(gpu, ref, [30], acc=acc)
+    gpu.reset_moments()
+    raw, U = gpu.moments()
+    assert not raw.any() and np.isnan(U)
+    compare_measured(gpu, ref, [20])
+    gpu.close()
+
+
+@pytest.mark.parametrize("name,options", [("C5a", {}), ("C5a", {"mode": 4}), ("C3-stretch", {})])
+def test_protocol_stretch_measured_in_kernel(name, options):
+    # the stretch of single updates of the protocol tests, as ONE measured launch: same E, M after every update
+    job = farm.JOBS[name]
+    c = wl.CONFIGS[job["cfg"]]
+    gpu = binding.Wolff(c.dim, c.L, c.J, c.T, c.seed if job["seed"] is None else job["seed"])
+    for k, v in options.items():
+        gpu.set_option(k, v)
+    gpu.set_spins(wl.cold(c.N))
+    ref = farm.result(name)
+    for b in ref["batches"]:
+        gpu.run(b["n"])
+    st = ref["stretch"]
+    gpu.set_option("measure", 1)
+    gpu.run(len(st["sizes"]))
+    E, M = gpu.series()
+    _, _, sz = gpu.observables(sizes=True)
+    assert np.array_equal(sz, st["sizes"])
+    assert np.array_equal(E, st["E"]) and np.array_equal(M, st["M"])
+    raw, U = gpu.moments()
+    acc = oracle.moments_raw(st["E"], st["M"])
+    assert np.array_equal(raw, acc) and abs(U - oracle.binder(acc)) < 1e-12
+    assert np.array_equal(farm.pack(gpu.get_spins()), st["bits"])
+    gpu.close()

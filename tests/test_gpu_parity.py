@@ -26,6 +26,8 @@ MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 3},
          {"mode": 0, "fill": 0, "small_cluster": 0},
          {"mode": 0, "fill": 2, "tile_ctas": 5, "tile_log": 4, "small_cluster": 0},
          {"mode": 0, "small_cluster": 1000000},
+         # an inbox of 32 entries: senders wait for the receiver all the time (back-pressure path)
+         {"mode": 0, "tile_log": 2, "tile_ctas": 4, "inbox_log": 5, "fill": 2, "small_cluster": 0},
          {"mode": 4, "speculative": 1, "up_threshold": 8, "down_threshold": 3, "cluster_up_threshold": 40, "grid_down_threshold": 20}]
 
 
@@ -97,7 +99,7 @@ def test_randomised_knobs_shared_memory_resident_kernel(case_seed):
         T = rng.choice([wl.TC_2D, 1.8, 3.0] if dim == 2 else [wl.TC_3D, 4.0, 5.0])
         opts = {"mode": 0, "small_cluster": 0, "tile_log": rng.choice([2, 3, 4, 5, 6]), "tile_ctas": rng.choice([0, 1, 2, 3, 7, 16, 64]),
                 "fill": rng.choice([0, 1, 2, 2]), "ring_cap": rng.choice([32, 64, 2048]), "idle_ns": rng.choice([0, 100, 1000]),
-                "fill_bufs": rng.choice([0, 1]), "fill_min_us": rng.choice([0, 30])}
+                "fill_bufs": rng.choice([0, 1]), "fill_min_us": rng.choice([0, 30]), "inbox_log": rng.choice([0, 5, 6, 9])}
         start = rng.choice([None, wl.cold(L ** dim), wl.blobs(dim, L, seed=rng.randrange(1000))])
         gpu, ref = make_pair(dim, L, 1.0, T, seed=rng.randrange(1 << 40), start=start, options=opts)
         compare_batched(gpu, ref, [rng.choice([1, 2, 5]), rng.choice([50, 300]), rng.choice([1, 500])])
@@ -163,6 +165,48 @@ def test_full_size_configs_literal_random_start(name):
     compare_batched(gpu, ref, [1000, 2000])
 
 
+def test_two_live_handles_with_different_plans_interleaved():
+    # the kernel's shared-memory attribute belongs to the process, not to a handle: a second handle of the same dim
+    # that makes a (smaller) plan must not break the launches of the first (regression: cudaErrorInvalidValue)
+    big, ref_big = make_pair(2, 1024, 1.0, wl.TC_2D, seed=5, start=wl.cold(1024 * 1024), options={"small_cluster": 0})
+    big.run(3)
+    small, ref_small = make_pair(2, 64, 1.0, wl.TC_2D, seed=6, options={"small_cluster": 0, "tile_log": 3, "fill": 0})
+    tiny, ref_tiny = make_pair(2, 16, 1.0, wl.TC_2D, seed=7, options={"small_cluster": 0, "tile_log": 2, "tile_ctas": 2})
+    ref_big.run(3)
+    for _ in range(3):
+        small.run(20); ref_small.run(20)
+        big.run(2); ref_big.run(2)
+        tiny.run(20); ref_tiny.run(20)
+        big.run(1); ref_big.run(1)
+    for g, r in ((big, ref_big), (small, ref_small), (tiny, ref_tiny)):
+        assert_same_state(g, r)
+        g.close()
+
+
+def test_watchdog_abort_is_sticky_across_queued_runs():
+    # a cold-start update of 2^24 spins takes milliseconds; with a 1 ms watchdog the first launch aborts.  The runs
+    # queued behind it must not continue from a half-grown cluster, and the abort must still be reported.
+    from paper_1110_0899_b200 import binding
+    c = wl.CONFIGS["C3"]
+    gpu = binding.Wolff(*c.create_args())
+    gpu.set_option("small_cluster", 0)
+    gpu.set_spins(wl.cold(c.N))
+    gpu.set_option("watchdog_ms", 1)
+    gpu.run(2)
+    gpu.run(2)
+    gpu.run(2)
+    with pytest.raises(binding.WolffError) as info:
+        gpu.observables()
+    assert info.value.code == binding.WOLFF_EINTERNAL
+    with pytest.raises(binding.WolffError):
+        gpu.run(1)                                  # the handle stays failed
+    gpu.close()
+    # the device and the library are fine: a fresh handle works
+    g2, ref = make_pair(2, 64, 1.0, wl.TC_2D, seed=3)
+    compare_batched(g2, ref, [50])
+    g2.close()
+
+
 def test_microbench_pass_floor_runs_as_intended():
     # the latency-roofline floor (wolff_microbench [7]): every lane must have won every claim, else the chain timed is not
     # the one DESIGN.md section 6 describes
@@ -200,7 +244,8 @@ def test_random_api_sequences(case_seed):
     rng = random.Random(2000 + case_seed)
     streams = [None, torch.cuda.Stream(), torch.cuda.Stream()]
     knobs = {"mode": [0, 0, 4, 1, 3], "small_cluster": [0, 16, 100000], "tile_log": [0, 2, 3, 4, 5], "tile_ctas": [0, 1, 3, 16],
-             "fill": [0, 1, 2], "fill_bufs": [0, 1], "ring_cap": [32, 2048], "idle_ns": [0, 1000], "fill_min_us": [0, 30]}
+             "fill": [0, 1, 2], "fill_bufs": [0, 1], "ring_cap": [32, 2048], "idle_ns": [0, 1000], "fill_min_us": [0, 30],
+             "inbox_log": [0, 5, 7]}
     for _ in range(40):
         dim = rng.choice([2, 3])
         L = rng.choice([8, 16, 32, 64] if dim == 2 else [4, 8, 16])
