@@ -2,14 +2,20 @@
 """bench.py -- throughput of the Wolff single-cluster hot path on B200, one JSON line.
 
 A "step" is one pass of the whole hot path over one batch:
-    wolff_run(h, U, stream)          -- U single-cluster updates as ONE persistent kernel launch (A1-A7)
+    wolff_run(h, U, stream)           -- U single-cluster updates as ONE persistent kernel launch (A1-A7)
     wolff_observables(h, E, M, sizes) -- the whole-lattice E/M reduction (A8) + read-back of the size log (A9)
 on the workload BASELINE.json's metric is quoted on: 2D L=4096 at T_c (primary; `value`) and 3D L=256 at T_c
 (reported under "secondary").  Start state: the 'equilibrated' variant of SURVEY.md 8(d) -- cold start followed by
 `--equil` untimed updates -- because the literal random start never reaches T_c-sized clusters within the configured
-1,000 + 10,000 updates; the literal variant is reported as updates/s under "literal_random_start".
+1,000 + 10,000 updates; the literal variant is reported as updates/s under "literal_random_start".  With the default
+U = 500 the driver's 20 steps are BASELINE.json's 10,000 measured updates.
+
+Every GPU figure has the oracle beside it, timed on the SAME clusters: the lattice and update index at the start of
+the timed region are copied out of the library and loaded into the oracle, which then runs a bounded prefix of exactly
+those updates on one host core (the algorithm is sequential; `cores` says so).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl b200|reference] [--workload C3] [--updates U]
+                    [--opt key=value ...]
 
 N > 1 (torchrun): replicas only -- every rank runs its own independent chain (seed + rank), no
 data-path collective; value = flipped spins of all ranks / max-over-ranks time.
@@ -31,6 +37,7 @@ if ROOT not in sys.path:
 
 METRIC = "flipped spins/sec & Wolff updates/sec, 2D L=4096 and 3D L=256 at T_c"
 UNIT = "flipped spins/s"
+DTYPE = "int8 spins / uint32 bond words / int64 sums"
 L2_FLUSH_BYTES = 256 << 20          # > 126 MB L2
 
 
@@ -43,10 +50,20 @@ def measured_peak_hbm():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-# ncu `--set full` DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of one launch of the growth kernel,
-# bytes: profiles/r1_growth_tiles_C3.md (a 10-update C3 launch: the 16 MiB lattice is read once in the prologue; the
-# write-back and all queue traffic stay in L2).  It does not grow with the updates per launch.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = 22624256 + 493056
+# ncu `--set full` DRAM traffic (dram__bytes_read.sum + dram__bytes_write.sum) of ONE launch of the growth kernel, by
+# (workload, growth mode): taken offline from the committed captures under profiles/ (the launch shape of each capture
+# is stated there).  Any other workload / mode / knob setting prints null -- never a figure from another configuration.
+NCU_TRAFFIC = {
+    ("C3", 0): {"bytes": 22624256 + 493056, "source": "profiles/r1_growth_tiles_C3.md (10-update launch; the traffic is the one lattice "
+                                                       "load per launch and does not grow with the updates)"},
+    ("C5a", 0): {"bytes": 66096640 + 15944960, "source": "profiles/r1_growth_tiles_C5a.md (200-update launch)"},
+}
+
+
+def ncu_traffic(workload: str, mode: int, options: dict):
+    if options:
+        return None
+    return NCU_TRAFFIC.get((workload, mode))
 
 
 class ClockSampler:
@@ -106,6 +123,14 @@ def algorithmic_bytes(dim: int, flipped: int, attempts: int) -> int:
     return flipped * (2 * dim + 8) + 4 * attempts
 
 
+def workload_config(c, equil: int, updates: int, world: int):
+    """The `config` object of the JSON line: the same for the CUDA arm and the reference arm."""
+    return {"workload": "%s, equilibrated variant: cold start + %d untimed updates, seed %d(+rank)" % (c.name, equil, c.seed),
+            "updates_per_step": updates, "step": "wolff_run(U) + wolff_observables (E, M, size log)",
+            "l2": "flushed between steps by a %d MiB write, outside the timed events" % (L2_FLUSH_BYTES >> 20),
+            "parallelism": "replicas only" if world > 1 else "single GPU"}
+
+
 # ====================================================================== N > 1: replicas only (DESIGN.md section 8)
 
 def all_reduce_scalar(x, op: str, world: int, device=None):
@@ -128,6 +153,59 @@ def aggregate_replicas(flipped: int, updates: int, total_ms: float, world: int, 
     return {"total_ms": ms, "flipped": f, "updates": u, "value": f / (ms * 1e-3), "updates_per_s": u / (ms * 1e-3)}
 
 
+# ====================================================================== the oracle beside every figure
+
+def oracle_on_same_clusters(c, seed: int, lattice, update_index: int, budget_s: float, max_updates: int, measured: bool = False):
+    """The oracle as it stands, one host core, started from the very state the GPU's timed region started from
+    (lattice bytes + update index + seed = the whole state), running a bounded prefix of exactly those updates.
+    measured=True: E and M by whole-lattice summation after every update, as the paper's CPU '+ measurement' column."""
+    import oracle
+    ref = oracle.OracleWolff(c.dim, c.L, c.J, c.T, seed)
+    ref.set_spins(lattice)
+    ref.update_index = update_index
+    flipped = n = 0
+    t0 = time.perf_counter()
+    while n < max_updates and time.perf_counter() - t0 < budget_s:
+        if measured:
+            sizes, _, _ = ref.run_logged(1)
+        else:
+            sizes = ref.run(1)
+        flipped += int(sizes[0])
+        n += 1
+    dt = time.perf_counter() - t0
+    ref.close()
+    return {"value": flipped / dt, "unit": UNIT, "updates_per_s": n / dt, "cores": 1, "kind": "oracle",
+            "sample": "%s, the first %d updates of the GPU's timed region (from update index %d, same lattice, same seed): "
+                      "%.1f s of CPU work, %d spins flipped%s" % (c.name, n, update_index, dt, flipped,
+                                                                  ", E and M summed over the lattice after every update" if measured else ""),
+            "host_cores_available": os.cpu_count()}
+
+
+def oracle_replicas(c, seeds, n_updates: int, budget_s: float, threads: int):
+    """`threads` independent oracle chains side by side (one per host core; the ctypes calls release the GIL): the
+    aggregate the host can reach on replicas.  Literal start (the oracle's own seed-derived lattice)."""
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+
+    def one(seed):
+        ref = oracle.OracleWolff(c.dim, c.L, c.J, c.T, seed)
+        t0 = time.perf_counter()
+        n = f = 0
+        while n < n_updates and time.perf_counter() - t0 < budget_s:
+            f += int(ref.run(100).sum())
+            n += 100
+        dt = time.perf_counter() - t0
+        ref.close()
+        return n, f, dt
+
+    with ThreadPoolExecutor(max_workers=threads) as pool:
+        res = list(pool.map(one, seeds[:threads]))
+    dt = max(r[2] for r in res)
+    return {"updates_per_s": sum(r[0] for r in res) / dt, "value": sum(r[1] for r in res) / dt, "unit": UNIT, "cores": threads,
+            "kind": "oracle", "one_core_updates_per_s": res[0][0] / res[0][2],
+            "sample": "%s literal random start, %d chains of up to %d updates side by side" % (c.name, threads, n_updates)}
+
+
 # ====================================================================== the CUDA arm
 
 def run_b200(args, rank: int, world: int):
@@ -146,6 +224,8 @@ def run_b200(args, rank: int, world: int):
     dev = torch.device("cuda", local_rank)
     stream = torch.cuda.Stream(device=dev)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    options = dict(args.opt)
+    launches = [0]
 
     def barrier():
         if world > 1:
@@ -153,33 +233,44 @@ def run_b200(args, rank: int, world: int):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def measure(cfg_name: str, updates: int, equil: int, steps: int, warmup: int, cold: bool):
+    def open_chain(cfg_name: str, seed: int, cold: bool, equil: int, extra=None):
         c = wl.CONFIGS[cfg_name]
-        seed = c.seed + rank
         h = binding.Wolff(c.dim, c.L, c.J, c.T, seed)
         if args.mode:
             h.set_option("mode", args.mode)
+        for k, v in list(options.items()) + list((extra or {}).items()):
+            h.set_option(k, v)
         if cold:
             h.set_spins(wl.cold(c.N))
         if equil:
             h.run(equil, stream=stream)
             h.observables()
+        return c, h
+
+    def measure(cfg_name: str, updates: int, equil: int, steps: int, warmup: int, cold: bool, seed_offset: int = 0,
+                depth_steps: int = 1, sample_clocks: bool = False):
+        """One timed leg.  Returns per-step device times, the kernel's own per-update durations, counters, the BFS depth
+        of the first `depth_steps` timed steps, and the state at the start of the timed region (for the oracle)."""
+        c = wl.CONFIGS[cfg_name]
+        seed = c.seed + rank + seed_offset
+        c, h = open_chain(cfg_name, seed, cold, equil)
         E_d = torch.zeros(1, dtype=torch.int64, device=dev)
         M_d = torch.zeros(1, dtype=torch.int64, device=dev)
         sizes_d = torch.zeros(updates, dtype=torch.int32, device=dev)
-        flipped = attempts = levels = 0
-        step_ms, growth_ms = [], []
+        ns_d = torch.zeros(updates, dtype=torch.int32, device=dev)
+        res = {"cfg": c, "h": h, "seed": seed, "flipped": 0, "attempts": 0, "levels": 0, "depth_updates": 0, "updates": updates * steps,
+               "step_ms": [], "growth_ms": [], "update_ns": []}
         # BFS depth of the clusters the timed steps grow (a property of the workload, DESIGN.md section 6): the
         # level-synchronous kernel (mode 4) replays the same updates from the same lattice, untimed, and counts levels
         twin = None
-        if args.mode == 0 and not args.no_depth:
+        if args.mode == 0 and not args.no_depth and depth_steps > 0:
             twin = binding.Wolff(c.dim, c.L, c.J, c.T, seed)
             twin.set_option("mode", 4)
             snapshot = torch.empty(c.N, dtype=torch.int8, device=dev)
 
-        def one_step(timed: bool):
-            nonlocal flipped, attempts, levels
-            if timed and twin is not None:
+        def one_step(timed: bool, index: int):
+            replay = timed and twin is not None and index < depth_steps
+            if replay:
                 h.get_spins_into(snapshot)
                 twin.set_spins(snapshot)
                 twin.update_index = h.update_index
@@ -195,38 +286,68 @@ def run_b200(args, rank: int, world: int):
                 e2.record(stream)
             e2.synchronize()
             if timed:
-                step_ms.append(e0.elapsed_time(e2))
-                growth_ms.append(e0.elapsed_time(e1))
+                launches[0] += 2
+                res["step_ms"].append(e0.elapsed_time(e2))
+                res["growth_ms"].append(e0.elapsed_time(e1))
                 st = h.stats()
-                flipped += st["flipped"]; attempts += st["claim_attempts"]
+                res["flipped"] += st["flipped"]; res["attempts"] += st["claim_attempts"]
                 assert int(sizes_d.sum().item()) == st["flipped"]
-                if twin is not None:
+                h.series_into(None, None, ns_d)
+                res["update_ns"].append(ns_d.cpu().numpy().astype(np.uint32).astype(np.float64))
+                if replay:
                     twin.run(updates, stream=stream)
                     ts = twin.stats()
                     assert ts["flipped"] == st["flipped"]
-                    st = ts
-                levels += st["levels_cta"] + st["levels_cluster"] + st["levels_grid"]
+                    res["levels"] += ts["levels_cta"] + ts["levels_cluster"] + ts["levels_grid"]
+                    res["depth_updates"] += updates
+                    res["depth_growth_ms"] = res.get("depth_growth_ms", 0.0) + e0.elapsed_time(e1)
 
-        for _ in range(warmup):
-            one_step(False)
+        for i in range(warmup):
+            one_step(False, i)
+        # the state the timed region starts from: lattice + update index (+ seed) is the whole state of a chain
+        res["start_lattice"] = h.get_spins()
+        res["start_index"] = h.update_index
         barrier()
-        t0 = time.perf_counter()
-        with ClockSampler(local_rank) as clocks:
-            for _ in range(steps):
-                one_step(True)
-            barrier()
-        wall = time.perf_counter() - t0
+        if sample_clocks:
+            with ClockSampler(local_rank) as clocks:
+                for i in range(steps):
+                    one_step(True, i)
+                barrier()
+            res["clocks"] = clocks.summary()
+        else:
+            for i in range(steps):
+                one_step(True, i)
         if twin is not None:
             twin.close()
-        res = {"cfg": c, "h": h, "flipped": flipped, "attempts": attempts, "levels": levels, "updates": updates * steps,
-               "step_ms": step_ms, "growth_ms": growth_ms, "wall_s": wall, "clocks": clocks.summary()}
+        ns = np.concatenate(res["update_ns"]) if res["update_ns"] else np.zeros(1)
+        res["ms_per_update_mean_in_kernel"] = float(ns.mean()) * 1e-6
+        res["ms_per_update_median_in_kernel"] = float(np.median(ns)) * 1e-6
         return res
 
-    def measurement_legs(h, cfg, n_updates: int):
-        """Row A8 on its own (the E/M reduction through the C-ABI, L2 flushed / warm) and the paper's '+ measurement'
-        protocol: E and M after EVERY update, i.e. run(1) + observables in a loop."""
+    def leg_summary(r, oracle_budget: float, oracle_max: int = 10 ** 9):
+        ms = sum(r["step_ms"])
+        out = {"value": r["flipped"] / (ms * 1e-3), "unit": UNIT, "updates_per_s": r["updates"] / (ms * 1e-3),
+               "updates_timed": r["updates"], "mean_cluster": r["flipped"] / max(r["updates"], 1),
+               "ms_per_update_mean": ms / max(r["updates"], 1), "ms_per_update_median": r["ms_per_update_median_in_kernel"],
+               "ms_per_update_note": "mean = device time of the steps / updates; median = the kernel's own per-update durations (wolff_get_series)"}
+        if r["depth_updates"]:
+            out["bfs_depth_per_update"] = r["levels"] / r["depth_updates"]
+            out["us_per_bfs_level"] = r["depth_growth_ms"] * 1e3 / max(r["levels"], 1)
+            out["bfs_depth_sample"] = "the first %d timed updates, replayed untimed by the level-synchronous kernel" % r["depth_updates"]
+        if rank == 0 and not args.no_cpu_baseline and oracle_budget > 0:
+            out["cpu_baseline"] = oracle_on_same_clusters(r["cfg"], r["seed"], r["start_lattice"], r["start_index"], oracle_budget, oracle_max)
+            out["gpu_over_one_cpu_core"] = out["value"] / out["cpu_baseline"]["value"] if out["cpu_baseline"]["value"] else None
+        return out
+
+    def measurement_legs(cfg_name: str, seed: int, lattice, index: int, n_updates: int, oracle_budget: float):
+        """Row A8 on its own, and the paper's '+ measurement' protocol (E and M after EVERY
+        update) three ways on the SAME updates, from the same state: update only; measured inside the persistent kernel
+        ("measure" = 1, ONE launch); and the host loop run(1) + observables per update (one launch per update)."""
+        c, h = open_chain(cfg_name, seed, False, 0)
+        lat_d = torch.from_numpy(lattice).to(dev)
         E_d = torch.zeros(1, dtype=torch.int64, device=dev)
         M_d = torch.zeros(1, dtype=torch.int64, device=dev)
+
         def timed_observables(cold: bool):
             best = None
             for _ in range(5):
@@ -241,49 +362,101 @@ def run_b200(args, rank: int, world: int):
                 ms = e0.elapsed_time(e1)
                 best = ms if best is None else min(best, ms)
             return best
+
+        def reset():
+            h.set_spins(lat_d)
+            h.update_index = index
+
+        def timed_run(measure: int, n: int):
+            reset()
+            h.set_option("measure", measure)
+            h.run(3, stream=stream); h.observables()       # the kernel choice of mode 0 and the tables settle
+            reset()
+            with torch.cuda.stream(stream):
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                h.run(n, stream=stream)
+                e1.record(stream)
+            e1.synchronize()
+            launches[0] += 1
+            return e0.elapsed_time(e1), h.stats()["flipped"]
+
+        reset()
         cold_ms, warm_ms = timed_observables(True), timed_observables(False)
+        plain_ms, flipped = timed_run(0, n_updates)
+        meas_ms, flipped_m = timed_run(1, n_updates)
+        assert flipped == flipped_m
+        # host loop: one launch + one whole-lattice reduction per update
+        h.set_option("measure", 0)
+        reset()
+        n_loop = min(n_updates, 50 if c.N > (1 << 22) and cfg_name == "C3" else 200)
         sz = torch.zeros(1, dtype=torch.int32, device=dev)
-        flipped = 0
+        loop_flipped = 0
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for _ in range(n_updates):
+        for _ in range(n_loop):
             h.run(1, stream=stream)
             h.observables_into(E_d, M_d, sz)
-            flipped += int(sz.item())
-        dt = time.perf_counter() - t0
+            loop_flipped += int(sz.item())
+        loop_dt = time.perf_counter() - t0
+        launches[0] += 2 * n_loop
         peak, _ = measured_peak_hbm()
-        return {"a8_energy_magnetisation": {"bound": "hbm", "bytes": cfg.N, "cold_l2_us": cold_ms * 1e3, "warm_l2_us": warm_ms * 1e3,
-                                            "cold_l2_gbs": cfg.N / (cold_ms * 1e-3) / 1e9, "warm_l2_gbs": cfg.N / (warm_ms * 1e-3) / 1e9,
-                                            "peak": peak, "frac_cold": cfg.N / (cold_ms * 1e-3) / 1e9 / peak,
-                                            "note": "wolff_observables(E, M) with device pointers: the reduction kernel, two 8-byte copies and "
-                                                    "a stream synchronise; at 16 MiB the call is launch-latency bound"},
-                "with_measurement_every_update": {"updates": n_updates, "updates_per_s": n_updates / dt, "value": flipped / dt, "unit": UNIT,
-                                                  "ms_per_update": dt * 1e3 / n_updates, "protocol": "run(1) + observables(E, M, size) per update, host wall clock"}}
+        out = {"a8_energy_magnetisation": {"bound": "hbm", "bytes": c.N, "cold_l2_us": cold_ms * 1e3, "warm_l2_us": warm_ms * 1e3,
+                                           "cold_l2_gbs": c.N / (cold_ms * 1e-3) / 1e9, "warm_l2_gbs": c.N / (warm_ms * 1e-3) / 1e9,
+                                           "peak": peak, "frac_cold": c.N / (cold_ms * 1e-3) / 1e9 / peak,
+                                           "note": "wolff_observables(E, M) as a call, device destinations written by the reduction kernel "
+                                                   "itself: launch + kernel + one small read-back of the control block + one synchronise"},
+               "with_measurement_every_update": {
+                   "updates": n_updates, "same_updates_same_state": True,
+                   "update_only_ms_per_update": plain_ms / n_updates,
+                   "in_kernel_ms_per_update": meas_ms / n_updates, "in_kernel_over_update_only": meas_ms / plain_ms,
+                   "in_kernel_value": flipped / (meas_ms * 1e-3), "unit": UNIT,
+                   "in_kernel_protocol": "set_option('measure', 1); run(%d): ONE launch, E and M after every update on the device" % n_updates,
+                   "host_loop_updates": n_loop, "host_loop_ms_per_update": loop_dt * 1e3 / n_loop,
+                   "host_loop_value": loop_flipped / loop_dt,
+                   "host_loop_protocol": "run(1) + observables(E, M, size) per update, host wall clock"}}
+        if rank == 0 and not args.no_cpu_baseline and oracle_budget > 0:
+            out["with_measurement_every_update"]["cpu_baseline"] = oracle_on_same_clusters(c, seed, lattice, index, oracle_budget, n_updates, measured=True)
+        h.close()
+        return out
 
-    def e2e(cfg_name: str, updates: int, steps: int, warmup: int, h):
-        """Same metric through the C-ABI with HOST buffers: every step copies the lattice in from pinned host
-        memory, runs, and reads E, M, the size log and the lattice back to the host."""
+    def batch_leg(cfg_name: str, R: int, n: int, cold: bool, equil: int, oracle_budget: float):
+        """R independent chains in ONE launch (wolff_batch_run): aggregate updates/s and flipped spins/s."""
         c = wl.CONFIGS[cfg_name]
-        lattice = torch.empty(c.N, dtype=torch.int8).pin_memory()
-        sizes = torch.empty(updates, dtype=torch.int32).pin_memory()
-        em = torch.zeros(2, dtype=torch.int64).pin_memory()
-        h.get_spins_into(lattice)
-        flipped = 0
-        def step():
-            h.set_spins(lattice)                                   # H2D: N bytes
-            h.run(updates, stream=stream)
-            h.observables_into(em.data_ptr(), em.data_ptr() + 8, sizes)   # D2H: 16 + 4*updates bytes
-            h.get_spins_into(lattice)                              # D2H: N bytes
-            return int(sizes.sum().item())
-        for _ in range(warmup):
-            step()
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(steps):
-            flipped += step()
-        barrier()
-        dt = time.perf_counter() - t0
-        return {"flipped": flipped, "seconds": dt, "h2d": c.N, "d2h": c.N + 16 + 4 * updates}
+        seeds = [c.seed + 1000 * rank + r for r in range(R)]
+        b = binding.WolffBatch(c.dim, c.L, c.J, [c.T] * R, seeds)
+        if cold:
+            b.set_spins(torch.ones(R * c.N, dtype=torch.int8, device=dev))
+        if equil:
+            b.run(equil, stream=stream)
+            b.stats()
+        best = None
+        for _ in range(2):
+            with torch.cuda.stream(stream):
+                flush.fill_(1)
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                b.run(n, stream=stream)
+                e1.record(stream)
+            e1.synchronize()
+            launches[0] += 1
+            st = b.stats()
+            ms = e0.elapsed_time(e1)
+            if best is None or ms < best[0]:
+                best = (ms, st)
+        b.close()
+        ms, st = best
+        agg = aggregate_replicas(st["flipped"], st["updates"], ms, world, dev)
+        out = {"workload": "%s, %s, %d chains (seeds %d..) in one launch, %d updates each after %d untimed" %
+                           (c.name, "cold start" if cold else "literal random start", R, seeds[0], n, equil),
+               "replicas": R * world, "updates_per_s": agg["updates_per_s"], "value": agg["value"], "unit": UNIT,
+               "mean_cluster": st["flipped"] / max(st["updates"], 1), "bfs_levels_per_update": st["levels"] / max(st["updates"], 1),
+               "ms": ms}
+        if rank == 0 and not args.no_cpu_baseline and oracle_budget > 0 and not cold:
+            cores = os.cpu_count() or 1
+            out["cpu_baseline_one_core"] = oracle_replicas(c, seeds, 20000, oracle_budget, 1)
+            out["cpu_baseline_all_cores"] = oracle_replicas(c, seeds, 20000, oracle_budget, cores)
+        return out
 
     def reduce_sum(x):
         return all_reduce_scalar(x, "sum", world, dev)
@@ -291,131 +464,190 @@ def run_b200(args, rank: int, world: int):
     def reduce_max(x):
         return all_reduce_scalar(x, "max", world, dev)
 
-    primary = measure(args.workload, args.updates, args.equil, args.steps, args.warmup, cold=True)
+    # ------------------------------------------------------------------ primary leg
+    primary = measure(args.workload, args.updates, args.equil, args.steps, args.warmup, cold=True, sample_clocks=True)
     c = primary["cfg"]
     agg = aggregate_replicas(primary["flipped"], primary["updates"], sum(primary["step_ms"]), world, dev)
     total_ms, updates_all, value = agg["total_ms"], agg["updates"], agg["value"]
 
-    e = e2e(args.workload, args.updates, args.steps, args.warmup, primary["h"])
+    def e2e(h):
+        """Same metric through the C-ABI with HOST buffers: every step copies the lattice in from pinned host
+        memory, runs, and reads E, M, the size log and the lattice back to the host."""
+        updates = args.updates
+        lattice = torch.empty(c.N, dtype=torch.int8).pin_memory()
+        sizes = torch.empty(updates, dtype=torch.int32).pin_memory()
+        em = torch.zeros(2, dtype=torch.int64).pin_memory()
+        h.get_spins_into(lattice)
+        flipped = 0
+
+        def step():
+            h.set_spins(lattice)                                   # H2D: N bytes
+            h.run(updates, stream=stream)
+            h.observables_into(em.data_ptr(), em.data_ptr() + 8, sizes)   # D2H: 16 + 4*updates bytes
+            h.get_spins_into(lattice)                              # D2H: N bytes
+            return int(sizes.sum().item())
+        for _ in range(args.warmup):
+            step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            flipped += step()
+        barrier()
+        dt = time.perf_counter() - t0
+        launches[0] += 3 * args.steps                              # validation, growth, E/M reduction
+        return {"flipped": flipped, "seconds": dt, "h2d": c.N, "d2h": c.N + 16 + 4 * updates}
+
+    e = e2e(primary["h"])
     e2e_value = reduce_sum(e["flipped"]) / reduce_max(e["seconds"])
+    primary["h"].close()
 
     peak, peak_src = measured_peak_hbm()
     alg_bytes = algorithmic_bytes(c.dim, primary["flipped"], primary["attempts"]) / args.steps
     avg_growth_s = sum(primary["growth_ms"]) / args.steps * 1e-3
     achieved = alg_bytes / avg_growth_s / 1e9
+    traffic = ncu_traffic(args.workload, args.mode, options)
+    summary = leg_summary(primary, args.cpu_seconds if world == 1 else 0.0)
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "int8 spins / uint32 bond words / int64 sums", "data": "synthetic",
-        "config": {"workload": "%s, equilibrated variant: cold start + %d untimed updates, seed %d(+rank)" % (c.name, args.equil, c.seed),
-                   "updates_per_step": args.updates, "step": "wolff_run(U) + wolff_observables (E, M, size log)",
-                   "l2": "flushed between steps by a %d MiB write, outside the timed events" % (L2_FLUSH_BYTES >> 20),
-                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "dtype": DTYPE, "data": "synthetic",
+        "config": workload_config(c, args.equil, args.updates, world),
+        "options": options,
         "updates_per_s": updates_all / (total_ms * 1e-3),
+        "updates_timed": primary["updates"],
         "mean_cluster": primary["flipped"] / primary["updates"],
-        "bfs_depth_per_update": primary["levels"] / primary["updates"],
-        "us_per_bfs_level": sum(primary["growth_ms"]) * 1e3 / max(primary["levels"], 1),
+        "ms_per_update_mean": summary["ms_per_update_mean"], "ms_per_update_median": summary["ms_per_update_median"],
         "clocks": primary["clocks"],
-        "gpu_launches": 2 * args.steps,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"]},
         "roofline": {"bound": "hbm", "kernel": ("growth_tiles_kernel" if args.mode == 0 else "growth_kernel") + " (persistent, one launch per step)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH, "peak_source": peak_src,
-                     "algorithmic_bytes_per_launch": alg_bytes,
-                     "note": "latency-bound by design: the path is a chain of dependent hops (BFS depth x hop latency), not a stream; "
-                             "see bfs_depth_per_update and us_per_bfs_level"},
+                     "traffic": traffic["bytes"] if traffic else None,
+                     "traffic_source": traffic["source"] if traffic else "no committed ncu capture for this workload / mode / options",
+                     "peak_source": peak_src, "algorithmic_bytes_per_launch": alg_bytes,
+                     "note": "the fraction is ~1e-3 by the nature of the path: a chain of dependent hops (BFS depth x hop latency) on a "
+                             "lattice that lives in shared memory, not a stream; latency_roofline is the bound that describes it"},
     }
+    for key in ("bfs_depth_per_update", "us_per_bfs_level", "bfs_depth_sample", "cpu_baseline", "gpu_over_one_cpu_core"):
+        if key in summary:
+            out[key] = summary[key]
 
-    if rank == 0 and world == 1 and not args.no_depth and args.mode == 0:
+    single = rank == 0 and world == 1
+    if single and not args.no_depth and args.mode == 0 and "bfs_depth_per_update" in summary:
         # latency roofline (DESIGN.md section 6): T_update >= BFS depth x t_pass, t_pass floor from wolff_microbench [7]
         micro = binding.microbench()
-        depth = primary["levels"] / primary["updates"]
+        depth = summary["bfs_depth_per_update"]
         floor_ms = depth * micro["smem_pass_floor_ns"] * 1e-6
-        achieved_ms = sum(primary["growth_ms"]) / primary["updates"]
-        out["latency_roofline"] = {"bfs_depth_per_update": depth, "t_pass_floor_ns": micro["smem_pass_floor_ns"],
+        achieved_ms = primary["depth_growth_ms"] / primary["depth_updates"]
+        out["latency_roofline"] = {"bound": "latency", "bfs_depth_per_update": depth, "t_pass_floor_ns": micro["smem_pass_floor_ns"],
                                    "bound_ms_per_update": floor_ms, "achieved_ms_per_update": achieved_ms,
-                                   "frac": floor_ms / achieved_ms if achieved_ms else None,
+                                   "frac": floor_ms / achieved_ms if achieved_ms else None, "sample": summary["bfs_depth_sample"],
                                    "microbench_ns": {k: v for k, v in micro.items()}}
-    if rank == 0 and world == 1 and not args.no_secondary:
-        out.update(measurement_legs(primary["h"], c, 50))
-        primary["h"].close()
+    if single and not args.no_secondary:
+        osec = args.leg_cpu_seconds
+        # spread over seeds (SURVEY.md 8(d) "Timing protocol"): the same leg on seeds +1, +2, fewer steps
+        seeds = {"seed %d" % c.seed: {"value": value, "updates": primary["updates"], "ms_per_update_mean": summary["ms_per_update_mean"],
+                                      "ms_per_update_median": summary["ms_per_update_median"], "mean_cluster": out["mean_cluster"]}}
+        for off in (1, 2):
+            r = measure(args.workload, args.updates, args.equil, max(2, args.steps // 5), 1, cold=True, seed_offset=off, depth_steps=0)
+            s = leg_summary(r, 0.0)
+            seeds["seed %d" % r["seed"]] = {k: s[k] for k in ("value", "ms_per_update_mean", "ms_per_update_median", "mean_cluster")}
+            seeds["seed %d" % r["seed"]]["updates"] = r["updates"]
+            r["h"].close()
+        out["seeds"] = seeds
+        out.update(measurement_legs(args.workload, primary["seed"], primary["start_lattice"], primary["start_index"], args.updates, osec))
+
         sec = measure(args.secondary, args.secondary_updates, args.equil, args.steps, args.warmup, cold=True)
         sc = sec["cfg"]
-        ms = sum(sec["step_ms"])
-        out["secondary"] = {"workload": sc.name + ", equilibrated variant", "value": sec["flipped"] / (ms * 1e-3), "unit": UNIT,
-                            "updates_per_s": sec["updates"] / (ms * 1e-3), "ms_per_step": ms / args.steps,
-                            "updates_per_step": args.secondary_updates, "mean_cluster": sec["flipped"] / sec["updates"],
-                            "bfs_depth_per_update": sec["levels"] / sec["updates"],
-                            "us_per_bfs_level": sum(sec["growth_ms"]) * 1e3 / max(sec["levels"], 1)}
-        out["secondary"].update(measurement_legs(sec["h"], sc, 500))
+        out["secondary"] = dict(workload=sc.name + ", equilibrated variant: cold start + %d untimed updates" % args.equil,
+                                updates_per_step=args.secondary_updates, ms_per_step=sum(sec["step_ms"]) / args.steps, **leg_summary(sec, osec))
         sec["h"].close()
+        out["secondary"].update(measurement_legs(args.secondary, sec["seed"], sec["start_lattice"], sec["start_index"],
+                                                 args.secondary_updates, osec))
         lit = {}
         for name in (args.workload, args.secondary, "C5b"):
-            r = measure(name, 1000, 1000, max(1, args.steps // 2), 1, cold=False)
-            ms = sum(r["step_ms"])
-            lit[wl.CONFIGS[name].name] = {"updates_per_s": r["updates"] / (ms * 1e-3), "mean_cluster": r["flipped"] / r["updates"]}
+            r = measure(name, 1000, 1000, max(1, args.steps // 2), 1, cold=False, depth_steps=0)
+            lit[wl.CONFIGS[name].name] = leg_summary(r, osec, oracle_max=r["updates"])
             r["h"].close()
         out["literal_random_start"] = lit
         # C5b (T = 5.0, disordered phase) from a cold start: equilibrium clusters of a few tens of spins
-        r = measure("C5b", 10000, 1000, max(1, args.steps // 2), 1, cold=True)
-        ms = sum(r["step_ms"])
-        out["c5b_equilibrated"] = {"workload": wl.CONFIGS["C5b"].name + ", cold start + 1000 untimed updates", "updates_per_s": r["updates"] / (ms * 1e-3),
-                                   "value": r["flipped"] / (ms * 1e-3), "unit": UNIT, "mean_cluster": r["flipped"] / r["updates"]}
+        r = measure("C5b", 10000, 1000, max(1, args.steps // 2), 1, cold=True, depth_steps=0)
+        out["c5b_equilibrated"] = dict(workload=wl.CONFIGS["C5b"].name + ", cold start + 1000 untimed updates", **leg_summary(r, osec, oracle_max=r["updates"]))
         r["h"].close()
-
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        out["cpu_baseline"] = cpu_baseline(args.workload, budget_s=args.cpu_seconds)
+    if not args.no_batch and (single or world > 1):
+        # f1: independent replicas in one launch (SURVEY.md 8(f) row 1) -- the small-cluster regime is where one chain
+        # cannot fill the chip
+        osec = args.leg_cpu_seconds if single else 0.0
+        out["batch_replicas"] = {
+            "C5b_literal": batch_leg("C5b", args.batch_replicas, 2000, False, 200, osec),
+            "C2_literal": batch_leg("C2", 4 * args.batch_replicas, 2000, False, 200, osec),
+            "C1_equilibrated": batch_leg("C1", 4 * args.batch_replicas, 2000, False, 1000, 0.0),
+            "C2_equilibrated": batch_leg("C2", args.batch_replicas // 2, 40, True, 300, 0.0),
+        }
+    out["gpu_launches"] = launches[0]
     return out
 
 
 # ====================================================================== the oracle arm (CPU)
 
-def cpu_baseline(cfg_name: str, budget_s: float):
-    """The oracle as it stands, one host core, on a bounded sample of the same workload."""
-    import oracle
-    from paper_1110_0899_b200 import workloads as wl
-    c = wl.CONFIGS[cfg_name]
-    ref = oracle.OracleWolff(*c.create_args())
-    ref.set_spins(wl.cold(c.N))
-    flipped = n = 0
-    t0 = time.perf_counter()
-    while time.perf_counter() - t0 < budget_s:
-        flipped += int(ref.run(1)[0])
-        n += 1
-    dt = time.perf_counter() - t0
-    return {"value": flipped / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "%s cold start, first %d updates (%.1f s of CPU work, %d spins flipped)" % (c.name, n, dt, flipped),
-            "updates_per_s": n / dt, "host_cores_available": os.cpu_count()}
-
-
 def run_reference(args):
-    """--impl reference: the oracle timed on the host; each step is a bounded sample of the workload."""
+    """--impl reference: the oracle, as it stands, on one host core, on the CUDA arm's workload and config.  The
+    chain is brought to the state the CUDA arm's timed region starts from -- cold start, `--equil` updates, the warm-up
+    steps -- by the CUDA library when a GPU is there (untimed: the sequential oracle needs minutes for it), else by
+    the oracle itself with a shorter equilibration; the timed steps run the oracle alone, each on a bounded number of
+    the very updates the CUDA arm times."""
     import oracle
     from paper_1110_0899_b200 import workloads as wl
     c = wl.CONFIGS[args.workload]
-    ref = oracle.OracleWolff(*c.create_args())
-    ref.set_spins(wl.cold(c.N))
+    seed = c.seed
+    ref = oracle.OracleWolff(c.dim, c.L, c.J, c.T, seed)
+    start = None
+    try:
+        import torch
+        if torch.cuda.is_available():
+            from paper_1110_0899_b200 import binding, build as cuda_build
+            cuda_build.build()
+            torch.cuda.set_device(0)
+            h = binding.Wolff(c.dim, c.L, c.J, c.T, seed)
+            h.set_spins(wl.cold(c.N))
+            h.run(args.equil + args.warmup * args.updates)          # what precedes the CUDA arm's timed region
+            ref.set_spins(h.get_spins())
+            ref.update_index = h.update_index
+            start = "state at update index %d taken from the CUDA library (cold start + %d + %d warm-up updates, untimed)" % (
+                h.update_index, args.equil, args.warmup * args.updates)
+            h.close()
+    except Exception as exc:                                       # no GPU / no library: the oracle equilibrates itself
+        sys.stderr.write("reference arm: CUDA equilibration unavailable (%s)\n" % exc)
+    if start is None:
+        ref.set_spins(wl.cold(c.N))
+        ref.run(args.reference_equil)
+        start = "cold start + %d oracle updates (no GPU for the equilibration: NOT the CUDA arm's clusters)" % args.reference_equil
     per_step = args.reference_updates
     for _ in range(args.warmup):
-        ref.run(per_step)
+        ref.run(1)                                                 # warm the caches; the chain moves on by W updates
     flipped = 0
     t0 = time.perf_counter()
     for _ in range(args.steps):
         flipped += int(ref.run(per_step).sum())
     dt = time.perf_counter() - t0
     value = flipped / dt
-    sample = "%s cold start, updates %d..%d (%d per step)" % (c.name, args.warmup * per_step,
-                                                             (args.warmup + args.steps) * per_step - 1, per_step)
+    sample = "%s; each step = %d consecutive updates of that chain (bounded sample of the %d-update step), %d steps timed" % (
+        start, per_step, args.updates, args.steps)
     return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "int8 spins / uint32 bond words / int64 sums", "data": "synthetic",
-            "config": {"workload": "%s, cold start (bounded sample)" % c.name, "updates_per_step": per_step,
-                       "step": "oracle_run(U)", "parallelism": "one host core"},
-            "updates_per_s": per_step * args.steps / dt,
+            "vs_baseline": None, "dtype": DTYPE, "data": "synthetic",
+            "config": workload_config(c, args.equil, args.updates, 1),
+            "updates_per_s": per_step * args.steps / dt, "mean_cluster": flipped / (per_step * args.steps),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
+
+
+def parse_opt(text: str):
+    key, _, value = text.partition("=")
+    if not key or not value:
+        raise argparse.ArgumentTypeError("expected key=value")
+    return key, int(value)
 
 
 def main():
@@ -425,15 +657,20 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workload", default="C3")
-    ap.add_argument("--updates", type=int, default=100, help="updates per step (primary workload)")
+    ap.add_argument("--updates", type=int, default=500, help="updates per step (primary workload); 20 steps = BASELINE's 10,000")
     ap.add_argument("--secondary", default="C5a")
     ap.add_argument("--secondary-updates", type=int, default=1000)
     ap.add_argument("--equil", type=int, default=1000, help="untimed equilibration updates after the cold start")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0)
-    ap.add_argument("--reference-updates", type=int, default=3)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="oracle budget beside the primary leg")
+    ap.add_argument("--leg-cpu-seconds", type=float, default=3.0, help="oracle budget beside each of the other legs")
+    ap.add_argument("--reference-updates", type=int, default=20, help="--impl reference: oracle updates per step")
+    ap.add_argument("--reference-equil", type=int, default=100, help="--impl reference without a GPU: oracle equilibration updates")
+    ap.add_argument("--batch-replicas", type=int, default=296, help="chains of the batch legs at 3D L=256 (x4 at the small lattices)")
     ap.add_argument("--mode", type=int, default=0, help="growth kernel: 0 = default (shared-memory-resident), 4 = level-synchronous tiers")
+    ap.add_argument("--opt", type=parse_opt, action="append", default=[], help="wolff_set_option key=value for every chain of the bench")
     ap.add_argument("--no-depth", action="store_true", help="skip the untimed BFS-depth replay of the timed updates")
     ap.add_argument("--no-secondary", action="store_true")
+    ap.add_argument("--no-batch", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":

@@ -140,8 +140,8 @@ WOLFF_API int wolff_reset_moments(wolff_handle h);
  *   "tile_ctas"            ... CTAs that share the lattice (0 = one per SM)
  *   "ring_cap"             ... entries of a CTA's shared-memory work ring (power of two; overflow spills to global memory)
  *   "inbox_log"            ... log2 of the entries of a CTA's inbox, the global-memory queue of claims other CTAs send it
- *                          (0 = auto: what one update can send at most, capped at 12; 5..24).  A sender that finds an
- *                          inbox full waits for its receiver, which never waits for anybody
+ *                          (0 = auto: what one update can send at most, no capacity checks; 5..24: a smaller inbox --
+ *                          a sender that finds it full waits for the receiver, which never waits for anybody)
  *   "fill"                 ... bond tables: 0 = never (Philox inline), 1 = filled by idle warps when updates are long
  *                          enough to pay for it (default), 2 = always
  *   "fill_bufs"            ... bond-table buffers: 0 = two (the running update and the next one) when they fit beside the
@@ -194,6 +194,43 @@ WOLFF_API int wolff_microbench(double *out_ns, int n_out);
 
 /* Free everything.  NULL is allowed. */
 WOLFF_API int wolff_destroy(wolff_handle h);
+
+/* ------------------------------------------------------------------------------------------------------------------
+ * A BATCH of R independent chains in one launch.
+ *
+ * The paper's physics results are sweeps over temperatures and lattice sizes (the temperature
+ * dependence of the timings, Fig. 1, and the Binder ratio U(T) for several L, Fig. 2, Eq. 3): many independent chains.
+ * A batch holds R chains of the same dim and L, chain r with its own J[r], T[r] and seed[r]; wolff_batch_run performs
+ * n_updates updates of EVERY chain in ONE persistent launch, one CTA per chain at a time (a CTA takes the next chain
+ * when it has finished one), so up to 8-16 chains per SM are in flight.  Chain r computes, bit for bit, what a single
+ * chain made by wolff_create(dim, L, J[r], T[r], seed[r]) computes: same start lattice, same site draws, same bond
+ * variables, same update index (the index is shared by the chains of a batch and advances by n_updates per run).
+ * Layouts are replica-major: E[r], M[r]; cluster_sizes[r * n_updates + k]; spins[r * N + i]; series likewise.
+ * Ownership, pointer kinds (host or device), error codes and blocking behaviour are those of the single-chain calls. */
+typedef struct wolff_batch_ctx *wolff_batch;
+
+/* J, T, seed: host arrays of R values.  1 <= R <= 2^20; the device must hold R * 5 N bytes. */
+WOLFF_API wolff_batch wolff_batch_create(int dim, int L, int R, const double *J, const double *T, const uint64_t *seed);
+WOLFF_API int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream);
+/* E[R], M[R] of the current lattices (whole-lattice sums); cluster_sizes[R * n_updates] of the most recent run. */
+WOLFF_API int wolff_batch_observables(wolff_batch b, int64_t *E, int64_t *M, uint32_t *cluster_sizes);
+WOLFF_API int wolff_batch_get_spins(wolff_batch b, int8_t *dst);           /* R * N bytes */
+WOLFF_API int wolff_batch_set_spins(wolff_batch b, const int8_t *src);     /* R * N bytes, each +1 or -1 */
+WOLFF_API int wolff_batch_get_state(wolff_batch b, uint64_t *update_index, uint64_t *thresholds /* R values */);
+WOLFF_API int wolff_batch_set_update_index(wolff_batch b, uint64_t update_index);
+/* Keys: "measure" 0 | 1 (E and M after every update of every chain, inside the kernel: see wolff_get_series);
+ * "threads" threads per CTA: 0 = auto (256 for few chains, 64 for many), 32, 64, 128, 256;
+ * "queue_cap" entries of a CTA's shared-memory copy of the frontier (wider frontiers are read from the member list). */
+WOLFF_API int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value);
+/* E and M after every update of the most recent (measured) run: R * n_updates values each. */
+WOLFF_API int wolff_batch_get_series(wolff_batch b, int64_t *E_series, int64_t *M_series);
+/* moments: R * 10 words (layout of wolff_get_moments); binder: R doubles (Eq. 3).  Host pointers. */
+WOLFF_API int wolff_batch_get_moments(wolff_batch b, uint64_t *moments, double *binder);
+WOLFF_API int wolff_batch_reset_moments(wolff_batch b);
+/* Counters of the most recent run (host pointer, 4 values): updates, flipped spins, BFS levels, claim attempts,
+ * summed over the chains. */
+WOLFF_API int wolff_batch_get_stats(wolff_batch b, uint64_t *stats);
+WOLFF_API int wolff_batch_destroy(wolff_batch b);
 
 /* Reason for the last failure on this thread (static storage, never NULL). */
 WOLFF_API const char *wolff_last_error(void);

@@ -37,6 +37,20 @@ _SIGNATURES = {
     "wolff_get_stats": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]),
     "wolff_microbench": (ctypes.c_int, [ctypes.POINTER(ctypes.c_double), ctypes.c_int]),
     "wolff_destroy": (ctypes.c_int, [ctypes.c_void_p]),
+    "wolff_batch_create": (ctypes.c_void_p, [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                                             ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_uint64)]),
+    "wolff_batch_run": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_uint64, ctypes.c_void_p]),
+    "wolff_batch_observables": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_batch_get_spins": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_batch_set_spins": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_batch_get_state": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_uint64)]),
+    "wolff_batch_set_update_index": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_uint64]),
+    "wolff_batch_set_option": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_char_p, ctypes.c_int64]),
+    "wolff_batch_get_series": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]),
+    "wolff_batch_get_moments": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64), ctypes.POINTER(ctypes.c_double)]),
+    "wolff_batch_reset_moments": (ctypes.c_int, [ctypes.c_void_p]),
+    "wolff_batch_get_stats": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]),
+    "wolff_batch_destroy": (ctypes.c_int, [ctypes.c_void_p]),
     "wolff_last_error": (ctypes.c_char_p, []),
 }
 
@@ -227,3 +241,118 @@ class Wolff:
         buf = (ctypes.c_uint64 * NSTATS)()
         self._check(self._lib.wolff_get_stats(self._h, buf))
         return dict(zip(STAT_NAMES, (int(x) for x in buf)))
+
+
+BATCH_STAT_NAMES = ("updates", "flipped", "levels", "claim_attempts")
+
+
+class WolffBatch:
+    """R independent chains of one shape in one launch (wolff_batch_create .. wolff_batch_destroy)."""
+
+    def __init__(self, dim: int, L: int, J, T, seed):
+        self._lib = load()
+        T = [float(t) for t in np.atleast_1d(T)]
+        R = len(T)
+        J = [float(j) for j in np.broadcast_to(np.atleast_1d(J), (R,))]
+        seed = [int(x) for x in np.broadcast_to(np.atleast_1d(np.asarray(seed, dtype=np.uint64)), (R,))]
+        self._h = self._lib.wolff_batch_create(int(dim), int(L), R, (ctypes.c_double * R)(*J), (ctypes.c_double * R)(*T),
+                                               (ctypes.c_uint64 * R)(*seed))
+        if not self._h:
+            raise WolffError(WOLFF_EINVAL, last_error())
+        self.dim, self.L, self.N, self.R = int(dim), int(L), int(L) ** int(dim), R
+        self.last_n = 0
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.wolff_batch_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc: int):
+        if rc != WOLFF_OK:
+            raise WolffError(rc, last_error())
+
+    def run(self, n_updates: int, stream=None):
+        self._check(self._lib.wolff_batch_run(self._h, int(n_updates), _stream_handle(stream)))
+        if n_updates:
+            self.last_n = int(n_updates)
+
+    def observables_into(self, E=None, M=None, cluster_sizes=None):
+        self._check(self._lib.wolff_batch_observables(self._h, _ptr(E), _ptr(M), _ptr(cluster_sizes)))
+
+    def observables(self, sizes: bool = False):
+        """(E[R], M[R]) of the current lattices, plus sizes[R, n] of the most recent run when sizes=True."""
+        E = np.zeros(self.R, dtype=np.int64)
+        M = np.zeros(self.R, dtype=np.int64)
+        out = np.empty((self.R, self.last_n), dtype=np.uint32) if sizes and self.last_n else None
+        self.observables_into(E, M, out)
+        if sizes:
+            return E, M, (out if out is not None else np.empty((self.R, 0), dtype=np.uint32))
+        return E, M
+
+    def get_spins_into(self, dst):
+        self._check(self._lib.wolff_batch_get_spins(self._h, _ptr(dst)))
+
+    def get_spins(self) -> np.ndarray:
+        out = np.empty((self.R, self.N), dtype=np.int8)
+        self.get_spins_into(out)
+        return out
+
+    def set_spins(self, src):
+        if isinstance(src, np.ndarray):
+            src = np.ascontiguousarray(src, dtype=np.int8).reshape(-1)
+            if src.size != self.R * self.N:
+                raise ValueError("need R * N = %d spins" % (self.R * self.N))
+        self._check(self._lib.wolff_batch_set_spins(self._h, _ptr(src)))
+
+    @property
+    def update_index(self) -> int:
+        u = ctypes.c_uint64()
+        self._check(self._lib.wolff_batch_get_state(self._h, ctypes.byref(u), None))
+        return int(u.value)
+
+    @update_index.setter
+    def update_index(self, u: int):
+        self._check(self._lib.wolff_batch_set_update_index(self._h, int(u)))
+
+    @property
+    def thresholds(self) -> np.ndarray:
+        buf = (ctypes.c_uint64 * self.R)()
+        self._check(self._lib.wolff_batch_get_state(self._h, None, buf))
+        return np.array([int(x) for x in buf], dtype=np.uint64)
+
+    def set_option(self, key: str, value: int):
+        self._check(self._lib.wolff_batch_set_option(self._h, key.encode(), int(value)))
+
+    def series(self):
+        """(E[R, n], M[R, n]) after every update of the most recent measured run."""
+        E = np.empty((self.R, self.last_n), dtype=np.int64)
+        M = np.empty((self.R, self.last_n), dtype=np.int64)
+        self._check(self._lib.wolff_batch_get_series(self._h, _ptr(E), _ptr(M)))
+        return E, M
+
+    def moments(self):
+        """(raw[R, 10], binder[R]): wolff_batch_get_moments."""
+        buf = (ctypes.c_uint64 * (10 * self.R))()
+        U = (ctypes.c_double * self.R)()
+        self._check(self._lib.wolff_batch_get_moments(self._h, buf, U))
+        return (np.array([int(x) for x in buf], dtype=np.uint64).reshape(self.R, 10), np.array([float(x) for x in U]))
+
+    def reset_moments(self):
+        self._check(self._lib.wolff_batch_reset_moments(self._h))
+
+    def stats(self) -> dict:
+        buf = (ctypes.c_uint64 * 4)()
+        self._check(self._lib.wolff_batch_get_stats(self._h, buf))
+        return dict(zip(BATCH_STAT_NAMES, (int(x) for x in buf)))

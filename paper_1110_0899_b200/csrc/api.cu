@@ -26,6 +26,11 @@ void set_error(const char *fmt, ...)
 
 }  // namespace
 
+namespace wolff {
+void set_error_v(const char *fmt, va_list ap) { vsnprintf(g_error, sizeof(g_error), fmt, ap); }
+uint64_t bond_threshold(double J, double T);
+}
+
 struct wolff_ctx {
     int dim = 0, L = 0;
     double J = 0, T = 0;
@@ -68,7 +73,7 @@ struct wolff_ctx {
     int tile_log_opt = 0;           // 0 = auto
     int tile_ctas_opt = 0;          // 0 = one CTA per SM
     uint32_t ring_cap = 2048;
-    int inbox_log_opt = 0;          // 0 = auto (at most 2^12 entries per CTA)
+    int inbox_log_opt = 0;          // 0 = auto: what one update can send at most (no capacity checks)
     int fill_mode = 1;              // bond tables: 0 off, 1 adaptive, 2 always
     uint64_t fill_min_us = 30;
     int fill_bufs = 0;              // 0 = two buffers when they fit, else one; 1 = one
@@ -131,8 +136,10 @@ int check_handle(wolff_ctx *h)
     return WOLFF_OK;
 }
 
+}  // namespace
+
 // Reading R7: p = -expm1(-2J/T) in IEEE double, thr = floor(p * 2^32) in [0, 2^32].
-uint64_t bond_threshold(double J, double T)
+uint64_t wolff::bond_threshold(double J, double T)
 {
     const double p = -std::expm1(-2.0 * J / T);
     if (!(p > 0.0)) return 0;
@@ -140,6 +147,8 @@ uint64_t bond_threshold(double J, double T)
     if (scaled >= 4294967296.0) return 4294967296ull;
     return (uint64_t)scaled;
 }
+
+namespace {
 
 uint32_t cta_capacity(const wolff_ctx *h) { return h->qcap / (2u * (uint32_t)h->dim); }   // next level must fit one buffer
 uint32_t cluster_capacity(const wolff_ctx *h) { return (uint32_t)h->cluster_ctas * (cta_capacity(h) & ~31u); }
@@ -229,14 +238,15 @@ int refresh_plan(wolff_ctx *h, cudaStream_t stream)
     tp.G = G;
     tp.magicG = ((1ull << 40) + G - 1) / G;
     tp.slots = slots;
-    // Inbox of a CTA: never more entries than one update can send it (every bond across the surface of its tiles once,
-    // the seed, the exit), and by default at most 2^12 -- a sender that finds the inbox full waits for the receiver
-    // (which never waits for anybody), and a small inbox stays in L2 lines that were touched a moment ago.
+    // Inbox of a CTA: by default what one update can send it at most (every bond across the surface of its tiles once,
+    // the seed, the control messages), so nothing can overflow and senders check nothing.  Knob "inbox_log": a smaller
+    // inbox; senders then check the capacity before each store and wait for the receiver, which never waits for anybody
+    // (the check costs throughput; the size of the inboxes does not: growth_tiles.cu, run_passes).
     const uint64_t surface = (uint64_t)slots * 2ull * dim * (1ull << ((dim - 1) * b));
     tp.in_log = ceil_log2(surface + 4);
-    const uint32_t in_log_max = h->inbox_log_opt > 0 ? (uint32_t)h->inbox_log_opt : 12u;
-    if (tp.in_log > in_log_max) tp.in_log = in_log_max;
     if (tp.in_log < 5u) tp.in_log = 5u;              // the receiver looks at 32 slots at a time
+    tp.bp = 0u;
+    if (h->inbox_log_opt > 0 && (uint32_t)h->inbox_log_opt < tp.in_log) { tp.in_log = (uint32_t)h->inbox_log_opt; tp.bp = 1u; }
     tp.in_cap = 1u << tp.in_log;
     tp.spill_log = ceil_log2((uint64_t)slots << (dim * b));
     tp.ring_cap = h->ring_cap;

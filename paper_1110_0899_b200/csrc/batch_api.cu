@@ -1,0 +1,396 @@
+// batch_api.cu -- the extern "C" boundary of the batch of chains declared in include/wolff.h (host side only).
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/wolff.h"
+#include "internal.h"
+
+using namespace wolff;
+
+// defined in api.cu: the thread-local error string shared by the whole library, and reading R7
+namespace wolff {
+void set_error_v(const char *fmt, va_list ap);
+uint64_t bond_threshold(double J, double T);
+}
+
+namespace {
+
+void set_error(const char *fmt, ...) __attribute__((format(printf, 1, 2)));
+void set_error(const char *fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    wolff::set_error_v(fmt, ap);
+    va_end(ap);
+}
+
+}  // namespace
+
+struct wolff_batch_ctx {
+    int dim = 0, L = 0;
+    uint32_t R = 0;
+    uint64_t N = 0;
+    size_t stride = 0;              // bytes between two lattices (N padded to 16)
+    uint64_t u = 0;                 // next update index (shared by all chains)
+    int device = 0, num_sms = 0;
+    Geometry geo{};
+    std::vector<uint64_t> thr, seed;
+    int8_t *spins = nullptr;
+    uint32_t *lists = nullptr;
+    uint32_t *sizes = nullptr;
+    long long *E_log = nullptr, *M_log = nullptr;
+    uint64_t log_cap = 0;           // updates per chain the logs can hold
+    uint2 *keys = nullptr;
+    unsigned long long *thr_dev = nullptr;
+    long long *EM = nullptr;
+    unsigned long long *moments = nullptr;
+    unsigned long long *acc = nullptr;      // E/M reduction scratch, 2 per chain
+    unsigned long long *stats = nullptr;    // 4 counters + the chain counter
+    uint64_t last_n = 0;
+    bool ran = false, last_measured = false, cuda_failed = false;
+    cudaStream_t last_stream = nullptr;
+    int measure = 0, threads_opt = 0;
+    uint32_t qcap = 1024;
+};
+
+namespace {
+
+class DeviceScope {
+public:
+    explicit DeviceScope(const wolff_batch_ctx *b)
+    {
+        if (!b) return;
+        if (cudaGetDevice(&prev_) != cudaSuccess) { cudaGetLastError(); prev_ = -1; }
+        if (prev_ != b->device) { cudaSetDevice(b->device); switched_ = true; }
+    }
+    ~DeviceScope() { if (switched_ && prev_ >= 0) cudaSetDevice(prev_); }
+private:
+    int prev_ = -1;
+    bool switched_ = false;
+};
+
+int fail_cuda(wolff_batch_ctx *b, cudaError_t e, const char *what)
+{
+    set_error("%s: %s", what, cudaGetErrorString(e));
+    if (b) b->cuda_failed = true;
+    return WOLFF_ECUDA;
+}
+
+#define CHECK_CUDA(b, call, what)                                   \
+    do {                                                            \
+        cudaError_t e_ = (call);                                    \
+        if (e_ != cudaSuccess) return fail_cuda((b), e_, (what));   \
+    } while (0)
+
+int check(wolff_batch_ctx *b)
+{
+    if (!b) { set_error("null batch handle"); return WOLFF_EINVAL; }
+    if (b->cuda_failed) { set_error("batch handle is in a failed CUDA state"); return WOLFF_ECUDA; }
+    return WOLFF_OK;
+}
+
+void free_all(wolff_batch_ctx *b)
+{
+    cudaFree(b->spins); cudaFree(b->lists); cudaFree(b->sizes); cudaFree(b->E_log); cudaFree(b->M_log);
+    cudaFree(b->keys); cudaFree(b->thr_dev); cudaFree(b->EM); cudaFree(b->moments); cudaFree(b->acc); cudaFree(b->stats);
+}
+
+// threads per CTA and CTAs of a launch: every chain resident at once when the chip can hold them
+void launch_shape(const wolff_batch_ctx *b, int *threads, int *grid)
+{
+    int t = b->threads_opt;
+    if (t == 0) {
+        const uint32_t per_sm = (b->R + (uint32_t)b->num_sms - 1u) / (uint32_t)b->num_sms;     // chains per SM
+        t = per_sm >= 8u ? 64 : (per_sm >= 3u ? 128 : 256);
+    }
+    int per_sm = 1;
+    if (batch_ctas_per_sm(b->dim, b->geo.pow2 != 0, t, b->qcap, &per_sm) != cudaSuccess || per_sm < 1) { cudaGetLastError(); per_sm = 1; }
+    uint64_t g = (uint64_t)per_sm * (uint64_t)b->num_sms;
+    if (g > b->R) g = b->R;
+    *threads = t;
+    *grid = (int)g;
+}
+
+}  // namespace
+
+extern "C" {
+
+wolff_batch wolff_batch_create(int dim, int L, int R, const double *J, const double *T, const uint64_t *seed)
+{
+    if (dim != 2 && dim != 3) { set_error("dim must be 2 or 3 (got %d)", dim); return nullptr; }
+    if (L < 2) { set_error("L must be >= 2 (got %d)", L); return nullptr; }
+    if (R < 1 || R > (1 << 20)) { set_error("R must be in [1, 2^20] (got %d)", R); return nullptr; }
+    if (!J || !T || !seed) { set_error("J, T and seed must point to R values each"); return nullptr; }
+    uint64_t N = 1;
+    for (int k = 0; k < dim; ++k) {
+        N *= (uint64_t)L;
+        if (N > (1ull << 31)) { set_error("N = L^dim exceeds 2^31"); return nullptr; }
+    }
+    for (int r = 0; r < R; ++r) {
+        if (!(J[r] >= 0.0) || !std::isfinite(J[r])) { set_error("J[%d] must be finite and >= 0", r); return nullptr; }
+        if (!(T[r] > 0.0) || !std::isfinite(T[r])) { set_error("T[%d] must be finite and > 0", r); return nullptr; }
+    }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        set_error("no usable CUDA device (%s); this library has no CPU fallback", cudaGetErrorString(e));
+        return nullptr;
+    }
+    wolff_batch_ctx *b = new (std::nothrow) wolff_batch_ctx();
+    if (!b) { set_error("out of host memory"); return nullptr; }
+    b->dim = dim; b->L = L; b->R = (uint32_t)R; b->N = N;
+    b->stride = (size_t)((N + 15ull) & ~15ull);
+    b->geo.L = (uint32_t)L; b->geo.N = (uint32_t)N; b->geo.LL = (uint32_t)((uint64_t)L * (uint64_t)L);
+    b->geo.pow2 = ((L & (L - 1)) == 0) ? 1u : 0u;
+    b->geo.logL = 0;
+    if (b->geo.pow2) while ((1u << b->geo.logL) < (uint32_t)L) ++b->geo.logL;
+    cudaDeviceProp prop{};
+    if (cudaGetDevice(&b->device) != cudaSuccess || cudaGetDeviceProperties(&prop, b->device) != cudaSuccess) {
+        set_error("cudaGetDeviceProperties failed"); delete b; return nullptr;
+    }
+    b->num_sms = prop.multiProcessorCount;
+    std::vector<uint2> keys((size_t)R);
+    b->thr.resize((size_t)R); b->seed.assign(seed, seed + R);
+    for (int r = 0; r < R; ++r) {
+        b->thr[(size_t)r] = bond_threshold(J[r], T[r]);
+        keys[(size_t)r] = make_uint2((uint32_t)seed[r], (uint32_t)(seed[r] >> 32));
+    }
+    const size_t Rz = (size_t)R;
+    bool ok = cudaMalloc(&b->spins, Rz * b->stride) == cudaSuccess && cudaMalloc(&b->lists, Rz * (size_t)N * sizeof(uint32_t)) == cudaSuccess &&
+              cudaMalloc(&b->keys, Rz * sizeof(uint2)) == cudaSuccess && cudaMalloc(&b->thr_dev, Rz * sizeof(unsigned long long)) == cudaSuccess &&
+              cudaMalloc(&b->EM, 2 * Rz * sizeof(long long)) == cudaSuccess && cudaMalloc(&b->moments, 10 * Rz * sizeof(unsigned long long)) == cudaSuccess &&
+              cudaMalloc(&b->acc, 2 * Rz * sizeof(unsigned long long)) == cudaSuccess && cudaMalloc(&b->stats, 8 * sizeof(unsigned long long)) == cudaSuccess;
+    if (!ok) {
+        cudaGetLastError();
+        set_error("device allocation failed for %d chains of N = %llu", R, (unsigned long long)N);
+        free_all(b); delete b;
+        return nullptr;
+    }
+    static_assert(sizeof(unsigned long long) == sizeof(uint64_t), "threshold layout");
+    e = cudaMemcpy(b->keys, keys.data(), Rz * sizeof(uint2), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(b->thr_dev, b->thr.data(), Rz * sizeof(uint64_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(b->moments, 0, 10 * Rz * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(b->EM, 0, 2 * Rz * sizeof(long long));
+    if (e == cudaSuccess) e = cudaMemset(b->stats, 0, 8 * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = cudaMemset(b->spins, 0, Rz * b->stride);
+    // every chain starts from its own seed-derived random lattice (reading R9), as wolff_create does
+    for (int r = 0; r < R && e == cudaSuccess; ++r)
+        e = launch_init_lattice(b->spins + (size_t)r * b->stride, b->geo.N, seed[r], b->num_sms, nullptr);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) {
+        set_error("batch initialisation failed: %s", cudaGetErrorString(e));
+        free_all(b); delete b;
+        return nullptr;
+    }
+    return b;
+}
+
+int wolff_batch_destroy(wolff_batch b)
+{
+    if (!b) return WOLFF_OK;
+    DeviceScope scope(b);
+    if (b->ran) cudaStreamSynchronize(b->last_stream);
+    free_all(b);
+    delete b;
+    return WOLFF_OK;
+}
+
+int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (n_updates == 0) return WOLFF_OK;
+    if (n_updates > (1ull << 32)) { set_error("n_updates too large for one call (max 2^32)"); return WOLFF_EINVAL; }
+    if (b->ran && (stream != b->last_stream || n_updates > b->log_cap))
+        CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+    if (n_updates > b->log_cap) {
+        uint64_t cap = b->log_cap ? b->log_cap : 1024;
+        while (cap < n_updates) cap *= 2;
+        uint32_t *fresh = nullptr;
+        long long *fresh_E = nullptr, *fresh_M = nullptr;
+        const size_t entries = (size_t)b->R * (size_t)cap;
+        if (cudaMalloc(&fresh, entries * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&fresh_E, entries * sizeof(long long)) != cudaSuccess ||
+            cudaMalloc(&fresh_M, entries * sizeof(long long)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(fresh); cudaFree(fresh_E); cudaFree(fresh_M);
+            set_error("cannot allocate the per-update logs for %u chains x %llu updates", b->R, (unsigned long long)n_updates);
+            return WOLFF_ENOMEM;
+        }
+        cudaFree(b->sizes); cudaFree(b->E_log); cudaFree(b->M_log);
+        b->sizes = fresh; b->E_log = fresh_E; b->M_log = fresh_M;
+        b->log_cap = cap;
+    }
+    if (b->measure)      // running E and M start from a whole-lattice evaluation of every chain
+        CHECK_CUDA(b, launch_batch_energy(b->spins, b->stride, b->geo, b->dim, b->R, b->acc, b->EM, b->num_sms, stream), "launch batch E/M reduction");
+    CHECK_CUDA(b, cudaMemsetAsync(b->stats, 0, 8 * sizeof(unsigned long long), stream), "cudaMemsetAsync(stats)");
+    BatchParams bp{};
+    bp.spins = b->spins; bp.lists = b->lists; bp.sizes = b->sizes; bp.E_log = b->E_log; bp.M_log = b->M_log;
+    bp.keys = b->keys; bp.thr = b->thr_dev; bp.EM = b->EM; bp.moments = b->moments; bp.stats = b->stats;
+    bp.next = reinterpret_cast<unsigned int *>(b->stats + 4);
+    bp.geo = b->geo; bp.lattice_stride = b->stride; bp.u0 = b->u; bp.n_updates = n_updates; bp.R = b->R;
+    bp.measure = b->measure ? 1u : 0u; bp.qcap = b->qcap;
+    int threads = 0, grid = 0;
+    launch_shape(b, &threads, &grid);
+    CHECK_CUDA(b, launch_growth_batch(bp, b->dim, grid, threads, stream), "launch batch growth kernel");
+    b->u += n_updates;
+    b->last_n = n_updates;
+    b->last_measured = b->measure != 0;
+    b->last_stream = stream;
+    b->ran = true;
+    return WOLFF_OK;
+}
+
+int wolff_batch_observables(wolff_batch b, int64_t *E, int64_t *M, uint32_t *cluster_sizes)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    cudaStream_t s = b->last_stream;
+    const size_t R = b->R;
+    if (E || M) {
+        CHECK_CUDA(b, launch_batch_energy(b->spins, b->stride, b->geo, b->dim, b->R, b->acc, b->EM, b->num_sms, s), "launch batch E/M reduction");
+        // (E, M) pairs -> the caller's two arrays (host or device): strided copies
+        if (E) CHECK_CUDA(b, cudaMemcpy2DAsync(E, sizeof(int64_t), b->EM, 2 * sizeof(long long), sizeof(int64_t), R, cudaMemcpyDefault, s), "copy E");
+        if (M) CHECK_CUDA(b, cudaMemcpy2DAsync(M, sizeof(int64_t), b->EM + 1, 2 * sizeof(long long), sizeof(int64_t), R, cudaMemcpyDefault, s), "copy M");
+    }
+    if (cluster_sizes && b->ran && b->last_n > 0)
+        CHECK_CUDA(b, cudaMemcpyAsync(cluster_sizes, b->sizes, R * (size_t)b->last_n * sizeof(uint32_t), cudaMemcpyDefault, s), "copy cluster sizes");
+    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_batch_get_spins(wolff_batch b, int8_t *dst)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    if (!dst) { set_error("dst is NULL"); return WOLFF_EINVAL; }
+    cudaStream_t s = b->last_stream;
+    CHECK_CUDA(b, cudaMemcpy2DAsync(dst, (size_t)b->N, b->spins, b->stride, (size_t)b->N, b->R, cudaMemcpyDefault, s), "copy lattices out");
+    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_batch_set_spins(wolff_batch b, const int8_t *src)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    if (!src) { set_error("src is NULL"); return WOLFF_EINVAL; }
+    cudaStream_t s = b->last_stream;
+    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    // stage in the member lists (4 N bytes per chain, idle between runs), validate there, then commit
+    int8_t *staging = reinterpret_cast<int8_t *>(b->lists);
+    const size_t total = (size_t)b->R * (size_t)b->N;
+    CHECK_CUDA(b, cudaMemcpyAsync(staging, src, total, cudaMemcpyDefault, s), "copy lattices in");
+    unsigned int *invalid = reinterpret_cast<unsigned int *>(b->stats + 6);
+    CHECK_CUDA(b, cudaMemsetAsync(invalid, 0, sizeof(unsigned int), s), "reset validation flag");
+    CHECK_CUDA(b, launch_validate_word(staging, total, invalid, b->num_sms, s), "launch validation");
+    unsigned int bad = 0;
+    CHECK_CUDA(b, cudaMemcpyAsync(&bad, invalid, sizeof(bad), cudaMemcpyDeviceToHost, s), "read validation flag");
+    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    if (bad) { set_error("batch set_spins: every byte must be +1 or -1"); return WOLFF_EINVAL; }
+    CHECK_CUDA(b, cudaMemcpy2DAsync(b->spins, b->stride, staging, (size_t)b->N, (size_t)b->N, b->R, cudaMemcpyDeviceToDevice, s), "commit lattices");
+    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_batch_get_state(wolff_batch b, uint64_t *update_index, uint64_t *thresholds)
+{
+    if (!b) { set_error("null batch handle"); return WOLFF_EINVAL; }
+    if (update_index) *update_index = b->u;
+    if (thresholds) memcpy(thresholds, b->thr.data(), (size_t)b->R * sizeof(uint64_t));
+    return WOLFF_OK;
+}
+
+int wolff_batch_set_update_index(wolff_batch b, uint64_t update_index)
+{
+    if (!b) { set_error("null batch handle"); return WOLFF_EINVAL; }
+    b->u = update_index;
+    return WOLFF_OK;
+}
+
+int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value)
+{
+    if (!b || !key) { set_error("null batch handle or key"); return WOLFF_EINVAL; }
+    if (!strcmp(key, "measure")) {
+        if (value != 0 && value != 1) { set_error("measure must be 0 or 1"); return WOLFF_EINVAL; }
+        b->measure = (int)value;
+    } else if (!strcmp(key, "threads")) {
+        if (value != 0 && value != 32 && value != 64 && value != 128 && value != 256) { set_error("threads must be 0 (auto), 32, 64, 128 or 256"); return WOLFF_EINVAL; }
+        b->threads_opt = (int)value;
+    } else if (!strcmp(key, "queue_cap")) {
+        if (value < 8 || value > 16384) { set_error("queue_cap must be in [8, 16384]"); return WOLFF_EINVAL; }
+        b->qcap = (uint32_t)value;
+    } else {
+        set_error("unknown batch option '%s'", key);
+        return WOLFF_EINVAL;
+    }
+    return WOLFF_OK;
+}
+
+int wolff_batch_get_series(wolff_batch b, int64_t *E_series, int64_t *M_series)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    if (!b->ran || !b->last_measured) {
+        set_error("the most recent wolff_batch_run was not a measured one (wolff_batch_set_option \"measure\" = 1)");
+        return WOLFF_EINVAL;
+    }
+    cudaStream_t s = b->last_stream;
+    const size_t bytes = (size_t)b->R * (size_t)b->last_n * sizeof(int64_t);
+    if (E_series) CHECK_CUDA(b, cudaMemcpyAsync(E_series, b->E_log, bytes, cudaMemcpyDefault, s), "copy E series");
+    if (M_series) CHECK_CUDA(b, cudaMemcpyAsync(M_series, b->M_log, bytes, cudaMemcpyDefault, s), "copy M series");
+    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_batch_get_moments(wolff_batch b, uint64_t *moments, double *binder)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    std::vector<uint64_t> host(10 * (size_t)b->R);
+    CHECK_CUDA(b, cudaMemcpyAsync(host.data(), b->moments, host.size() * sizeof(uint64_t), cudaMemcpyDeviceToHost, b->last_stream), "read moments");
+    CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+    if (moments) memcpy(moments, host.data(), host.size() * sizeof(uint64_t));
+    if (binder) {
+        const long double two64 = 18446744073709551616.0L;
+        for (uint32_t r = 0; r < b->R; ++r) {
+            const uint64_t *m = host.data() + 10 * (size_t)r;
+            const long double n = (long double)m[0], s2 = (long double)m[6] * two64 + (long double)m[5], s4 = (long double)m[8] * two64 + (long double)m[7];
+            binder[r] = (m[0] == 0 || s2 == 0.0L) ? std::nan("") : (double)(1.0L - (n * s4) / (3.0L * s2 * s2));
+        }
+    }
+    return WOLFF_OK;
+}
+
+int wolff_batch_reset_moments(wolff_batch b)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    CHECK_CUDA(b, cudaMemsetAsync(b->moments, 0, 10 * (size_t)b->R * sizeof(unsigned long long), b->last_stream), "clear moments");
+    CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+int wolff_batch_get_stats(wolff_batch b, uint64_t *stats)
+{
+    int rc = check(b);
+    if (rc) return rc;
+    DeviceScope scope(b);
+    if (!stats) { set_error("stats is NULL"); return WOLFF_EINVAL; }
+    CHECK_CUDA(b, cudaMemcpyAsync(stats, b->stats, 4 * sizeof(uint64_t), cudaMemcpyDeviceToHost, b->last_stream), "read stats");
+    CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+    return WOLFF_OK;
+}
+
+}  // extern "C"

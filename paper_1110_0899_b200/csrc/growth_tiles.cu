@@ -53,9 +53,7 @@ namespace {
 #ifndef WOLFF_WIDE
 #define WOLFF_WIDE 1
 #endif
-#ifndef WOLFF_BACKPRESSURE
-#define WOLFF_BACKPRESSURE 1      // 0: probe builds without the inbox capacity check (the host must then size the inboxes for the worst case)
-#endif
+
 constexpr unsigned int kWide = WOLFF_WIDE;         // sites per lane group and pass: a warp holds up to kWide * 32 / (2 dim) sites
 constexpr uint32_t kEmpty = 0xFFFFFFFFu;
 constexpr int kT = kTileThreads;
@@ -343,6 +341,7 @@ __device__ __forceinline__ void raise_abort(Control *ctl, unsigned int code) { s
 // receiver never waits for a sender (it only claims, and feeds its ring or spill list), so this wait always ends.
 __device__ __noinline__ void wait_inbox(const TileParams &tp, uint32_t own, unsigned int pos)
 {
+    if (!tp.bp) return;            // worst-case inboxes: nothing can overflow
     unsigned int polls = 0;
     while (pos - ld_relaxed_u32(tp.gihead + own) >= tp.in_cap) {
         if ((++polls & 0x3FFu) == 0u && ld_relaxed_u32(&tp.g.ctl->error) != 0u) return;     // the launch is being aborted
@@ -585,7 +584,11 @@ struct WorkerState {
 // Passes until the warp holds no site (READY) or for at most 32 passes (!READY: the caller looks again whether the
 // tables have become complete).  POS: the seed spin s0 of the running update is +1 (claim = OR), else -1 (AND).
 // READY: every tile of this CTA has its bond table of this update, so no state is checked and no Philox runs here.
-template <int DIM, bool POS, bool READY>
+// BP: the inboxes are smaller than what one update can send (knob "inbox_log"), so a sender checks the capacity
+// before it stores a message (wait_inbox).  With worst-case inboxes (the default) the check does not exist: measured
+// on B200 the check costs 15 % (C3) / 40 % (C5a) of the throughput -- one more L2 load in flight per message and a
+// call in the pass -- while the size of the inboxes (2^12 against 2^16 entries per CTA at C5a) makes no difference.
+template <int DIM, bool POS, bool READY, bool BP>
 __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, const Layout &ly, const Tiling<DIM> &tg, uint32_t *stage,
                                            unsigned int c, WorkerState &ws, Tally &tl)
 {
@@ -625,9 +628,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     unsigned int budget = 32u;
 
     auto send = [&](unsigned int j) {
-#if WOLFF_BACKPRESSURE
-        if (msg_pos[j] - msg_seen[j] >= tp.in_cap) wait_inbox(tp, msg_own[j], msg_pos[j]);
-#endif
+        if (BP && msg_pos[j] - msg_seen[j] >= tp.in_cap) wait_inbox(tp, msg_own[j], msg_pos[j]);
         st_relaxed_u64(tp.inbox + ((size_t)msg_own[j] << tp.in_log) + (msg_pos[j] & in_mask),
                        pack_msg(kKindClaim, (msg_pos[j] >> tp.in_log) & 1u, krel, msg_na[j], POS ? 1 : -1));
         msg_valid[j] = false;
@@ -724,15 +725,14 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
                 if (msg_valid[j]) send(j);
                 // the atomic writes the loop-carried register itself (an in-out operand, 32 bits: a 64-bit result needs an
                 // aligned register pair, which ptxas then copies out of -- and a copy waits for the L2 round trip here)
-#if WOLFF_BACKPRESSURE
-                asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.global.add.u32 %0, [%2], 1;\n"
-                             " @p ld.relaxed.gpu.global.u32 %1, [%4];\n}"
-                             : "+r"(msg_pos[j]), "+r"(msg_seen[j]) : "l"(tp.gtail + own[j]), "r"((unsigned int)cand_r[j]), "l"(tp.gihead + own[j])
-                             : "memory");
-#else
-                asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %2, 0;\n @p atom.global.add.u32 %0, [%1], 1;\n}"
-                             : "+r"(msg_pos[j]) : "l"(tp.gtail + own[j]), "r"((unsigned int)cand_r[j]) : "memory");
-#endif
+                if (BP)
+                    asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %3, 0;\n @p atom.global.add.u32 %0, [%2], 1;\n"
+                                 " @p ld.relaxed.gpu.global.u32 %1, [%4];\n}"
+                                 : "+r"(msg_pos[j]), "+r"(msg_seen[j]) : "l"(tp.gtail + own[j]), "r"((unsigned int)cand_r[j]), "l"(tp.gihead + own[j])
+                                 : "memory");
+                else
+                    asm volatile("{\n .reg .pred p;\n setp.ne.u32 p, %2, 0;\n @p atom.global.add.u32 %0, [%1], 1;\n}"
+                                 : "+r"(msg_pos[j]) : "l"(tp.gtail + own[j]), "r"((unsigned int)cand_r[j]) : "memory");
                 if (cand_r[j]) {
                     msg_own[j] = own[j];
                     msg_na[j] = na[j];
@@ -910,12 +910,20 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         ws.krel = ld_vol(&sh.krel);
         while (ws.nsites != 0u) {
             const bool ready = tables && ld_vol(&sh.ready_tag[ws.krel & (tp.nbuf - 1u)]) == ws.krel + 1u;
-            if (ws.s0 > 0) {
-                if (ready) run_passes<DIM, true, true>(tp, sh, ly, tg, stage, c, ws, tl);
-                else run_passes<DIM, true, false>(tp, sh, ly, tg, stage, c, ws, tl);
+            if (tp.bp) {
+                if (ws.s0 > 0) {
+                    if (ready) run_passes<DIM, true, true, true>(tp, sh, ly, tg, stage, c, ws, tl);
+                    else run_passes<DIM, true, false, true>(tp, sh, ly, tg, stage, c, ws, tl);
+                } else {
+                    if (ready) run_passes<DIM, false, true, true>(tp, sh, ly, tg, stage, c, ws, tl);
+                    else run_passes<DIM, false, false, true>(tp, sh, ly, tg, stage, c, ws, tl);
+                }
+            } else if (ws.s0 > 0) {
+                if (ready) run_passes<DIM, true, true, false>(tp, sh, ly, tg, stage, c, ws, tl);
+                else run_passes<DIM, true, false, false>(tp, sh, ly, tg, stage, c, ws, tl);
             } else {
-                if (ready) run_passes<DIM, false, true>(tp, sh, ly, tg, stage, c, ws, tl);
-                else run_passes<DIM, false, false>(tp, sh, ly, tg, stage, c, ws, tl);
+                if (ready) run_passes<DIM, false, true, false>(tp, sh, ly, tg, stage, c, ws, tl);
+                else run_passes<DIM, false, false, false>(tp, sh, ly, tg, stage, c, ws, tl);
             }
         }
     }
@@ -1212,7 +1220,7 @@ __device__ __forceinline__ void build_tables(const TileParams &tp, const Layout 
 }
 
 template <int DIM>
-__global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const TileParams tp)
+__global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const __grid_constant__ TileParams tp)
 {
     extern __shared__ __align__(16) unsigned char smem_t[];
     __shared__ TShared sh;

@@ -95,6 +95,7 @@ struct TileParams {
     uint32_t G;                      // CTAs (one per SM, all co-resident)
     uint32_t slots;                  // tiles per CTA (upper bound)
     uint32_t in_log, in_cap;         // inbox entries per CTA (a power of two, at least 32)
+    uint32_t bp;                     // 1: in_cap is below what one update can send a CTA: senders check the capacity (back-pressure)
     uint32_t spill_log;              // spill entries per CTA (at least the sites the CTA owns)
     uint32_t ring_cap;               // entries of the shared-memory ring (power of two)
     unsigned long long watchdog_ns;  // an update longer than this aborts the launch
@@ -110,6 +111,28 @@ struct TileParams {
     // faces[((slot * G + owner) * dim + d) * B^(dim-1) + f], one byte per site
     int8_t *faces;
 };
+
+// R independent chains in one launch, one CTA per chain at a time (growth_batch.cu).
+struct BatchParams {
+    int8_t *spins;                   // R lattices, lattice_stride bytes apart
+    uint32_t *lists;                 // R member lists of N entries (the list of the running cluster; its tail is the frontier)
+    uint32_t *sizes;                 // [R][n_updates] cluster sizes of this launch
+    long long *E_log, *M_log;        // [R][n_updates] E, M after every update (measure)
+    const uint2 *keys;               // [R] Philox key = seed of the chain
+    const unsigned long long *thr;   // [R] bond threshold of the chain
+    long long *EM;                   // [R][2] E, M of every chain: the last whole-lattice evaluation / the running values
+    unsigned long long *moments;     // [R][10] accumulated sums (layout: wolff_get_moments)
+    unsigned long long *stats;       // [4] updates, flipped spins, levels, claim attempts of this launch
+    unsigned int *next;              // the next chain to be taken by a CTA (zeroed per launch)
+    Geometry geo;
+    size_t lattice_stride;
+    unsigned long long u0;           // first update index of this launch (shared by all chains)
+    unsigned long long n_updates;
+    uint32_t R;
+    uint32_t measure;
+    uint32_t qcap;                   // entries per shared-memory frontier buffer
+};
+constexpr int kBatchMaxThreads = 256;
 
 // Launch shape of the persistent kernel.
 struct GrowthLaunch {
@@ -131,8 +154,15 @@ cudaError_t growth_max_clusters(int dim, bool pow2, const GrowthLaunch &l, int *
 size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, uint32_t nbuf);
 cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm);
 cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes, cudaStream_t stream);
+// batch of chains: CTAs of `threads` threads, `grid` of them; co-resident CTAs per SM; E, M of every chain into EM
+cudaError_t launch_growth_batch(const BatchParams &bp, int dim, int grid, int threads, cudaStream_t stream);
+cudaError_t batch_ctas_per_sm(int dim, bool pow2, int threads, uint32_t qcap, int *per_sm);
+cudaError_t launch_batch_energy(const int8_t *spins, size_t stride, const Geometry &geo, int dim, uint32_t R, unsigned long long *acc,
+                                long long *EM, int num_sms, cudaStream_t stream);
 cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, int num_sms, cudaStream_t stream);
 cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, int num_sms, cudaStream_t stream);
+// n_bytes spins (16-byte aligned buffer) are all +1 / -1, else *invalid |= 1
+cudaError_t launch_validate_word(const int8_t *spins, size_t n_bytes, unsigned int *invalid, int num_sms, cudaStream_t stream);
 // E and M of the lattice into ctl->E, ctl->M and, when not null, into the DEVICE words E_dst, M_dst
 cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo, int dim, Control *ctl,
                                         long long *E_dst, long long *M_dst, int num_sms, cudaStream_t stream);

@@ -59,12 +59,12 @@ __device__ __forceinline__ bool word_valid(uint32_t w)
     return w == (0x01010101u | (s * 0xFEu));
 }
 
-__global__ void __launch_bounds__(kThreads) validate_kernel(const int8_t *spins, uint32_t N, Control *ctl)
+__global__ void __launch_bounds__(kThreads) validate_kernel(const int8_t *spins, size_t N, unsigned int *invalid)
 {
     bool bad = false;
-    const uint32_t chunks = N / 16u;
+    const size_t chunks = N / 16u;
     const uint4 *const v = reinterpret_cast<const uint4 *>(spins);
-    for (uint32_t c = blockIdx.x * blockDim.x + threadIdx.x; c < chunks; c += gridDim.x * blockDim.x) {
+    for (size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x; c < chunks; c += (size_t)gridDim.x * blockDim.x) {
         const uint4 a = v[c];
         bad |= !(word_valid(a.x) && word_valid(a.y) && word_valid(a.z) && word_valid(a.w));
     }
@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(kThreads) validate_kernel(const int8_t *spins,
         const int8_t b = spins[chunks * 16u + threadIdx.x];
         bad |= (b != 1 && b != -1);
     }
-    if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(&ctl->invalid, 1u);
+    if (__any_sync(0xFFFFFFFFu, bad) && (threadIdx.x & 31) == 0) atomicOr(invalid, 1u);
 }
 
 // ---------------------------------------------------------------- E / M reduction
@@ -209,8 +209,13 @@ cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, int nu
 
 cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, int num_sms, cudaStream_t stream)
 {
-    const int grid = grid_for((N + 15u) / 16u, num_sms, 8);
-    validate_kernel<<<grid, kThreads, 0, stream>>>(spins, N, ctl);
+    return launch_validate_word(spins, (size_t)N, &ctl->invalid, num_sms, stream);
+}
+
+cudaError_t launch_validate_word(const int8_t *spins, size_t n_bytes, unsigned int *invalid, int num_sms, cudaStream_t stream)
+{
+    const int grid = grid_for((n_bytes + 15u) / 16u, num_sms, 8);
+    validate_kernel<<<grid, kThreads, 0, stream>>>(spins, n_bytes, invalid);
     return cudaGetLastError();
 }
 
