@@ -448,7 +448,7 @@ def run_b200(args, rank: int, world: int):
         ms, st = best
         agg = aggregate_replicas(st["flipped"], st["updates"], ms, world, dev)
         out = {"workload": "%s, %s, %d chains (seeds %d..) in one launch, %d updates each after %d untimed" %
-                           (c.name, "cold start" if cold else "literal random start", R, seeds[0], n, equil),
+                           (c.name, "cold start" if cold else "random start", R, seeds[0], n, equil),
                "replicas": R * world, "updates_per_s": agg["updates_per_s"], "value": agg["value"], "unit": UNIT,
                "mean_cluster": st["flipped"] / max(st["updates"], 1), "bfs_levels_per_update": st["levels"] / max(st["updates"], 1),
                "ms": ms}

@@ -220,7 +220,12 @@ WOLFF_API int wolff_batch_get_state(wolff_batch b, uint64_t *update_index, uint6
 WOLFF_API int wolff_batch_set_update_index(wolff_batch b, uint64_t update_index);
 /* Keys: "measure" 0 | 1 (E and M after every update of every chain, inside the kernel: see wolff_get_series);
  * "threads" threads per CTA: 0 = auto (256 for few chains, 64 for many), 32, 64, 128, 256;
- * "queue_cap" entries of a CTA's shared-memory copy of the frontier (wider frontiers are read from the member list). */
+ * "queue_cap" entries of a CTA's shared-memory copy of the frontier (wider frontiers are read from the member list);
+ * "resident" where a chain's lattice lives while a CTA works on it: 1 = the int8 lattice in global memory (L2 / HBM);
+ *   2 = bit-packed in the CTA's shared memory, one bit per spin (N <= about 1.8 million: 2D L = 1024 is 128 KiB) plus, in
+ *   a measured run, one mark bit per spin (then N <= about 900,000; a run that does not fit returns WOLFF_EINVAL),
+ *   packed from / unpacked to the int8 lattice around the chain's turn;
+ *   0 = auto: 2 when a plane is at most 32 KiB (several chains per SM stay in flight), else 1.  Never changes a result. */
 WOLFF_API int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value);
 /* E and M after every update of the most recent (measured) run: R * n_updates values each. */
 WOLFF_API int wolff_batch_get_series(wolff_batch b, int64_t *E_series, int64_t *M_series);

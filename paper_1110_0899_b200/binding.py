@@ -13,7 +13,8 @@ import threading
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libwolff_b200.so")
+# WOLFF_B200_LIB: another build of the same library (the bounds-checked one: `python -m paper_1110_0899_b200.build --checked`)
+LIB_PATH = os.environ.get("WOLFF_B200_LIB") or os.path.join(HERE, "libwolff_b200.so")
 
 WOLFF_OK, WOLFF_EINVAL, WOLFF_ENOMEM, WOLFF_ECUDA, WOLFF_EINTERNAL = 0, -1, -2, -3, -4
 NSTATS = 16

@@ -11,6 +11,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB_NAME = "libwolff_b200.so"
 LIB_PATH = os.path.join(HERE, LIB_NAME)
+CHECKED_LIB_PATH = os.path.join(HERE, "libwolff_b200_checked.so")
 SOURCES = ["api.cu", "batch_api.cu", "growth.cu", "growth_batch.cu", "growth_tiles.cu", "measure.cu", "microbench.cu"]
 HEADERS = ["internal.h", "device_common.cuh", "expand.cuh", os.path.join(ROOT, "include", "wolff.h")]
 NVCC_COMPILE_FLAGS = [
@@ -33,21 +34,27 @@ def _header_paths():
     return [h if os.path.isabs(h) else os.path.join(CSRC, h) for h in HEADERS] + [os.path.abspath(__file__)]
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB_PATH):
+def needs_build(lib_path: str = LIB_PATH) -> bool:
+    if not os.path.exists(lib_path):
         return True
     deps = [os.path.join(CSRC, s) for s in SOURCES] + _header_paths()
-    return os.path.getmtime(LIB_PATH) < max(os.path.getmtime(d) for d in deps)
+    return os.path.getmtime(lib_path) < max(os.path.getmtime(d) for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
     """One nvcc per source file, side by side (the files share no device code, so there is no device link), then one
     link.  Objects are kept under paper_1110_0899_b200/build/ (git-ignored) and reused while they are newer than
-    their source and every header."""
-    if not force and not needs_build():
-        return LIB_PATH
+    their source and every header.
+
+    checked=True builds libwolff_b200_checked.so with -DWOLFF_CHECKED (every queue, list, tile and bit-plane index is
+    compared with its bound before use: device_common.cuh); load it with WOLFF_B200_LIB=<path> (binding.py)."""
+    lib_path = CHECKED_LIB_PATH if checked else LIB_PATH
+    if not force and not needs_build(lib_path):
+        return lib_path
     nvcc = nvcc_path()
     extra = os.environ.get("WOLFF_NVCC_EXTRA", "").split()      # e.g. -DWOLFF_PROFILE (per-section cycle counters)
+    if checked:
+        extra.append("-DWOLFF_CHECKED")
     os.makedirs(OBJ_DIR, exist_ok=True)
     tag = ("_" + "".join(c if c.isalnum() else "_" for c in " ".join(extra))) if extra else ""
     newest_header = max(os.path.getmtime(h) for h in _header_paths())
@@ -73,14 +80,14 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 sys.stderr.write(err)
     if failed:
         raise RuntimeError("nvcc failed:\n" + "\n".join(failed))
-    tmp = LIB_PATH + ".tmp.%d" % os.getpid()
+    tmp = lib_path + ".tmp.%d" % os.getpid()
     cmd = [nvcc] + NVCC_LINK_FLAGS + ["-o", tmp] + objs
     proc = subprocess.run(cmd, capture_output=True, text=True)
     if proc.returncode != 0:
         raise RuntimeError("link failed:\n%s\n%s" % (" ".join(cmd), proc.stderr))
-    os.replace(tmp, LIB_PATH)
-    return LIB_PATH
+    os.replace(tmp, lib_path)
+    return lib_path
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv))

@@ -50,6 +50,7 @@ struct wolff_ctx {
     uint64_t sizes_cap = 0;         // entries allocated in each of the four logs
     int measure = 0;                // in-kernel measurement after every update
     bool last_measured = false;     // the most recent run was a measured one
+    bool em_valid = false;          // the control block holds E and M of the current lattice
     uint64_t last_n = 0;            // updates in the most recent wolff_run
     Control *ctl = nullptr;
     cudaStream_t last_stream = nullptr;
@@ -303,7 +304,8 @@ int digest_control(wolff_ctx *h, const Control &c)
 {
     if (!h->ran) return WOLFF_OK;
     if (c.error != 0) {
-        set_error("device watchdog: an update or a grid barrier did not complete (error flag %u)", c.error);
+        if (c.error >= 1000u) set_error("checked build: index out of bounds in a growth kernel (code %u)", c.error - 1000u);
+        else set_error("device watchdog: an update or a grid barrier did not complete (error flag %u)", c.error);
         h->cuda_failed = true;
         return WOLFF_EINTERNAL;
     }
@@ -489,8 +491,9 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
             // the level-synchronous kernel keeps running E and M: it starts from a whole-lattice evaluation (into the
             // control block) and marks the members of the running cluster in the spin bytes (claim_with_bits)
             p.claim_bits = 0xFCu;
-            CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, nullptr, nullptr, h->num_sms, stream),
-                       "launch E/M reduction");
+            if (!h->em_valid)
+                CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, nullptr, nullptr, h->num_sms, stream),
+                           "launch E/M reduction");
         }
         effective_thresholds(h, &p);
         rc = refresh_shape(h);
@@ -504,6 +507,7 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     h->u += n_updates;
     h->last_n = n_updates;
     h->last_measured = h->measure != 0;
+    h->em_valid = h->measure != 0;      // a measured run leaves E and M of the final lattice in the control block
     h->last_stream = stream;
     h->ran = true;
     h->run_since_set = true;
@@ -529,9 +533,11 @@ int wolff_observables(wolff_handle h, int64_t *E, int64_t *M, uint32_t *cluster_
         if (e == cudaSuccess && (attr.type == cudaMemoryTypeDevice || attr.type == cudaMemoryTypeManaged))
             dev_dst[k] = reinterpret_cast<long long *>(dst[k]);
     }
-    if (E || M)
+    if (E || M) {
         CHECK_CUDA(h, launch_energy_magnetisation(h->spins, h->geo, h->dim, h->ctl, dev_dst[0], dev_dst[1], h->num_sms, s),
                    "launch E/M reduction");
+        h->em_valid = true;
+    }
     if (cluster_sizes && h->last_n > 0)
         CHECK_CUDA(h, cudaMemcpyAsync(cluster_sizes, h->sizes, (size_t)h->last_n * sizeof(uint32_t), cudaMemcpyDefault, s),
                    "copy cluster sizes");
@@ -577,6 +583,7 @@ int wolff_set_spins(wolff_handle h, const int8_t *src)
     CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     if (invalid) { set_error("set_spins: every byte must be +1 or -1"); return WOLFF_EINVAL; }
     CHECK_CUDA(h, cudaMemcpyAsync(h->spins, staging, (size_t)h->N, cudaMemcpyDeviceToDevice, s), "commit lattice");
+    h->em_valid = false;
     h->have_mean = false;           // a new lattice: nothing is known about its clusters
     h->run_since_set = false;
     CHECK_CUDA(h, cudaStreamSynchronize(s), "cudaStreamSynchronize");
@@ -687,6 +694,13 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
     } else if (!strcmp(key, "cooperative")) {
         if (value != 0 && value != 1) { set_error("cooperative must be 0 or 1"); return WOLFF_EINVAL; }
         h->cooperative = (int)value;
+#ifdef WOLFF_CHECKED
+    } else if (!strcmp(key, "check_selftest")) {
+        // checked builds only: one failing WOLFF_CHECK on the handle's control block, so that a test can see that the checks
+        // are compiled in and that a violation reaches the caller (WOLFF_EINTERNAL at the next synchronising call)
+        h->ran = true;
+        CHECK_CUDA(h, launch_check_selftest(h->ctl, h->last_stream), "launch check self-test");
+#endif
     } else {
         set_error("unknown option '%s'", key);
         return WOLFF_EINVAL;

@@ -52,8 +52,11 @@ struct wolff_batch_ctx {
     unsigned long long *stats = nullptr;    // 4 counters + the chain counter
     uint64_t last_n = 0;
     bool ran = false, last_measured = false, cuda_failed = false;
+    bool em_valid = false;          // EM holds E and M of the current lattices (a measured run or an evaluation left them there)
     cudaStream_t last_stream = nullptr;
     int measure = 0, threads_opt = 0;
+    int resident = 0;               // 0 auto, 1 int8 lattice in global memory, 2 bit-packed lattice in shared memory
+    size_t smem_optin = 0;
     uint32_t qcap = 1024;
 };
 
@@ -99,8 +102,19 @@ void free_all(wolff_batch_ctx *b)
     cudaFree(b->keys); cudaFree(b->thr_dev); cudaFree(b->EM); cudaFree(b->moments); cudaFree(b->acc); cudaFree(b->stats);
 }
 
+// Does this batch run on the bit-packed shared-memory-resident lattice?  "resident" 2: whenever the planes fit one CTA;
+// auto: when they are small enough (32 KiB) that several chains per SM stay in flight.
+bool use_bits(const wolff_batch_ctx *b)
+{
+    if (b->resident == 1) return false;
+    const size_t planes = batch_smem_bytes(b->geo.N, 0, true, b->measure != 0);
+    const size_t all = batch_smem_bytes(b->geo.N, b->qcap, true, b->measure != 0);
+    if (all + 1024 > b->smem_optin) return false;
+    return b->resident == 2 || planes <= (32u << 10);
+}
+
 // threads per CTA and CTAs of a launch: every chain resident at once when the chip can hold them
-void launch_shape(const wolff_batch_ctx *b, int *threads, int *grid)
+void launch_shape(const wolff_batch_ctx *b, bool bits, int *threads, int *grid)
 {
     int t = b->threads_opt;
     if (t == 0) {
@@ -108,7 +122,8 @@ void launch_shape(const wolff_batch_ctx *b, int *threads, int *grid)
         t = per_sm >= 8u ? 64 : (per_sm >= 3u ? 128 : 256);
     }
     int per_sm = 1;
-    if (batch_ctas_per_sm(b->dim, b->geo.pow2 != 0, t, b->qcap, &per_sm) != cudaSuccess || per_sm < 1) { cudaGetLastError(); per_sm = 1; }
+    const size_t smem = batch_smem_bytes(b->geo.N, b->qcap, bits, b->measure != 0);
+    if (batch_ctas_per_sm(b->dim, b->geo.pow2 != 0, bits, t, smem, &per_sm) != cudaSuccess || per_sm < 1) { cudaGetLastError(); per_sm = 1; }
     uint64_t g = (uint64_t)per_sm * (uint64_t)b->num_sms;
     if (g > b->R) g = b->R;
     *threads = t;
@@ -153,6 +168,7 @@ wolff_batch wolff_batch_create(int dim, int L, int R, const double *J, const dou
         set_error("cudaGetDeviceProperties failed"); delete b; return nullptr;
     }
     b->num_sms = prop.multiProcessorCount;
+    b->smem_optin = prop.sharedMemPerBlockOptin;
     std::vector<uint2> keys((size_t)R);
     b->thr.resize((size_t)R); b->seed.assign(seed, seed + R);
     for (int r = 0; r < R; ++r) {
@@ -207,6 +223,11 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if (n_updates == 0) return WOLFF_OK;
     if (n_updates > (1ull << 32)) { set_error("n_updates too large for one call (max 2^32)"); return WOLFF_EINVAL; }
+    if (b->resident == 2 && batch_smem_bytes(b->geo.N, b->qcap, true, b->measure != 0) + 1024 > b->smem_optin) {
+        set_error("resident = 2: the bit planes of N = %llu spins (%d of them%s) and the frontier buffers do not fit one CTA's shared memory",
+                  (unsigned long long)b->N, b->measure ? 2 : 1, b->measure ? ": a measured run keeps a mark per spin" : "");
+        return WOLFF_EINVAL;
+    }
     if (b->ran && (stream != b->last_stream || n_updates > b->log_cap))
         CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
     if (n_updates > b->log_cap) {
@@ -226,7 +247,7 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
         b->sizes = fresh; b->E_log = fresh_E; b->M_log = fresh_M;
         b->log_cap = cap;
     }
-    if (b->measure)      // running E and M start from a whole-lattice evaluation of every chain
+    if (b->measure && !b->em_valid)      // running E and M start from a whole-lattice evaluation of every chain
         CHECK_CUDA(b, launch_batch_energy(b->spins, b->stride, b->geo, b->dim, b->R, b->acc, b->EM, b->num_sms, stream), "launch batch E/M reduction");
     CHECK_CUDA(b, cudaMemsetAsync(b->stats, 0, 8 * sizeof(unsigned long long), stream), "cudaMemsetAsync(stats)");
     BatchParams bp{};
@@ -236,11 +257,13 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
     bp.geo = b->geo; bp.lattice_stride = b->stride; bp.u0 = b->u; bp.n_updates = n_updates; bp.R = b->R;
     bp.measure = b->measure ? 1u : 0u; bp.qcap = b->qcap;
     int threads = 0, grid = 0;
-    launch_shape(b, &threads, &grid);
-    CHECK_CUDA(b, launch_growth_batch(bp, b->dim, grid, threads, stream), "launch batch growth kernel");
+    const bool bits = use_bits(b);
+    launch_shape(b, bits, &threads, &grid);
+    CHECK_CUDA(b, launch_growth_batch(bp, b->dim, bits, grid, threads, stream), "launch batch growth kernel");
     b->u += n_updates;
     b->last_n = n_updates;
     b->last_measured = b->measure != 0;
+    b->em_valid = b->measure != 0;       // a measured run leaves the running values in EM; an unmeasured one outdates them
     b->last_stream = stream;
     b->ran = true;
     return WOLFF_OK;
@@ -255,6 +278,7 @@ int wolff_batch_observables(wolff_batch b, int64_t *E, int64_t *M, uint32_t *clu
     const size_t R = b->R;
     if (E || M) {
         CHECK_CUDA(b, launch_batch_energy(b->spins, b->stride, b->geo, b->dim, b->R, b->acc, b->EM, b->num_sms, s), "launch batch E/M reduction");
+        b->em_valid = true;
         // (E, M) pairs -> the caller's two arrays (host or device): strided copies
         if (E) CHECK_CUDA(b, cudaMemcpy2DAsync(E, sizeof(int64_t), b->EM, 2 * sizeof(long long), sizeof(int64_t), R, cudaMemcpyDefault, s), "copy E");
         if (M) CHECK_CUDA(b, cudaMemcpy2DAsync(M, sizeof(int64_t), b->EM + 1, 2 * sizeof(long long), sizeof(int64_t), R, cudaMemcpyDefault, s), "copy M");
@@ -296,6 +320,7 @@ int wolff_batch_set_spins(wolff_batch b, const int8_t *src)
     CHECK_CUDA(b, cudaMemcpyAsync(&bad, invalid, sizeof(bad), cudaMemcpyDeviceToHost, s), "read validation flag");
     CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     if (bad) { set_error("batch set_spins: every byte must be +1 or -1"); return WOLFF_EINVAL; }
+    b->em_valid = false;
     CHECK_CUDA(b, cudaMemcpy2DAsync(b->spins, b->stride, staging, (size_t)b->N, (size_t)b->N, b->R, cudaMemcpyDeviceToDevice, s), "commit lattices");
     CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
     return WOLFF_OK;
@@ -325,6 +350,13 @@ int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value)
     } else if (!strcmp(key, "threads")) {
         if (value != 0 && value != 32 && value != 64 && value != 128 && value != 256) { set_error("threads must be 0 (auto), 32, 64, 128 or 256"); return WOLFF_EINVAL; }
         b->threads_opt = (int)value;
+    } else if (!strcmp(key, "resident")) {
+        if (value < 0 || value > 2) { set_error("resident must be 0 (auto), 1 (int8 lattice in global memory) or 2 (bit-packed in shared memory)"); return WOLFF_EINVAL; }
+        if (value == 2 && batch_smem_bytes(b->geo.N, b->qcap, true, false) + 1024 > b->smem_optin) {
+            set_error("resident = 2: a bit plane of N = %llu spins does not fit one CTA's shared memory", (unsigned long long)b->N);
+            return WOLFF_EINVAL;
+        }
+        b->resident = (int)value;
     } else if (!strcmp(key, "queue_cap")) {
         if (value < 8 || value > 16384) { set_error("queue_cap must be in [8, 16384]"); return WOLFF_EINVAL; }
         b->qcap = (uint32_t)value;
@@ -388,8 +420,15 @@ int wolff_batch_get_stats(wolff_batch b, uint64_t *stats)
     if (rc) return rc;
     DeviceScope scope(b);
     if (!stats) { set_error("stats is NULL"); return WOLFF_EINVAL; }
-    CHECK_CUDA(b, cudaMemcpyAsync(stats, b->stats, 4 * sizeof(uint64_t), cudaMemcpyDeviceToHost, b->last_stream), "read stats");
+    uint64_t host[8];
+    CHECK_CUDA(b, cudaMemcpyAsync(host, b->stats, sizeof(host), cudaMemcpyDeviceToHost, b->last_stream), "read stats");
     CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+    memcpy(stats, host, 4 * sizeof(uint64_t));
+    if (host[7] != 0) {      // set by checked builds only (-DWOLFF_CHECKED): an index was out of its bounds
+        set_error("checked build: index out of bounds in the batch kernel (code %llu)", (unsigned long long)host[7]);
+        b->cuda_failed = true;
+        return WOLFF_EINTERNAL;
+    }
     return WOLFF_OK;
 }
 

@@ -8,6 +8,23 @@
 
 namespace wolff {
 
+// ---------------------------------------------------------------- checked builds
+// -DWOLFF_CHECKED: every index the growth kernels compute for a queue, a list, a tile or a bit plane is compared with
+// its bound before it is used; a violation stores 1000 + code into the error word (the handle then reports
+// WOLFF_EINTERNAL with that code) and the access is skipped.  compute-sanitizer is closed on the pool this library was
+// developed on, so this is the memory check that can be run there (profiles/ holds the summary of such a run); the
+// release build contains none of it.
+#ifdef WOLFF_CHECKED
+__device__ __forceinline__ bool wolff_check_failed(void *errword, unsigned int code)
+{
+    asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(errword), "r"(1000u + code) : "memory");
+    return false;
+}
+#define WOLFF_CHECK(errword, cond, code) ((cond) ? true : wolff::wolff_check_failed((void *)(errword), (unsigned int)(code)))
+#else
+#define WOLFF_CHECK(errword, cond, code) (true)
+#endif
+
 // ---------------------------------------------------------------- Philox4x32-10 (reading R11)
 // Salmon et al., SC'11.  One round maps (c0,c1,c2,c3) to
 // (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)); the key is bumped by the Weyl

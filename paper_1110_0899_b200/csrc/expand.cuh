@@ -148,8 +148,9 @@ __device__ __forceinline__ int boundary_partial(const Geometry &geo, const int8_
 // warp on *dst_count (ballot/popc aggregation).  Must be called by all 32 lanes of a warp.
 template <int DIM, bool POW2, bool SPEC>
 __device__ __forceinline__ void expand_sites(const GrowthParams &p, int s0, uint32_t u_lo, uint32_t u_hi, bool valid,
-                                             uint32_t i, uint32_t *dst, unsigned int *dst_count, unsigned int &attempts)
+                                             uint32_t i, uint32_t *dst, unsigned int *dst_count, uint32_t dst_cap, unsigned int &attempts)
 {
+    (void)dst_cap;       // entries dst[] can hold: looked at by checked builds only
     uint32_t nbr[2 * DIM];
     unsigned int won;
     uint32_t x, y, z;
@@ -170,7 +171,8 @@ __device__ __forceinline__ void expand_sites(const GrowthParams &p, int s0, uint
         const unsigned int lt = bit - 1u;
 #pragma unroll
         for (int k = 0; k < 2 * DIM; ++k) {
-            if (ballots[k] & bit) dst[base + __popc(ballots[k] & lt)] = nbr[k];
+            if ((ballots[k] & bit) && WOLFF_CHECK(&p.ctl->error, base + __popc(ballots[k] & lt) < dst_cap && nbr[k] < p.geo.N, 20))
+                dst[base + __popc(ballots[k] & lt)] = nbr[k];
             base += __popc(ballots[k]);
         }
     }

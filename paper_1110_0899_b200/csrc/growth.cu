@@ -174,7 +174,7 @@ __device__ __forceinline__ unsigned int grid_levels(const GrowthParams &p, Share
                 const bool valid = idx < end;
                 const uint32_t site = valid ? __ldcg(p.clist + lo + idx) : 0u;
                 // winners go straight to the global list: one atomic on the tail per warp
-                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, p.clist, &ctl->tail, c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, p.clist, &ctl->tail, p.geo.N, c.attempts);
             }
         }
         // every thread's list writes happen-before thread 0's release (bar.sync, then atom.acq_rel)
@@ -251,7 +251,8 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
             // has logged it already
             if (p.measure) {
                 const uint32_t base = size0 + (uint32_t)(added - n) + before;
-                for (unsigned int e = tid; e < mine; e += T) p.clist[base + e] = cur[e];
+                for (unsigned int e = tid; e < mine; e += T)
+                    if (WOLFF_CHECK(&ctl->error, base + e < p.geo.N, 22)) p.clist[base + e] = cur[e];
             }
         }
         first = false;
@@ -331,7 +332,7 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
                 const unsigned int idx = pass + tid;
                 const bool valid = idx < mine;
                 const uint32_t site = valid ? cur[idx] : 0u;
-                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, p.qcap, c.attempts);
             }
         } else {
             ++c.levels_rebalanced;
@@ -351,7 +352,7 @@ __device__ __forceinline__ unsigned int cluster_levels(const GrowthParams &p, Sh
                     }
                     site = (owner == r) ? cur[off] : ld_dsmem_u32(map_to_rank(sh_cur, owner) + 4u * off);
                 }
-                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, dst_count, p.qcap, c.attempts);
             }
         }
 #ifdef WOLFF_PROFILE
@@ -507,12 +508,13 @@ __global__ void __launch_bounds__(kGrowthThreads, 1) growth_kernel(const GrowthP
                 const unsigned int idx = pass + tid;
                 const bool valid = idx < n;
                 const uint32_t site = valid ? cur[idx] : 0u;
-                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, &sh.lcnt[lvl1], c.attempts);
+                expand_sites<DIM, POW2, SPEC>(p, s0, u_lo, u_hi, valid, site, nxt, &sh.lcnt[lvl1], p.qcap, c.attempts);
             }
             __syncthreads();
             const unsigned int n1 = sh.lcnt[lvl1];
             if (p.measure)                                            // member log of a measured run
-                for (unsigned int e = tid; e < n1; e += T) p.clist[(uint32_t)size + e] = nxt[e];
+                for (unsigned int e = tid; e < n1; e += T)
+                    if (WOLFF_CHECK(&ctl->error, (uint32_t)size + e < p.geo.N, 21)) p.clist[(uint32_t)size + e] = nxt[e];
             size += n1;
             lvl = lvl1;
             uint32_t *t = cur; cur = nxt; nxt = t;

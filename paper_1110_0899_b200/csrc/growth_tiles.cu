@@ -109,6 +109,18 @@ __device__ __forceinline__ unsigned int lds_u32(uint32_t saddr)
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
     return v;
 }
+__device__ __forceinline__ unsigned int lds_u8(uint32_t saddr)
+{
+    unsigned int v;
+    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint4 lds_v4(uint32_t saddr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(saddr) : "memory");
+    return v;
+}
 __device__ __forceinline__ void sts_u32(uint32_t saddr, unsigned int v)
 {
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
@@ -306,6 +318,7 @@ __device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uin
         sbase = __shfl_sync(kFullMask, sbase, 0);
         uint32_t *const seg = tp.spill + ((size_t)c << tp.spill_log);
         const uint32_t smask = (1u << tp.spill_log) - 1u;
+        WOLFF_CHECK(&tp.g.ctl->error, sbase + n - ld_vol64(&sh.spill_head) <= (1ull << tp.spill_log), 3);
         for (unsigned int j = lane; j < n; j += 32u) {
             const unsigned long long pos = sbase + (unsigned long long)j;
             st_relaxed_u32(seg + ((uint32_t)pos & smask), (items[j] << 1) | spill_tag(pos, tp.spill_log));
@@ -414,7 +427,7 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
         const unsigned int b0 = __ballot_sync(kFullMask, all || blk.x < tp.thr32);
         const unsigned int b1 = __ballot_sync(kFullMask, all || blk.y < tp.thr32);
         const unsigned int b2 = DIM == 3 ? __ballot_sync(kFullMask, all || blk.z < tp.thr32) : 0u;
-        if (lane < (unsigned int)DIM)
+        if (lane < (unsigned int)DIM && WOLFF_CHECK(&p.ctl->error, f.buf < tp.nbuf && f.slot < ly.myslots && f.chunk < ly.wpt, 4))
             ly.bond[(f.buf * DIM + lane) * ly.plane + f.slot * ly.wpt + f.chunk] = lane == 0u ? b0 : (lane == 1u ? b1 : b2);
     } else {
         // 32 sites of the low-d face: the bond each of them has with its -d neighbour (owned by that neighbour)
@@ -427,7 +440,8 @@ __device__ __forceinline__ bool fill_step(const TileParams &tp, TShared &sh, con
         const uint4 blk = philox4x32_10(gn, kDomainBond, (uint32_t)u, (uint32_t)(u >> 32), p.key0, p.key1);
         const uint32_t r = d == 0u ? blk.x : (d == 1u ? blk.y : blk.z);
         const unsigned int bb = __ballot_sync(kFullMask, valid && (all || r < tp.thr32));
-        if (lane == 0) ly.halo[((f.buf * DIM + d) * tp.slots + f.slot) * ly.fw + (j - d * ly.fw)] = bb;
+        if (lane == 0 && WOLFF_CHECK(&p.ctl->error, f.buf < tp.nbuf && d < (uint32_t)DIM && f.slot < ly.myslots && j - d * ly.fw < ly.fw, 5))
+            ly.halo[((f.buf * DIM + d) * tp.slots + f.slot) * ly.fw + (j - d * ly.fw)] = bb;
     }
     if (lane == 0) ++tl.chunks;
     if (++f.chunk == ly.wpt + DIM * ly.fw) {
@@ -451,46 +465,58 @@ __device__ __forceinline__ void bar_sync_named(unsigned int id, unsigned int nth
 {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
-__device__ __forceinline__ unsigned int popc_sign4(const uint4 &v)
+// Sign bits of up to eight words in ONE population count: the sign bits sit at bits 7, 15, 23, 31 of a word, so word j
+// shifted right by j lands on bits 7-j of every byte.  (POPC runs at a quarter of the ALU rate: with one per word the
+// sums below were bound by it.)
+__device__ __forceinline__ unsigned int merge4(unsigned int a, unsigned int b, unsigned int c, unsigned int d)
 {
-    return __popc(v.x & 0x80808080u) + __popc(v.y & 0x80808080u) + __popc(v.z & 0x80808080u) + __popc(v.w & 0x80808080u);
+    return (a & 0x80808080u) | ((b & 0x80808080u) >> 1) | ((c & 0x80808080u) >> 2) | ((d & 0x80808080u) >> 3);
 }
-__device__ __forceinline__ unsigned int unequal4(const uint4 &a, const uint4 &b)
-{
-    return __popc((a.x ^ b.x) & 0x80808080u) + __popc((a.y ^ b.y) & 0x80808080u) + __popc((a.z ^ b.z) & 0x80808080u) +
-           __popc((a.w ^ b.w) & 0x80808080u);
-}
+__device__ __forceinline__ unsigned int merge4(const uint4 &v) { return merge4(v.x, v.y, v.z, v.w); }
+__device__ __forceinline__ uint4 xor4(const uint4 &a, const uint4 &b) { return make_uint4(a.x ^ b.x, a.y ^ b.y, a.z ^ b.z, a.w ^ b.w); }
 
 template <int DIM>
-__device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, const Layout &ly, unsigned int c, unsigned int ptid,
-                                          unsigned int P, unsigned int krel)
+__device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, uint32_t lat_s, uint32_t nbr_s, uint32_t myslots, unsigned int c,
+                                          unsigned int ptid, unsigned int P, unsigned int krel)
 {
+    // lat_s: the tiles, nbr_s: the table of neighbouring tiles (shared-window addresses)
     constexpr unsigned int ND = 2u * DIM;
     const Tiling<DIM> tg(tp);
     Control *ctl = tp.g.ctl;
-    const uint32_t b = tg.b, B = 1u << b, m = tg.m, TS = 1u << tg.ts_log;
-    const uint32_t F = 1u << ((DIM - 1) * b), F4 = F >> 2;             // bytes / words of one face (B >= 4: F >= 4)
-    const unsigned char *const lat = reinterpret_cast<const unsigned char *>(ly.lat);
+    const uint32_t b = tg.b, B = 1u << b, m = tg.m;
+    const uint32_t f_log = (DIM - 1) * b, F = 1u << f_log;            // sites of one face
     const unsigned char *const faces = reinterpret_cast<const unsigned char *>(tp.faces);
-    // ---- 1. the low faces of my tiles -> global memory, four sites per store
+    unsigned char *const faces_out = reinterpret_cast<unsigned char *>(tp.faces);
+#ifdef WOLFF_PROFILE
+    const bool prof = ptid == 0u && c == 1u;
+    unsigned long long pt[6] = {0, 0, 0, 0, 0, 0};
+    if (prof) pt[0] = globaltimer_ns();
+#endif
+    // ---- 1. the low faces of my tiles -> global memory.  x = 0 (a byte every B in the tile): one site per lane, so that
+    // a warp's loads spread over the banks; y = 0 / z = 0 (runs of B consecutive bytes): four sites per lane.
+    for (uint32_t idx = ptid; idx < (myslots << f_log); idx += P) {
+        const uint32_t slot = idx >> f_log, f = idx & (F - 1u);
+        faces_out[(size_t)((slot * tp.G + c) * DIM) * F + f] = (unsigned char)lds_u8(lat_s + (slot << tg.ts_log) + (f << b));
+    }
     {
         unsigned int *const fout = reinterpret_cast<unsigned int *>(tp.faces);
-        const uint32_t nwords = ly.myslots * DIM * F4;
+        const uint32_t f4_log = f_log - 2u;                           // log2 of the words of one face (B >= 4)
+        const uint32_t nwords = (myslots * (DIM - 1)) << f4_log;
         for (uint32_t idx = ptid; idx < nwords; idx += P) {
-            const uint32_t slot = idx / (DIM * F4), rem = idx - slot * (DIM * F4), d = rem / F4, f0 = (rem - d * F4) << 2;
-            const uint32_t low = (1u << (d * b)) - 1u;
-            uint32_t word = 0;
-#pragma unroll
-            for (uint32_t j = 0; j < 4u; ++j) {
-                const uint32_t f = f0 + j;
-                const uint32_t w = (f & low) | ((f >> (d * b)) << ((d + 1u) * b));     // coordinate d = 0
-                word |= (uint32_t)lat[(slot << tg.ts_log) + w] << (8u * j);
-            }
-            fout[((slot * tp.G + c) * DIM + d) * F4 + (f0 >> 2)] = word;
+            const uint32_t sd = idx >> f4_log, slot = sd / (DIM - 1), d = 1u + (sd - slot * (DIM - 1)), f0 = (idx & ((1u << f4_log) - 1u)) << 2;
+            const uint32_t low = (1u << (d * b)) - 1u;                // f = x | z << b (y = 0)  or  x | y << b (z = 0)
+            fout[(((slot * tp.G + c) * DIM + d) << f4_log) + (f0 >> 2)] =
+                lds_u32(lat_s + (slot << tg.ts_log) + ((f0 & low) | ((f0 >> (d * b)) << ((d + 1u) * b))));
         }
     }
     __threadfence();
+#ifdef WOLFF_PROFILE
+    if (prof) pt[1] = globaltimer_ns();
+#endif
     bar_sync_named(1u, P);
+#ifdef WOLFF_PROFILE
+    if (prof) pt[2] = globaltimer_ns();
+#endif
     if (ptid == 0u) {
         atomicAdd(&ctl->meas_arrive_a, 1u);
         const unsigned int target = (krel + 1u) * tp.G;
@@ -499,47 +525,88 @@ __device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, co
             if ((++polls & 0xFFu) == 0u && ld_relaxed_u32(&ctl->error) != 0u) break;
     }
     bar_sync_named(1u, P);
+#ifdef WOLFF_PROFILE
+    if (prof) pt[3] = globaltimer_ns();
+#endif
     // ---- 2. my tiles: negative spins and unequal forward bonds
     unsigned int un = 0, ng = 0;
     auto face_of = [&](uint32_t slot, uint32_t d) -> const unsigned char * {
-        const uint32_t nt = ly.nbrtab[slot * ND + 2u * d];                  // (owner << 16) | slot of the +d neighbouring tile
+        const uint32_t nt = lds_u32(nbr_s + (slot * ND + 2u * d) * 4u);       // (owner << 16) | slot of the +d neighbouring tile
         return faces + (size_t)(((nt & 0xFFFFu) * tp.G + (nt >> 16)) * DIM + d) * F;
     };
     if (b >= 4u) {
-        const uint32_t cpt_log = tg.ts_log - 4u, total = ly.myslots << cpt_log;
-        for (uint32_t ch = ptid; ch < total; ch += P) {
+        // (a) the bonds inside my tiles: shared memory only, 16 sites per load
+        const uint32_t cpt_log = tg.ts_log - 4u, total = myslots << cpt_log;
+        auto chunk = [&](uint32_t ch) {
             const uint32_t slot = ch >> cpt_log, w0 = (ch & ((1u << cpt_log) - 1u)) << 4;
             const uint32_t x0 = w0 & m, y = (w0 >> b) & m, z = DIM == 3 ? (w0 >> (2u * b)) : 0u;
-            const unsigned char *const at = lat + (slot << tg.ts_log) + w0;
-            const uint4 a = *reinterpret_cast<const uint4 *>(at);
-            ng += popc_sign4(a);
-            // +x: the 16 sites shifted by one byte; the 17th is the next site of the row, or the +x tile's low-x face
-            const uint32_t nb = x0 + 16u < B ? (uint32_t)at[16] : (uint32_t)__ldcg(face_of(slot, 0u) + (w0 >> b));
-            un += __popc((a.x ^ __funnelshift_r(a.x, a.y, 8)) & 0x80808080u) + __popc((a.y ^ __funnelshift_r(a.y, a.z, 8)) & 0x80808080u) +
-                  __popc((a.z ^ __funnelshift_r(a.z, a.w, 8)) & 0x80808080u) + __popc((a.w ^ __funnelshift_r(a.w, nb, 8)) & 0x80808080u);
-            const uint4 by = y + 1u < B ? *reinterpret_cast<const uint4 *>(at + B)
-                                        : __ldcg(reinterpret_cast<const uint4 *>(face_of(slot, 1u) + (x0 | (z << b))));
-            un += unequal4(a, by);
-            if (DIM == 3) {
-                const uint4 bz = z + 1u < B ? *reinterpret_cast<const uint4 *>(at + (B << b))
-                                            : __ldcg(reinterpret_cast<const uint4 *>(face_of(slot, 2u) + (x0 | (y << b))));
-                un += unequal4(a, bz);
+            const uint32_t at = lat_s + (slot << tg.ts_log) + w0;
+            const uint4 a = lds_v4(at);
+            // forward rows: inside the tile, else the row itself (equal words count nothing; the bond is counted in (b))
+            const uint4 by = lds_v4(y + 1u < B ? at + B : at);
+            const uint4 bz = DIM == 3 ? lds_v4(z + 1u < B ? at + (B << b) : at) : a;
+            // +x: the 16 sites shifted by one byte; the 17th is the next site of the row -- or, at the end of the row, a
+            // copy of the 16th, so that the bond across the tile border counts nothing here
+            const uint32_t nb = x0 + 16u < B ? lds_u8(at + 16u) : (a.w >> 24);
+            ng += __popc(merge4(a));
+            const unsigned int bx = merge4(a.x ^ __funnelshift_r(a.x, a.y, 8), a.y ^ __funnelshift_r(a.y, a.z, 8),
+                                           a.z ^ __funnelshift_r(a.z, a.w, 8), a.w ^ __funnelshift_r(a.w, nb, 8));
+            un += __popc(bx | (merge4(xor4(a, by)) >> 4));
+            if (DIM == 3) un += __popc(merge4(xor4(a, bz)));
+        };
+        uint32_t ch = ptid;
+        for (; ch + P < total; ch += 2u * P) { chunk(ch); chunk(ch + P); }
+        if (ch < total) chunk(ch);
+        // (b1) the bonds across the +x border of a tile: my site x = B - 1 against the next tile's x = 0 (global memory),
+        // one site per lane, eight global loads in flight per lane (a trip costs one L2 round trip, not eight)
+        constexpr uint32_t kSites = 8;
+        const uint32_t nsites = myslots << f_log;
+        for (uint32_t i0 = ptid; i0 < nsites; i0 += P * kSites) {
+            unsigned int theirs[kSites], mine[kSites];
+#pragma unroll
+            for (uint32_t j = 0; j < kSites; ++j) {
+                const uint32_t idx = i0 + j * P, ii = idx < nsites ? idx : 0u, slot = ii >> f_log, f = ii & (F - 1u);
+                theirs[j] = __ldcg(face_of(slot, 0u) + f);
+                mine[j] = lds_u8(lat_s + (slot << tg.ts_log) + (f << b) + m);
             }
+#pragma unroll
+            for (uint32_t j = 0; j < kSites; ++j)
+                if (i0 + j * P < nsites) un += ((mine[j] ^ theirs[j]) >> 7) & 1u;
+        }
+        // (b2) across the +y / +z borders: 16 sites per load on both sides, four tasks per trip, their global loads first
+        const uint32_t g_log = f_log - 4u;                            // log2 of the 16-site groups of one face
+        const uint32_t tasks = (myslots * (DIM - 1)) << g_log;
+        constexpr uint32_t kTasks = 4;
+        for (uint32_t t0 = ptid; t0 < tasks; t0 += P * kTasks) {
+            uint4 theirs[kTasks], mine[kTasks];
+            bool on[kTasks];
+#pragma unroll
+            for (uint32_t j = 0; j < kTasks; ++j) {
+                const uint32_t t = t0 + j * P;
+                on[j] = t < tasks;
+                const uint32_t tt = on[j] ? t : 0u, sd = tt >> g_log, slot = sd / (DIM - 1), d = 1u + (sd - slot * (DIM - 1));
+                const uint32_t f0 = (tt & ((1u << g_log) - 1u)) << 4, low = (1u << (d * b)) - 1u;
+                theirs[j] = __ldcg(reinterpret_cast<const uint4 *>(face_of(slot, d) + f0));
+                mine[j] = lds_v4(lat_s + (slot << tg.ts_log) + ((f0 & low) | ((f0 >> (d * b)) << ((d + 1u) * b)) | (m << (d * b))));   // coordinate d = B - 1
+            }
+#pragma unroll
+            for (uint32_t j = 0; j < kTasks; ++j)
+                if (on[j]) un += __popc(merge4(xor4(mine[j], theirs[j])));
         }
     } else {
         // tiles narrower than a 16-byte load (test configurations): one site at a time
-        const uint32_t total = ly.myslots << tg.ts_log;
+        const uint32_t total = myslots << tg.ts_log;
         for (uint32_t idx = ptid; idx < total; idx += P) {
             const uint32_t slot = idx >> tg.ts_log, w = idx & tg.ts_mask;
-            const uint32_t s = lat[idx];
-            ng += s >> 7;
+            const uint32_t s0b = lds_u8(lat_s + idx);
+            ng += s0b >> 7;
 #pragma unroll
             for (uint32_t d = 0; d < (uint32_t)DIM; ++d) {
                 const uint32_t low = (1u << (d * b)) - 1u;
                 uint32_t nbv;
-                if (((w >> (d * b)) & m) != m) nbv = lat[idx + (1u << (d * b))];
+                if (((w >> (d * b)) & m) != m) nbv = lds_u8(lat_s + idx + (1u << (d * b)));
                 else nbv = __ldcg(face_of(slot, d) + ((w & low) | ((w >> ((d + 1u) * b)) << (d * b))));
-                un += ((s ^ nbv) >> 7) & 1u;
+                un += ((s0b ^ nbv) >> 7) & 1u;
             }
         }
     }
@@ -549,7 +616,17 @@ __device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, co
         if (un) atomicAdd(&sh.meas_un, (unsigned long long)un);
         if (ng) atomicAdd(&sh.meas_ng, (unsigned long long)ng);
     }
+#ifdef WOLFF_PROFILE
+    if (prof) pt[4] = globaltimer_ns();
+#endif
     bar_sync_named(1u, P);
+#ifdef WOLFF_PROFILE
+    if (prof) {
+        pt[5] = globaltimer_ns();
+        // [2] faces  [3] wait for the CTA's warps  [4] wait for all CTAs  [5] sums  [6] wait for the CTA's warps again
+        for (int i = 0; i < 5; ++i) atomicAdd(&ctl->stats[2 + i], pt[i + 1] - pt[i]);
+    }
+#endif
     if (ptid == 0u) {
         const unsigned long long tun = ld_vol64(&sh.meas_un), tng = ld_vol64(&sh.meas_ng);
         st_vol64(&sh.meas_un, 0ull);
@@ -671,6 +748,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
                 st[j] = lds_u32(state_s + slot[j] * 4u);                              // state first: see fill_step()
                 bw[j] = lds_u32(baddr);
             }
+            if (have[j] && !WOLFF_CHECK(&p.ctl->error, local[j] ? na[j] < (ly.myslots << tg.ts_log) : own[j] < tp.G, 1)) { have[j] = false; local[j] = true; na[j] = 0u; }
             if (local[j]) spw[j] = lds_u32(lat_s + (na[j] & ~3u));                    // gather
             bytemask[j] = 0xFFu << ((na[j] & 3u) * 8u);
         }
@@ -758,11 +836,13 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
         if (total == 0u) return 1;                               // the warp runs dry
         uint32_t *const st_out = stage + sbuf;
         const uint32_t out_s = stage_s + sbuf * 4u;
+        const unsigned int sbuf_prev = sbuf; (void)sbuf_prev;
         sbuf ^= 32u * W;
         unsigned int before = 0;
 #pragma unroll
         for (unsigned int j = 0; j < W; ++j) {
-            if (won[j]) sts_u32(out_s + (before + __popc(wb[j] & lt)) * 4u, na[j]);
+            if (won[j] && WOLFF_CHECK(&p.ctl->error, sbuf_prev + before + __popc(wb[j] & lt) < (unsigned int)kStage, 8))
+                sts_u32(out_s + (before + __popc(wb[j] & lt)) * 4u, na[j]);
             before += __popc(wb[j]);
         }
         __syncwarp();
@@ -854,7 +934,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
         if (n == 0u) {
             mreq = __shfl_sync(kFullMask, mreq, 0);
             if (mreq != meas_done) {                                   // the update is over everywhere: measure (see measure_phase)
-                measure_phase<DIM>(tp, sh, ly, c, ptid, P, mreq - 1u);
+                measure_phase<DIM>(tp, sh, smem_addr(ly.lat), smem_addr(ly.nbrtab), ly.myslots, c, ptid, P, mreq - 1u);
                 meas_done = mreq;
                 continue;
             }
@@ -969,7 +1049,7 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
             if (what == 1u) {
                 if (lane == 0) { __threadfence_block(); st_vol(&sh.meas_req, krel_m + 1u); }
                 __syncwarp();
-                measure_phase<DIM>(tp, sh, ly, c, lane, c == 0u ? kT - 32u : kT, krel_m);
+                measure_phase<DIM>(tp, sh, smem_addr(ly.lat), smem_addr(ly.nbrtab), ly.myslots, c, lane, c == 0u ? kT - 32u : kT, krel_m);
                 continue;
             }
             break;
@@ -977,7 +1057,7 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
         const uint32_t addr = lo >> 1;
         int s0 = (lo & 1u) ? -1 : 1;
         bool win = false;
-        if (mine) {
+        if (mine && WOLFF_CHECK(&p.ctl->error, addr < (ly.myslots << (DIM * tp.tile_log)) && (unsigned long long)(hi & (kMaxK - 1u)) < p.n_updates, 2)) {
             if (kind == kKindSeed) s0 = (int)vol(reinterpret_cast<const signed char *>(ly.lat) + addr);   // A1: the seed spin
             win = claim_and_flip(ly.lat, addr, s0);
             ++tl.attempts;
@@ -1045,6 +1125,7 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
             const uint32_t i0 = (uint32_t)__umul64hi(rr, (unsigned long long)p.geo.N);
             uint32_t own, addr;
             tg.locate(i0, own, addr);
+            WOLFF_CHECK(&ctl->error, i0 < p.geo.N && own < G && addr < (tp.slots << (DIM * tp.tile_log)), 7);
             const unsigned int pos = atomicAdd(tp.gtail + own, 1u);
             wait_inbox(tp, own, pos);
             st_relaxed_u64(tp.inbox + ((size_t)own << tp.in_log) + (pos & in_mask),
@@ -1084,6 +1165,9 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
             prev = a;
         }
         if (p.measure && !aborted) {
+#ifdef WOLFF_PROFILE
+            const unsigned long long tm0 = globaltimer_ns();
+#endif
             // "+ measurement": every CTA evaluates its tiles (measure_phase); the request travels like the exit message
             for (unsigned int base = 0; base < G; base += 256u) {
                 unsigned int pos[8];
@@ -1122,6 +1206,9 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
                 }
             }
             if (__shfl_sync(kFullMask, bad, 0)) aborted = true;
+#ifdef WOLFF_PROFILE
+            if (lane == 0) atomicAdd(&ctl->stats[8], globaltimer_ns() - tm0);     // the monitor's view of one measurement
+#endif
         }
     }
     if (p.measure && lane == 0 && !aborted && p.n_updates > 0) { ctl->E = lastE; ctl->M = lastM; mom.store(ctl->moments); }
@@ -1170,6 +1257,7 @@ __device__ __forceinline__ void copy_tiles_vec(const TileParams &tp, const Layou
             const uint32_t a = (idx < total ? idx : 0u) * VB;
             const uint32_t gi = ly.origin[a >> tg.ts_log] + tg.spread(a & tg.ts_mask);
             gp[u] = reinterpret_cast<V *>(tp.g.spins + gi);
+            WOLFF_CHECK(&tp.g.ctl->error, idx >= total || (size_t)gi + VB <= (((size_t)tp.g.geo.N + 15u) & ~(size_t)15u), 6);
             if (idx < total) v[u] = LOAD ? __ldcg(gp[u]) : loc[idx];
         }
 #pragma unroll
@@ -1271,7 +1359,7 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const __grid_consta
     copy_tiles<DIM, false>(tp, ly);
 #ifdef WOLFF_PROFILE
     __syncthreads();
-    if (tid == 0 && c == 0) {
+    if (tid == 0 && c == 0 && !tp.g.measure) {     // (a measured profiling run uses these slots for the measurement's phases)
         tp.g.ctl->stats[4] = tk1 - tk0; tp.g.ctl->stats[5] = tk2 - tk1; tp.g.ctl->stats[6] = globaltimer_ns() - tk2;
     }
 #endif
@@ -1292,8 +1380,8 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const __grid_consta
         if (tl.ring_pushes) atomicAdd(&ctl->stats[12], (unsigned long long)tl.ring_pushes);
         if (tl.spills) atomicAdd(&ctl->stats[14], (unsigned long long)tl.spills);
 #ifdef WOLFF_PROFILE
-        if (tl.cyc_pass) atomicAdd(&ctl->stats[2], tl.cyc_pass);
-        if (tl.lanes) atomicAdd(&ctl->stats[3], tl.lanes);
+        if (tl.cyc_pass && !tp.g.measure) atomicAdd(&ctl->stats[2], tl.cyc_pass);
+        if (tl.lanes && !tp.g.measure) atomicAdd(&ctl->stats[3], tl.lanes);
 #endif
     }
 }

@@ -155,10 +155,15 @@ size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t rin
 cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm);
 cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes, cudaStream_t stream);
 // batch of chains: CTAs of `threads` threads, `grid` of them; co-resident CTAs per SM; E, M of every chain into EM
-cudaError_t launch_growth_batch(const BatchParams &bp, int dim, int grid, int threads, cudaStream_t stream);
-cudaError_t batch_ctas_per_sm(int dim, bool pow2, int threads, uint32_t qcap, int *per_sm);
+// bits: the bit-packed shared-memory-resident variant; its shared memory: the frontier buffers + N/8 bytes per plane
+size_t batch_smem_bytes(uint32_t N, uint32_t qcap, bool bits, bool measure);
+cudaError_t launch_growth_batch(const BatchParams &bp, int dim, bool bits, int grid, int threads, cudaStream_t stream);
+cudaError_t batch_ctas_per_sm(int dim, bool pow2, bool bits, int threads, size_t smem, int *per_sm);
 cudaError_t launch_batch_energy(const int8_t *spins, size_t stride, const Geometry &geo, int dim, uint32_t R, unsigned long long *acc,
                                 long long *EM, int num_sms, cudaStream_t stream);
+#ifdef WOLFF_CHECKED
+cudaError_t launch_check_selftest(Control *ctl, cudaStream_t stream);      // one failing WOLFF_CHECK (code 99)
+#endif
 cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, int num_sms, cudaStream_t stream);
 cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, int num_sms, cudaStream_t stream);
 // n_bytes spins (16-byte aligned buffer) are all +1 / -1, else *invalid |= 1

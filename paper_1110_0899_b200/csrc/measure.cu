@@ -120,6 +120,14 @@ __device__ __forceinline__ void block_accumulate(unsigned long long unequal, uns
 // uses any: the kernel is a few microseconds long, so what it needs is bytes in flight.
 constexpr int kU = 4;
 
+// Sign bits of four words in one word: they sit at bits 7, 15, 23, 31, so word j shifted right by j lands on bit 7 - j of
+// every byte; two such merges (the second shifted by 4) give eight words per population count (POPC runs at a quarter
+// of the ALU rate).
+__device__ __forceinline__ uint32_t merge4(uint32_t a, uint32_t b, uint32_t c, uint32_t d)
+{
+    return (a & kSignMask) | ((b & kSignMask) >> 1) | ((c & kSignMask) >> 2) | ((d & kSignMask) >> 3);
+}
+
 template <int DIM>
 __global__ void __launch_bounds__(kThreads) energy_magnetisation_vec16(const int8_t *__restrict__ spins, Geometry g, Control *ctl,
                                                                        long long *E_dst, long long *M_dst)
@@ -155,17 +163,12 @@ __global__ void __launch_bounds__(kThreads) energy_magnetisation_vec16(const int
         }
 #pragma unroll
         for (int u = 0; u < kU; ++u) {
-            uint32_t acc = 0, neg = 0;
-            acc += __popc((a[u].x ^ __funnelshift_r(a[u].x, a[u].y, 8)) & kSignMask);
-            acc += __popc((a[u].y ^ __funnelshift_r(a[u].y, a[u].z, 8)) & kSignMask);
-            acc += __popc((a[u].z ^ __funnelshift_r(a[u].z, a[u].w, 8)) & kSignMask);
-            acc += __popc((a[u].w ^ __funnelshift_r(a[u].w, nb[u], 8)) & kSignMask);
-            neg += __popc(a[u].x & kSignMask) + __popc(a[u].y & kSignMask) + __popc(a[u].z & kSignMask) + __popc(a[u].w & kSignMask);
-            acc += __popc((a[u].x ^ by[u].x) & kSignMask) + __popc((a[u].y ^ by[u].y) & kSignMask) +
-                   __popc((a[u].z ^ by[u].z) & kSignMask) + __popc((a[u].w ^ by[u].w) & kSignMask);
-            if (DIM == 3)
-                acc += __popc((a[u].x ^ bz[u].x) & kSignMask) + __popc((a[u].y ^ bz[u].y) & kSignMask) +
-                       __popc((a[u].z ^ bz[u].z) & kSignMask) + __popc((a[u].w ^ bz[u].w) & kSignMask);
+            const uint32_t neg = __popc(merge4(a[u].x, a[u].y, a[u].z, a[u].w));
+            const uint32_t bx = merge4(a[u].x ^ __funnelshift_r(a[u].x, a[u].y, 8), a[u].y ^ __funnelshift_r(a[u].y, a[u].z, 8),
+                                       a[u].z ^ __funnelshift_r(a[u].z, a[u].w, 8), a[u].w ^ __funnelshift_r(a[u].w, nb[u], 8));
+            const uint32_t byb = merge4(a[u].x ^ by[u].x, a[u].y ^ by[u].y, a[u].z ^ by[u].z, a[u].w ^ by[u].w);
+            uint32_t acc = __popc(bx | (byb >> 4));
+            if (DIM == 3) acc += __popc(merge4(a[u].x ^ bz[u].x, a[u].y ^ bz[u].y, a[u].z ^ bz[u].z, a[u].w ^ bz[u].w));
             if (on[u]) { unequal += acc; negative += neg; }
         }
     }
@@ -206,6 +209,15 @@ cudaError_t launch_init_lattice(int8_t *spins, uint32_t N, uint64_t seed, int nu
     init_lattice_kernel<<<grid, kThreads, 0, stream>>>(spins, N, (uint32_t)seed, (uint32_t)(seed >> 32));
     return cudaGetLastError();
 }
+
+#ifdef WOLFF_CHECKED
+__global__ void check_selftest_kernel(Control *ctl) { WOLFF_CHECK(&ctl->error, ctl == nullptr, 99); }
+cudaError_t launch_check_selftest(Control *ctl, cudaStream_t stream)
+{
+    check_selftest_kernel<<<1, 1, 0, stream>>>(ctl);
+    return cudaGetLastError();
+}
+#endif
 
 cudaError_t launch_validate(const int8_t *spins, uint32_t N, Control *ctl, int num_sms, cudaStream_t stream)
 {

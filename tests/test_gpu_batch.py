@@ -65,21 +65,28 @@ def sweep(R, lo, hi):
     return [lo + (hi - lo) * r / max(R - 1, 1) for r in range(R)]
 
 
+# where a chain's lattice lives during its turn: the int8 lattice in global memory, or bit-packed in shared memory
+RESIDENT = [1, 2]
+
+
+@pytest.mark.parametrize("resident", RESIDENT)
 @pytest.mark.parametrize("measured", [False, True])
 @pytest.mark.parametrize("dim,L,Tlo,Thi", [(2, 32, 1.8, 3.2), (3, 12, 3.8, 5.4), (2, 20, 2.0, 2.6), (3, 8, 4.2, 4.8)])
-def test_temperature_sweep_of_160_replicas(dim, L, Tlo, Thi, measured):
+def test_temperature_sweep_of_160_replicas(dim, L, Tlo, Thi, measured, resident):
     # more replicas than SMs: every CTA slot of the chip is in use, chains queue for CTAs; one T and seed per replica
     R = 160
     T = sweep(R, Tlo, Thi)
     seeds = [1000 + 7 * r for r in range(R)]
-    gpu, refs = make_batch(dim, L, T, seeds, options={"measure": int(measured)})
+    gpu, refs = make_batch(dim, L, T, seeds, options={"measure": int(measured), "resident": resident})
     assert_same_lattices(gpu, refs, "start lattices (reading R9)")
     compare(gpu, refs, [1, 40, 200], measured=measured)
     gpu.close()
 
 
 @pytest.mark.parametrize("options", [{"threads": 32}, {"threads": 64, "queue_cap": 8}, {"threads": 128, "queue_cap": 8, "measure": 1},
-                                      {"threads": 256, "measure": 1}, {"threads": 32, "queue_cap": 16, "measure": 1}])
+                                      {"threads": 256, "measure": 1}, {"threads": 32, "queue_cap": 16, "measure": 1},
+                                      {"threads": 32, "resident": 2}, {"threads": 64, "queue_cap": 8, "resident": 2, "measure": 1},
+                                      {"threads": 256, "resident": 2, "measure": 1}, {"threads": 128, "queue_cap": 8, "resident": 1}])
 def test_launch_shapes_and_tiny_frontier_buffers(options):
     # queue_cap 8: every level wider than 8 sites is read back from the member list in global memory
     R = 24
@@ -89,27 +96,39 @@ def test_launch_shapes_and_tiny_frontier_buffers(options):
     gpu.close()
 
 
+@pytest.mark.parametrize("resident", RESIDENT)
 @pytest.mark.parametrize("measured", [False, True])
-def test_wide_frontiers_p_one_and_p_zero(measured):
+def test_wide_frontiers_p_one_and_p_zero(measured, resident):
     # chain 0: p = 1 from a cold start (the first cluster is the whole lattice); chain 1: p = 0 (only the seed flips);
     # chain 2: T_c; non-power-of-two L
     for dim, L in [(2, 100), (3, 20)]:
         N = L ** dim
         gpu, refs = make_batch(dim, L, [0.04, 1.0, wl.TC_2D if dim == 2 else wl.TC_3D], [3, 4, 5], J=[1.0, 0.0, 1.0],
-                               options={"measure": int(measured)}, start=np.stack([wl.cold(N)] * 3))
+                               options={"measure": int(measured), "resident": resident}, start=np.stack([wl.cold(N)] * 3))
         assert gpu.thresholds.tolist()[:2] == [1 << 32, 0]
         compare(gpu, refs, [1, 2, 10], measured=measured)
         gpu.close()
 
 
-def test_medium_lattices_equilibrated_variant():
-    # C2-sized chains from a cold start: frontiers of hundreds of sites, clusters of 10^5..10^6 spins, in one CTA each
+@pytest.mark.parametrize("resident", RESIDENT)
+def test_medium_lattices_equilibrated_variant(resident):
+    # C2-sized chains from a cold start: frontiers of hundreds of sites, clusters of 10^5..10^6 spins, in one CTA each.
+    # resident 2: the 128 KiB sign plane of 2D L=1024 fills one SM's shared memory; the mark plane
+    # of a measured run does not fit beside it, so the measured part runs 3D L=64 (two planes of 32 KiB)
     c = wl.CONFIGS["C2"]
     R = 3
-    gpu, refs = make_batch(c.dim, c.L, [c.T, 2.2, 2.35], [1, 2, 3], start=np.stack([wl.cold(c.N)] * R))
+    gpu, refs = make_batch(c.dim, c.L, [c.T, 2.2, 2.35], [1, 2, 3], start=np.stack([wl.cold(c.N)] * R), options={"resident": resident})
     compare(gpu, refs, [1, 12])
-    gpu.set_option("measure", 1)
-    compare(gpu, refs, [6], measured=True)
+    if resident == 2:
+        gpu.set_option("measure", 1)
+        with pytest.raises(binding.WolffError):
+            gpu.run(1)
+        gpu.close()
+        gpu, refs = make_batch(3, 64, [wl.TC_3D, 4.3, 4.7], [1, 2, 3], start=np.stack([wl.cold(64 ** 3)] * R), options={"resident": 2, "measure": 1})
+        compare(gpu, refs, [2, 30], measured=True)
+    else:
+        gpu.set_option("measure", 1)
+        compare(gpu, refs, [6], measured=True)
     gpu.close()
 
 
