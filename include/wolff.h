@@ -160,6 +160,8 @@ WOLFF_API int wolff_reset_moments(wolff_handle h);
  *   "cooperative"          1 (default) = cooperative launch, 0 = plain launch of a grid sized to be co-resident
  *   "speculative"          level-synchronous kernel: 1 = no neighbour gather, the claim atomic is issued for every active
  *                          bond and its returned byte says whether the neighbour was parallel (default 0)
+ *   "check_selftest"       bounds-checked builds only (-DWOLFF_CHECKED, libwolff_b200_checked.so): makes one check fail on
+ *                          purpose, so that a test can see the report arrive (WOLFF_EINTERNAL at the next call)
  * Thresholds are clamped to what the shared-memory queues can hold.  Unknown key or out-of-range
  * value: WOLFF_EINVAL. */
 WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);
