@@ -121,24 +121,35 @@ WOLFF_API int wolff_get_series(wolff_handle h, int64_t *E_series, int64_t *M_ser
 WOLFF_API int wolff_get_moments(wolff_handle h, uint64_t *moments, double *binder);
 WOLFF_API int wolff_reset_moments(wolff_handle h);
 
-/* Tuning / test knobs; never change the result.  Two growth kernels implement wolff_run:
- *  - the shared-memory-resident, barrier-free kernel (lattice tiles live in the CTAs' shared memory for the
- *    launch, claims across CTAs travel as messages, bond variables come from tables filled ahead of time):
- *    used whenever L is a power of two >= 4 and the lattice fits the chip's shared memory;
+/* Tuning / test knobs; never change the result.  Three growth kernels implement wolff_run:
+ *  - the shared-memory-resident, barrier-free kernel of all SMs (int8 lattice tiles live in the CTAs' shared memory
+ *    for the launch, claims across CTAs travel as messages, bond variables come from tables filled ahead of time):
+ *    applies when L is a power of two >= 4 and the lattice fits the chip's shared memory; the fastest on clusters of
+ *    tens of thousands of spins and more (the BASELINE lattices at T_c);
+ *  - the cluster-resident, bit-packed, barrier-free kernel (one bit per spin in the distributed shared memory of ONE
+ *    thread-block cluster of up to 16 CTAs; a claim is one atomic on the word that holds the spin, in whichever CTA
+ *    holds it; the warp that draws the seed site expands it itself): applies when L is a power of two, N >= 32 and
+ *    N / 8 bytes fit one cluster (N <= 2^24); the fastest on small and medium clusters (the literal random start of
+ *    the BASELINE configs, T above T_c, 3D L = 128);
  *  - the level-synchronous kernel, which runs each BFS level in one of three tiers by frontier width n: one
- *    CTA (n <= up), one thread-block cluster (n <= cluster_up), the whole grid (above): used otherwise.
+ *    CTA (n <= up), one thread-block cluster (n <= cluster_up), the whole grid (above): any L.
  * Keys:
- *   "mode"                 0 = shared-memory-resident kernel where it applies, else level-synchronous tiers
- *                          (default); level-synchronous kernel only: 4 = tiers by frontier width, 1 = every level
+ *   "mode"                 0 = chosen by the mean cluster size of the last finished run, see "small_cluster" (default);
+ *                          5 = the cluster-resident kernel whenever it applies (else as mode 0);
+ *                          level-synchronous kernel only: 4 = tiers by frontier width, 1 = every level
  *                          grid-wide, 2 = one CTA whenever the frontier fits its shared-memory queue, 3 = the
  *                          cluster whenever it fits
- *   "measure"              1 = E and M after every update inside the kernel (see wolff_get_series); default 0
+ *   "measure"              1 = E and M after every update inside the kernel (see wolff_get_series); default 0.  The
+ *                          cluster-resident kernel does not measure: a measured run uses one of the other two
  *   "small_cluster"        mode 0: when the last finished run (seen at the caller's next synchronising call) had a mean
- *                          cluster below this size, the next run uses the level-synchronous kernel, whose fixed
- *                          cost per update is lower (default 16; 0 = never)
+ *                          cluster below this size, the next run uses the cluster-resident kernel (default 32768; 0 =
+ *                          never); where that kernel does not apply, runs with a mean cluster below min(16, this) use
+ *                          the level-synchronous kernel, whose fixed cost per update is lower than the first kernel's
+ *   "resident_ctas"        cluster-resident kernel: CTAs of the cluster, at most (1, 2, 4, 8 or 16; default 16)
  *   "tile_log"             shared-memory-resident kernel: log2 of the tile side (0 = auto: 6 in 2D, 4 in 3D)
  *   "tile_ctas"            ... CTAs that share the lattice (0 = one per SM)
- *   "ring_cap"             ... entries of a CTA's shared-memory work ring (power of two; overflow spills to global memory)
+ *   "ring_cap"             ... entries of a CTA's shared-memory work ring (power of two; overflow spills to global memory);
+ *                          also the ring of the cluster-resident kernel
  *   "inbox_log"            ... log2 of the entries of a CTA's inbox, the global-memory queue of claims other CTAs send it
  *                          (0 = auto: what one update can send at most, no capacity checks; 5..24: a smaller inbox --
  *                          a sender that finds it full waits for the receiver, which never waits for anybody)
@@ -175,6 +186,7 @@ WOLFF_API int wolff_set_option(wolff_handle h, const char *key, int64_t value);
  *   [11] messages between CTAs                      [12] sites handed over through the ring
  *   [13] warp passes (profiling builds)             [14] sites spilled to global memory
  *   [15] bond-table chunks filled (32 sites each)
+ * cluster-resident kernel: [0], [1], [7], [9], [12], [13], [14] as above; [11] sites taken out of another CTA's ring
  * Blocks until the run has finished. */
 #define WOLFF_NSTATS 16
 WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);

@@ -90,8 +90,16 @@ struct wolff_ctx {
     uint32_t *tile_spill = nullptr;
     uint32_t *tile_fill = nullptr;
     int8_t *tile_faces = nullptr;   // in-kernel measurement: the low faces of every tile
+    // cluster-resident bit-packed kernel (growth_cluster.cu): plan and the device state that goes with it
+    int resident_ctas = 16;         // largest cluster the plan may use
+    bool cl_dirty = true;
+    bool cl_ok = false;
+    ClusterParams cp{};
+    size_t cl_smem = 0;
+    uint32_t *cl_spill = nullptr;
+    unsigned long long *cl_spill_ctr = nullptr;
     // kernel choice in mode 0: mean cluster size of the last finished run (read when the caller next synchronises)
-    uint64_t small_cluster = 16;    // below this mean size the level-synchronous kernel runs (its fixed cost per update is lower); 0 = never
+    uint64_t small_cluster = 32768; // below this mean size mode 0 leaves the kernel of all SMs for the cluster-resident one; 0 = never
     bool have_mean = false;
     bool run_since_set = false;     // a run has been queued since the lattice was last loaded: its counters describe this lattice
     double mean_cluster = 0.0;
@@ -196,6 +204,59 @@ void free_tile_state(wolff_ctx *h)
 }
 
 uint32_t ceil_log2(uint64_t v) { uint32_t l = 0; while ((1ull << l) < v) ++l; return l; }
+
+void free_cluster_state(wolff_ctx *h)
+{
+    cudaFree(h->cl_spill); h->cl_spill = nullptr;
+    cudaFree(h->cl_spill_ctr); h->cl_spill_ctr = nullptr;
+}
+
+// (Re)derive the launch shape of growth_cluster.cu: the largest cluster (at most "cluster_ctas" CTAs) whose CTAs each
+// hold a power-of-two number of 32-bit words of the bit lattice, the ring and the stages in their shared memory.
+// cl_ok == false (L not a power of two, fewer than 32 spins, or the lattice does not fit one cluster) is not an error.
+int refresh_cluster_plan(wolff_ctx *h, cudaStream_t stream)
+{
+    if (!h->cl_dirty) return WOLFF_OK;
+    if (h->ran) CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+    free_cluster_state(h);
+    h->cl_ok = false;
+    h->cl_dirty = false;
+    if (!h->geo.pow2 || h->N < 32 || h->N > (1ull << 31)) return WOLFF_OK;
+    const uint64_t words = h->N / 32;
+    uint32_t nC = 16;
+    while (nC > 1 && (nC > (uint32_t)h->resident_ctas || nC > words)) nC >>= 1;
+    size_t smem = 0;
+    int clusters = 0;
+    // the largest cluster allowed: a CTA's share of the lattice (words / nC, a power of two) must fit its shared memory
+    smem = cluster_smem_bytes((uint32_t)(words / nC), h->ring_cap);
+    if (smem + 1024 > h->smem_optin) return WOLFF_OK;
+    cudaError_t e = cluster_prepare(h->dim, nC, smem, &clusters);
+    if (e != cudaSuccess || clusters < 1) { cudaGetLastError(); return WOLFF_OK; }
+    ClusterParams &cp = h->cp;
+    cp = ClusterParams{};
+    cp.nC = nC;
+    cp.wpc = (uint32_t)(words / nC);
+    cp.wpc_log = ceil_log2(cp.wpc);
+    cp.ring_cap = h->ring_cap;
+    cp.spill_log = ceil_log2(h->N);
+    cp.watchdog_ns = h->watchdog_ms * 1000000ull;
+    cp.thr32 = (uint32_t)h->thr;
+    cp.thr_all = (h->thr >> 32) != 0 ? 1u : 0u;
+    cp.idle_ns = h->idle_ns;
+    h->cl_smem = smem;
+    const size_t spill_bytes = ((size_t)1 << cp.spill_log) * sizeof(uint32_t);
+    if (cudaMalloc(&h->cl_spill, spill_bytes) != cudaSuccess || cudaMalloc(&h->cl_spill_ctr, 2 * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaGetLastError();
+        free_cluster_state(h);
+        return WOLFF_OK;
+    }
+    CHECK_CUDA(h, cudaMemsetAsync(h->cl_spill, 0, spill_bytes, stream), "clear spill list");
+    CHECK_CUDA(h, cudaMemsetAsync(h->cl_spill_ctr, 0, 2 * sizeof(unsigned long long), stream), "clear spill counters");
+    cp.spill = h->cl_spill;
+    cp.spill_ctr = h->cl_spill_ctr;
+    h->cl_ok = true;
+    return WOLFF_OK;
+}
 
 // (Re)derive the tiling of growth_tiles.cu from the knobs and allocate its inboxes, spill lists and counters.
 // plan_ok == false (L not a power of two, L < 4, or the lattice does not fit the chip's shared memory) is not an
@@ -411,6 +472,7 @@ int wolff_destroy(wolff_handle h)
     cudaFree(h->M_log);
     cudaFree(h->ctl);
     free_tile_state(h);
+    free_cluster_state(h);
     delete h;
     return WOLFF_OK;
 }
@@ -458,8 +520,41 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
         rc = refresh_plan(h, stream);
         if (rc) return rc;
     }
+    // kernel choice in mode 0, by the mean cluster of the last finished run: below "small_cluster" spins the
+    // cluster-resident kernel (its update costs what its few passes cost: no cooperative grid, no messages, no poll over
+    // 148 CTAs), above it the shared-memory-resident kernel of all SMs; where the cluster-resident kernel does not apply
+    // (L not a power of two, in-kernel measurement) clusters of a handful of spins go to the level-synchronous kernel
     const bool small = h->small_cluster > 0 && h->have_mean && h->mean_cluster < (double)h->small_cluster;
-    bool tiled = h->mode == 0 && h->plan_ok && !small;
+    const bool tiny = small && h->mean_cluster < 16.0;
+    bool clustered = false;
+    if ((h->mode == 5 || (h->mode == 0 && small)) && !h->measure) {
+        rc = refresh_cluster_plan(h, stream);
+        if (rc) return rc;
+        clustered = h->cl_ok;
+    }
+    if (clustered) {
+        // the monitor publishes the update index relative to the launch in 31 bits
+        const uint64_t chunk = 1ull << 30;
+        for (uint64_t done = 0; done < n_updates && clustered; done += chunk) {
+            ClusterParams cp = h->cp;
+            cp.g = p;
+            cp.g.u0 = h->u + done;
+            cp.g.n_updates = n_updates - done < chunk ? n_updates - done : chunk;
+            cp.g.sizes = h->sizes + done;
+            cp.g.ns_log = h->ns_log + done;
+            const cudaError_t e = launch_growth_cluster(cp, h->dim, h->cl_smem, stream);
+            if (e == cudaErrorLaunchOutOfResources || e == cudaErrorInvalidConfiguration || e == cudaErrorCooperativeLaunchTooLarge) {
+                cudaGetLastError();       // the SMs of one GPC cannot be had right now: not a fault of the handle
+                if (done == 0) { clustered = false; break; }
+            }
+            CHECK_CUDA(h, e, "launch cluster-resident growth kernel");
+        }
+    }
+    if (h->mode == 5 && !clustered) {
+        rc = refresh_plan(h, stream);
+        if (rc) return rc;
+    }
+    bool tiled = !clustered && (h->mode == 0 || h->mode == 5) && h->plan_ok && !tiny;
     if (tiled) {
         // shared-memory-resident kernel; a message carries the update index relative to the launch in 29 bits
         const uint64_t chunk = (1ull << 29) - 1;
@@ -486,7 +581,7 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
             CHECK_CUDA(h, e, "launch tiled growth kernel");
         }
     }
-    if (!tiled) {
+    if (!tiled && !clustered) {
         if (h->measure) {
             // the level-synchronous kernel keeps running E and M: it starts from a whole-lattice evaluation (into the
             // control block) and marks the members of the running cluster in the spin bytes (claim_with_bits)
@@ -611,50 +706,50 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
     DeviceScope scope(h);
     const uint32_t up_max = cta_capacity(h);
     if (!strcmp(key, "mode")) {
-        if (value < 0 || value > 4) { set_error("mode must be 0, 1, 2, 3 or 4"); return WOLFF_EINVAL; }
+        if (value < 0 || value > 5) { set_error("mode must be 0, 1, 2, 3, 4 or 5"); return WOLFF_EINVAL; }
         h->mode = (int)value;
     } else if (!strcmp(key, "tile_log")) {
         if (value != 0 && (value < 2 || value > 12)) { set_error("tile_log must be 0 (auto) or in [2, 12]"); return WOLFF_EINVAL; }
         h->tile_log_opt = (int)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "tile_ctas")) {
         if (value < 0 || value > 1 << 16) { set_error("tile_ctas must be in [0, 65536]"); return WOLFF_EINVAL; }
         h->tile_ctas_opt = (int)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "watchdog_ms")) {
         if (value < 1 || value > 3600000) { set_error("watchdog_ms must be in [1, 3600000]"); return WOLFF_EINVAL; }
         h->watchdog_ms = (uint64_t)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "small_cluster")) {
         if (value < 0 || value > (int64_t)0x7FFFFFFF) { set_error("small_cluster must be in [0, 2^31)"); return WOLFF_EINVAL; }
         h->small_cluster = (uint64_t)value;
     } else if (!strcmp(key, "fill")) {
         if (value < 0 || value > 2) { set_error("fill must be 0 (never), 1 (adaptive) or 2 (always)"); return WOLFF_EINVAL; }
         h->fill_mode = (int)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "fill_bufs")) {
         if (value < 0 || value > 2) { set_error("fill_bufs must be 0 (auto), 1 or 2"); return WOLFF_EINVAL; }
         h->fill_bufs = (int)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "fill_min_us")) {
         if (value < 0 || value > 1000000) { set_error("fill_min_us must be in [0, 1000000]"); return WOLFF_EINVAL; }
         h->fill_min_us = (uint64_t)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "idle_ns")) {
         if (value < 0 || value > 1000000) { set_error("idle_ns must be in [0, 1000000]"); return WOLFF_EINVAL; }
         h->idle_ns = (uint32_t)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "ring_cap")) {
         if (value < 32 || value > 32768 || (value & (value - 1)) != 0) { set_error("ring_cap must be a power of two in [32, 32768]"); return WOLFF_EINVAL; }
         h->ring_cap = (uint32_t)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "measure")) {
         if (value != 0 && value != 1) { set_error("measure must be 0 or 1"); return WOLFF_EINVAL; }
         h->measure = (int)value;
     } else if (!strcmp(key, "inbox_log")) {
         if (value != 0 && (value < 5 || value > 24)) { set_error("inbox_log must be 0 (auto) or in [5, 24]"); return WOLFF_EINVAL; }
         h->inbox_log_opt = (int)value;
-        h->plan_dirty = true;
+        h->plan_dirty = h->cl_dirty = true;
     } else if (!strcmp(key, "up_threshold")) {
         if (value < 0 || value > (int64_t)up_max) { set_error("up_threshold must be in [0, %u]", up_max); return WOLFF_EINVAL; }
         h->up = (uint32_t)value;
@@ -686,6 +781,13 @@ int wolff_set_option(wolff_handle h, const char *key, int64_t value)
             h->shape_dirty = true;
             return WOLFF_EINVAL;
         }
+    } else if (!strcmp(key, "resident_ctas")) {
+        if (value != 1 && value != 2 && value != 4 && value != 8 && value != 16) {
+            set_error("resident_ctas must be 1, 2, 4, 8 or 16");
+            return WOLFF_EINVAL;
+        }
+        h->resident_ctas = (int)value;
+        h->cl_dirty = true;
     } else if (!strcmp(key, "speculative")) {
         if (value != 0 && value != 1) { set_error("speculative must be 0 or 1"); return WOLFF_EINVAL; }
         h->spec = (int)value;

@@ -112,6 +112,22 @@ struct TileParams {
     int8_t *faces;
 };
 
+// Cluster-resident bit-packed kernel (growth_cluster.cu).  The lattice (L a power of two, N >= 32 nC) is held as one bit
+// per spin in the distributed shared memory of ONE thread-block cluster of nC CTAs: word w (sites 32 w .. 32 w + 31)
+// lives in CTA w / wpc.  The spill list and its two counters run on across launches (nothing is reset).
+struct ClusterParams {
+    GrowthParams g;
+    uint32_t nC;                     // CTAs of the cluster (1, 2, 4, 8 or 16)
+    uint32_t wpc, wpc_log;           // 32-bit words of the bit lattice per CTA (a power of two)
+    uint32_t ring_cap;               // entries of a CTA's shared-memory ring (power of two)
+    uint32_t *spill;                 // 2^spill_log entries (>= N): overflow of the rings, shared by the cluster
+    uint32_t spill_log;
+    unsigned long long *spill_ctr;   // [0] entries ever pushed, [1] entries ever taken
+    unsigned long long watchdog_ns;  // an update longer than this aborts the launch
+    uint32_t thr32, thr_all;         // low word of the bond threshold; thr_all = 1 when thr = 2^32 (every bond active)
+    uint32_t idle_ns;                // longest sleep of an idle warp between two polls of its ring
+};
+
 // R independent chains in one launch, one CTA per chain at a time (growth_batch.cu).
 struct BatchParams {
     int8_t *spins;                   // R lattices, lattice_stride bytes apart
@@ -145,6 +161,7 @@ struct GrowthLaunch {
 
 constexpr int kGrowthThreads = 512;
 constexpr int kTileThreads = 384;
+constexpr int kClusterThreads = 512;
 
 // launchers (defined next to their kernels)
 cudaError_t launch_growth(const GrowthParams &p, int dim, const GrowthLaunch &l, cudaStream_t stream);
@@ -154,6 +171,10 @@ cudaError_t growth_max_clusters(int dim, bool pow2, const GrowthLaunch &l, int *
 size_t tiles_smem_bytes(int dim, uint32_t tile_log, uint32_t slots, uint32_t ring_cap, uint32_t nbuf);
 cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm);
 cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes, cudaStream_t stream);
+// cluster-resident kernel: shared memory needed, attributes + co-resident clusters, launch of one cluster of cp.nC CTAs
+size_t cluster_smem_bytes(uint32_t wpc, uint32_t ring_cap);
+cudaError_t cluster_prepare(int dim, uint32_t nC, size_t smem_bytes, int *max_clusters);
+cudaError_t launch_growth_cluster(const ClusterParams &cp, int dim, size_t smem_bytes, cudaStream_t stream);
 // batch of chains: CTAs of `threads` threads, `grid` of them; co-resident CTAs per SM; E, M of every chain into EM
 // bits: the bit-packed shared-memory-resident variant; its shared memory: the frontier buffers + N/8 bytes per plane
 size_t batch_smem_bytes(uint32_t N, uint32_t qcap, bool bits, bool measure);

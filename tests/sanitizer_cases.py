@@ -10,7 +10,8 @@
 line is the one that has been run.)  Each case runs a short chain through the C-ABI and checks it against the oracle,
 so a run that a tool slowed down by two orders of magnitude still proves that the kernels did their work.  Knobs make the small lattices exercise what the
 large ones do: tiny tiles on few CTAs (every hop a message), a 32-entry ring (spills), a 32-entry inbox
-(back-pressure), bond tables on and off, every tier of the level-synchronous kernel, in-kernel measurement, the batch.
+(back-pressure), bond tables on and off, every tier of the level-synchronous kernel, the cluster-resident kernel on 1 to 16 CTAs,
+in-kernel measurement, the batch.
 Summaries of the runs are kept under profiles/ (SURVEY.md section 4 tier 4, section 5 "Race detection").
 """
 import os
@@ -40,6 +41,14 @@ TIERS = [
     (2, 24, 2.0, {"mode": 4, "up_threshold": 8, "down_threshold": 3, "cluster_up_threshold": 40, "grid_down_threshold": 20, "measure": 1}),
     (3, 6, 4.2, {"mode": 2, "measure": 1}),
     (2, 16, 2.2, {"mode": 4, "speculative": 1}),
+]
+
+
+CLUSTER = [
+    (2, 16, wl.TC_2D, {"mode": 5}),
+    (3, 8, wl.TC_3D, {"mode": 5, "resident_ctas": 4, "ring_cap": 32, "idle_ns": 0}),
+    (2, 32, 2.0, {"mode": 5, "resident_ctas": 2, "ring_cap": 32}),
+    (3, 8, 4.0, {"mode": 0, "small_cluster": 1 << 30, "resident_ctas": 1}),
 ]
 
 
@@ -94,6 +103,10 @@ def main(which):
         for case in TIERS:
             single_chain(*case)
             done.append("tiers %s" % (case[3],))
+    if which in ("all", "cluster"):
+        for case in CLUSTER:
+            single_chain(*case)
+            done.append("cluster %s" % (case[3],))
     if which in ("all", "batch"):
         for measure, threads, resident in [(0, 32, 1), (1, 64, 1), (1, 256, 2), (0, 64, 2)]:
             batch(measure, threads, resident)

@@ -28,11 +28,15 @@ MODES = [{"mode": 0}, {"mode": 1}, {"mode": 2}, {"mode": 3},
          {"mode": 0, "small_cluster": 1000000},
          # an inbox of 32 entries: senders wait for the receiver all the time (back-pressure path)
          {"mode": 0, "tile_log": 2, "tile_ctas": 4, "inbox_log": 5, "fill": 2, "small_cluster": 0},
-         {"mode": 4, "speculative": 1, "up_threshold": 8, "down_threshold": 3, "cluster_up_threshold": 40, "grid_down_threshold": 20}]
+         {"mode": 4, "speculative": 1, "up_threshold": 8, "down_threshold": 3, "cluster_up_threshold": 40, "grid_down_threshold": 20},
+         # cluster-resident bit-packed kernel (mode 5; lattices it does not apply to fall through to mode 0): the largest
+         # cluster, two CTAs with a 32-entry ring (sites spill to global memory, peers steal), one CTA alone
+         {"mode": 5}, {"mode": 5, "resident_ctas": 2, "ring_cap": 32, "idle_ns": 0}, {"mode": 5, "resident_ctas": 1},
+         {"mode": 5, "resident_ctas": 4, "ring_cap": 64}]
 
 
 # ------------------------------------------------------------------ BASELINE config C1, exactly as written
-@pytest.mark.parametrize("options", MODES[:4])
+@pytest.mark.parametrize("options", MODES[:4] + [{"mode": 5}])
 def test_config_c1_every_update(options):
     c = wl.CONFIGS["C1"]
     gpu, ref = make_pair(*c.create_args(), options=options)
@@ -100,6 +104,25 @@ def test_randomised_knobs_shared_memory_resident_kernel(case_seed):
         opts = {"mode": 0, "small_cluster": 0, "tile_log": rng.choice([2, 3, 4, 5, 6]), "tile_ctas": rng.choice([0, 1, 2, 3, 7, 16, 64]),
                 "fill": rng.choice([0, 1, 2, 2]), "ring_cap": rng.choice([32, 64, 2048]), "idle_ns": rng.choice([0, 100, 1000]),
                 "fill_bufs": rng.choice([0, 1]), "fill_min_us": rng.choice([0, 30]), "inbox_log": rng.choice([0, 5, 6, 9])}
+        start = rng.choice([None, wl.cold(L ** dim), wl.blobs(dim, L, seed=rng.randrange(1000))])
+        gpu, ref = make_pair(dim, L, 1.0, T, seed=rng.randrange(1 << 40), start=start, options=opts)
+        compare_batched(gpu, ref, [rng.choice([1, 2, 5]), rng.choice([50, 300]), rng.choice([1, 500])])
+        gpu.close()
+
+
+@pytest.mark.parametrize("case_seed", range(2))
+def test_randomised_knobs_cluster_resident_kernel(case_seed):
+    # 25 short chains per seed on the cluster-resident bit-packed kernel: random lattice (down to 32 spins, one word),
+    # temperature, start, cluster size (1 .. 16 CTAs) and ring size (32 entries: sites spill to global memory and come
+    # back; peers steal), in mode 5 and through the kernel choice of mode 0
+    import random
+    rng = random.Random(3000 + case_seed)
+    for _ in range(25):
+        dim = rng.choice([2, 3])
+        L = rng.choice([8, 16, 32, 64, 128] if dim == 2 else [4, 8, 16, 32])
+        T = rng.choice([wl.TC_2D, 1.8, 3.0] if dim == 2 else [wl.TC_3D, 4.0, 5.0])
+        opts = {"mode": rng.choice([5, 5, 0]), "small_cluster": 1 << 30, "resident_ctas": rng.choice([1, 2, 4, 8, 16]),
+                "ring_cap": rng.choice([32, 64, 2048]), "idle_ns": rng.choice([0, 100, 1000])}
         start = rng.choice([None, wl.cold(L ** dim), wl.blobs(dim, L, seed=rng.randrange(1000))])
         gpu, ref = make_pair(dim, L, 1.0, T, seed=rng.randrange(1 << 40), start=start, options=opts)
         compare_batched(gpu, ref, [rng.choice([1, 2, 5]), rng.choice([50, 300]), rng.choice([1, 500])])
@@ -181,6 +204,16 @@ def test_two_live_handles_with_different_plans_interleaved():
     for g, r in ((big, ref_big), (small, ref_small), (tiny, ref_tiny)):
         assert_same_state(g, r)
         g.close()
+    # the same for the cluster-resident kernel: clusters of 16, 4 and 1 CTAs of one kernel function, interleaved
+    a, ref_a = make_pair(3, 32, 1.0, wl.TC_3D, seed=8, options={"mode": 5})
+    b, ref_b = make_pair(3, 16, 1.0, wl.TC_3D, seed=9, options={"mode": 5, "resident_ctas": 4})
+    c, ref_c = make_pair(3, 8, 1.0, wl.TC_3D, seed=10, options={"mode": 5, "resident_ctas": 1, "ring_cap": 32})
+    for _ in range(3):
+        for g, r, n in ((a, ref_a, 30), (b, ref_b, 50), (c, ref_c, 70)):
+            g.run(n); r.run(n)
+    for g, r in ((a, ref_a), (b, ref_b), (c, ref_c)):
+        assert_same_state(g, r)
+        g.close()
 
 
 def test_watchdog_abort_is_sticky_across_queued_runs():
@@ -243,7 +276,7 @@ def test_random_api_sequences(case_seed):
     import torch
     rng = random.Random(2000 + case_seed)
     streams = [None, torch.cuda.Stream(), torch.cuda.Stream()]
-    knobs = {"mode": [0, 0, 4, 1, 3], "small_cluster": [0, 16, 100000], "tile_log": [0, 2, 3, 4, 5], "tile_ctas": [0, 1, 3, 16],
+    knobs = {"mode": [0, 0, 4, 1, 3, 5], "small_cluster": [0, 16, 100000], "resident_ctas": [1, 2, 4, 16], "tile_log": [0, 2, 3, 4, 5], "tile_ctas": [0, 1, 3, 16],
              "fill": [0, 1, 2], "fill_bufs": [0, 1], "ring_cap": [32, 2048], "idle_ns": [0, 1000], "fill_min_us": [0, 30],
              "inbox_log": [0, 5, 7]}
     for _ in range(40):
