@@ -12,6 +12,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB_NAME = "libwolff_b200.so"
 LIB_PATH = os.path.join(HERE, LIB_NAME)
 CHECKED_LIB_PATH = os.path.join(HERE, "libwolff_b200_checked.so")
+JITTER_LIB_PATH = os.path.join(HERE, "libwolff_b200_jitter.so")
 SOURCES = ["api.cu", "batch_api.cu", "growth.cu", "growth_batch.cu", "growth_cluster.cu", "growth_tiles.cu", "measure.cu", "microbench.cu"]
 HEADERS = ["internal.h", "device_common.cuh", "expand.cuh", os.path.join(ROOT, "include", "wolff.h")]
 NVCC_COMPILE_FLAGS = [
@@ -41,20 +42,24 @@ def needs_build(lib_path: str = LIB_PATH) -> bool:
     return os.path.getmtime(lib_path) < max(os.path.getmtime(d) for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, checked: bool = False, jitter: bool = False) -> str:
     """One nvcc per source file, side by side (the files share no device code, so there is no device link), then one
     link.  Objects are kept under paper_1110_0899_b200/build/ (git-ignored) and reused while they are newer than
     their source and every header.
 
     checked=True builds libwolff_b200_checked.so with -DWOLFF_CHECKED (every queue, list, tile and bit-plane index is
-    compared with its bound before use: device_common.cuh); load it with WOLFF_B200_LIB=<path> (binding.py)."""
-    lib_path = CHECKED_LIB_PATH if checked else LIB_PATH
+    compared with its bound before use: device_common.cuh); load it with WOLFF_B200_LIB=<path> (binding.py).
+    jitter=True builds libwolff_b200_jitter.so with -DWOLFF_CHECKED -DWOLFF_JITTER (random sleeps between the steps of the
+    lock-free protocols, device_common.cuh)."""
+    lib_path = JITTER_LIB_PATH if jitter else (CHECKED_LIB_PATH if checked else LIB_PATH)
     if not force and not needs_build(lib_path):
         return lib_path
     nvcc = nvcc_path()
     extra = os.environ.get("WOLFF_NVCC_EXTRA", "").split()      # e.g. -DWOLFF_PROFILE (per-section cycle counters)
-    if checked:
+    if checked or jitter:
         extra.append("-DWOLFF_CHECKED")
+    if jitter:
+        extra.append("-DWOLFF_JITTER")
     os.makedirs(OBJ_DIR, exist_ok=True)
     tag = ("_" + "".join(c if c.isalnum() else "_" for c in " ".join(extra))) if extra else ""
     newest_header = max(os.path.getmtime(h) for h in _header_paths())
@@ -90,4 +95,4 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False) -> 
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv, jitter="--jitter" in sys.argv))

@@ -25,6 +25,28 @@ __device__ __forceinline__ bool wolff_check_failed(void *errword, unsigned int c
 #define WOLFF_CHECK(errword, cond, code) (true)
 #endif
 
+// ---------------------------------------------------------------- schedule-perturbing builds
+// -DWOLFF_JITTER: the lock-free protocols of the growth kernels (ring reserve / put / take, inbox slot / message,
+// pending counts and publishing, work stealing, termination) are correct for every interleaving of their steps, not
+// only for the ones the hardware usually produces.  This build makes unusual interleavings common: at every marked
+// point between two steps of a protocol a thread sleeps, one time in four, for a pseudo-random 0-2 microseconds
+// (thousands of cycles: longer than any of the protocol's round trips).  With compute-sanitizer's racecheck closed on
+// the development pool, running the parity cases on this build is the race test that can be run there
+// (tests/test_gpu_checked.py, profiles/r2_checked_build.md); the release build contains none of it.
+#ifdef WOLFF_JITTER
+__device__ __forceinline__ void wolff_jitter(unsigned int id)
+{
+    unsigned int t;
+    asm volatile("mov.u32 %0, %%clock;" : "=r"(t));
+    unsigned int h = t ^ (id * 0x9E3779B9u) ^ (threadIdx.x * 0x85EBCA6Bu) ^ (blockIdx.x * 0xC2B2AE35u);
+    h ^= h >> 15; h *= 0x2C1B3C6Du; h ^= h >> 12;
+    if ((h & 3u) == 0u) __nanosleep(h >> 21);
+}
+#define WOLFF_JITTER_POINT(id) wolff::wolff_jitter((unsigned int)(id))
+#else
+#define WOLFF_JITTER_POINT(id) ((void)0)
+#endif
+
 // ---------------------------------------------------------------- Philox4x32-10 (reading R11)
 // Salmon et al., SC'11.  One round maps (c0,c1,c2,c3) to
 // (hi(M1*c2)^c1^k0, lo(M1*c2), hi(M0*c0)^c3^k1, lo(M0*c0)); the key is bumped by the Weyl

@@ -166,6 +166,7 @@ __device__ __forceinline__ void hand_over(const ClusterParams &cp, uint32_t head
     }
     ok = __shfl_sync(kFullMask, ok, 0);
     base = __shfl_sync(kFullMask, base, 0);
+    WOLFF_JITTER_POINT(1);           // reserved, not yet filled
     if (ok) {
         // the entry of the lap before has been acquired (head moved past it) but may not have been taken yet
         for (unsigned int j = lane; j < n; j += 32u) {
@@ -178,6 +179,7 @@ __device__ __forceinline__ void hand_over(const ClusterParams &cp, uint32_t head
         if (lane == 0) sbase = atomicAdd(cp.spill_ctr, (unsigned long long)n);
         sbase = __shfl_sync(kFullMask, sbase, 0);
         const uint32_t smask = (1u << cp.spill_log) - 1u;
+        WOLFF_JITTER_POINT(2);
         for (unsigned int j = lane; j < n; j += 32u) {
             const unsigned long long pos = sbase + (unsigned long long)j;
             st_relaxed_u32_g(cp.spill + ((uint32_t)pos & smask), (items[j] << 1) | spill_tag(pos, cp.spill_log));
@@ -255,7 +257,7 @@ __device__ __forceinline__ void run_passes(const ClusterParams &cp, uint32_t bit
         uint32_t *const st_out = stage + sbuf;
         const uint32_t out_s = stage_s + sbuf * 4u;
         sbuf ^= 32u;
-        if (won) sts_u32(out_s + __popc(wb & lt) * 4u, n);
+        if (won && WOLFF_CHECK(&p.ctl->error, n < p.geo.N && (wi >> cp.wpc_log) < cp.nC && __popc(wb & lt) < 32, 32)) sts_u32(out_s + __popc(wb & lt) * 4u, n);
         __syncwarp();
         nsites = total < S ? total : S;
         if (q < S && q < nsites) a = lds_u32(out_s + q * 4u);
@@ -275,6 +277,7 @@ __device__ __forceinline__ void run_passes(const ClusterParams &cp, uint32_t bit
             }
             // counted (the atomic has returned: the addition has been performed) before another warp can see them
             if (lane == 0) (void)cl_atom_add64(pc_c, (unsigned long long)(total - S));
+            WOLFF_JITTER_POINT(3);
             __syncwarp();
             hand_over(cp, head_c, ring_c, st_out + S, total - S, tl);
 #ifdef WOLFF_PROFILE
@@ -288,6 +291,7 @@ __device__ __forceinline__ void run_passes(const ClusterParams &cp, uint32_t bit
     }
     // ---- dry: one reduction hands back the warp's units and adds the spins it claimed
     const unsigned int wsum = __reduce_add_sync(kFullMask, mywon);
+    WOLFF_JITTER_POINT(4);           // claims made, units not yet handed back
     if (!MONITOR && lane == 0) cl_red_add64(pc_c, ((unsigned long long)wsum << 32) - (unsigned long long)ws.units);
     ws.nsites = 0u; ws.mywon = MONITOR ? wsum : 0u; ws.sbuf = sbuf; ws.a = a;
 }
@@ -349,6 +353,7 @@ __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh
                 sp_pos = shd;
                 backlog = st - shd > 0xFFFFFFFFull ? 0xFFFFFFFFu : (unsigned int)(st - shd);
             }
+            WOLFF_JITTER_POINT(6);   // the peers' rings as they were a while ago
             const unsigned int cand = __ballot_sync(kFullMask, backlog != 0u);
             if (cand == 0u) continue;
             // the first candidate after the own rank, cyclically: thieves spread over the victims
@@ -374,6 +379,7 @@ __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh
             h = __shfl_sync(kFullMask, h, 0);
         }
         idle = 0;
+        WOLFF_JITTER_POINT(5);       // entries acquired (head moved), not yet taken out of their slots
 #ifdef WOLFF_PROFILE
         const long long tt0 = clock64();
 #endif
@@ -403,8 +409,9 @@ __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh
         ws.a = __shfl_sync(kFullMask, ent, q & 31u);
         ws.nsites = n;
         ws.units = n;
-        // the update these sites belong to: written into every CTA (and read back) by the monitor before its seed site
-        // entered a ring
+        WOLFF_JITTER_POINT(8);
+        // the update these sites belong to: written into every CTA (and read back) by the monitor before the first site
+        // of the update left its hands
         const unsigned int upd = *reinterpret_cast<volatile unsigned int *>(&sh.upd);
         const unsigned long long u = p.u0 + (unsigned long long)(upd >> 1);
 #ifdef WOLFF_PROFILE
@@ -450,6 +457,7 @@ __device__ __forceinline__ void monitor_warp(const ClusterParams &cp, CShared &s
         }
         s0neg = __shfl_sync(kFullMask, s0neg, 0);
         i0 = __shfl_sync(kFullMask, i0, 0);
+        WOLFF_JITTER_POINT(7);
         ws.a = lane < ND ? i0 : 0u;          // the lanes of site 0
         ws.nsites = 1u;
         ws.units = 0u;

@@ -309,6 +309,7 @@ __device__ __forceinline__ void hand_over(const TileParams &tp, TShared &sh, uin
     if (lane == 0) ok = ring_reserve(sh, tp.ring_cap, n, base) ? 1u : 0u;
     ok = __shfl_sync(kFullMask, ok, 0);
     base = __shfl_sync(kFullMask, base, 0);
+    WOLFF_JITTER_POINT(11);          // reserved, not yet filled
     if (ok) {
         for (unsigned int j = lane; j < n; j += 32u) ring_put(ring + ((base + j) & rmask), items[j]);
         if (lane == 0) tl.ring_pushes += n;
@@ -336,6 +337,7 @@ __device__ __noinline__ void publish(const TileParams &tp, TShared &sh, unsigned
     while (atomicCAS(&sh.pub_lock, 0u, 1u) != 0u) { }
     const unsigned long long I = ld_vol64(&sh.ihead);
     __threadfence_block();
+    WOLFF_JITTER_POINT(12);          // between the look at ihead and the look at pending
     if (ld_vol(&sh.pending) == 0u) {
         const unsigned int a = atomicExch(&sh.claimed, 0u);
         if (a) atomicAdd(tp.added, (unsigned long long)a);
@@ -705,6 +707,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
     unsigned int budget = 32u;
 
     auto send = [&](unsigned int j) {
+        WOLFF_JITTER_POINT(13);      // slot counted in gtail, message not yet stored
         if (BP && msg_pos[j] - msg_seen[j] >= tp.in_cap) wait_inbox(tp, msg_own[j], msg_pos[j]);
         st_relaxed_u64(tp.inbox + ((size_t)msg_own[j] << tp.in_log) + (msg_pos[j] & in_mask),
                        pack_msg(kKindClaim, (msg_pos[j] >> tp.in_log) & 1u, krel, msg_na[j], POS ? 1 : -1));
@@ -881,6 +884,7 @@ __device__ __forceinline__ void run_passes(const TileParams &tp, TShared &sh, co
 #pragma unroll
     for (unsigned int j = 0; j < W; ++j) if (msg_valid[j]) send(j);
     const unsigned int wsum = __reduce_add_sync(kFullMask, mywon);
+    WOLFF_JITTER_POINT(14);          // messages sent, units not yet handed back
     if (lane == 0) {
         if (wsum) red_shared_add(claimed_s, wsum);
         __threadfence_block();
@@ -954,6 +958,7 @@ __device__ __forceinline__ void worker_warp(const TileParams &tp, TShared &sh, c
             continue;
         }
         idle = 0;
+        WOLFF_JITTER_POINT(15);      // entries acquired (head moved), not yet taken out of their slots
         if (watcher) { watcher = false; if (lane == 0) st_vol(&sh.watcher, 0u); }
         h = __shfl_sync(kFullMask, h, 0);
         from_spill = __shfl_sync(kFullMask, from_spill, 0);
@@ -1077,10 +1082,12 @@ __device__ __forceinline__ void receiver_warp(const TileParams &tp, TShared &sh,
             atomicAdd(&sh.pending, w + 1u);            // the winners, and a token that keeps the CTA busy until they are queued
             if (w) atomicAdd(&sh.claimed, w);
             __threadfence_block();
+            WOLFF_JITTER_POINT(16);                    // pending raised, ihead not yet moved
             st_vol64(&sh.ihead, ih);                   // after pending: see publish()
             __threadfence_block();
         }
         if (win) stage[__popc(wb & lt)] = addr;
+        WOLFF_JITTER_POINT(17);
         __syncwarp();
         if (w) hand_over(tp, sh, ly.ring, stage, w, c, tl);
         __syncwarp();
@@ -1141,6 +1148,7 @@ __device__ __forceinline__ void monitor_warp(const TileParams &tp, Tally &tl)
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) d += __shfl_xor_sync(kFullMask, d, o);
             fence_acq_rel_gpu();      // every gtail (and `added`) is read after every gdone
+            WOLFF_JITTER_POINT(18);
             for (unsigned int cc = lane; cc < G; cc += 32u) t += ld_relaxed_u32(tp.gtail + cc);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(kFullMask, t, o);

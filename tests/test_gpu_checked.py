@@ -24,6 +24,21 @@ def test_checked_build_runs_clean_on_the_stress_cases():
 
 
 @pytest.mark.gpu
+def test_schedule_perturbing_build_runs_clean_on_the_stress_cases():
+    # -DWOLFF_JITTER: random sleeps of up to 2 us between the steps of every lock-free protocol of the growth kernels
+    # (ring reserve / put / take, inbox slot / message, pending counts, publishing, stealing, termination), so that
+    # interleavings the hardware rarely produces become common; every case is compared with the oracle, three rounds
+    from paper_1110_0899_b200 import build
+    lib = build.build(jitter=True)
+    env = dict(os.environ, WOLFF_B200_LIB=lib)
+    for which in ("tiles", "cluster", "tiles", "cluster", "tiles", "cluster"):
+        out = subprocess.run([sys.executable, os.path.join(ROOT, "tests", "sanitizer_cases.py"), which], env=env, capture_output=True, text=True,
+                             timeout=900)
+        assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-4000:]
+        assert "sanitizer cases passed" in out.stdout
+
+
+@pytest.mark.gpu
 def test_checked_build_reports_a_violation():
     # the check itself must be alive: the checked build honours a test hook that feeds it an index past its bound
     from paper_1110_0899_b200 import build
