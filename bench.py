@@ -54,10 +54,19 @@ def measured_peak_hbm():
 # (workload, growth mode): taken offline from the committed captures under profiles/ (the launch shape of each capture
 # is stated there).  Any other workload / mode / knob setting prints null -- never a figure from another configuration.
 NCU_TRAFFIC = {
-    ("C3", 0): {"bytes": 22624256 + 493056, "source": "profiles/r1_growth_tiles_C3.md (10-update launch; the traffic is the one lattice "
-                                                       "load per launch and does not grow with the updates)"},
-    ("C5a", 0): {"bytes": 66096640 + 15944960, "source": "profiles/r1_growth_tiles_C5a.md (200-update launch)"},
+    ("C3", 0): {"bytes": 26623488 + 1387264, "source": "profiles/r2_growth_tiles_C3.md (50-update launch; the traffic is the one lattice "
+                                                        "load per launch plus the queues, and does not grow with the updates)"},
+    ("C5a", 0): {"bytes": 54497536 + 8451584, "source": "profiles/r2_growth_tiles_C5a.md (200-update launch)"},
 }
+
+
+def kernel_of(stats: dict) -> str:
+    """Which growth kernel the most recent run used, from its counters (wolff_get_stats)."""
+    if stats["levels_cta"] + stats["levels_cluster"] + stats["levels_grid"] > 0:
+        return "growth_kernel (level-synchronous tiers)"
+    if stats["fill_chunks"] + stats["inline_passes"] > 0:
+        return "growth_tiles_kernel (int8 tiles in the shared memory of all SMs)"
+    return "growth_cluster_kernel (bit-packed lattice in one cluster's distributed shared memory)"
 
 
 def ncu_traffic(workload: str, mode: int, options: dict):
@@ -290,6 +299,7 @@ def run_b200(args, rank: int, world: int):
                 res["step_ms"].append(e0.elapsed_time(e2))
                 res["growth_ms"].append(e0.elapsed_time(e1))
                 st = h.stats()
+                res["kernel"] = kernel_of(st)
                 res["flipped"] += st["flipped"]; res["attempts"] += st["claim_attempts"]
                 assert int(sizes_d.sum().item()) == st["flipped"]
                 h.series_into(None, None, ns_d)
@@ -326,7 +336,7 @@ def run_b200(args, rank: int, world: int):
 
     def leg_summary(r, oracle_budget: float, oracle_max: int = 10 ** 9):
         ms = sum(r["step_ms"])
-        out = {"value": r["flipped"] / (ms * 1e-3), "unit": UNIT, "updates_per_s": r["updates"] / (ms * 1e-3),
+        out = {"value": r["flipped"] / (ms * 1e-3), "unit": UNIT, "updates_per_s": r["updates"] / (ms * 1e-3), "kernel": r.get("kernel"),
                "updates_timed": r["updates"], "mean_cluster": r["flipped"] / max(r["updates"], 1),
                "ms_per_update_mean": ms / max(r["updates"], 1), "ms_per_update_median": r["ms_per_update_median_in_kernel"],
                "ms_per_update_note": "mean = device time of the steps / updates; median = the kernel's own per-update durations (wolff_get_series)"}
@@ -570,6 +580,13 @@ def run_b200(args, rank: int, world: int):
             lit[wl.CONFIGS[name].name] = leg_summary(r, osec, oracle_max=r["updates"])
             r["h"].close()
         out["literal_random_start"] = lit
+        # the other BASELINE configs ("reported for all five configs"), equilibrated variant
+        others = {}
+        for name, upd in (("C1", 1000), ("C2", 1000), ("C4", 1000)):
+            r = measure(name, upd, args.equil, max(2, args.steps // 2), 1, cold=name != "C1", depth_steps=0)
+            others[wl.CONFIGS[name].name] = leg_summary(r, osec, oracle_max=r["updates"])
+            r["h"].close()
+        out["other_configs_equilibrated"] = others
         # C5b (T = 5.0, disordered phase) from a cold start: equilibrium clusters of a few tens of spins
         r = measure("C5b", 10000, 1000, max(1, args.steps // 2), 1, cold=True, depth_steps=0)
         out["c5b_equilibrated"] = dict(workload=wl.CONFIGS["C5b"].name + ", cold start + 1000 untimed updates", **leg_summary(r, osec, oracle_max=r["updates"]))

@@ -202,8 +202,12 @@ WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
  *       ld.shared (spin, bond bit) -> atom.shared (claim) -> ballot/popc -> st.shared -> __syncwarp -> ld.shared;
  *       this is the floor of t_pass in the latency roofline T_update >= depth x t_pass
  *   [8] fraction of lanes that won their claim in [7] (1.0 when the chain ran as intended; not a time)
+ * between two CTAs of one thread-block cluster (the links of the cluster-resident kernel):
+ *   [9] dependent ld.shared::cluster on the peer's shared memory, one lane    [10] dependent atom.shared::cluster.or with
+ *   return on the peer, one lane    [11] ... one warp, 32 scattered words    [12] a word stored into the peer's shared
+ *   memory until a warp polling there sees it, one way
  * Not part of the measured path. */
-#define WOLFF_NMICRO 9
+#define WOLFF_NMICRO 13
 WOLFF_API int wolff_microbench(double *out_ns, int n_out);
 
 /* Free everything.  NULL is allowed. */

@@ -108,7 +108,8 @@ def _stream_handle(stream):
 
 
 MICRO_NAMES = ("l2_load_lane_ns", "l2_load_warp_ns", "l2_atomic_lane_ns", "l2_atomic_warp_ns", "syncthreads_ns",
-               "philox_x3_ns", "grid_barrier_ns", "smem_pass_floor_ns", "smem_pass_win_fraction")
+               "philox_x3_ns", "grid_barrier_ns", "smem_pass_floor_ns", "smem_pass_win_fraction",
+               "dsmem_load_lane_ns", "dsmem_atomic_lane_ns", "dsmem_atomic_warp_ns", "dsmem_store_to_poll_ns")
 
 
 def microbench() -> dict:

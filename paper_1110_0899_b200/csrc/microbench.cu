@@ -162,6 +162,92 @@ __global__ void __launch_bounds__(32, 1) smem_pass_kernel(int iters, double *out
     if (lane == 0) { out[7] = (double)(t1 - t0) / iters; out[8] = (double)won_total / (32.0 * iters); }
 }
 
+// out[9..12]: the links of the cluster-resident kernel (growth_cluster.cu) between two CTAs of one thread-block
+// cluster: out[9] = ns per dependent ld.shared::cluster on the PEER's shared memory (one lane), out[10] = ns per dependent
+// atom.shared::cluster.or with return on the peer (one lane), out[11] = the same with 32 lanes on 32 scattered words,
+// out[12] = ns one way for a word stored into the peer's shared memory to be seen by a warp polling there (half of a
+// ping-pong round trip).
+__device__ __forceinline__ uint32_t mb_smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t mb_mapa(uint32_t a, uint32_t r)
+{
+    uint32_t o;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(o) : "r"(a), "r"(r));
+    return o;
+}
+__device__ __forceinline__ uint32_t mb_cl_ld(uint32_t a)
+{
+    uint32_t v;
+    asm volatile("ld.volatile.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory");
+    return v;
+}
+__device__ __forceinline__ void mb_cl_st(uint32_t a, uint32_t v) { asm volatile("st.volatile.shared::cluster.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ uint32_t mb_cl_or(uint32_t a, uint32_t v)
+{
+    uint32_t o;
+    asm volatile("atom.shared::cluster.or.b32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory");
+    return o;
+}
+__device__ __forceinline__ void mb_cluster_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t mb_cluster_rank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(32, 1) dsmem_kernel(int iters, double *out)
+{
+    extern __shared__ __align__(16) unsigned int dyn[];
+    constexpr unsigned int kWords = 8192;             // 32 KiB of the peer's shared memory
+    __shared__ unsigned int flag;
+    const unsigned int lane = threadIdx.x, rank = mb_cluster_rank();
+    for (unsigned int i = lane; i < kWords; i += 32u) dyn[i] = 0u;
+    if (lane == 0) flag = 0u;
+    mb_cluster_sync();
+    const uint32_t mask = kWords - 1u;
+    if (rank == 0u) {
+        const uint32_t peer = mb_mapa(mb_smem_addr(dyn), 1u);
+        if (lane == 0) {
+            uint32_t idx = 12345u & mask;
+            unsigned long long t0 = globaltimer_ns();
+            for (int k = 0; k < iters; ++k) { const uint32_t v = mb_cl_ld(peer + idx * 4u); idx = (idx * 1664525u + 1013904223u + v) & mask; }
+            unsigned long long t1 = globaltimer_ns();
+            out[9] = (double)(t1 - t0) / iters;
+            t0 = globaltimer_ns();
+            for (int k = 0; k < iters; ++k) { const uint32_t v = mb_cl_or(peer + idx * 4u, 0u); idx = (idx * 1664525u + 1013904223u + v) & mask; }
+            t1 = globaltimer_ns();
+            out[10] = (double)(t1 - t0) / iters + (idx == 0xFFFFFFFFu ? 1.0 : 0.0);
+        }
+        __syncwarp();
+        uint32_t idx = (lane * 2654435761u) & mask;
+        const unsigned long long t0 = globaltimer_ns();
+        for (int k = 0; k < iters; ++k) { const uint32_t v = mb_cl_or(peer + idx * 4u, 0u); idx = (idx * 1664525u + 1013904223u + v + lane) & mask; }
+        const unsigned long long t1 = globaltimer_ns();
+        if (lane == 0) out[11] = (double)(t1 - t0) / iters + (idx == 0xFFFFFFFFu ? 1.0 : 0.0);
+    }
+    mb_cluster_sync();
+    if (lane == 0) {
+        const uint32_t mine = mb_smem_addr(&flag), theirs = mb_mapa(mine, rank ^ 1u);
+        if (rank == 0u) {
+            const unsigned long long t0 = globaltimer_ns();
+            for (int k = 1; k <= iters; ++k) {
+                mb_cl_st(theirs, (uint32_t)k);
+                while (mb_cl_ld(mine) != (uint32_t)k) { }
+            }
+            out[12] = (double)(globaltimer_ns() - t0) / (2.0 * iters);
+        } else {
+            for (int k = 1; k <= iters; ++k) {
+                while (mb_cl_ld(mine) != (uint32_t)k) { }
+                mb_cl_st(theirs, (uint32_t)k);
+            }
+        }
+    }
+    mb_cluster_sync();
+}
+
 }  // namespace
 }  // namespace wolff
 
@@ -195,6 +281,10 @@ extern "C" WOLFF_API int wolff_microbench(double *out_host, int n_out)
         const size_t smem = (64u << 10) + (64u << 10) / 8u + 32u * sizeof(unsigned int);
         e = cudaFuncSetAttribute(smem_pass_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) smem_pass_kernel<<<1, 32, smem>>>(4 * 496, out);
+    }
+    if (e == cudaSuccess) {
+        dsmem_kernel<<<2, 32, 8192 * sizeof(unsigned int)>>>(iters, out);
+        e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e == cudaSuccess) e = cudaMemcpy(out_host, out, sizeof(double) * WOLFF_NMICRO, cudaMemcpyDeviceToHost);

@@ -248,6 +248,9 @@ def test_microbench_pass_floor_runs_as_intended():
     assert m["smem_pass_win_fraction"] == 1.0
     assert 20.0 < m["smem_pass_floor_ns"] < 2000.0
     assert m["l2_load_lane_ns"] > m["smem_pass_floor_ns"] / 10.0
+    # the links of the cluster-resident kernel: a claim on a peer's shared memory is cheaper than one through L2
+    assert 20.0 < m["dsmem_atomic_lane_ns"] < m["l2_atomic_lane_ns"]
+    assert 20.0 < m["dsmem_load_lane_ns"] < 1000.0 and 20.0 < m["dsmem_store_to_poll_ns"] < 2000.0
 
 
 @pytest.mark.parametrize("name", ["C1", "C2", "C4"])
