@@ -530,7 +530,7 @@ def run_b200(args, rank: int, world: int):
         "ms_per_update_mean": summary["ms_per_update_mean"], "ms_per_update_median": summary["ms_per_update_median"],
         "clocks": primary["clocks"],
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": e["h2d"], "d2h_bytes_per_step": e["d2h"]},
-        "roofline": {"bound": "hbm", "kernel": ("growth_tiles_kernel" if args.mode == 0 else "growth_kernel") + " (persistent, one launch per step)",
+        "roofline": {"bound": "hbm", "kernel": primary.get("kernel", "?") + " (persistent, one launch per step)",
                      "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic["bytes"] if traffic else None,
                      "traffic_source": traffic["source"] if traffic else "no committed ncu capture for this workload / mode / options",
