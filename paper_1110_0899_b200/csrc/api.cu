@@ -100,6 +100,7 @@ struct wolff_ctx {
     unsigned long long *cl_spill_ctr = nullptr;
     // kernel choice in mode 0: mean cluster size of the last finished run (read when the caller next synchronises)
     uint64_t small_cluster = 32768; // below this mean size mode 0 leaves the kernel of all SMs for the cluster-resident one; 0 = never
+                                    // (set by wolff_create: 8192 in 2D, 32768 in 3D)
     bool have_mean = false;
     bool run_since_set = false;     // a run has been queued since the lattice was last loaded: its counters describe this lattice
     double mean_cluster = 0.0;
@@ -412,6 +413,7 @@ wolff_handle wolff_create(int dim, int L, double J, double T, uint64_t seed)
     if (!h) { set_error("out of host memory"); return nullptr; }
     h->dim = dim; h->L = L; h->J = J; h->T = T; h->seed = seed; h->N = N;
     h->thr = bond_threshold(J, T);
+    h->small_cluster = dim == 2 ? 8192 : 32768;     // measured crossover of the two barrier-free kernels
     h->geo.L = (uint32_t)L;
     h->geo.N = (uint32_t)N;
     h->geo.LL = (uint32_t)((uint64_t)L * (uint64_t)L);
