@@ -126,10 +126,11 @@ struct Geometry {
     uint32_t pow2;   // 1 when L is a power of two
 };
 
+// Coordinates of site i (reading R5).
 template <int DIM, bool POW2>
-__device__ __forceinline__ void neighbours(const Geometry &g, uint32_t i, uint32_t (&nbr)[2 * DIM])
+__device__ __forceinline__ void site_coords(const Geometry &g, uint32_t i, uint32_t &x, uint32_t &y, uint32_t &z)
 {
-    uint32_t x, y, z = 0;
+    z = 0;
     if (POW2) {
         const uint32_t mask = g.L - 1u;
         x = i & mask;
@@ -141,6 +142,13 @@ __device__ __forceinline__ void neighbours(const Geometry &g, uint32_t i, uint32
         y = t % g.L;
         if (DIM == 3) z = t / g.L;
     }
+}
+
+// nbr[2d] = +d neighbour, nbr[2d+1] = -d neighbour of site i at (x, y, z), periodic.
+template <int DIM>
+__device__ __forceinline__ void neighbours_at(const Geometry &g, uint32_t i, uint32_t x, uint32_t y, uint32_t z,
+                                              uint32_t (&nbr)[2 * DIM])
+{
     const uint32_t Lm1 = g.L - 1u;
     nbr[0] = (x == Lm1) ? i - Lm1 : i + 1u;
     nbr[1] = (x == 0u) ? i + Lm1 : i - 1u;
@@ -152,6 +160,14 @@ __device__ __forceinline__ void neighbours(const Geometry &g, uint32_t i, uint32
         nbr[4] = (z == Lm1) ? i - zwrap : i + g.LL;
         nbr[5] = (z == 0u) ? i + zwrap : i - g.LL;
     }
+}
+
+template <int DIM, bool POW2>
+__device__ __forceinline__ void neighbours(const Geometry &g, uint32_t i, uint32_t (&nbr)[2 * DIM])
+{
+    uint32_t x, y, z;
+    site_coords<DIM, POW2>(g, i, x, y, z);
+    neighbours_at<DIM>(g, i, x, y, z, nbr);
 }
 
 // ---------------------------------------------------------------- spins

@@ -12,42 +12,6 @@ namespace wolff {
 
 constexpr unsigned int kFullMask = 0xFFFFFFFFu;
 
-// Coordinates of site i (reading R5).
-template <int DIM, bool POW2>
-__device__ __forceinline__ void site_coords(const Geometry &g, uint32_t i, uint32_t &x, uint32_t &y, uint32_t &z)
-{
-    z = 0;
-    if (POW2) {
-        const uint32_t mask = g.L - 1u;
-        x = i & mask;
-        y = (i >> g.logL) & mask;
-        if (DIM == 3) z = i >> (2u * g.logL);
-    } else {
-        x = i % g.L;
-        const uint32_t t = i / g.L;
-        y = t % g.L;
-        if (DIM == 3) z = t / g.L;
-    }
-}
-
-// nbr[2d] = +d neighbour, nbr[2d+1] = -d neighbour of site i at (x, y, z), periodic.
-template <int DIM>
-__device__ __forceinline__ void neighbours_at(const Geometry &g, uint32_t i, uint32_t x, uint32_t y, uint32_t z,
-                                              uint32_t (&nbr)[2 * DIM])
-{
-    const uint32_t Lm1 = g.L - 1u;
-    nbr[0] = (x == Lm1) ? i - Lm1 : i + 1u;
-    nbr[1] = (x == 0u) ? i + Lm1 : i - 1u;
-    const uint32_t ywrap = g.LL - g.L;                 // L*(L-1)
-    nbr[2] = (y == Lm1) ? i - ywrap : i + g.L;
-    nbr[3] = (y == 0u) ? i + ywrap : i - g.L;
-    if (DIM == 3) {
-        const uint32_t zwrap = g.N - g.LL;             // L*L*(L-1)
-        nbr[4] = (z == Lm1) ? i - zwrap : i + g.LL;
-        nbr[5] = (z == 0u) ? i + zwrap : i - g.LL;
-    }
-}
-
 // A2-A4 for one site per lane.  On return nbr[] holds the 2*DIM neighbour ids, bit k of `won` is set
 // when THIS lane flipped nbr[k] from s0 to -s0 (so nbr[k] is a new member of the cluster), and
 // (x, y, z) are the site's coordinates.  Lanes with valid == false do nothing and return won = 0.
