@@ -42,8 +42,8 @@ struct alignas(128) Control {
     unsigned int invalid;                      // set_spins validation
     unsigned int ticket;                       // E/M reduction: CTAs done
     unsigned int pad0;
-    unsigned long long acc_unequal;            // E/M reduction scratch
-    unsigned long long acc_negative;
+    unsigned long long acc_unequal;            // E/M reduction scratch: #unequal bonds | #negative spins << 33
+    unsigned long long acc_negative;           // (unused)
     long long E;                               // result of the last reduction; with in-kernel measurement: the
     long long M;                               // running values after the last measured update
     unsigned long long moments[10];            // in-kernel measurement: accumulated sums (layout: wolff_get_moments)

@@ -92,16 +92,18 @@ __device__ __forceinline__ void block_accumulate(unsigned long long unequal, uns
     if (threadIdx.x == 0) {
         unsigned long long un = 0, ng = 0;
         for (int w = 0; w < kThreads / 32; ++w) { un += s_un[w]; ng += s_ng[w]; }
-        if (un) atomicAdd(&ctl->acc_unequal, un);
-        if (ng) atomicAdd(&ctl->acc_negative, ng);
+        // one atomic per CTA on one word: #unequal (at most dim * N < 2^33) in the low 33 bits, #negative (at most N <= 2^31)
+        // above them.  Hundreds of CTAs finish within a microsecond of each other and their atomics on one address are
+        // served one after the other, so every atomic saved is time off the kernel's tail.
+        atomicAdd(&ctl->acc_unequal, un | (ng << 33));
         __threadfence();
         const unsigned int t = atomicAdd(&ctl->ticket, 1u);
         last = (t == gridDim.x - 1u);
         if (last) {
             // every other CTA's contribution is visible: its fence preceded its ticket
             __threadfence();
-            const unsigned long long tun = atomicAdd(&ctl->acc_unequal, 0ull);
-            const unsigned long long tng = atomicAdd(&ctl->acc_negative, 0ull);
+            const unsigned long long packed = atomicAdd(&ctl->acc_unequal, 0ull);
+            const unsigned long long tun = packed & ((1ull << 33) - 1ull), tng = packed >> 33;
             const long long Ev = 2ll * (long long)tun - (long long)dim * (long long)N;
             const long long Mv = (long long)N - 2ll * (long long)tng;
             ctl->E = Ev;
@@ -109,7 +111,6 @@ __device__ __forceinline__ void block_accumulate(unsigned long long unequal, uns
             if (E_dst) *E_dst = Ev;          // the caller's device words: no bounce through the host
             if (M_dst) *M_dst = Mv;
             ctl->acc_unequal = 0ull;
-            ctl->acc_negative = 0ull;
             ctl->ticket = 0u;
         }
     }
@@ -235,8 +236,9 @@ cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo
                                         long long *E_dst, long long *M_dst, int num_sms, cudaStream_t stream)
 {
     if (geo.L % 16u == 0u) {
-        // one wave, kU chunks per thread: 4 CTAs of 256 threads per SM at 16 MiB
-        const int grid = grid_for((geo.N / 16u + kU - 1) / kU, num_sms, 8);
+        // kU chunks in flight per thread, a few CTAs per SM (every CTA ends with two atomics on the same two words)
+        // (measured on B200, 16 MiB, cold L2, ncu: 12.7 / 9.7 / 11.1 us with 2 / 4 / 8 CTAs per SM)
+        const int grid = grid_for((geo.N / 16u + kU - 1) / kU, num_sms, 4);
         if (dim == 2) energy_magnetisation_vec16<2><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
         else          energy_magnetisation_vec16<3><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
     } else {
