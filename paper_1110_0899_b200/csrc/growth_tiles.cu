@@ -150,7 +150,8 @@ struct alignas(16) TShared {
     unsigned int watcher;               // 1 while some idle worker warp holds the watch (polls the ring without backing off)
     unsigned int ready_tag[2];          // k + 1 when EVERY tile of the CTA has its bits of update k in buffer k & 1
     unsigned int meas_req;              // k + 1 once the monitor has asked for the measurement after update k (in-kernel measurement)
-    unsigned long long meas_un, meas_ng;   // ... this CTA's sums of one evaluation: unequal forward bonds, negative spins
+    unsigned int meas_un, meas_ng;      // ... this CTA's sums of one evaluation: unequal forward bonds, negative spins (a CTA
+                                        // holds fewer than 2^18 spins: 32 bits, i.e. native shared-memory reductions)
     unsigned long long ihead;           // inbox messages consumed (written by the receiver warp only)
     unsigned long long spill_head, spill_tail;   // running positions in the CTA's global spill list (kept across launches)
 };
@@ -615,8 +616,8 @@ __device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, ui
     un = __reduce_add_sync(kFullMask, un);
     ng = __reduce_add_sync(kFullMask, ng);
     if ((threadIdx.x & 31u) == 0u) {
-        if (un) atomicAdd(&sh.meas_un, (unsigned long long)un);
-        if (ng) atomicAdd(&sh.meas_ng, (unsigned long long)ng);
+        if (un) red_shared_add(smem_addr(&sh.meas_un), un);
+        if (ng) red_shared_add(smem_addr(&sh.meas_ng), ng);
     }
 #ifdef WOLFF_PROFILE
     if (prof) pt[4] = globaltimer_ns();
@@ -630,9 +631,9 @@ __device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, ui
     }
 #endif
     if (ptid == 0u) {
-        const unsigned long long tun = ld_vol64(&sh.meas_un), tng = ld_vol64(&sh.meas_ng);
-        st_vol64(&sh.meas_un, 0ull);
-        st_vol64(&sh.meas_ng, 0ull);
+        const unsigned long long tun = ld_vol(&sh.meas_un), tng = ld_vol(&sh.meas_ng);
+        st_vol(&sh.meas_un, 0u);
+        st_vol(&sh.meas_ng, 0u);
         if (tun) atomicAdd(&ctl->meas_unequal, tun);
         if (tng) atomicAdd(&ctl->meas_negative, tng);
         __threadfence();
@@ -1340,7 +1341,7 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const __grid_consta
         sh.ready_tag[0] = sh.ready_tag[1] = 0u;
         sh.watcher = 0u;
         sh.meas_req = 0u;
-        sh.meas_un = sh.meas_ng = 0ull;
+        sh.meas_un = sh.meas_ng = 0u;
         sh.fill_on = tp.fill_mode == 0u ? 0u : (tp.fill_mode == 2u ? 1u : tp.gfill[c]);
         sh.ihead = ld_relaxed_u64(tp.gdone + c);          // everything ever sent to this CTA was consumed by the last launch
         sh.spill_head = sh.spill_tail = ld_relaxed_u64(tp.gspill + c);
