@@ -520,6 +520,7 @@ __device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, ui
 #ifdef WOLFF_PROFILE
     if (prof) pt[2] = globaltimer_ns();
 #endif
+    // (summing the bonds inside the tiles before this wait instead of after it changes nothing: measured)
     if (ptid == 0u) {
         atomicAdd(&ctl->meas_arrive_a, 1u);
         const unsigned int target = (krel + 1u) * tp.G;
@@ -540,26 +541,40 @@ __device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, ui
     if (b >= 4u) {
         // (a) the bonds inside my tiles: shared memory only, 16 sites per load
         const uint32_t cpt_log = tg.ts_log - 4u, total = myslots << cpt_log;
+        // spins are +1 / -1 bytes, so a signed 8-bit dot product of two words IS the sum of four bond products s_i s_j
+        // (and against 0x01010101 the sum of four spins): one IDP4A per word and direction instead of mask, shift, merge
+        // and population count.  #unequal = (#bonds - sum of products) / 2, #negative = (#spins - sum of spins) / 2.
+        int dps = 0, sps = 0;
+        unsigned int nch = 0;
         auto chunk = [&](uint32_t ch) {
             const uint32_t slot = ch >> cpt_log, w0 = (ch & ((1u << cpt_log) - 1u)) << 4;
             const uint32_t x0 = w0 & m, y = (w0 >> b) & m, z = DIM == 3 ? (w0 >> (2u * b)) : 0u;
             const uint32_t at = lat_s + (slot << tg.ts_log) + w0;
             const uint4 a = lds_v4(at);
-            // forward rows: inside the tile, else the row itself (equal words count nothing; the bond is counted in (b))
+            // forward rows: inside the tile, else the row itself (a product of a spin with itself counts as an equal
+            // pair, i.e. nothing unequal; the bond is counted in (b))
             const uint4 by = lds_v4(y + 1u < B ? at + B : at);
             const uint4 bz = DIM == 3 ? lds_v4(z + 1u < B ? at + (B << b) : at) : a;
             // +x: the 16 sites shifted by one byte; the 17th is the next site of the row -- or, at the end of the row, a
             // copy of the 16th, so that the bond across the tile border counts nothing here
             const uint32_t nb = x0 + 16u < B ? lds_u8(at + 16u) : (a.w >> 24);
-            ng += __popc(merge4(a));
-            const unsigned int bx = merge4(a.x ^ __funnelshift_r(a.x, a.y, 8), a.y ^ __funnelshift_r(a.y, a.z, 8),
-                                           a.z ^ __funnelshift_r(a.z, a.w, 8), a.w ^ __funnelshift_r(a.w, nb, 8));
-            un += __popc(bx | (merge4(xor4(a, by)) >> 4));
-            if (DIM == 3) un += __popc(merge4(xor4(a, bz)));
+            sps = __dp4a((int)a.x, 0x01010101, sps); sps = __dp4a((int)a.y, 0x01010101, sps);
+            sps = __dp4a((int)a.z, 0x01010101, sps); sps = __dp4a((int)a.w, 0x01010101, sps);
+            dps = __dp4a((int)a.x, (int)__funnelshift_r(a.x, a.y, 8), dps); dps = __dp4a((int)a.y, (int)__funnelshift_r(a.y, a.z, 8), dps);
+            dps = __dp4a((int)a.z, (int)__funnelshift_r(a.z, a.w, 8), dps); dps = __dp4a((int)a.w, (int)__funnelshift_r(a.w, nb, 8), dps);
+            dps = __dp4a((int)a.x, (int)by.x, dps); dps = __dp4a((int)a.y, (int)by.y, dps);
+            dps = __dp4a((int)a.z, (int)by.z, dps); dps = __dp4a((int)a.w, (int)by.w, dps);
+            if (DIM == 3) {
+                dps = __dp4a((int)a.x, (int)bz.x, dps); dps = __dp4a((int)a.y, (int)bz.y, dps);
+                dps = __dp4a((int)a.z, (int)bz.z, dps); dps = __dp4a((int)a.w, (int)bz.w, dps);
+            }
+            ++nch;
         };
         uint32_t ch = ptid;
         for (; ch + P < total; ch += 2u * P) { chunk(ch); chunk(ch + P); }
         if (ch < total) chunk(ch);
+        un += (unsigned int)(((int)(nch * 16u * (unsigned int)DIM) - dps) >> 1);
+        ng += (unsigned int)(((int)(nch * 16u) - sps) >> 1);
         // (b1) the bonds across the +x border of a tile: my site x = B - 1 against the next tile's x = 0 (global memory),
         // one site per lane, eight global loads in flight per lane (a trip costs one L2 round trip, not eight)
         constexpr uint32_t kSites = 8;
@@ -594,7 +609,8 @@ __device__ __noinline__ void measure_phase(const TileParams &tp, TShared &sh, ui
             }
 #pragma unroll
             for (uint32_t j = 0; j < kTasks; ++j)
-                if (on[j]) un += __popc(merge4(xor4(mine[j], theirs[j])));
+                if (on[j]) un += (unsigned int)((16 - __dp4a((int)mine[j].x, (int)theirs[j].x, __dp4a((int)mine[j].y, (int)theirs[j].y,
+                                                     __dp4a((int)mine[j].z, (int)theirs[j].z, __dp4a((int)mine[j].w, (int)theirs[j].w, 0))))) >> 1);
         }
     } else {
         // tiles narrower than a 16-byte load (test configurations): one site at a time
