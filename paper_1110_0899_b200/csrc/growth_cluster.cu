@@ -27,8 +27,11 @@
 //     units of outstanding work: a warp that takes n sites holds n units until it runs dry; sites handed to a ring
 //     are added BEFORE they become visible (an atomic with return, so the addition has been performed).  When a warp
 //     runs dry one remote reduction subtracts its units and adds the spins it claimed, so the monitor warp (CTA 0)
-//     that reads pending == 0 reads the complete cluster size in the same word.  It logs the size, draws the next seed
-//     site (A1) and hands it to the ring of the CTA that holds it.
+//     that reads pending == 0 reads the complete cluster size in the same word;
+//   - the monitor warp draws the seed site (A1), flips its bit and EXPANDS IT ITSELF, as a worker would; its own unit and
+//     claims never touch the shared word, and only when a site is about to leave its hands does it publish the update's
+//     index and seed spin to every CTA.  A cluster of a handful of spins (the literal random start of the BASELINE configs,
+//     T above T_c) is complete after its few passes, without a hand-over, a poll or a remote word besides the spins'.
 //
 // The int8 lattice in global memory stays the authoritative copy between launches: every CTA packs its slab of the
 // lattice in the prologue and unpacks it in the epilogue (N bytes each way per launch, by 16 SMs).
