@@ -128,13 +128,14 @@ WOLFF_API int wolff_reset_moments(wolff_handle h);
  *    tens of thousands of spins and more (the BASELINE lattices at T_c);
  *  - the cluster-resident, bit-packed, barrier-free kernel (one bit per spin in the distributed shared memory of ONE
  *    thread-block cluster of up to 16 CTAs; a claim is one atomic on the word that holds the spin, in whichever CTA
- *    holds it; the warp that draws the seed site expands it itself): applies when L is a power of two, N >= 32 and
- *    N / 8 bytes fit one cluster (N <= 2^24); the fastest on small and medium clusters (the literal random start of
- *    the BASELINE configs, T above T_c, 3D L = 128);
+ *    holds it; the warp that draws the seed site expands it itself): applies to any L with N <= 2^24 (N / 8 bytes fit
+ *    one cluster); the fastest on small and medium clusters (the literal random start of the BASELINE configs, T above
+ *    T_c, 3D L = 128) and on every lattice the first kernel does not apply to (L not a power of two);
  *  - the level-synchronous kernel, which runs each BFS level in one of three tiers by frontier width n: one
  *    CTA (n <= up), one thread-block cluster (n <= cluster_up), the whole grid (above): any L.
  * Keys:
- *   "mode"                 0 = chosen by the mean cluster size of the last finished run, see "small_cluster" (default);
+ *   "mode"                 0 = chosen by the lattice and the mean cluster size of the last finished run, see
+ *                          "small_cluster" (default);
  *                          5 = the cluster-resident kernel whenever it applies (else as mode 0);
  *                          level-synchronous kernel only: 4 = tiers by frontier width, 1 = every level
  *                          grid-wide, 2 = one CTA whenever the frontier fits its shared-memory queue, 3 = the

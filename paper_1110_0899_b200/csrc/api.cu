@@ -214,7 +214,7 @@ void free_cluster_state(wolff_ctx *h)
 
 // (Re)derive the launch shape of growth_cluster.cu: the largest cluster (at most "cluster_ctas" CTAs) whose CTAs each
 // hold a power-of-two number of 32-bit words of the bit lattice, the ring and the stages in their shared memory.
-// cl_ok == false (L not a power of two, fewer than 32 spins, or the lattice does not fit one cluster) is not an error.
+// cl_ok == false (the lattice does not fit one cluster: more than 2^24 spins) is not an error.
 int refresh_cluster_plan(wolff_ctx *h, cudaStream_t stream)
 {
     if (!h->cl_dirty) return WOLFF_OK;
@@ -222,22 +222,29 @@ int refresh_cluster_plan(wolff_ctx *h, cudaStream_t stream)
     free_cluster_state(h);
     h->cl_ok = false;
     h->cl_dirty = false;
-    if (!h->geo.pow2 || h->N < 32 || h->N > (1ull << 31)) return WOLFF_OK;
-    const uint64_t words = h->N / 32;
+    // sites are carried in 24 bits and divided by L and L^2 with 40-bit reciprocals: N <= 2^24, L^2 <= 2^16 in 3D
+    if (h->N > (1ull << 24) || (h->dim == 3 && (uint64_t)h->L * h->L > (1ull << 16))) return WOLFF_OK;
+    const uint64_t words = (h->N + 31) / 32;
     uint32_t nC = 16;
     while (nC > 1 && (nC > (uint32_t)h->resident_ctas || nC > words)) nC >>= 1;
     size_t smem = 0;
     int clusters = 0;
-    // the largest cluster allowed: a CTA's share of the lattice (words / nC, a power of two) must fit its shared memory
-    smem = cluster_smem_bytes((uint32_t)(words / nC), h->ring_cap);
+    // the largest cluster allowed: a CTA's share of the lattice (a power of two of words, at least words / nC) must fit
+    // its shared memory
+    uint32_t wpc = 1;
+    while ((uint64_t)wpc * nC < words) wpc <<= 1;
+    smem = cluster_smem_bytes(wpc, h->ring_cap);
     if (smem + 1024 > h->smem_optin) return WOLFF_OK;
-    cudaError_t e = cluster_prepare(h->dim, nC, smem, &clusters);
+    cudaError_t e = cluster_prepare(h->dim, h->geo.pow2 != 0, nC, smem, &clusters);
     if (e != cudaSuccess || clusters < 1) { cudaGetLastError(); return WOLFF_OK; }
     ClusterParams &cp = h->cp;
     cp = ClusterParams{};
     cp.nC = nC;
-    cp.wpc = (uint32_t)(words / nC);
+    cp.wpc = wpc;
     cp.wpc_log = ceil_log2(cp.wpc);
+    cp.words = (uint32_t)words;
+    cp.magicL = ((1ull << 40) + (uint64_t)h->L - 1) / (uint64_t)h->L;
+    cp.magicLL = ((1ull << 40) + (uint64_t)h->geo.LL - 1) / (uint64_t)h->geo.LL;
     cp.ring_cap = h->ring_cap;
     cp.spill_log = ceil_log2(h->N);
     cp.watchdog_ns = h->watchdog_ms * 1000000ull;
@@ -529,7 +536,8 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     const bool small = h->small_cluster > 0 && h->have_mean && h->mean_cluster < (double)h->small_cluster;
     const bool tiny = small && h->mean_cluster < 16.0;
     bool clustered = false;
-    if ((h->mode == 5 || (h->mode == 0 && small)) && !h->measure) {
+    // (a lattice the kernel of all SMs does not apply to -- L not a power of two -- runs here whatever its clusters)
+    if ((h->mode == 5 || (h->mode == 0 && (small || !h->plan_ok))) && !h->measure) {
         rc = refresh_cluster_plan(h, stream);
         if (rc) return rc;
         clustered = h->cl_ok;

@@ -7,7 +7,8 @@
 // lattice in the shared memory of all 148 SMs, and a claim that crosses into another CTA's tiles travels through L2
 // (an atomic for the inbox slot, a store, the receiver's poll: 1.5-3 us per hop, which is what bounds it in 3D where
 // 16^3 tiles make 0.16 such hops per spin).  Here the lattice is ONE BIT PER SPIN (the sign), so every BASELINE
-// lattice (<= 2^24 spins = 2 MiB) fits the distributed shared memory of ONE thread-block cluster of 16 CTAs, and
+// lattice (<= 2^24 spins = 2 MiB) fits the distributed shared memory of ONE thread-block cluster of 16 CTAs (any L: the
+// coordinates of a site come from shifts when L is a power of two, from two multiplications otherwise), and
 //
 //   - claim-and-flip (A4) is ONE atomic on the 32-bit word holding the neighbour's bit, wherever that word lives:
 //     atom.shared::cluster.or / .and on the own CTA's window (about 40 ns as a dependent operation) or on a peer's
@@ -78,12 +79,6 @@ __device__ __forceinline__ unsigned long long cl_ld_u64(uint32_t a)
     return v;
 }
 __device__ __forceinline__ void cl_st_u32(uint32_t a, uint32_t v) { asm volatile("st.volatile.shared::cluster.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
-__device__ __forceinline__ uint32_t cl_atom_add(uint32_t a, uint32_t v)
-{
-    uint32_t o;
-    asm volatile("atom.shared::cluster.add.u32 %0, [%1], %2;" : "=r"(o) : "r"(a), "r"(v) : "memory");
-    return o;
-}
 __device__ __forceinline__ uint32_t cl_atom_xor(uint32_t a, uint32_t v)
 {
     uint32_t o;
@@ -210,7 +205,9 @@ struct CWorker {
 // the cluster's pending / claimed word; before the first site of the update leaves its hands it writes the update's
 // index and seed spin into every CTA and reads them back (the load returns only after the store has been performed
 // there), so every warp that later takes a site of this update finds them.
-template <int DIM, bool POS, bool MONITOR>
+// POW2: L is a power of two (coordinates by shifts and masks); else by two multiplications with ceil(2^40 / divisor), exact
+// for sites below 2^24 and divisors up to 2^16 (the host checks both).
+template <int DIM, bool POS, bool MONITOR, bool POW2>
 __device__ __forceinline__ void run_passes(const ClusterParams &cp, uint32_t bits_s, uint32_t pc_c, uint32_t head_c, uint32_t ring_c, uint32_t *stage,
                                            uint32_t u_lo, uint32_t u_hi, CWorker &ws, CTally &tl)
 {
@@ -221,6 +218,11 @@ __device__ __forceinline__ void run_passes(const ClusterParams &cp, uint32_t bit
     const unsigned int q = lane / ND, k = lane - q * ND, d = k >> 1, sgn = k & 1u;
     const uint32_t Lmask = p.geo.L - 1u;
     const uint32_t sh_d = d * p.geo.logL, fmask = Lmask << sh_d, delta = sgn ? 0xFFFFFFFFu : 1u;
+    // any L: this lane's stride L^d, its magic, and the steps to the neighbour inside the lattice / across the wrap
+    const uint32_t stride = d == 0u ? 1u : (d == 1u ? p.geo.L : p.geo.LL);
+    const unsigned long long magic_s = d == 0u ? (1ull << 40) : (d == 1u ? cp.magicL : cp.magicLL);
+    const uint32_t edge_c = sgn ? 0u : Lmask;                                        // coordinate at which the neighbour wraps
+    const uint32_t step_in = sgn ? 0u - stride : stride, step_wrap = sgn ? Lmask * stride : 0u - Lmask * stride;
     const uint32_t wmask = cp.wpc - 1u;
     const uint32_t stage_s = smem_addr(stage);
     uint32_t a = ws.a;
@@ -233,7 +235,14 @@ __device__ __forceinline__ void run_passes(const ClusterParams &cp, uint32_t bit
 #endif
         const bool have = q < S && q < nsites;               // lanes 30, 31 in 3D (q = S) never hold a site
         // ---- this lane's neighbour (periodic) and the owner of the bond between them (reading R6)
-        const uint32_t n = (a & ~fmask) | ((((a >> sh_d) + delta) & Lmask) << sh_d);
+        uint32_t n;
+        if (POW2) {
+            n = (a & ~fmask) | ((((a >> sh_d) + delta) & Lmask) << sh_d);
+        } else {
+            const uint32_t q1 = (uint32_t)(((unsigned long long)a * magic_s) >> 40);                         // a div L^d
+            const uint32_t c = q1 - (uint32_t)(((unsigned long long)q1 * cp.magicL) >> 40) * p.geo.L;         // ... mod L
+            n = a + (c == edge_c ? step_wrap : step_in);
+        }
         // ---- A3: the bond variable, one Philox block per lane (word d of the block of the bond's owner)
         const uint4 blk = philox4x32_10(sgn ? n : a, kDomainBond, u_lo, u_hi, p.key0, p.key1);
         const uint32_t r = d == 0u ? blk.x : (d == 1u ? blk.y : blk.z);
@@ -299,7 +308,7 @@ __device__ __forceinline__ void run_passes(const ClusterParams &cp, uint32_t bit
     ws.nsites = 0u; ws.mywon = MONITOR ? wsum : 0u; ws.sbuf = sbuf; ws.a = a;
 }
 
-template <int DIM>
+template <int DIM, bool POW2>
 __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh, uint32_t bits_s, uint32_t ring_s, uint32_t *stage, unsigned int rank,
                                             CTally &tl)
 {
@@ -421,15 +430,15 @@ __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh
         tl.cyc_take += (unsigned long long)(clock64() - tt0);
         ++tl.takes;
 #endif
-        if (upd & 1u) run_passes<DIM, false, false>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
-        else          run_passes<DIM, true, false>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
+        if (upd & 1u) run_passes<DIM, false, false, POW2>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
+        else          run_passes<DIM, true, false, POW2>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
     }
 }
 
 // CTA 0 only: the update loop ("(v) Go to (i)").  Draws the seed site of update u (A1, reading R8), flips
 // it, expands it (run_passes<MONITOR>); when sites have left its hands it waits for the pending count to return to zero;
 // logs the size (A7).
-template <int DIM>
+template <int DIM, bool POW2>
 __device__ __forceinline__ void monitor_warp(const ClusterParams &cp, CShared &sh, uint32_t bits_s, uint32_t ring_s, uint32_t *stage, CTally &tl)
 {
     constexpr unsigned int ND = 2u * DIM;
@@ -467,8 +476,8 @@ __device__ __forceinline__ void monitor_warp(const ClusterParams &cp, CShared &s
         ws.mywon = 0u;
         ws.upd_v = ((unsigned int)k << 1) | s0neg;
         ws.handed = false;
-        if (s0neg) run_passes<DIM, false, true>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
-        else       run_passes<DIM, true, true>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
+        if (s0neg) run_passes<DIM, false, true, POW2>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
+        else       run_passes<DIM, true, true, POW2>(cp, bits_s, pc_c, head_c, ring_c, stage, (uint32_t)u, (uint32_t)(u >> 32), ws, tl);
         unsigned int size = 1u + ws.mywon;     // the seed and what this warp claimed itself
         if (ws.handed) {
             // sites have left this warp's hands: the update is complete when nothing is pending anywhere
@@ -509,7 +518,7 @@ __device__ __forceinline__ void monitor_warp(const ClusterParams &cp, CShared &s
     }
 }
 
-template <int DIM>
+template <int DIM, bool POW2>
 __global__ void __launch_bounds__(kCT, 1) growth_cluster_kernel(const __grid_constant__ ClusterParams cp)
 {
     extern __shared__ __align__(16) unsigned char smem_c[];
@@ -534,26 +543,42 @@ __global__ void __launch_bounds__(kCT, 1) growth_cluster_kernel(const __grid_con
         sh.watcher = 0u;
     }
     // ---- prologue: my slab of the lattice, one bit per spin (bit = 1: spin -1); word w of the lattice = sites 32 w ..
-    const uint4 *const src = reinterpret_cast<const uint4 *>(p.spins) + (size_t)rank * cp.wpc * 2u;
+    // (the last word of the lattice may be partial and the last CTAs may hold fewer words than wpc, or none)
+    const uint4 *const src = reinterpret_cast<const uint4 *>(p.spins);
     for (uint32_t w = tid; w < cp.wpc; w += kCT) {
-        const uint4 lo = __ldcg(src + 2u * w), hi = __ldcg(src + 2u * w + 1u);
-        bits[w] = pack16(lo) | (pack16(hi) << 16);
+        const uint32_t gw = rank * cp.wpc + w, first = gw * 32u;
+        uint32_t v = 0u;
+        if (gw < cp.words) {
+            if (first + 32u <= p.geo.N) {
+                const uint4 lo = __ldcg(src + 2u * (size_t)gw), hi = __ldcg(src + 2u * (size_t)gw + 1u);
+                v = pack16(lo) | (pack16(hi) << 16);
+            } else {
+                for (uint32_t i = first; i < p.geo.N; ++i) v |= (p.spins[i] < 0 ? 1u : 0u) << (i - first);
+            }
+        }
+        bits[w] = v;
     }
     cluster.sync();                  // every CTA's shared memory is initialised before a peer touches it
 
     if (!dead) {
-        if (warp == 0u && rank == 0u) monitor_warp<DIM>(cp, sh, smem_addr(bits), smem_addr(ring), stage, tl);
-        else worker_warp<DIM>(cp, sh, smem_addr(bits), smem_addr(ring), stage + warp * kCStage, rank, tl);
+        if (warp == 0u && rank == 0u) monitor_warp<DIM, POW2>(cp, sh, smem_addr(bits), smem_addr(ring), stage, tl);
+        else worker_warp<DIM, POW2>(cp, sh, smem_addr(bits), smem_addr(ring), stage + warp * kCStage, rank, tl);
     }
     cluster.sync();                  // no peer touches this CTA's shared memory any more
 
     // ---- epilogue: my slab back to the int8 lattice
     if (!dead) {
-        uint4 *const dst = reinterpret_cast<uint4 *>(p.spins) + (size_t)rank * cp.wpc * 2u;
+        uint4 *const dst = reinterpret_cast<uint4 *>(p.spins);
         for (uint32_t w = tid; w < cp.wpc; w += kCT) {
+            const uint32_t gw = rank * cp.wpc + w, first = gw * 32u;
+            if (gw >= cp.words) continue;
             const uint32_t b = bits[w];
-            dst[2u * w] = unpack16(b & 0xFFFFu);
-            dst[2u * w + 1u] = unpack16(b >> 16);
+            if (first + 32u <= p.geo.N) {
+                dst[2u * (size_t)gw] = unpack16(b & 0xFFFFu);
+                dst[2u * (size_t)gw + 1u] = unpack16(b >> 16);
+            } else {
+                for (uint32_t i = first; i < p.geo.N; ++i) p.spins[i] = ((b >> (i - first)) & 1u) ? (int8_t)-1 : (int8_t)1;
+            }
         }
     }
     Control *ctl = p.ctl;
@@ -574,21 +599,21 @@ __global__ void __launch_bounds__(kCT, 1) growth_cluster_kernel(const __grid_con
     }
 }
 
-template <int DIM>
+template <int DIM, bool POW2>
 cudaError_t set_attributes(size_t smem_bytes, int nC)
 {
-    const void *fn = reinterpret_cast<const void *>(&growth_cluster_kernel<DIM>);
+    const void *fn = reinterpret_cast<const void *>(&growth_cluster_kernel<DIM, POW2>);
     cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return e;
     if (nC > 8) e = cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     return e;
 }
 
-template <int DIM>
+template <int DIM, bool POW2>
 cudaError_t launch_one(const ClusterParams &cp, size_t smem_bytes, cudaStream_t stream, int *max_clusters)
 {
     // per-process kernel attributes: another live handle may have changed them since this one made its plan
-    cudaError_t e = set_attributes<DIM>(smem_bytes, (int)cp.nC);
+    cudaError_t e = set_attributes<DIM, POW2>(smem_bytes, (int)cp.nC);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3(cp.nC);
@@ -602,8 +627,8 @@ cudaError_t launch_one(const ClusterParams &cp, size_t smem_bytes, cudaStream_t 
     attr.val.clusterDim.z = 1;
     cfg.attrs = &attr;
     cfg.numAttrs = 1;
-    if (max_clusters) return cudaOccupancyMaxActiveClusters(max_clusters, growth_cluster_kernel<DIM>, &cfg);
-    return cudaLaunchKernelEx(&cfg, growth_cluster_kernel<DIM>, cp);
+    if (max_clusters) return cudaOccupancyMaxActiveClusters(max_clusters, growth_cluster_kernel<DIM, POW2>, &cfg);
+    return cudaLaunchKernelEx(&cfg, growth_cluster_kernel<DIM, POW2>, cp);
 }
 
 }  // namespace
@@ -613,16 +638,24 @@ size_t cluster_smem_bytes(uint32_t wpc, uint32_t ring_cap)
     return ((size_t)wpc + (size_t)ring_cap + (size_t)kCWarps * kCStage) * sizeof(uint32_t);
 }
 
-cudaError_t cluster_prepare(int dim, uint32_t nC, size_t smem_bytes, int *max_clusters)
+namespace {
+cudaError_t dispatch(const ClusterParams &cp, int dim, bool pow2, size_t smem_bytes, cudaStream_t stream, int *max_clusters)
+{
+    if (dim == 2) return pow2 ? launch_one<2, true>(cp, smem_bytes, stream, max_clusters) : launch_one<2, false>(cp, smem_bytes, stream, max_clusters);
+    return pow2 ? launch_one<3, true>(cp, smem_bytes, stream, max_clusters) : launch_one<3, false>(cp, smem_bytes, stream, max_clusters);
+}
+}  // namespace
+
+cudaError_t cluster_prepare(int dim, bool pow2, uint32_t nC, size_t smem_bytes, int *max_clusters)
 {
     ClusterParams cp{};
     cp.nC = nC;
-    return dim == 2 ? launch_one<2>(cp, smem_bytes, nullptr, max_clusters) : launch_one<3>(cp, smem_bytes, nullptr, max_clusters);
+    return dispatch(cp, dim, pow2, smem_bytes, nullptr, max_clusters);
 }
 
 cudaError_t launch_growth_cluster(const ClusterParams &cp, int dim, size_t smem_bytes, cudaStream_t stream)
 {
-    return dim == 2 ? launch_one<2>(cp, smem_bytes, stream, nullptr) : launch_one<3>(cp, smem_bytes, stream, nullptr);
+    return dispatch(cp, dim, cp.g.geo.pow2 != 0u, smem_bytes, stream, nullptr);
 }
 
 }  // namespace wolff

@@ -112,13 +112,15 @@ struct TileParams {
     int8_t *faces;
 };
 
-// Cluster-resident bit-packed kernel (growth_cluster.cu).  The lattice (L a power of two, N >= 32 nC) is held as one bit
-// per spin in the distributed shared memory of ONE thread-block cluster of nC CTAs: word w (sites 32 w .. 32 w + 31)
-// lives in CTA w / wpc.  The spill list and its two counters run on across launches (nothing is reset).
+// Cluster-resident bit-packed kernel (growth_cluster.cu).  The lattice (any L, N <= 2^24) is held as one bit per spin in
+// the distributed shared memory of ONE thread-block cluster of nC CTAs: word w (sites 32 w .. 32 w + 31) lives in CTA
+// w / wpc (the last word may be partial, the last CTAs may hold fewer words, or none).  The spill list and its two counters run on across launches (nothing is reset).
 struct ClusterParams {
     GrowthParams g;
     uint32_t nC;                     // CTAs of the cluster (1, 2, 4, 8 or 16)
     uint32_t wpc, wpc_log;           // 32-bit words of the bit lattice per CTA (a power of two)
+    uint32_t words;                  // words of the whole lattice: ceil(N / 32)
+    unsigned long long magicL, magicLL;   // ceil(2^40 / L), ceil(2^40 / L^2): a div L for a < 2^24 when L is not a power of two
     uint32_t ring_cap;               // entries of a CTA's shared-memory ring (power of two)
     uint32_t *spill;                 // 2^spill_log entries (>= N): overflow of the rings, shared by the cluster
     uint32_t spill_log;
@@ -173,7 +175,7 @@ cudaError_t tiles_prepare(int dim, size_t smem_bytes, int *ctas_per_sm);
 cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes, cudaStream_t stream);
 // cluster-resident kernel: shared memory needed, attributes + co-resident clusters, launch of one cluster of cp.nC CTAs
 size_t cluster_smem_bytes(uint32_t wpc, uint32_t ring_cap);
-cudaError_t cluster_prepare(int dim, uint32_t nC, size_t smem_bytes, int *max_clusters);
+cudaError_t cluster_prepare(int dim, bool pow2, uint32_t nC, size_t smem_bytes, int *max_clusters);
 cudaError_t launch_growth_cluster(const ClusterParams &cp, int dim, size_t smem_bytes, cudaStream_t stream);
 // batch of chains: CTAs of `threads` threads, `grid` of them; co-resident CTAs per SM; E, M of every chain into EM
 // bits: the bit-packed shared-memory-resident variant; its shared memory: the frontier buffers + N/8 bytes per plane

@@ -49,6 +49,7 @@ CLUSTER = [
     (3, 8, wl.TC_3D, {"mode": 5, "resident_ctas": 4, "ring_cap": 32, "idle_ns": 0}),
     (2, 32, 2.0, {"mode": 5, "resident_ctas": 2, "ring_cap": 32}),
     (3, 8, 4.0, {"mode": 0, "small_cluster": 1 << 30, "resident_ctas": 1}),
+    (2, 21, 2.1, {"mode": 0, "resident_ctas": 4, "ring_cap": 32}),          # L not a power of two, a partial last word
 ]
 
 

@@ -112,14 +112,14 @@ def test_randomised_knobs_shared_memory_resident_kernel(case_seed):
 
 @pytest.mark.parametrize("case_seed", range(2))
 def test_randomised_knobs_cluster_resident_kernel(case_seed):
-    # 25 short chains per seed on the cluster-resident bit-packed kernel: random lattice (down to 32 spins, one word),
+    # 25 short chains per seed on the cluster-resident bit-packed kernel: random lattice (any L, a partial last word),
     # temperature, start, cluster size (1 .. 16 CTAs) and ring size (32 entries: sites spill to global memory and come
     # back; peers steal), in mode 5 and through the kernel choice of mode 0
     import random
     rng = random.Random(3000 + case_seed)
     for _ in range(25):
         dim = rng.choice([2, 3])
-        L = rng.choice([8, 16, 32, 64, 128] if dim == 2 else [4, 8, 16, 32])
+        L = rng.choice([8, 16, 32, 64, 128, 7, 30, 100] if dim == 2 else [4, 8, 16, 32, 5, 11, 24])
         T = rng.choice([wl.TC_2D, 1.8, 3.0] if dim == 2 else [wl.TC_3D, 4.0, 5.0])
         opts = {"mode": rng.choice([5, 5, 0]), "small_cluster": 1 << 30, "resident_ctas": rng.choice([1, 2, 4, 8, 16]),
                 "ring_cap": rng.choice([32, 64, 2048]), "idle_ns": rng.choice([0, 100, 1000])}
