@@ -430,11 +430,13 @@ def run_b200(args, rank: int, world: int):
         h.close()
         return out
 
-    def batch_leg(cfg_name: str, R: int, n: int, cold: bool, equil: int, oracle_budget: float):
-        """R independent chains in ONE launch (wolff_batch_run): aggregate updates/s and flipped spins/s."""
+    def batch_leg(cfg_name: str, R: int, n: int, cold: bool, equil: int, oracle_budget: float, batch_options=None):
+        """R independent chains in ONE call (wolff_batch_run): aggregate updates/s and flipped spins/s."""
         c = wl.CONFIGS[cfg_name]
         seeds = [c.seed + 1000 * rank + r for r in range(R)]
         b = binding.WolffBatch(c.dim, c.L, c.J, [c.T] * R, seeds)
+        for k, v in (batch_options or {}).items():
+            b.set_option(k, v)
         if cold:
             b.set_spins(torch.ones(R * c.N, dtype=torch.int8, device=dev))
         if equil:
@@ -449,7 +451,7 @@ def run_b200(args, rank: int, world: int):
                 b.run(n, stream=stream)
                 e1.record(stream)
             e1.synchronize()
-            launches[0] += 1
+            launches[0] += R if (batch_options or {}).get("resident") == 3 else 1
             st = b.stats()
             ms = e0.elapsed_time(e1)
             if best is None or ms < best[0]:
@@ -457,8 +459,10 @@ def run_b200(args, rank: int, world: int):
         b.close()
         ms, st = best
         agg = aggregate_replicas(st["flipped"], st["updates"], ms, world, dev)
-        out = {"workload": "%s, %s, %d chains (seeds %d..) in one launch, %d updates each after %d untimed" %
-                           (c.name, "cold start" if cold else "random start", R, seeds[0], n, equil),
+        out = {"workload": "%s, %s, %d chains (seeds %d..) in one %s, %d updates each after %d untimed" %
+                           (c.name, "cold start" if cold else "random start", R, seeds[0],
+                            "call: one thread-block cluster per chain, 7 chains side by side" if (batch_options or {}).get("resident") == 3 else "launch",
+                            n, equil),
                "replicas": R * world, "updates_per_s": agg["updates_per_s"], "value": agg["value"], "unit": UNIT,
                "mean_cluster": st["flipped"] / max(st["updates"], 1), "bfs_levels_per_update": st["levels"] / max(st["updates"], 1),
                "ms": ms}
@@ -600,6 +604,9 @@ def run_b200(args, rank: int, world: int):
             "C2_literal": batch_leg("C2", 4 * args.batch_replicas, 2000, False, 200, osec),
             "C1_equilibrated": batch_leg("C1", 4 * args.batch_replicas, 2000, False, 1000, 0.0),
             "C2_equilibrated": batch_leg("C2", args.batch_replicas // 2, 40, True, 300, 0.0),
+            # the metric's own workloads as replicas: every chain in one 16-CTA cluster (cluster-resident kernel)
+            "C3_equilibrated_one_cluster_per_chain": batch_leg("C3", 14, 50, True, 300, 0.0, {"resident": 3}),
+            "C5a_equilibrated_one_cluster_per_chain": batch_leg("C5a", 14, 300, True, 300, 0.0, {"resident": 3}),
         }
     out["gpu_launches"] = launches[0]
     return out

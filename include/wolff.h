@@ -221,7 +221,8 @@ WOLFF_API int wolff_destroy(wolff_handle h);
  * dependence of the timings, Fig. 1, and the Binder ratio U(T) for several L, Fig. 2, Eq. 3): many independent chains.
  * A batch holds R chains of the same dim and L, chain r with its own J[r], T[r] and seed[r]; wolff_batch_run performs
  * n_updates updates of EVERY chain in ONE persistent launch, one CTA per chain at a time (a CTA takes the next chain
- * when it has finished one), so up to 8-16 chains per SM are in flight.  Chain r computes, bit for bit, what a single
+ * when it has finished one), so up to 8-16 chains per SM are in flight (or, "resident" = 3, one thread-block cluster per
+ * chain: one launch per chain, seven side by side).  Chain r computes, bit for bit, what a single
  * chain made by wolff_create(dim, L, J[r], T[r], seed[r]) computes: same start lattice, same site draws, same bond
  * variables, same update index (the index is shared by the chains of a batch and advances by n_updates per run).
  * Layouts are replica-major: E[r], M[r]; cluster_sizes[r * n_updates + k]; spins[r * N + i]; series likewise.
@@ -244,6 +245,11 @@ WOLFF_API int wolff_batch_set_update_index(wolff_batch b, uint64_t update_index)
  *   2 = bit-packed in the CTA's shared memory, one bit per spin (N <= about 1.8 million: 2D L = 1024 is 128 KiB) plus, in
  *   a measured run, one mark bit per spin (then N <= about 900,000; a run that does not fit returns WOLFF_EINVAL),
  *   packed from / unpacked to the int8 lattice around the chain's turn;
+ *   3 = bit-packed in the distributed shared memory of one thread-block cluster per chain (N <= 2^24: 2D L = 4096 and
+ *   3D L = 256 are 2 MiB = 16 CTAs): every chain is one launch of the cluster-resident kernel of wolff_run, the launches
+ *   spread over the library's own streams (behind the caller's stream, which continues behind them), so that as many
+ *   chains run side by side as clusters fit the chip (7 of 16 CTAs on a B200); no in-kernel measurement (a measured run
+ *   returns WOLFF_EINVAL), at most 2^30 updates per call;
  *   0 = auto: 2 when a plane is at most 32 KiB (several chains per SM stay in flight), else 1.  Never changes a result. */
 WOLFF_API int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value);
 /* E and M after every update of the most recent (measured) run: R * n_updates values each. */

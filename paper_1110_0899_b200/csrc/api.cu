@@ -222,31 +222,9 @@ int refresh_cluster_plan(wolff_ctx *h, cudaStream_t stream)
     free_cluster_state(h);
     h->cl_ok = false;
     h->cl_dirty = false;
-    // sites are carried in 24 bits and divided by L and L^2 with 40-bit reciprocals: N <= 2^24, L^2 <= 2^16 in 3D
-    if (h->N > (1ull << 24) || (h->dim == 3 && (uint64_t)h->L * h->L > (1ull << 16))) return WOLFF_OK;
-    const uint64_t words = (h->N + 31) / 32;
-    uint32_t nC = 16;
-    while (nC > 1 && (nC > (uint32_t)h->resident_ctas || nC > words)) nC >>= 1;
-    size_t smem = 0;
-    int clusters = 0;
-    // the largest cluster allowed: a CTA's share of the lattice (a power of two of words, at least words / nC) must fit
-    // its shared memory
-    uint32_t wpc = 1;
-    while ((uint64_t)wpc * nC < words) wpc <<= 1;
-    smem = cluster_smem_bytes(wpc, h->ring_cap);
-    if (smem + 1024 > h->smem_optin) return WOLFF_OK;
-    cudaError_t e = cluster_prepare(h->dim, h->geo.pow2 != 0, nC, smem, &clusters);
-    if (e != cudaSuccess || clusters < 1) { cudaGetLastError(); return WOLFF_OK; }
     ClusterParams &cp = h->cp;
-    cp = ClusterParams{};
-    cp.nC = nC;
-    cp.wpc = wpc;
-    cp.wpc_log = ceil_log2(cp.wpc);
-    cp.words = (uint32_t)words;
-    cp.magicL = ((1ull << 40) + (uint64_t)h->L - 1) / (uint64_t)h->L;
-    cp.magicLL = ((1ull << 40) + (uint64_t)h->geo.LL - 1) / (uint64_t)h->geo.LL;
-    cp.ring_cap = h->ring_cap;
-    cp.spill_log = ceil_log2(h->N);
+    size_t smem = 0;
+    if (!cluster_plan(h->dim, h->geo, h->resident_ctas, h->ring_cap, h->smem_optin, &cp, &smem, nullptr)) return WOLFF_OK;
     cp.watchdog_ns = h->watchdog_ms * 1000000ull;
     cp.thr32 = (uint32_t)h->thr;
     cp.thr_all = (h->thr >> 32) != 0 ? 1u : 0u;

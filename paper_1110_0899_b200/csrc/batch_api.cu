@@ -55,10 +55,25 @@ struct wolff_batch_ctx {
     bool em_valid = false;          // EM holds E and M of the current lattices (a measured run or an evaluation left them there)
     cudaStream_t last_stream = nullptr;
     int measure = 0, threads_opt = 0;
-    int resident = 0;               // 0 auto, 1 int8 lattice in global memory, 2 bit-packed lattice in shared memory
+    int resident = 0;               // 0 auto, 1 int8 lattice in global memory, 2 bit-packed lattice in shared memory,
+                                    // 3 one thread-block cluster per chain (growth_cluster.cu), chains side by side on streams
     size_t smem_optin = 0;
     uint32_t qcap = 1024;
+    // resident = 3: the launch shape of the cluster-resident kernel and, per chain, a control block, a spill list and its
+    // two counters; the per-update durations the kernel records; the streams the chains' launches are spread over
+    bool cl_ready = false;
+    ClusterParams cl{};
+    size_t cl_smem = 0;
+    Control *cl_ctl = nullptr;
+    uint32_t *cl_spill = nullptr;
+    unsigned long long *cl_ctr = nullptr;
+    uint32_t *cl_ns = nullptr;
+    uint64_t cl_ns_cap = 0;
+    std::vector<cudaStream_t> cl_streams;
+    std::vector<cudaEvent_t> cl_events;     // one per stream, and the last one for the caller's stream
 };
+
+constexpr int kClusterStreams = 8;          // seven clusters of 16 CTAs are resident at a time on a B200
 
 namespace {
 
@@ -98,6 +113,10 @@ int check(wolff_batch_ctx *b)
 
 void free_all(wolff_batch_ctx *b)
 {
+    cudaFree(b->cl_ctl); cudaFree(b->cl_spill); cudaFree(b->cl_ctr); cudaFree(b->cl_ns);
+    for (cudaStream_t s : b->cl_streams) cudaStreamDestroy(s);
+    for (cudaEvent_t e : b->cl_events) cudaEventDestroy(e);
+    b->cl_streams.clear(); b->cl_events.clear();
     cudaFree(b->spins); cudaFree(b->lists); cudaFree(b->sizes); cudaFree(b->E_log); cudaFree(b->M_log);
     cudaFree(b->keys); cudaFree(b->thr_dev); cudaFree(b->EM); cudaFree(b->moments); cudaFree(b->acc); cudaFree(b->stats);
 }
@@ -111,6 +130,93 @@ bool use_bits(const wolff_batch_ctx *b)
     const size_t all = batch_smem_bytes(b->geo.N, b->qcap, true, b->measure != 0);
     if (all + 1024 > b->smem_optin) return false;
     return b->resident == 2 || planes <= (32u << 10);
+}
+
+// resident = 3: plan and per-chain state of the cluster-resident kernel (once per handle)
+int prepare_clusters(wolff_batch_ctx *b)
+{
+    if (b->cl_ready) return WOLFF_OK;
+    if (!cluster_plan(b->dim, b->geo, 16, 2048, b->smem_optin, &b->cl, &b->cl_smem, nullptr)) {
+        set_error("resident = 3: a lattice of N = %llu spins does not fit one thread-block cluster (at most 2^24)", (unsigned long long)b->N);
+        return WOLFF_EINVAL;
+    }
+    const size_t R = b->R, cap = (size_t)1 << b->cl.spill_log;
+    if (cudaMalloc(&b->cl_ctl, R * sizeof(Control)) != cudaSuccess || cudaMalloc(&b->cl_spill, R * cap * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&b->cl_ctr, R * 2 * sizeof(unsigned long long)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(b->cl_ctl); cudaFree(b->cl_spill); cudaFree(b->cl_ctr);
+        b->cl_ctl = nullptr; b->cl_spill = nullptr; b->cl_ctr = nullptr;
+        set_error("resident = 3: cannot allocate the spill lists of %u chains", b->R);
+        return WOLFF_ENOMEM;
+    }
+    CHECK_CUDA(b, cudaMemset(b->cl_ctl, 0, R * sizeof(Control)), "clear control blocks");
+    CHECK_CUDA(b, cudaMemset(b->cl_spill, 0, R * cap * sizeof(uint32_t)), "clear spill lists");
+    CHECK_CUDA(b, cudaMemset(b->cl_ctr, 0, R * 2 * sizeof(unsigned long long)), "clear spill counters");
+    const int ns = (int)(b->R < (uint32_t)kClusterStreams ? b->R : (uint32_t)kClusterStreams);
+    for (int i = 0; i < ns; ++i) {
+        cudaStream_t s = nullptr;
+        CHECK_CUDA(b, cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking), "cudaStreamCreate");
+        b->cl_streams.push_back(s);
+    }
+    for (int i = 0; i <= ns; ++i) {
+        cudaEvent_t e = nullptr;
+        CHECK_CUDA(b, cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
+        b->cl_events.push_back(e);
+    }
+    b->cl.watchdog_ns = 20000ull * 1000000ull;
+    b->cl.idle_ns = 1000;
+    b->cl_ready = true;
+    return WOLFF_OK;
+}
+
+// resident = 3: every chain is one launch of the cluster-resident kernel (one cluster of up to 16 CTAs); the launches are
+// spread over a few streams, so that as many chains run side by side as clusters fit the chip (7 of 16 CTAs on a B200).
+// The streams start behind the caller's stream and the caller's stream continues behind them.
+int run_clusters(wolff_batch_ctx *b, uint64_t n_updates, cudaStream_t stream)
+{
+    int rc = prepare_clusters(b);
+    if (rc) return rc;
+    if (n_updates > (1ull << 30)) { set_error("resident = 3: at most 2^30 updates per call"); return WOLFF_EINVAL; }
+    if (n_updates > b->cl_ns_cap) {
+        uint32_t *fresh = nullptr;
+        if (cudaMalloc(&fresh, (size_t)b->R * (size_t)b->log_cap * sizeof(uint32_t)) != cudaSuccess) {
+            cudaGetLastError();
+            set_error("cannot allocate the per-update durations for %u chains", b->R);
+            return WOLFF_ENOMEM;
+        }
+        cudaFree(b->cl_ns);
+        b->cl_ns = fresh;
+        b->cl_ns_cap = b->log_cap;
+    }
+    // counters of the growth kernel start from zero at every launch; the error flags stay
+    CHECK_CUDA(b, cudaMemset2DAsync(b->cl_ctl, sizeof(Control), 0, kControlClearBytes, b->R, stream), "clear control blocks");
+    const size_t ns = b->cl_streams.size(), cap = (size_t)1 << b->cl.spill_log;
+    cudaEvent_t start = b->cl_events[ns];
+    CHECK_CUDA(b, cudaEventRecord(start, stream), "cudaEventRecord");
+    for (size_t i = 0; i < ns; ++i) CHECK_CUDA(b, cudaStreamWaitEvent(b->cl_streams[i], start, 0), "cudaStreamWaitEvent");
+    for (uint32_t r = 0; r < b->R; ++r) {
+        ClusterParams cp = b->cl;
+        GrowthParams &g = cp.g;
+        g.spins = b->spins + (size_t)r * b->stride;
+        g.clist = nullptr;
+        g.sizes = b->sizes + (size_t)r * (size_t)n_updates;
+        g.ctl = b->cl_ctl + r;
+        g.geo = b->geo;
+        g.key0 = (uint32_t)b->seed[r]; g.key1 = (uint32_t)(b->seed[r] >> 32);
+        g.thr = b->thr[r]; g.u0 = b->u; g.n_updates = n_updates;
+        g.measure = 0u; g.claim_bits = 0xFEu;
+        g.ns_log = b->cl_ns + (size_t)r * (size_t)n_updates;
+        cp.thr32 = (uint32_t)b->thr[r];
+        cp.thr_all = (b->thr[r] >> 32) != 0 ? 1u : 0u;
+        cp.spill = b->cl_spill + (size_t)r * cap;
+        cp.spill_ctr = b->cl_ctr + 2 * (size_t)r;
+        CHECK_CUDA(b, launch_growth_cluster(cp, b->dim, b->cl_smem, b->cl_streams[r % ns]), "launch cluster-resident growth kernel");
+    }
+    for (size_t i = 0; i < ns; ++i) {
+        CHECK_CUDA(b, cudaEventRecord(b->cl_events[i], b->cl_streams[i]), "cudaEventRecord");
+        CHECK_CUDA(b, cudaStreamWaitEvent(stream, b->cl_events[i], 0), "cudaStreamWaitEvent");
+    }
+    return WOLFF_OK;
 }
 
 // threads per CTA and CTAs of a launch: every chain resident at once when the chip can hold them
@@ -247,6 +353,18 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
         b->sizes = fresh; b->E_log = fresh_E; b->M_log = fresh_M;
         b->log_cap = cap;
     }
+    if (b->resident == 3) {
+        if (b->measure) { set_error("resident = 3 does not measure inside the kernel: use resident 0, 1 or 2 for a measured run"); return WOLFF_EINVAL; }
+        rc = run_clusters(b, n_updates, stream);
+        if (rc) return rc;
+        b->u += n_updates;
+        b->last_n = n_updates;
+        b->last_measured = false;
+        b->em_valid = false;
+        b->last_stream = stream;
+        b->ran = true;
+        return WOLFF_OK;
+    }
     if (b->measure && !b->em_valid)      // running E and M start from a whole-lattice evaluation of every chain
         CHECK_CUDA(b, launch_batch_energy(b->spins, b->stride, b->geo, b->dim, b->R, b->acc, b->EM, b->num_sms, stream), "launch batch E/M reduction");
     CHECK_CUDA(b, cudaMemsetAsync(b->stats, 0, 8 * sizeof(unsigned long long), stream), "cudaMemsetAsync(stats)");
@@ -351,7 +469,15 @@ int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value)
         if (value != 0 && value != 32 && value != 64 && value != 128 && value != 256) { set_error("threads must be 0 (auto), 32, 64, 128 or 256"); return WOLFF_EINVAL; }
         b->threads_opt = (int)value;
     } else if (!strcmp(key, "resident")) {
-        if (value < 0 || value > 2) { set_error("resident must be 0 (auto), 1 (int8 lattice in global memory) or 2 (bit-packed in shared memory)"); return WOLFF_EINVAL; }
+        if (value < 0 || value > 3) {
+            set_error("resident must be 0 (auto), 1 (int8 lattice in global memory), 2 (bit-packed in one CTA's shared memory) or 3 (bit-packed in one cluster's)");
+            return WOLFF_EINVAL;
+        }
+        if (value == 3) {
+            DeviceScope scope(b);
+            const int rc3 = prepare_clusters(b);
+            if (rc3) return rc3;
+        }
         if (value == 2 && batch_smem_bytes(b->geo.N, b->qcap, true, false) + 1024 > b->smem_optin) {
             set_error("resident = 2: a bit plane of N = %llu spins does not fit one CTA's shared memory", (unsigned long long)b->N);
             return WOLFF_EINVAL;
@@ -421,6 +547,22 @@ int wolff_batch_get_stats(wolff_batch b, uint64_t *stats)
     DeviceScope scope(b);
     if (!stats) { set_error("stats is NULL"); return WOLFF_EINVAL; }
     uint64_t host[8];
+    if (b->resident == 3 && b->cl_ready) {
+        // one control block per chain: sum the counters, look at the error flags
+        std::vector<Control> ctl(b->R);
+        CHECK_CUDA(b, cudaMemcpyAsync(ctl.data(), b->cl_ctl, (size_t)b->R * sizeof(Control), cudaMemcpyDeviceToHost, b->last_stream), "read control blocks");
+        CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+        memset(stats, 0, 4 * sizeof(uint64_t));
+        for (uint32_t r = 0; r < b->R; ++r) {
+            if (ctl[r].error != 0) {
+                set_error("chain %u: %s (error flag %u)", r, ctl[r].error >= 1000u ? "checked build: index out of bounds" : "device watchdog", ctl[r].error);
+                b->cuda_failed = true;
+                return WOLFF_EINTERNAL;
+            }
+            stats[0] += ctl[r].stats[0]; stats[1] += ctl[r].stats[1]; stats[3] += ctl[r].stats[7];
+        }
+        return WOLFF_OK;
+    }
     CHECK_CUDA(b, cudaMemcpyAsync(host, b->stats, sizeof(host), cudaMemcpyDeviceToHost, b->last_stream), "read stats");
     CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
     memcpy(stats, host, 4 * sizeof(uint64_t));

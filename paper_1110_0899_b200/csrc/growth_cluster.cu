@@ -646,6 +646,41 @@ cudaError_t dispatch(const ClusterParams &cp, int dim, bool pow2, size_t smem_by
 }
 }  // namespace
 
+// The launch shape for a lattice: the largest cluster (at most max_ctas CTAs) whose CTAs each hold a power-of-two number
+// of 32-bit words of the bit lattice, the ring and the stages in their shared memory.  false: the lattice does not fit
+// one cluster (more than 2^24 spins), or no such cluster can be resident.
+bool cluster_plan(int dim, const Geometry &geo, int max_ctas, uint32_t ring_cap, size_t smem_optin, ClusterParams *cp, size_t *smem_bytes,
+                  int *max_clusters)
+{
+    // sites are carried in 24 bits and divided by L and L^2 with 40-bit reciprocals: N <= 2^24, L^2 <= 2^16 in 3D
+    const uint64_t N = geo.N;
+    if (N > (1ull << 24) || (dim == 3 && (uint64_t)geo.L * geo.L > (1ull << 16))) return false;
+    const uint64_t words = (N + 31) / 32;
+    uint32_t nC = 16;
+    while (nC > 1 && (nC > (uint32_t)max_ctas || nC > words)) nC >>= 1;
+    uint32_t wpc = 1;
+    while ((uint64_t)wpc * nC < words) wpc <<= 1;
+    const size_t smem = cluster_smem_bytes(wpc, ring_cap);
+    if (smem + 1024 > smem_optin) return false;
+    int clusters = 0;
+    const cudaError_t e = cluster_prepare(dim, geo.pow2 != 0u, nC, smem, &clusters);
+    if (e != cudaSuccess || clusters < 1) { cudaGetLastError(); return false; }
+    *cp = ClusterParams{};
+    cp->nC = nC;
+    cp->wpc = wpc;
+    cp->wpc_log = 0;
+    while ((1u << cp->wpc_log) < wpc) ++cp->wpc_log;
+    cp->words = (uint32_t)words;
+    cp->magicL = ((1ull << 40) + (uint64_t)geo.L - 1) / (uint64_t)geo.L;
+    cp->magicLL = ((1ull << 40) + (uint64_t)geo.LL - 1) / (uint64_t)geo.LL;
+    cp->ring_cap = ring_cap;
+    cp->spill_log = 0;
+    while ((1ull << cp->spill_log) < N) ++cp->spill_log;
+    *smem_bytes = smem;
+    if (max_clusters) *max_clusters = clusters;
+    return true;
+}
+
 cudaError_t cluster_prepare(int dim, bool pow2, uint32_t nC, size_t smem_bytes, int *max_clusters)
 {
     ClusterParams cp{};

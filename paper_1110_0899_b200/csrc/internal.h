@@ -176,6 +176,9 @@ cudaError_t launch_growth_tiles(const TileParams &tp, int dim, size_t smem_bytes
 // cluster-resident kernel: shared memory needed, attributes + co-resident clusters, launch of one cluster of cp.nC CTAs
 size_t cluster_smem_bytes(uint32_t wpc, uint32_t ring_cap);
 cudaError_t cluster_prepare(int dim, bool pow2, uint32_t nC, size_t smem_bytes, int *max_clusters);
+// fills nC, wpc, wpc_log, words, magicL, magicLL, ring_cap, spill_log of *cp; false when the lattice does not fit one cluster
+bool cluster_plan(int dim, const Geometry &geo, int max_ctas, uint32_t ring_cap, size_t smem_optin, ClusterParams *cp, size_t *smem_bytes,
+                  int *max_clusters);
 cudaError_t launch_growth_cluster(const ClusterParams &cp, int dim, size_t smem_bytes, cudaStream_t stream);
 // batch of chains: CTAs of `threads` threads, `grid` of them; co-resident CTAs per SM; E, M of every chain into EM
 // bits: the bit-packed shared-memory-resident variant; its shared memory: the frontier buffers + N/8 bytes per plane

@@ -132,6 +132,45 @@ def test_medium_lattices_equilibrated_variant(resident):
     gpu.close()
 
 
+@pytest.mark.parametrize("dim,L,Tlo,Thi", [(2, 32, 1.8, 3.2), (3, 12, 3.8, 5.4), (2, 20, 2.0, 2.6), (3, 16, 4.2, 4.8)])
+def test_one_cluster_per_chain_sweep(dim, L, Tlo, Thi):
+    # "resident" = 3: every chain is grown by its own thread-block cluster (the cluster-resident bit-packed kernel), the
+    # launches side by side on the library's streams; 40 replicas with their own T and seed, L a power of two and not
+    R = 40
+    gpu, refs = make_batch(dim, L, sweep(R, Tlo, Thi), [2000 + 3 * r for r in range(R)], options={"resident": 3})
+    assert_same_lattices(gpu, refs, "start lattices (reading R9)")
+    compare(gpu, refs, [1, 40, 200])
+    st = gpu.stats()
+    assert st["updates"] == R * 200
+    gpu.set_option("measure", 1)
+    with pytest.raises(binding.WolffError):
+        gpu.run(1)                                   # this residency does not measure inside the kernel
+    gpu.set_option("measure", 0)
+    gpu.set_option("resident", 1)                    # the same chains continue on another kernel
+    compare(gpu, refs, [30])
+    gpu.close()
+
+
+def test_one_cluster_per_chain_full_size():
+    # C5a-sized chains at T_c from a cold start (clusters of 10^5 .. 10^7 spins, 16 CTAs per chain, 7 chains side by side)
+    # and p = 1 / p = 0 chains on a lattice that is not a power of two
+    import torch
+    c = wl.CONFIGS["C5a"]
+    R = 9
+    gpu, refs = make_batch(c.dim, c.L, [c.T] * R, [c.seed + r for r in range(R)], options={"resident": 3},
+                           start=np.stack([wl.cold(c.N)] * R))
+    gpu.run(3, stream=torch.cuda.Stream())
+    _, _, sz = gpu.observables(sizes=True)
+    for r, ref in enumerate(refs):
+        assert np.array_equal(sz[r], ref.run(3))
+    assert_same_lattices(gpu, refs, "C5a x 9")
+    gpu.close()
+    N = 100 * 100
+    gpu, refs = make_batch(2, 100, [0.04, 1.0, wl.TC_2D], [3, 4, 5], J=[1.0, 0.0, 1.0], options={"resident": 3}, start=np.stack([wl.cold(N)] * 3))
+    compare(gpu, refs, [1, 2, 10])
+    gpu.close()
+
+
 def test_split_runs_index_jumps_and_bad_input():
     R = 5
     T = sweep(R, 2.0, 2.6)
