@@ -109,7 +109,7 @@ def main(which):
             single_chain(*case)
             done.append("cluster %s" % (case[3],))
     if which in ("all", "batch"):
-        for measure, threads, resident in [(0, 32, 1), (1, 64, 1), (1, 256, 2), (0, 64, 2)]:
+        for measure, threads, resident in [(0, 32, 1), (1, 64, 1), (1, 256, 2), (0, 64, 2), (0, 64, 3)]:
             batch(measure, threads, resident)
             done.append("batch measure=%d threads=%d resident=%d" % (measure, threads, resident))
     for d in done:

@@ -20,7 +20,7 @@ def test_checked_build_runs_clean_on_the_stress_cases():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "tests", "sanitizer_cases.py")], env=env, capture_output=True, text=True,
                          timeout=900)
     assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-4000:]
-    assert "sanitizer cases passed: 20" in out.stdout
+    assert "sanitizer cases passed: 21" in out.stdout
 
 
 @pytest.mark.gpu
