@@ -102,11 +102,14 @@ WOLFF_API int wolff_set_update_index(wolff_handle h, uint64_t update_index);
  * without leaving the persistent kernel, logs them on the device, and adds them to exact integer accumulators:
  *   - shared-memory-resident kernel: after each update every CTA sums the tiles it holds (the low faces of the tiles are
  *     exchanged through global memory); cost per update independent of the cluster, a few microseconds;
+ *   - cluster-resident kernel (L a multiple of 32): after each update every CTA of the cluster counts the negative spins
+ *     and the unequal forward bonds of its slab of the bit lattice (32 spins per population count) and sends its sums to
+ *     CTA 0 in one reduction; cost per update independent of the cluster;
  *   - level-synchronous kernel: M changes by -2 s0 |C|; E by 2 * sum over the cluster's boundary bonds (member i,
  *     non-member j) of s0 s_j, counted in a pass over the update's member list while every member still carries a mark
  *     in bit 1 of its byte (the role of the flag the paper packs into the spin word); cost
  *     proportional to the cluster.
- * Both give exactly the values wolff_observables would return after each update.
+ * All give exactly the values wolff_observables would return after each update.
  *
  * wolff_get_series: the per-update series of the MOST RECENT wolff_run, n_updates entries each: E and M after each
  * update (needs "measure" = 1 during that run, else WOLFF_EINVAL) and the duration of each update in nanoseconds as
@@ -141,7 +144,9 @@ WOLFF_API int wolff_reset_moments(wolff_handle h);
  *                          grid-wide, 2 = one CTA whenever the frontier fits its shared-memory queue, 3 = the
  *                          cluster whenever it fits
  *   "measure"              1 = E and M after every update inside the kernel (see wolff_get_series); default 0.  The
- *                          cluster-resident kernel does not measure: a measured run uses one of the other two
+ *                          cluster-resident kernel measures when L is a multiple of 32 (population counts over its bit
+ *                          lattice after each update: cost independent of the cluster); otherwise, and for clusters of
+ *                          a handful of spins, a measured run uses one of the other two
  *   "small_cluster"        mode 0: when the last finished run (seen at the caller's next synchronising call) had a mean
  *                          cluster below this size, the next run uses the cluster-resident kernel (default: the measured
  *                          crossover, 8192 in 2D and 32768 in 3D; 0 = never); where that kernel does not apply, runs with a mean cluster below min(16, this) use
@@ -248,8 +253,8 @@ WOLFF_API int wolff_batch_set_update_index(wolff_batch b, uint64_t update_index)
  *   3 = bit-packed in the distributed shared memory of one thread-block cluster per chain (N <= 2^24: 2D L = 4096 and
  *   3D L = 256 are 2 MiB = 16 CTAs): every chain is one launch of the cluster-resident kernel of wolff_run, the launches
  *   spread over the library's own streams (behind the caller's stream, which continues behind them), so that as many
- *   chains run side by side as clusters fit the chip (7 of 16 CTAs on a B200); no in-kernel measurement (a measured run
- *   returns WOLFF_EINVAL), at most 2^30 updates per call;
+ *   chains run side by side as clusters fit the chip (7 of 16 CTAs on a B200); in-kernel measurement when L is a multiple
+ *   of 32 (else a measured run returns WOLFF_EINVAL); at most 2^30 updates per call;
  *   0 = auto: 2 when a plane is at most 32 KiB (several chains per SM stay in flight), else 1.  Never changes a result. */
 WOLFF_API int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value);
 /* E and M after every update of the most recent (measured) run: R * n_updates values each. */

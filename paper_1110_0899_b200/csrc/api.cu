@@ -509,13 +509,16 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     }
     // kernel choice in mode 0, by the mean cluster of the last finished run: below "small_cluster" spins the
     // cluster-resident kernel (its update costs what its few passes cost: no cooperative grid, no messages, no poll over
-    // 148 CTAs), above it the shared-memory-resident kernel of all SMs; where the cluster-resident kernel does not apply
-    // (L not a power of two, in-kernel measurement) clusters of a handful of spins go to the level-synchronous kernel
+    // 148 CTAs), above it the shared-memory-resident kernel of all SMs; measured runs on clusters of a handful of spins go
+    // to the level-synchronous kernel
     const bool small = h->small_cluster > 0 && h->have_mean && h->mean_cluster < (double)h->small_cluster;
     const bool tiny = small && h->mean_cluster < 16.0;
     bool clustered = false;
     // (a lattice the kernel of all SMs does not apply to -- L not a power of two -- runs here whatever its clusters)
-    if ((h->mode == 5 || (h->mode == 0 && (small || !h->plan_ok))) && !h->measure) {
+    // (it measures inside the kernel when L is a multiple of 32; below 16 spins per cluster a measured run is cheaper on
+    // the level-synchronous kernel, whose measurement costs what the cluster costs, not what the lattice costs)
+    const bool cl_measures = h->L % 32 == 0;
+    if ((h->mode == 5 || (h->mode == 0 && (small || !h->plan_ok) && !(h->measure && tiny))) && (!h->measure || cl_measures)) {
         rc = refresh_cluster_plan(h, stream);
         if (rc) return rc;
         clustered = h->cl_ok;
@@ -530,6 +533,9 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
             cp.g.n_updates = n_updates - done < chunk ? n_updates - done : chunk;
             cp.g.sizes = h->sizes + done;
             cp.g.ns_log = h->ns_log + done;
+            cp.g.E_log = h->E_log + done;
+            cp.g.M_log = h->M_log + done;
+            if (h->measure && cp.idle_ns > 200u) cp.idle_ns = 200u;     // every warp of the cluster is waited for after each update
             const cudaError_t e = launch_growth_cluster(cp, h->dim, h->cl_smem, stream);
             if (e == cudaErrorLaunchOutOfResources || e == cudaErrorInvalidConfiguration || e == cudaErrorCooperativeLaunchTooLarge) {
                 cudaGetLastError();       // the SMs of one GPC cannot be had right now: not a fault of the handle

@@ -190,6 +190,10 @@ int run_clusters(wolff_batch_ctx *b, uint64_t n_updates, cudaStream_t stream)
     }
     // counters of the growth kernel start from zero at every launch; the error flags stay
     CHECK_CUDA(b, cudaMemset2DAsync(b->cl_ctl, sizeof(Control), 0, kControlClearBytes, b->R, stream), "clear control blocks");
+    const bool measure = b->measure != 0;
+    if (measure)      // the kernel accumulates into its control block: start from the batch's sums
+        CHECK_CUDA(b, cudaMemcpy2DAsync(&b->cl_ctl[0].moments, sizeof(Control), b->moments, 10 * sizeof(unsigned long long),
+                                        10 * sizeof(unsigned long long), b->R, cudaMemcpyDeviceToDevice, stream), "moments -> control blocks");
     const size_t ns = b->cl_streams.size(), cap = (size_t)1 << b->cl.spill_log;
     cudaEvent_t start = b->cl_events[ns];
     CHECK_CUDA(b, cudaEventRecord(start, stream), "cudaEventRecord");
@@ -204,8 +208,11 @@ int run_clusters(wolff_batch_ctx *b, uint64_t n_updates, cudaStream_t stream)
         g.geo = b->geo;
         g.key0 = (uint32_t)b->seed[r]; g.key1 = (uint32_t)(b->seed[r] >> 32);
         g.thr = b->thr[r]; g.u0 = b->u; g.n_updates = n_updates;
-        g.measure = 0u; g.claim_bits = 0xFEu;
+        g.measure = measure ? 1u : 0u; g.claim_bits = 0xFEu;
+        g.E_log = b->E_log + (size_t)r * (size_t)n_updates;
+        g.M_log = b->M_log + (size_t)r * (size_t)n_updates;
         g.ns_log = b->cl_ns + (size_t)r * (size_t)n_updates;
+        if (measure) cp.idle_ns = 200;
         cp.thr32 = (uint32_t)b->thr[r];
         cp.thr_all = (b->thr[r] >> 32) != 0 ? 1u : 0u;
         cp.spill = b->cl_spill + (size_t)r * cap;
@@ -215,6 +222,12 @@ int run_clusters(wolff_batch_ctx *b, uint64_t n_updates, cudaStream_t stream)
     for (size_t i = 0; i < ns; ++i) {
         CHECK_CUDA(b, cudaEventRecord(b->cl_events[i], b->cl_streams[i]), "cudaEventRecord");
         CHECK_CUDA(b, cudaStreamWaitEvent(stream, b->cl_events[i], 0), "cudaStreamWaitEvent");
+    }
+    if (measure) {
+        CHECK_CUDA(b, cudaMemcpy2DAsync(b->moments, 10 * sizeof(unsigned long long), &b->cl_ctl[0].moments, sizeof(Control),
+                                        10 * sizeof(unsigned long long), b->R, cudaMemcpyDeviceToDevice, stream), "control blocks -> moments");
+        CHECK_CUDA(b, cudaMemcpy2DAsync(b->EM, 2 * sizeof(long long), &b->cl_ctl[0].E, sizeof(Control), 2 * sizeof(long long), b->R,
+                                        cudaMemcpyDeviceToDevice, stream), "control blocks -> E, M");
     }
     return WOLFF_OK;
 }
@@ -354,13 +367,16 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
         b->log_cap = cap;
     }
     if (b->resident == 3) {
-        if (b->measure) { set_error("resident = 3 does not measure inside the kernel: use resident 0, 1 or 2 for a measured run"); return WOLFF_EINVAL; }
+        if (b->measure && b->L % 32 != 0) {
+            set_error("resident = 3 measures inside the kernel only when L is a multiple of 32 (L = %d): use resident 0, 1 or 2", b->L);
+            return WOLFF_EINVAL;
+        }
         rc = run_clusters(b, n_updates, stream);
         if (rc) return rc;
         b->u += n_updates;
         b->last_n = n_updates;
-        b->last_measured = false;
-        b->em_valid = false;
+        b->last_measured = b->measure != 0;
+        b->em_valid = b->measure != 0;
         b->last_stream = stream;
         b->ran = true;
         return WOLFF_OK;

@@ -36,6 +36,9 @@
 //
 // The int8 lattice in global memory stays the authoritative copy between launches: every CTA packs its slab of the
 // lattice in the prologue and unpacks it in the epilogue (N bytes each way per launch, by 16 SMs).
+//
+// "measure" = 1 (L a multiple of 32): E and M after EVERY update inside the kernel, by population counts over the bit
+// lattice (measure_slab), logged and accumulated as in the other kernels.
 #include <cooperative_groups.h>
 
 #include "expand.cuh"
@@ -121,7 +124,11 @@ struct alignas(16) CShared {
     unsigned int upd;                   // (krel << 1) | (seed spin is -1) of the running update, written by the monitor
     unsigned int stop;                  // the launch is over (or aborted)
     unsigned int watcher;               // 1 while some idle warp of this CTA holds the watch
-    unsigned int pad;
+    unsigned int meas_req;              // k + 1 once the monitor has asked for the measurement after update k ("measure" = 1)
+    // in-kernel measurement: this CTA's sums of one evaluation and the warps that have added theirs
+    unsigned int meas_un, meas_ng, meas_warps, pad;
+    // CTA 0 only: the cluster's sums of one evaluation, [CTAs arrived : 13 | negative spins : 25 | unequal bonds : 26]
+    unsigned long long meas_acc;
 };
 
 struct CTally {
@@ -183,6 +190,54 @@ __device__ __forceinline__ void hand_over(const ClusterParams &cp, uint32_t head
             st_relaxed_u32_g(cp.spill + ((uint32_t)pos & smask), (items[j] << 1) | spill_tag(pos, cp.spill_log));
         }
         if (lane == 0) tl.spills += n;
+    }
+}
+
+// ------------------------------------------------------------------------------------------ in-kernel measurement
+// "+ measurement": E and M of the whole lattice after an update, evaluated where the lattice is
+// -- one bit per spin in the cluster's shared memory -- without leaving the kernel: 32 spins per word, so
+//   #negative = popc(word),  #unequal bonds in direction d = popc(word ^ word of the +d neighbours)
+// (+x: the word shifted by one bit, its last bit from the next word of the row; +y, +z: the word L/32 or L^2/32 words
+// further on, wrapping; a word of another CTA's slab is read through its shared::cluster address).  Needs L to be a
+// multiple of 32 (the host checks).  Called by every warp of the cluster but the monitor, between two updates; the CTA's
+// last warp sends the CTA's sums and its arrival to CTA 0 in ONE remote reduction.
+template <int DIM>
+__device__ __noinline__ void measure_slab(const ClusterParams &cp, CShared &sh, uint32_t bits_s, unsigned int rank, unsigned int ptid, unsigned int P)
+{
+    const Geometry &g = cp.g.geo;
+    const uint32_t W = g.L >> 5, wmask = cp.wpc - 1u;
+    const uint32_t plane = g.L * W;                                   // words of one z-plane (of the lattice in 2D)
+    auto ldw = [&](uint32_t gw) { return cl_ld_u32(mapa(bits_s + ((gw & wmask) << 2), gw >> cp.wpc_log)); };
+    unsigned int un = 0, ng = 0;
+    for (uint32_t w = ptid; w < cp.wpc; w += P) {
+        const uint32_t gw = rank * cp.wpc + w;
+        if (gw >= cp.words) break;
+        const uint32_t word = lds_u32(bits_s + (w << 2));
+        const uint32_t row = gw / W, xw = gw - row * W;               // row = y + L z
+        const uint32_t z = DIM == 3 ? row / g.L : 0u, y = row - z * g.L;
+        const uint32_t wx = ldw(xw + 1u == W ? gw + 1u - W : gw + 1u);
+        const uint32_t wy = ldw(y + 1u == g.L ? gw + W - plane : gw + W);
+        ng += __popc(word);
+        un += __popc(word ^ ((word >> 1) | (wx << 31))) + __popc(word ^ wy);
+        if (DIM == 3) un += __popc(word ^ ldw(z + 1u == g.L ? gw + plane - cp.words : gw + plane));
+    }
+    un = __reduce_add_sync(kFullMask, un);
+    ng = __reduce_add_sync(kFullMask, ng);
+    if ((threadIdx.x & 31u) == 0u) {
+        if (un) atomicAdd(&sh.meas_un, un);
+        if (ng) atomicAdd(&sh.meas_ng, ng);
+        __threadfence_block();
+        if (atomicAdd(&sh.meas_warps, 1u) == P / 32u - 1u) {
+            // the last warp of this CTA: every other warp's sums are in (its fence preceded its count)
+            __threadfence_block();
+            const unsigned long long tun = *reinterpret_cast<volatile unsigned int *>(&sh.meas_un);
+            const unsigned long long tng = *reinterpret_cast<volatile unsigned int *>(&sh.meas_ng);
+            *reinterpret_cast<volatile unsigned int *>(&sh.meas_un) = 0u;
+            *reinterpret_cast<volatile unsigned int *>(&sh.meas_ng) = 0u;
+            *reinterpret_cast<volatile unsigned int *>(&sh.meas_warps) = 0u;
+            __threadfence_block();
+            cl_red_add64(mapa(smem_addr(&sh.meas_acc), 0u), tun | (tng << 26) | (1ull << 51));
+        }
     }
 }
 
@@ -321,16 +376,19 @@ __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh
     const uint32_t head_c = mapa(head_s, rank), ring_c = mapa(ring_s, rank), pc_c = mapa(smem_addr(&sh.pc), 0u);
     const uint32_t smask = (1u << cp.spill_log) - 1u;
     bool watcher = false;
-    unsigned int idle = 0;
+    unsigned int idle = 0, meas_done = 0;
+    // in-kernel measurement: every warp of the cluster but the monitor takes part
+    const unsigned int P = rank == 0u ? kCT - 32u : kCT, ptid = rank == 0u ? threadIdx.x - 32u : threadIdx.x;
     CWorker ws;
 
     for (;;) {
         // ---- take up to S sites: the own ring; as the CTA's watch also a peer's ring or the spill list
-        unsigned int n = 0, h = 0, stop = 0, src = rank;      // src: rank whose ring the sites come from, 32 = the spill list
+        unsigned int n = 0, h = 0, stop = 0, mreq = 0, src = rank;      // src: rank whose ring the sites come from, 32 = the spill list
         unsigned long long sp_pos = 0;
         if (lane == 0) {
             const unsigned long long ht = cl_ld_u64(head_c);
             stop = *reinterpret_cast<volatile unsigned int *>(&sh.stop);
+            mreq = *reinterpret_cast<volatile unsigned int *>(&sh.meas_req);
             h = (unsigned int)ht;
             const unsigned int t = (unsigned int)(ht >> 32);
             if (t != h) {
@@ -340,6 +398,12 @@ __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh
         }
         n = __shfl_sync(kFullMask, n, 0);
         if (n == 0u) {
+            mreq = __shfl_sync(kFullMask, mreq, 0);
+            if (mreq != meas_done) {                               // the update is over everywhere: measure (measure_slab)
+                measure_slab<DIM>(cp, sh, bits_s, rank, ptid, P);
+                meas_done = mreq;
+                continue;
+            }
             if (__shfl_sync(kFullMask, stop, 0)) break;            // launch over
             if (!watcher) {
                 unsigned int got = 0;
@@ -451,6 +515,10 @@ __device__ __forceinline__ void monitor_warp(const ClusterParams &cp, CShared &s
     unsigned int prev_claimed = 0;
     unsigned long long flipped = 0, polls_total = 0;
     bool aborted = false;
+    Moments mom;
+    long long lastE = 0, lastM = 0;
+    if (p.measure && lane == 0) mom.load(ctl->moments);
+    const uint32_t mreq_s = smem_addr(&sh.meas_req), macc_c = mapa(smem_addr(&sh.meas_acc), 0u);
     CWorker ws;
     ws.upd_s = smem_addr(&sh.upd);
     for (unsigned long long k = 0; k < p.n_updates && !aborted; ++k) {
@@ -508,7 +576,33 @@ __device__ __forceinline__ void monitor_warp(const ClusterParams &cp, CShared &s
             const unsigned long long dt = globaltimer_ns() - t0;
             p.ns_log[k] = dt > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)dt;
         }
+        if (p.measure && !aborted) {
+            // "+ measurement": every CTA evaluates its slab (measure_slab); the sums and the arrivals come back in one word
+            if (lane < cp.nC) cl_st_u32(mapa(mreq_s, lane), (unsigned int)k + 1u);
+            unsigned int bad = 0;
+            if (lane == 0) {
+                unsigned long long acc;
+                unsigned int polls = 0;
+                while (((acc = cl_ld_u64(macc_c)) >> 51) != (unsigned long long)cp.nC) {
+                    if ((++polls & 0x3FFu) == 0u) {
+                        if (ld_relaxed_u32(&ctl->error) != 0u) { bad = 1; break; }
+                        if (globaltimer_ns() - t0 > cp.watchdog_ns) { raise_abort(ctl, 6u); bad = 1; break; }
+                    }
+                }
+                if (!bad) {
+                    *reinterpret_cast<volatile unsigned long long *>(&sh.meas_acc) = 0ull;     // every CTA has arrived: nobody adds until the next request
+                    const long long un = (long long)(acc & ((1ull << 26) - 1ull)), ng = (long long)((acc >> 26) & ((1ull << 25) - 1ull));
+                    lastE = 2ll * un - (long long)DIM * (long long)p.geo.N;
+                    lastM = (long long)p.geo.N - 2ll * ng;
+                    p.E_log[k] = lastE;
+                    p.M_log[k] = lastM;
+                    mom.add(lastE, lastM);
+                }
+            }
+            if (__shfl_sync(kFullMask, bad, 0)) aborted = true;
+        }
     }
+    if (p.measure && lane == 0 && !aborted && p.n_updates > 0) { ctl->E = lastE; ctl->M = lastM; mom.store(ctl->moments); }
     // everybody leaves
     if (lane < cp.nC) cl_st_u32(mapa(stop_s, lane), 1u);
     if (lane == 0) {
@@ -541,6 +635,9 @@ __global__ void __launch_bounds__(kCT, 1) growth_cluster_kernel(const __grid_con
         sh.upd = 0u;
         sh.stop = dead ? 1u : 0u;
         sh.watcher = 0u;
+        sh.meas_req = 0u;
+        sh.meas_un = sh.meas_ng = sh.meas_warps = 0u;
+        sh.meas_acc = 0ull;
     }
     // ---- prologue: my slab of the lattice, one bit per spin (bit = 1: spin -1); word w of the lattice = sites 32 w ..
     // (the last word of the lattice may be partial and the last CTAs may hold fewer words than wpc, or none)

@@ -1,8 +1,8 @@
 """In-kernel measurement ("measure" = 1) against the oracle: E and M after EVERY update, bit-exact.
 
 PAPER.md:126, 138, 147 (the "+ measurement" columns) and Eq. 3.  The CUDA path evaluates E and M
-inside the persistent kernel (growth_tiles.cu: every CTA sums the tiles it holds; growth.cu: running values from the
-cluster's boundary bonds); the oracle sums the whole lattice after every update (oracle_run_logged) and accumulates the
+inside the persistent kernel (growth_tiles.cu: every CTA sums the tiles it holds; growth_cluster.cu: population counts over
+the bit lattice; growth.cu: running values from the cluster's boundary bonds); the oracle sums the whole lattice after every update (oracle_run_logged) and accumulates the
 moments by their definition (oracle_moments).  Everything is integer: tolerance none, except the Binder ratio, a
 double computed from identical integers on both sides (1e-12).
 """
@@ -45,7 +45,7 @@ MEASURE_MODES = [dict(o, measure=1) for o in MODES]
 
 
 @pytest.mark.parametrize("options", [{"mode": 0, "small_cluster": 0}, {"mode": 0}, {"mode": 4}, {"mode": 1},
-                                      {"mode": 0, "small_cluster": 0, "fill": 2, "tile_log": 4}])
+                                      {"mode": 0, "small_cluster": 0, "fill": 2, "tile_log": 4}, {"mode": 5}])
 def test_config_c1_measured_every_update(options):
     c = wl.CONFIGS["C1"]
     gpu, ref = make_pair(*c.create_args(), options=dict(options, measure=1))
@@ -79,7 +79,25 @@ def test_p_one_cold_start_measured(dim, L, options):
     gpu.close()
 
 
-@pytest.mark.parametrize("options", [{"mode": 0, "small_cluster": 0}, {"mode": 4}, {"mode": 3}, {"mode": 1}])
+@pytest.mark.parametrize("options", [{"mode": 5}, {"mode": 5, "resident_ctas": 2, "ring_cap": 32}, {"mode": 5, "resident_ctas": 1, "idle_ns": 0},
+                                      {"mode": 0, "small_cluster": 1 << 30}])
+@pytest.mark.parametrize("dim,L,T", [(2, 32, wl.TC_2D), (2, 96, 2.2), (3, 32, wl.TC_3D), (2, 128, 2.0), (3, 64, 4.4), (2, 160, wl.TC_2D)])
+def test_cluster_resident_kernel_measured(dim, L, T, options):
+    # the cluster-resident kernel measures by population counts over its bit lattice when L is a multiple of 32 (L a power of
+    # two and not; one word per row at L = 32); every spin in one cluster from a cold start, then ragged blobs
+    gpu, ref = make_pair(dim, L, 1.0, T, seed=90 + L, options=dict(options, measure=1))
+    acc = compare_measured(gpu, ref, [1, 2, 60])
+    gpu.set_spins(wl.cold(L ** dim)); ref.set_spins(wl.cold(L ** dim))
+    acc = compare_measured(gpu, ref, [1, 5], acc=acc)
+    gpu.set_spins(wl.blobs(dim, L, seed=5)); ref.set_spins(wl.blobs(dim, L, seed=5))
+    compare_measured(gpu, ref, [1] * 3 + [30], acc=acc)
+    st = gpu.stats()
+    if options["mode"] == 5:         # (mode 0 sends measured runs on clusters of a handful of spins to the level-synchronous kernel)
+        assert st["levels_cta"] + st["levels_cluster"] + st["levels_grid"] + st["fill_chunks"] + st["inline_passes"] == 0    # it was this kernel
+    gpu.close()
+
+
+@pytest.mark.parametrize("options", [{"mode": 0, "small_cluster": 0}, {"mode": 4}, {"mode": 3}, {"mode": 1}, {"mode": 5}])
 @pytest.mark.parametrize("name,n", [("C2", 150), ("C4", 100)])
 def test_medium_configs_measured(name, n, options):
     c = wl.CONFIGS[name]
@@ -108,7 +126,7 @@ def test_moments_run_on_across_runs_and_reset():
     gpu.close()
 
 
-@pytest.mark.parametrize("name,options", [("C5a", {}), ("C5a", {"mode": 4}), ("C3-stretch", {})])
+@pytest.mark.parametrize("name,options", [("C5a", {}), ("C5a", {"mode": 4}), ("C3-stretch", {}), ("C5a", {"mode": 5})])
 def test_protocol_stretch_measured_in_kernel(name, options):
     # the stretch of single updates of the protocol tests, as ONE measured launch: same E, M after every update
     job = farm.JOBS[name]
