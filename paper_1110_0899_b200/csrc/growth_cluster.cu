@@ -201,7 +201,7 @@ __device__ __forceinline__ void hand_over(const ClusterParams &cp, uint32_t head
 // further on, wrapping; a word of another CTA's slab is read through its shared::cluster address).  Needs L to be a
 // multiple of 32 (the host checks).  Called by every warp of the cluster but the monitor, between two updates; the CTA's
 // last warp sends the CTA's sums and its arrival to CTA 0 in ONE remote reduction.
-template <int DIM>
+template <int DIM, bool POW2>
 __device__ __noinline__ void measure_slab(const ClusterParams &cp, CShared &sh, uint32_t bits_s, unsigned int rank, unsigned int ptid, unsigned int P)
 {
     const Geometry &g = cp.g.geo;
@@ -213,8 +213,14 @@ __device__ __noinline__ void measure_slab(const ClusterParams &cp, CShared &sh, 
         const uint32_t gw = rank * cp.wpc + w;
         if (gw >= cp.words) break;
         const uint32_t word = lds_u32(bits_s + (w << 2));
-        const uint32_t row = gw / W, xw = gw - row * W;               // row = y + L z
-        const uint32_t z = DIM == 3 ? row / g.L : 0u, y = row - z * g.L;
+        uint32_t row, xw, y, z;                                       // row = y + L z
+        if (POW2) {
+            row = gw >> (g.logL - 5u); xw = gw & (W - 1u);
+            z = DIM == 3 ? row >> g.logL : 0u; y = row & (g.L - 1u);
+        } else {
+            row = gw / W; xw = gw - row * W;
+            z = DIM == 3 ? row / g.L : 0u; y = row - z * g.L;
+        }
         const uint32_t wx = ldw(xw + 1u == W ? gw + 1u - W : gw + 1u);
         const uint32_t wy = ldw(y + 1u == g.L ? gw + W - plane : gw + W);
         ng += __popc(word);
@@ -400,7 +406,7 @@ __device__ __forceinline__ void worker_warp(const ClusterParams &cp, CShared &sh
         if (n == 0u) {
             mreq = __shfl_sync(kFullMask, mreq, 0);
             if (mreq != meas_done) {                               // the update is over everywhere: measure (measure_slab)
-                measure_slab<DIM>(cp, sh, bits_s, rank, ptid, P);
+                measure_slab<DIM, POW2>(cp, sh, bits_s, rank, ptid, P);
                 meas_done = mreq;
                 continue;
             }
