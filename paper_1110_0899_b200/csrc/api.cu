@@ -518,7 +518,11 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     // (it measures inside the kernel when L is a multiple of 32; below 16 spins per cluster a measured run is cheaper on
     // the level-synchronous kernel, whose measurement costs what the cluster costs, not what the lattice costs)
     const bool cl_measures = h->L % 32 == 0;
-    if ((h->mode == 5 || (h->mode == 0 && (small || !h->plan_ok) && !(h->measure && tiny))) && (!h->measure || cl_measures)) {
+    // (a launch of this kernel packs and unpacks the lattice with 16 SMs: 9 us + 50 us per 2^24 spins, against 11 us for a
+    // launch of the level-synchronous kernel and 32 us for the kernel of all SMs.  A call of a few updates on a large
+    // lattice -- the host loop run(1) + observables -- is therefore left to those two: fewer than N / 2^20 updates)
+    const bool brief = n_updates < (h->N >> 20) && (tiny || h->plan_ok);
+    if ((h->mode == 5 || (h->mode == 0 && (small || !h->plan_ok) && !(h->measure && tiny) && !brief)) && (!h->measure || cl_measures)) {
         rc = refresh_cluster_plan(h, stream);
         if (rc) return rc;
         clustered = h->cl_ok;
@@ -548,7 +552,7 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
         rc = refresh_plan(h, stream);
         if (rc) return rc;
     }
-    bool tiled = !clustered && (h->mode == 0 || h->mode == 5) && h->plan_ok && !tiny;
+    bool tiled = !clustered && (h->mode == 0 || h->mode == 5) && h->plan_ok && !tiny;      // (tiny: the level-synchronous kernel)
     if (tiled) {
         // shared-memory-resident kernel; a message carries the update index relative to the launch in 29 bits
         const uint64_t chunk = (1ull << 29) - 1;

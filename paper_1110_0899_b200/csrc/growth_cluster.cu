@@ -648,18 +648,29 @@ __global__ void __launch_bounds__(kCT, 1) growth_cluster_kernel(const __grid_con
     // ---- prologue: my slab of the lattice, one bit per spin (bit = 1: spin -1); word w of the lattice = sites 32 w ..
     // (the last word of the lattice may be partial and the last CTAs may hold fewer words than wpc, or none)
     const uint4 *const src = reinterpret_cast<const uint4 *>(p.spins);
-    for (uint32_t w = tid; w < cp.wpc; w += kCT) {
-        const uint32_t gw = rank * cp.wpc + w, first = gw * 32u;
-        uint32_t v = 0u;
-        if (gw < cp.words) {
-            if (first + 32u <= p.geo.N) {
-                const uint4 lo = __ldcg(src + 2u * (size_t)gw), hi = __ldcg(src + 2u * (size_t)gw + 1u);
-                v = pack16(lo) | (pack16(hi) << 16);
-            } else {
-                for (uint32_t i = first; i < p.geo.N; ++i) v |= (p.spins[i] < 0 ? 1u : 0u) << (i - first);
+    {
+        // four words (eight 16-byte loads) in flight per thread: the slab is a megabyte per SM, and what the copy waits for
+        // is the latency of L2 / HBM, not their bandwidth
+        constexpr uint32_t U = 4;
+        for (uint32_t w0 = tid; w0 < cp.wpc; w0 += kCT * U) {
+            uint4 lo[U], hi[U];
+            bool full[U];
+#pragma unroll
+            for (uint32_t u = 0; u < U; ++u) {
+                const uint32_t w = w0 + u * kCT, gw = rank * cp.wpc + w;
+                full[u] = w < cp.wpc && gw < cp.words && gw * 32u + 32u <= p.geo.N;
+                if (full[u]) { lo[u] = __ldcg(src + 2u * (size_t)gw); hi[u] = __ldcg(src + 2u * (size_t)gw + 1u); }
+            }
+#pragma unroll
+            for (uint32_t u = 0; u < U; ++u) {
+                const uint32_t w = w0 + u * kCT, gw = rank * cp.wpc + w, first = gw * 32u;
+                if (w >= cp.wpc) continue;
+                uint32_t v = 0u;
+                if (full[u]) v = pack16(lo[u]) | (pack16(hi[u]) << 16);
+                else if (gw < cp.words) for (uint32_t i = first; i < p.geo.N; ++i) v |= (p.spins[i] < 0 ? 1u : 0u) << (i - first);
+                bits[w] = v;
             }
         }
-        bits[w] = v;
     }
     cluster.sync();                  // every CTA's shared memory is initialised before a peer touches it
 
