@@ -149,7 +149,9 @@ WOLFF_API int wolff_reset_moments(wolff_handle h);
  *                          a handful of spins, a measured run uses one of the other two
  *   "small_cluster"        mode 0: when the last finished run (seen at the caller's next synchronising call) had a mean
  *                          cluster below this size, the next run uses the cluster-resident kernel (default: the measured
- *                          crossover, 8192 in 2D and 32768 in 3D; 0 = never); where that kernel does not apply, runs with a mean cluster below min(16, this) use
+ *                          crossover, 8192 in 2D and 32768 in 3D; 0 = never) -- unless the call is for fewer than N / 2^20
+ *                          updates, which the launch of that kernel (it packs the lattice with 16 SMs) would dominate;
+ *                          where that kernel does not apply, runs with a mean cluster below min(16, this) use
  *                          the level-synchronous kernel, whose fixed cost per update is lower than the first kernel's
  *   "resident_ctas"        cluster-resident kernel: CTAs of the cluster, at most (1, 2, 4, 8 or 16; default 16)
  *   "tile_log"             shared-memory-resident kernel: log2 of the tile side (0 = auto: 6 in 2D, 4 in 3D)
