@@ -135,6 +135,48 @@ def test_neighbours_brute_force(dim, L):
     assert set(edge_cover.values()) == {2}
 
 
+# ------------------------------------------------------------------ bond variable layout (readings R6, R10)
+
+def test_bond_layout_recomputed_from_the_philox_block():
+    """oracle.bond_active is word d of Philox(key = seed, ctr = (owner_lo, BOND << 30 | owner_hi, u_lo, u_hi)) < thr: the block
+    is recomputed here from the documented layout (R10) with the known-answer-pinned Philox, for seeds with a high
+    word, update indices beyond 2^32 and owners up to 2^31 - 1.  A bond stream that ignored u, the seed's high word, the
+    direction or the domain tag fails here."""
+    rng = np.random.default_rng(20260611)
+    for _ in range(400):
+        seed = int(rng.integers(0, 1 << 63)) * 2 + int(rng.integers(0, 2))
+        u = int(rng.integers(0, 1 << 40)) + (int(rng.integers(0, 2)) << 45)
+        owner = int(rng.integers(0, 1 << 31))
+        d = int(rng.integers(0, 3))
+        thr = int(rng.integers(0, (1 << 32) + 1))
+        x = oracle.philox4x32_10([owner & 0xFFFFFFFF, (0 << 30) | (owner >> 32), u & 0xFFFFFFFF, u >> 32],
+                                 [seed & 0xFFFFFFFF, seed >> 32])
+        assert oracle.bond_active(seed, u, owner, d, thr) == (x[d] < thr)
+        # the same counter in the SITE / INIT domains is another block: the three streams are disjoint
+        assert x != oracle.philox4x32_10([owner & 0xFFFFFFFF, 1 << 30, u & 0xFFFFFFFF, u >> 32], [seed & 0xFFFFFFFF, seed >> 32])
+    # thr = 0: no bond; thr = 2^32: every bond
+    assert not any(oracle.bond_active(5, 9, o, d, 0) for o in range(200) for d in range(3))
+    assert all(oracle.bond_active(5, 9, o, d, 1 << 32) for o in range(200) for d in range(3))
+
+
+def test_bond_stream_depends_on_update_seed_and_direction_and_has_the_right_density():
+    thr = oracle.threshold(1.0, wl.TC_2D)
+    p = thr / 2.0 ** 32
+    n = 10_000
+    base = np.array([oracle.bond_active(77, 3, o, 0, thr) for o in range(n)])
+    sd_diff = (n * 2 * p * (1 - p) * (1 - 2 * p * (1 - p))) ** 0.5      # two independent streams differ with prob. 2 p (1 - p)
+    for other in (np.array([oracle.bond_active(77, 4, o, 0, thr) for o in range(n)]),                    # next update
+                  np.array([oracle.bond_active(77, 3 + (1 << 32), o, 0, thr) for o in range(n)]),        # high word of u
+                  np.array([oracle.bond_active(77 + (1 << 32), 3, o, 0, thr) for o in range(n)]),        # high word of the seed
+                  np.array([oracle.bond_active(77, 3, o, 1, thr) for o in range(n)])):                   # other direction
+        assert abs(int((base != other).sum()) - n * 2 * p * (1 - p)) < 5 * sd_diff
+    # active fraction over 10^5 edges = thr / 2^32 within 4 sigma (PAPER.md:120: p = 1 - exp(-2 J / T))
+    m = 100_000
+    act = sum(oracle.bond_active(123456789, 11, o % 50_000, o // 50_000, thr) for o in range(m))
+    assert abs(act - m * p) < 4 * (m * p * (1 - p)) ** 0.5
+    assert abs(p - (1 - np.exp(-2 / wl.TC_2D))) < 1e-9
+
+
 # ------------------------------------------------------------------ start lattice (reading R9)
 
 def test_start_lattice_bits_and_balance():
