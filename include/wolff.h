@@ -269,6 +269,42 @@ WOLFF_API int wolff_batch_reset_moments(wolff_batch b);
 WOLFF_API int wolff_batch_get_stats(wolff_batch b, uint64_t *stats);
 WOLFF_API int wolff_batch_destroy(wolff_batch b);
 
+/* ------------------------------------------------------------------------------------------------------------------
+ * E and M without any allocation, for callers that cannot let a library allocate on the device.
+ *
+ * Everything above works on a handle, and making a handle calls cudaMalloc.  Some host programs cannot afford that: a
+ * simulation that gave the whole card to its own arena at start-up (cudaMalloc then finds nothing); a service that
+ * must stay inside a fixed memory budget once it is initialised; a program with a latency-critical loop on other
+ * streams of the device, which cudaMalloc / cudaFree stall while they run.  For them this one call computes, from a
+ * lattice that lives in THEIR device memory, the same two integers wolff_observables returns: E = - sum over bonds
+ * s_i s_j (each bond once, units of J, periodic; Eq. 2) and M = sum s_i ("measurement of energy and
+ * magnetization").  It calls no cudaMalloc, cudaFree or other allocating routine, and makes no staging
+ * copies.
+ *
+ *   spins_dev   the lattice: N = L^dim bytes, +1 / -1, x fastest, in memory of the CURRENT device (or managed memory);
+ *               16-byte aligned when L is a multiple of 16.  Read only; the bytes are not validated.
+ *   dim, L      2 or 3; L >= 2; N <= WOLFF_NOALLOC_MAX_SITES (2^28: 2D up to L = 16384, 3D up to L = 645) -- larger
+ *               lattices are refused with WOLFF_EINVAL, because the scratch memory is fixed in size
+ *   E_dev, M_dev  one int64 each, in memory of the current device, managed memory or pinned host memory; either may be
+ *               NULL.  Caller-owned, written by the kernel.
+ *   cuda_stream a cudaStream_t passed as void* (NULL = the legacy default stream).  The call enqueues a 256-byte
+ *               memset and one kernel there and returns without waiting: the results are in E_dev / M_dev once the
+ *               stream has reached that point.
+ *
+ * Scratch memory: the partial sums of the reduction (one 16-byte slot per 16,384 sites) and a ticket live in a
+ * file-scope __device__ array of 256.25 KiB inside the library image; every GPU on which the library is loaded holds
+ * that much from load until the process exits.  All calls of a process share it, and it keeps what the last call left:
+ * the ticket is cleared on the stream in front of every launch, the slots are overwritten before they are read.  Two
+ * calls whose kernels can OVERLAP on the GPU (different streams without an ordering between them, or several host
+ * threads) race on it and give wrong sums; calls on one stream, or ordered by events, are fine.
+ * The FIRST call on each device looks the array's device address up (cudaGetSymbolAddress, with that device current)
+ * and keeps it; make that first call before any stream capture begins on the thread.
+ * Errors: WOLFF_EINVAL (dim, L, size beyond the limit, NULL / misaligned / host / other-device pointers),
+ * WOLFF_ECUDA (the lookup, the memset or the launch failed); the text is in wolff_last_error(). */
+#define WOLFF_NOALLOC_MAX_SITES (1u << 28)
+WOLFF_API int wolff_energy_magnetisation_noalloc(const int8_t *spins_dev, int dim, int L, int64_t *E_dev, int64_t *M_dev,
+                                                 void *cuda_stream);
+
 /* Reason for the last failure on this thread (static storage, never NULL). */
 WOLFF_API const char *wolff_last_error(void);
 

@@ -52,8 +52,11 @@ _SIGNATURES = {
     "wolff_batch_reset_moments": (ctypes.c_int, [ctypes.c_void_p]),
     "wolff_batch_get_stats": (ctypes.c_int, [ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]),
     "wolff_batch_destroy": (ctypes.c_int, [ctypes.c_void_p]),
+    "wolff_energy_magnetisation_noalloc": (ctypes.c_int, [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_void_p,
+                                                         ctypes.c_void_p, ctypes.c_void_p]),
     "wolff_last_error": (ctypes.c_char_p, []),
 }
+NOALLOC_MAX_SITES = 1 << 28
 
 _lock = threading.Lock()
 _lib = None
@@ -119,6 +122,18 @@ def microbench() -> dict:
     if rc != WOLFF_OK:
         raise WolffError(rc, "wolff_microbench failed")
     return dict(zip(MICRO_NAMES, (float(x) for x in buf)))
+
+
+def energy_magnetisation_noalloc(spins, dim: int, L: int, E_out=None, M_out=None, stream=None):
+    """wolff_energy_magnetisation_noalloc: E and M of a lattice the caller already holds on the current device, for
+    programs that cannot let the library allocate there (the card belongs to their own arena, their memory budget is
+    fixed after start-up, or a cudaMalloc would stall their other streams).  `spins`: device tensor (or address) of
+    L**dim int8 values +1 / -1; `E_out`, `M_out`: one int64 each in device, managed or pinned host memory, either may be
+    None.  Nothing is allocated and nothing is waited for: the values are there once `stream` has run the kernel.  At
+    most NOALLOC_MAX_SITES sites; calls that can overlap on the GPU race on the shared scratch memory (see wolff.h)."""
+    rc = load().wolff_energy_magnetisation_noalloc(_ptr(spins), int(dim), int(L), _ptr(E_out), _ptr(M_out), _stream_handle(stream))
+    if rc != WOLFF_OK:
+        raise WolffError(rc, last_error())
 
 
 class Wolff:

@@ -13,7 +13,7 @@ LIB_NAME = "libwolff_b200.so"
 LIB_PATH = os.path.join(HERE, LIB_NAME)
 CHECKED_LIB_PATH = os.path.join(HERE, "libwolff_b200_checked.so")
 JITTER_LIB_PATH = os.path.join(HERE, "libwolff_b200_jitter.so")
-SOURCES = ["api.cu", "batch_api.cu", "growth.cu", "growth_batch.cu", "growth_cluster.cu", "growth_tiles.cu", "measure.cu", "microbench.cu"]
+SOURCES = ["api.cu", "batch_api.cu", "growth.cu", "growth_batch.cu", "growth_cluster.cu", "growth_tiles.cu", "measure.cu", "microbench.cu", "noalloc.cu"]
 HEADERS = ["internal.h", "device_common.cuh", "expand.cuh", os.path.join(ROOT, "include", "wolff.h")]
 NVCC_COMPILE_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",
