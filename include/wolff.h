@@ -30,7 +30,9 @@
  *     aborted one do nothing, and the next synchronising call returns WOLFF_EINTERNAL.
  *   - Calls make the handle's device current for their own duration and restore the
  *     caller's current device before they return.
- *   - A handle is not thread-safe; distinct handles are independent.
+ *   - A handle is not thread-safe; distinct handles are independent, also when different host threads drive handles
+ *     of different lattice sizes: the one piece of per-process kernel state, the dynamic shared-memory limit of each
+ *     kernel, is only ever set to a single value (the device's maximum), never to a handle's own need.
  *   - There is no CPU fallback: without a usable CUDA device wolff_create fails.
  */
 #ifndef WOLFF_B200_H
@@ -81,16 +83,20 @@ WOLFF_API int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream);
  * pointers may be NULL; each may be host or device memory.  Blocks until done. */
 WOLFF_API int wolff_observables(wolff_handle h, int64_t *E, int64_t *M, uint32_t *cluster_sizes);
 
-/* Copy the lattice (N bytes, +1/-1, x fastest) to dst (host or device).  Blocks. */
+/* Copy the lattice (N bytes, +1/-1, x fastest) to dst (host or device).  Blocks.  The spins S_i = +/-1 of PAPER.md:36-40
+ * (Eq. 2), one int8 each (the paper packs spin and in-cluster flag into one word; here
+ * the flip itself is the claim, so the byte is the spin and nothing else). */
 WOLFF_API int wolff_get_spins(wolff_handle h, int8_t *dst);
 
-/* Load a lattice (N bytes, each +1 or -1; host or device).  Used for cold starts, crafted
+/* Load a lattice (N bytes, each +1 or -1; host or device).  Used for cold starts (the
+ * "equilibrated" benchmark variant; PAPER.md:126 measures at T_c), crafted
  * cases and resuming.  Values other than +/-1 give WOLFF_EINVAL and leave the lattice
  * unchanged.  Blocks. */
 WOLFF_API int wolff_set_spins(wolff_handle h, const int8_t *src);
 
-/* Update index (number of updates done since creation, or as set) and the integer bond
- * threshold in [0, 2^32].  Either pointer may be NULL (host pointers). */
+/* Update index (number of updates done since creation, or as set: the count of step (v) of
+ * PAPER.md:48, which keys the site draw and the bond variables, R8/R10) and the integer bond
+ * threshold in [0, 2^32] (p = 1 - exp(-2J/T); R7).  Either pointer may be NULL (host pointers). */
 WOLFF_API int wolff_get_state(wolff_handle h, uint64_t *update_index, uint64_t *threshold);
 
 /* Set the update index (to resume a chain: lattice + index + seed is the whole state). */
@@ -218,7 +224,7 @@ WOLFF_API int wolff_get_stats(wolff_handle h, uint64_t *stats);
 #define WOLFF_NMICRO 13
 WOLFF_API int wolff_microbench(double *out_ns, int n_out);
 
-/* Free everything.  NULL is allowed. */
+/* Free everything wolff_create allocated (lattice, cluster list of PAPER.md:50, control block, logs).  NULL is allowed. */
 WOLFF_API int wolff_destroy(wolff_handle h);
 
 /* ------------------------------------------------------------------------------------------------------------------
@@ -257,7 +263,12 @@ WOLFF_API int wolff_batch_set_update_index(wolff_batch b, uint64_t update_index)
  *   spread over the library's own streams (behind the caller's stream, which continues behind them), so that as many
  *   chains run side by side as clusters fit the chip (7 of 16 CTAs on a B200); in-kernel measurement when L is a multiple
  *   of 32 (else a measured run returns WOLFF_EINVAL); at most 2^30 updates per call;
- *   0 = auto: 2 when a plane is at most 32 KiB (several chains per SM stay in flight), else 1.  Never changes a result. */
+ *   0 = auto: 2 when a plane is at most 32 KiB (several chains per SM stay in flight), else 1.  Never changes a result.
+ * "watchdog_ms" ("resident" = 3): an update that takes longer aborts its chain's launch (default 20000).
+ * A chain whose kernel aborted (watchdog; an out-of-bounds index in a checked build) is reported like a single chain's:
+ * EVERY synchronising batch call (observables, get/set_spins, get_series, get/reset_moments, get_stats) looks at the
+ * chains' error words after it has waited, returns WOLFF_EINTERNAL naming the first such chain, and the batch stays
+ * failed (its lattices, logs and moments are then unfinished). */
 WOLFF_API int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value);
 /* E and M after every update of the most recent (measured) run: R * n_updates values each. */
 WOLFF_API int wolff_batch_get_series(wolff_batch b, int64_t *E_series, int64_t *M_series);
@@ -305,7 +316,8 @@ WOLFF_API int wolff_batch_destroy(wolff_batch b);
 WOLFF_API int wolff_energy_magnetisation_noalloc(const int8_t *spins_dev, int dim, int L, int64_t *E_dev, int64_t *M_dev,
                                                  void *cuda_stream);
 
-/* Reason for the last failure on this thread (static storage, never NULL). */
+/* Reason for the last failure on this thread (static storage, never NULL).  Not part of the method: the error
+ * behaviour of the boundary ("Conventions" above). */
 WOLFF_API const char *wolff_last_error(void);
 
 #ifdef __cplusplus

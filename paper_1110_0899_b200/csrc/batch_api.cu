@@ -59,6 +59,7 @@ struct wolff_batch_ctx {
                                     // 3 one thread-block cluster per chain (growth_cluster.cu), chains side by side on streams
     size_t smem_optin = 0;
     uint32_t qcap = 1024;
+    uint64_t watchdog_ms = 20000;   // resident = 3: an update that takes longer aborts its chain's launch
     // resident = 3: the launch shape of the cluster-resident kernel and, per chain, a control block, a spill list and its
     // two counters; the per-update durations the kernel records; the streams the chains' launches are spread over
     bool cl_ready = false;
@@ -108,6 +109,38 @@ int check(wolff_batch_ctx *b)
 {
     if (!b) { set_error("null batch handle"); return WOLFF_EINVAL; }
     if (b->cuda_failed) { set_error("batch handle is in a failed CUDA state"); return WOLFF_ECUDA; }
+    return WOLFF_OK;
+}
+
+// Every synchronising batch call ends here: wait for the stream, then look at what the kernels reported on the device.
+// resident = 3: each chain's control block has a sticky error word (watchdog codes, 1000 + code in checked builds);
+// the other kernels report through stats[7] (checked builds only).  An aborted chain has a half-grown cluster and
+// unfinished logs, so the handle is marked failed, as a single chain's is (wolff.h: WOLFF_EINTERNAL).
+int sync_and_check(wolff_batch_ctx *b)
+{
+    cudaStream_t s = b->last_stream;
+    if (b->cl_ready && b->ran) {
+        std::vector<unsigned int> err(b->R);
+        CHECK_CUDA(b, cudaMemcpy2DAsync(err.data(), sizeof(unsigned int), &b->cl_ctl[0].error, sizeof(Control), sizeof(unsigned int), b->R,
+                                        cudaMemcpyDeviceToHost, s), "read the chains' error words");
+        CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+        for (uint32_t r = 0; r < b->R; ++r) {
+            if (err[r] == 0u) continue;
+            if (err[r] >= 1000u) set_error("chain %u: checked build: index out of bounds in the cluster-resident kernel (code %u)", r, err[r] - 1000u);
+            else set_error("chain %u: device watchdog: an update did not complete (error flag %u)", r, err[r]);
+            b->cuda_failed = true;
+            return WOLFF_EINTERNAL;
+        }
+        return WOLFF_OK;
+    }
+    unsigned long long flag = 0;
+    CHECK_CUDA(b, cudaMemcpyAsync(&flag, b->stats + 7, sizeof(flag), cudaMemcpyDeviceToHost, s), "read the batch kernel's check word");
+    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    if (flag != 0) {
+        set_error("checked build: index out of bounds in the batch kernel (code %llu)", flag);
+        b->cuda_failed = true;
+        return WOLFF_EINTERNAL;
+    }
     return WOLFF_OK;
 }
 
@@ -163,7 +196,7 @@ int prepare_clusters(wolff_batch_ctx *b)
         CHECK_CUDA(b, cudaEventCreateWithFlags(&e, cudaEventDisableTiming), "cudaEventCreate");
         b->cl_events.push_back(e);
     }
-    b->cl.watchdog_ns = 20000ull * 1000000ull;
+    b->cl.watchdog_ns = b->watchdog_ms * 1000000ull;
     b->cl.idle_ns = 1000;
     b->cl_ready = true;
     return WOLFF_OK;
@@ -419,8 +452,7 @@ int wolff_batch_observables(wolff_batch b, int64_t *E, int64_t *M, uint32_t *clu
     }
     if (cluster_sizes && b->ran && b->last_n > 0)
         CHECK_CUDA(b, cudaMemcpyAsync(cluster_sizes, b->sizes, R * (size_t)b->last_n * sizeof(uint32_t), cudaMemcpyDefault, s), "copy cluster sizes");
-    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
-    return WOLFF_OK;
+    return sync_and_check(b);
 }
 
 int wolff_batch_get_spins(wolff_batch b, int8_t *dst)
@@ -431,8 +463,7 @@ int wolff_batch_get_spins(wolff_batch b, int8_t *dst)
     if (!dst) { set_error("dst is NULL"); return WOLFF_EINVAL; }
     cudaStream_t s = b->last_stream;
     CHECK_CUDA(b, cudaMemcpy2DAsync(dst, (size_t)b->N, b->spins, b->stride, (size_t)b->N, b->R, cudaMemcpyDefault, s), "copy lattices out");
-    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
-    return WOLFF_OK;
+    return sync_and_check(b);
 }
 
 int wolff_batch_set_spins(wolff_batch b, const int8_t *src)
@@ -442,7 +473,8 @@ int wolff_batch_set_spins(wolff_batch b, const int8_t *src)
     DeviceScope scope(b);
     if (!src) { set_error("src is NULL"); return WOLFF_EINVAL; }
     cudaStream_t s = b->last_stream;
-    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
+    rc = sync_and_check(b);
+    if (rc) return rc;
     // stage in the member lists (4 N bytes per chain, idle between runs), validate there, then commit
     int8_t *staging = reinterpret_cast<int8_t *>(b->lists);
     const size_t total = (size_t)b->R * (size_t)b->N;
@@ -499,6 +531,10 @@ int wolff_batch_set_option(wolff_batch b, const char *key, int64_t value)
             return WOLFF_EINVAL;
         }
         b->resident = (int)value;
+    } else if (!strcmp(key, "watchdog_ms")) {
+        if (value < 1 || value > 3600000) { set_error("watchdog_ms must be in [1, 3600000]"); return WOLFF_EINVAL; }
+        b->watchdog_ms = (uint64_t)value;
+        b->cl.watchdog_ns = b->watchdog_ms * 1000000ull;
     } else if (!strcmp(key, "queue_cap")) {
         if (value < 8 || value > 16384) { set_error("queue_cap must be in [8, 16384]"); return WOLFF_EINVAL; }
         b->qcap = (uint32_t)value;
@@ -522,8 +558,7 @@ int wolff_batch_get_series(wolff_batch b, int64_t *E_series, int64_t *M_series)
     const size_t bytes = (size_t)b->R * (size_t)b->last_n * sizeof(int64_t);
     if (E_series) CHECK_CUDA(b, cudaMemcpyAsync(E_series, b->E_log, bytes, cudaMemcpyDefault, s), "copy E series");
     if (M_series) CHECK_CUDA(b, cudaMemcpyAsync(M_series, b->M_log, bytes, cudaMemcpyDefault, s), "copy M series");
-    CHECK_CUDA(b, cudaStreamSynchronize(s), "cudaStreamSynchronize");
-    return WOLFF_OK;
+    return sync_and_check(b);
 }
 
 int wolff_batch_get_moments(wolff_batch b, uint64_t *moments, double *binder)
@@ -533,7 +568,8 @@ int wolff_batch_get_moments(wolff_batch b, uint64_t *moments, double *binder)
     DeviceScope scope(b);
     std::vector<uint64_t> host(10 * (size_t)b->R);
     CHECK_CUDA(b, cudaMemcpyAsync(host.data(), b->moments, host.size() * sizeof(uint64_t), cudaMemcpyDeviceToHost, b->last_stream), "read moments");
-    CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+    rc = sync_and_check(b);
+    if (rc) return rc;
     if (moments) memcpy(moments, host.data(), host.size() * sizeof(uint64_t));
     if (binder) {
         const long double two64 = 18446744073709551616.0L;
@@ -552,8 +588,7 @@ int wolff_batch_reset_moments(wolff_batch b)
     if (rc) return rc;
     DeviceScope scope(b);
     CHECK_CUDA(b, cudaMemsetAsync(b->moments, 0, 10 * (size_t)b->R * sizeof(unsigned long long), b->last_stream), "clear moments");
-    CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
-    return WOLFF_OK;
+    return sync_and_check(b);
 }
 
 int wolff_batch_get_stats(wolff_batch b, uint64_t *stats)

@@ -208,3 +208,35 @@ def test_full_size_literal_random_start_replicas():
     gpu, refs = make_batch(c.dim, c.L, [c.T] * R, [c.seed + r for r in range(R)])
     compare(gpu, refs, [1000])
     gpu.close()
+
+
+def test_one_cluster_per_chain_abort_is_reported_by_every_synchronising_call():
+    """resident = 3: a chain whose kernel aborted (here: a 1 ms watchdog on a cold-start update of four million spins,
+    which one 16-CTA cluster cannot finish in that time) has a half-grown cluster and unfinished logs.  The single-chain
+    API reports that at the next synchronising call (WOLFF_EINTERNAL, handle failed: wolff.h); the batch must too, from
+    whichever call comes first -- not only from wolff_batch_get_stats."""
+    L, R = 2048, 2
+    cold = np.stack([wl.cold(L * L)] * R)
+    for first_call in ("observables", "get_spins", "series", "moments", "set_spins", "reset_moments"):
+        gpu = binding.WolffBatch(2, L, 1.0, [0.5] * R, [11, 12])
+        gpu.set_option("resident", 3)
+        gpu.set_option("measure", 1)
+        gpu.set_spins(cold)
+        gpu.set_option("watchdog_ms", 1)
+        gpu.run(2)
+        with pytest.raises(binding.WolffError) as info:
+            {"observables": gpu.observables, "get_spins": gpu.get_spins, "series": gpu.series, "moments": gpu.moments,
+             "set_spins": lambda: gpu.set_spins(cold), "reset_moments": gpu.reset_moments}[first_call]()
+        assert info.value.code == binding.WOLFF_EINTERNAL, first_call
+        assert "watchdog" in str(info.value)
+        with pytest.raises(binding.WolffError):
+            gpu.run(1)                              # the handle stays failed
+        gpu.close()
+    # the same start with the default watchdog finishes and is correct: both chains flip nearly the whole lattice
+    gpu = binding.WolffBatch(2, L, 1.0, [0.5] * R, [11, 12])
+    gpu.set_option("resident", 3)
+    gpu.set_spins(cold)
+    gpu.run(1)
+    E, M, sz = gpu.observables(sizes=True)
+    assert all(int(s) > 0.9 * L * L for s in sz[:, 0]) and all(int(m) < 0 for m in M)
+    gpu.close()
