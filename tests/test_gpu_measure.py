@@ -150,3 +150,50 @@ def test_protocol_stretch_measured_in_kernel(name, options):
     assert np.array_equal(raw, acc) and abs(U - oracle.binder(acc)) < 1e-12
     assert np.array_equal(farm.pack(gpu.get_spins()), st["bits"])
     gpu.close()
+
+
+def _measured_without_reevaluation(gpu, ref, n, acc):
+    """A measured run followed ONLY by series() / moments(): no wolff_observables, so the next measured run must start from
+    the running E and M the previous kernel left on the device (the em_valid carry-over of api.cu / batch_api.cu)."""
+    gpu.run(n)
+    E, M = gpu.series()
+    rs, rE, rM = ref.run_logged(n)
+    assert np.array_equal(E, rE) and np.array_equal(M, rM), "series differ"
+    acc = oracle.moments_raw(rE, rM, acc=acc)
+    assert np.array_equal(gpu.moments()[0], acc)
+    return acc
+
+
+@pytest.mark.parametrize("dim,L,T", [(2, 64, wl.TC_2D), (3, 32, wl.TC_3D), (2, 96, 2.2)])
+def test_running_energy_carries_over_between_measured_runs_and_kernels(dim, L, T):
+    gpu, ref = make_pair(dim, L, 1.0, T, seed=17 + L, options={"measure": 1})
+    tiled = {"mode": 0, "small_cluster": 0}
+    cluster = {"mode": 5}
+    levels = {"mode": 4}
+    acc = None
+    for options, n in ((tiled, 20), (tiled, 15), (cluster, 20), (cluster, 10), (levels, 12), (levels, 9), (tiled, 7), (levels, 5),
+                       (cluster, 6), (tiled, 4)):
+        for k, v in options.items():
+            gpu.set_option(k, v)
+        acc = _measured_without_reevaluation(gpu, ref, n, acc)
+    assert_same_state(gpu, ref, "after ten measured runs without a whole-lattice evaluation in between")
+    gpu.close()
+
+
+def test_running_energy_carries_over_in_a_batch():
+    import test_gpu_batch as tb
+    T = [2.0, wl.TC_2D, 2.6]
+    gpu, refs = tb.make_batch(2, 64, T, [5, 6, 7], options={"measure": 1})
+    acc = [None] * gpu.R
+    for resident, n in ((3, 12), (3, 8), (1, 10), (2, 9), (3, 6), (1, 5)):
+        gpu.set_option("resident", resident)
+        gpu.run(n)
+        Es, Ms = gpu.series()
+        raw, _ = gpu.moments()
+        for r, ref in enumerate(refs):
+            _, rE, rM = ref.run_logged(n)
+            assert np.array_equal(Es[r], rE) and np.array_equal(Ms[r], rM), "chain %d, resident %d" % (r, resident)
+            acc[r] = oracle.moments_raw(rE, rM, acc=acc[r])
+            assert np.array_equal(raw[r], acc[r])
+    tb.assert_same_lattices(gpu, refs, "after six measured batch runs without an evaluation in between")
+    gpu.close()
