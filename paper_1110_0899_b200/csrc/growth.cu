@@ -573,7 +573,7 @@ template <int DIM, bool POW2, bool SPEC>
 cudaError_t prepare_one(const GrowthLaunch &l, int *max_clusters)
 {
     const void *fn = reinterpret_cast<const void *>(&growth_kernel<DIM, POW2, SPEC>);
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)l.smem_bytes);
+    cudaError_t e = allow_max_dynamic_smem(fn);
     if (e != cudaSuccess) return e;
     if (l.cluster_ctas > 8) {
         e = cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);

@@ -397,8 +397,8 @@ __global__ void batch_finish_energy_kernel(unsigned long long *acc, long long *E
 template <int DIM, bool POW2, bool BITS>
 cudaError_t launch_one(const BatchParams &bp, int grid, int threads, size_t smem, cudaStream_t stream)
 {
-    // per-process kernel attribute: set at every launch (another batch may have set a smaller value)
-    const cudaError_t e = cudaFuncSetAttribute(growth_batch_kernel<DIM, POW2, BITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // per-process kernel attribute: only ever raised to the device's maximum (internal.h)
+    const cudaError_t e = allow_max_dynamic_smem(reinterpret_cast<const void *>(&growth_batch_kernel<DIM, POW2, BITS>));
     if (e != cudaSuccess) return e;
     growth_batch_kernel<DIM, POW2, BITS><<<grid, threads, smem, stream>>>(bp);
     return cudaGetLastError();
@@ -407,7 +407,7 @@ cudaError_t launch_one(const BatchParams &bp, int grid, int threads, size_t smem
 template <int DIM, bool POW2, bool BITS>
 cudaError_t occupancy_one(int threads, size_t smem, int *per_sm)
 {
-    const cudaError_t e = cudaFuncSetAttribute(growth_batch_kernel<DIM, POW2, BITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const cudaError_t e = allow_max_dynamic_smem(reinterpret_cast<const void *>(&growth_batch_kernel<DIM, POW2, BITS>));
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, growth_batch_kernel<DIM, POW2, BITS>, threads, smem);
 }

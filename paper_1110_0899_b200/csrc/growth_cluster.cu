@@ -717,7 +717,8 @@ template <int DIM, bool POW2>
 cudaError_t set_attributes(size_t smem_bytes, int nC)
 {
     const void *fn = reinterpret_cast<const void *>(&growth_cluster_kernel<DIM, POW2>);
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    (void)smem_bytes;
+    cudaError_t e = allow_max_dynamic_smem(fn);
     if (e != cudaSuccess) return e;
     if (nC > 8) e = cudaFuncSetAttribute(fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     return e;

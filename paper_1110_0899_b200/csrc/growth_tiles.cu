@@ -1414,10 +1414,9 @@ __global__ void __launch_bounds__(kT, 1) growth_tiles_kernel(const __grid_consta
 template <int DIM>
 cudaError_t launch_one(const TileParams &tp, size_t smem_bytes, cudaStream_t stream)
 {
-    // the attribute belongs to the kernel function, i.e. to the process: another live handle of the same dim may have
-    // made its plan (and set a smaller value) since this handle made its own
+    // the attribute belongs to the kernel function, i.e. to the process: only ever raised to the device's maximum (internal.h)
     const void *fn = reinterpret_cast<const void *>(&growth_tiles_kernel<DIM>);
-    const cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    const cudaError_t ea = allow_max_dynamic_smem(fn);
     if (ea != cudaSuccess) return ea;
     void *args[] = { const_cast<TileParams *>(&tp) };
     return cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(&growth_tiles_kernel<DIM>), dim3(tp.G), dim3(kT), args,
@@ -1428,7 +1427,7 @@ template <int DIM>
 cudaError_t prepare_one(size_t smem_bytes, int *ctas_per_sm)
 {
     const void *fn = reinterpret_cast<const void *>(&growth_tiles_kernel<DIM>);
-    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    cudaError_t e = allow_max_dynamic_smem(fn);
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, growth_tiles_kernel<DIM>, kT, smem_bytes);
 }

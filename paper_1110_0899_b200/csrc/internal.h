@@ -2,6 +2,9 @@
 #pragma once
 #include <cstddef>
 #include <cstdint>
+#include <mutex>
+#include <utility>
+#include <vector>
 #include <cuda_runtime.h>
 
 #include "device_common.cuh"
@@ -164,6 +167,35 @@ struct GrowthLaunch {
 constexpr int kGrowthThreads = 512;
 constexpr int kTileThreads = 384;
 constexpr int kClusterThreads = 512;
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function (per device), not to a handle.  If every
+// handle set it to its own need, two host threads driving handles of different L could interleave set(A), set(B smaller),
+// launch(A) and A's launch would be refused.  So the library only ever sets ONE value per kernel: the most the device
+// allows it (the opt-in maximum minus the kernel's static shared memory).  Setting it again, from any thread, changes
+// nothing, and every handle's launch fits under it; occupancy follows the shared memory a launch asks for, not this cap.
+inline cudaError_t allow_max_dynamic_smem(const void *fn)
+{
+    static std::mutex mu;
+    static std::vector<std::pair<const void *, int>> done;      // (kernel, device) pairs already raised: a launch pays one lookup
+    int dev = 0, optin = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        for (const auto &d : done)
+            if (d.first == fn && d.second == dev) return cudaSuccess;
+    }
+    e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    if (e != cudaSuccess) return e;
+    cudaFuncAttributes fa{};
+    e = cudaFuncGetAttributes(&fa, fn);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes);
+    if (e != cudaSuccess) return e;
+    std::lock_guard<std::mutex> lock(mu);
+    done.emplace_back(fn, dev);
+    return cudaSuccess;
+}
 
 // launchers (defined next to their kernels)
 cudaError_t launch_growth(const GrowthParams &p, int dim, const GrowthLaunch &l, cudaStream_t stream);
