@@ -125,7 +125,10 @@ WOLFF_API int wolff_get_series(wolff_handle h, int64_t *E_series, int64_t *M_ser
 /* Accumulated over all measured updates since creation or the last reset, ten 64-bit words (host pointer):
  *   [0] n   [1] sum E (two's complement)   [2] sum |M|   [3],[4] sum E^2 (low, high word)
  *   [5],[6] sum M^2   [7],[8] sum M^4   [9] 0
- * exact integers (M^4 reaches 2^96 at 2^24 spins, hence 128 bits), and the Binder ratio of PAPER.md Eq. 3,
+ * exact integers (M^4 reaches 2^96 at 2^24 spins, hence 128 bits).  They stay exact while samples x N^4 < 2^128: any
+ * number of samples up to N = 2^16, 2^32 samples at N = 2^24, 2^16 at N = 2^28, 16 at N = 2^31; a measured wolff_run
+ * (or wolff_batch_run) that would take the count past that bound is refused with WOLFF_EINVAL before anything is
+ * launched (reset the moments to go on).  And the Binder ratio of PAPER.md Eq. 3,
  * U = 1 - <M^4> / (3 <M^2>^2), from them (NaN without samples).  Either pointer may be NULL.  Blocks. */
 WOLFF_API int wolff_get_moments(wolff_handle h, uint64_t *moments, double *binder);
 WOLFF_API int wolff_reset_moments(wolff_handle h);

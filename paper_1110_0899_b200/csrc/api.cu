@@ -47,7 +47,9 @@ struct wolff_ctx {
     uint32_t *ns_log = nullptr;     // per-update duration of the most recent run
     long long *E_log = nullptr;     // per-update E, M of the most recent run ("measure" = 1)
     long long *M_log = nullptr;
-    uint64_t sizes_cap = 0;         // entries allocated in each of the four logs
+    uint64_t sizes_cap = 0;         // entries allocated in the size and duration logs
+    uint64_t em_cap = 0;            // entries allocated in E_log and M_log (allocated by the first measured run)
+    uint64_t meas_count = 0;        // samples in the moment accumulators (host-side count, for the overflow bound)
     int measure = 0;                // in-kernel measurement after every update
     bool last_measured = false;     // the most recent run was a measured one
     bool em_valid = false;          // the control block holds E and M of the current lattice
@@ -476,22 +478,48 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
         // the size log and control block are about to be reused: finish the previous run first
         CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
     }
+    if (h->measure) {
+        // the 128-bit accumulators are exact while samples * N^4 < 2^128 (sum M^4 is the largest; |M| <= N): any number of
+        // samples up to N = 2^16, 2^32 at N = 2^24, 2^16 at N = 2^28, 16 at N = 2^31.  Beyond that they would wrap without
+        // a trace (the oracle's wrap the same way, so no parity test could see it): refuse instead.
+        const unsigned __int128 n2 = (unsigned __int128)h->N * h->N, n4 = n2 * n2;       // <= 2^124
+        const unsigned __int128 limit = ~(unsigned __int128)0 / n4;
+        if ((unsigned __int128)h->meas_count + n_updates > limit) {
+            set_error("measured run refused: %llu + %llu samples of M^4 <= N^4 (N = %llu) would overflow the 128-bit moment "
+                      "accumulators; call wolff_reset_moments first (or run with \"measure\" = 0)",
+                      (unsigned long long)h->meas_count, (unsigned long long)n_updates, (unsigned long long)h->N);
+            return WOLFF_EINVAL;
+        }
+    }
     if (n_updates > h->sizes_cap) {
         if (h->ran) CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
         uint64_t cap = h->sizes_cap ? h->sizes_cap : 1024;
         while (cap < n_updates) cap *= 2;
         uint32_t *fresh = nullptr, *fresh_ns = nullptr;
-        long long *fresh_E = nullptr, *fresh_M = nullptr;
-        if (cudaMalloc(&fresh, (size_t)cap * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&fresh_ns, (size_t)cap * sizeof(uint32_t)) != cudaSuccess ||
-            cudaMalloc(&fresh_E, (size_t)cap * sizeof(long long)) != cudaSuccess || cudaMalloc(&fresh_M, (size_t)cap * sizeof(long long)) != cudaSuccess) {
+        if (cudaMalloc(&fresh, (size_t)cap * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&fresh_ns, (size_t)cap * sizeof(uint32_t)) != cudaSuccess) {
             cudaGetLastError();
-            cudaFree(fresh); cudaFree(fresh_ns); cudaFree(fresh_E); cudaFree(fresh_M);
+            cudaFree(fresh); cudaFree(fresh_ns);
             set_error("cannot allocate the per-update logs for %llu updates", (unsigned long long)n_updates);
             return WOLFF_ENOMEM;
         }
-        cudaFree(h->sizes); cudaFree(h->ns_log); cudaFree(h->E_log); cudaFree(h->M_log);
-        h->sizes = fresh; h->ns_log = fresh_ns; h->E_log = fresh_E; h->M_log = fresh_M;
+        cudaFree(h->sizes); cudaFree(h->ns_log);
+        h->sizes = fresh; h->ns_log = fresh_ns;
         h->sizes_cap = cap;
+    }
+    if (h->measure && n_updates > h->em_cap) {
+        // E and M after every update: 16 bytes per update, allocated only once a measured run asks for them
+        if (h->ran) CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+        const uint64_t cap = h->sizes_cap;
+        long long *fresh_E = nullptr, *fresh_M = nullptr;
+        if (cudaMalloc(&fresh_E, (size_t)cap * sizeof(long long)) != cudaSuccess || cudaMalloc(&fresh_M, (size_t)cap * sizeof(long long)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(fresh_E); cudaFree(fresh_M);
+            set_error("cannot allocate the per-update E / M logs for %llu updates", (unsigned long long)n_updates);
+            return WOLFF_ENOMEM;
+        }
+        cudaFree(h->E_log); cudaFree(h->M_log);
+        h->E_log = fresh_E; h->M_log = fresh_M;
+        h->em_cap = cap;
     }
     GrowthParams p{};
     p.spins = h->spins; p.clist = h->clist; p.sizes = h->sizes; p.ctl = h->ctl; p.geo = h->geo;
@@ -537,8 +565,8 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
             cp.g.n_updates = n_updates - done < chunk ? n_updates - done : chunk;
             cp.g.sizes = h->sizes + done;
             cp.g.ns_log = h->ns_log + done;
-            cp.g.E_log = h->E_log + done;
-            cp.g.M_log = h->M_log + done;
+            cp.g.E_log = h->measure ? h->E_log + done : nullptr;
+            cp.g.M_log = h->measure ? h->M_log + done : nullptr;
             if (h->measure && cp.idle_ns > 200u) cp.idle_ns = 200u;     // every warp of the cluster is waited for after each update
             const cudaError_t e = launch_growth_cluster(cp, h->dim, h->cl_smem, stream);
             if (e == cudaErrorLaunchOutOfResources || e == cudaErrorInvalidConfiguration || e == cudaErrorCooperativeLaunchTooLarge) {
@@ -563,8 +591,8 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
             tp.g.n_updates = n_updates - done < chunk ? n_updates - done : chunk;
             tp.g.sizes = h->sizes + done;
             tp.g.ns_log = h->ns_log + done;
-            tp.g.E_log = h->E_log + done;
-            tp.g.M_log = h->M_log + done;
+            tp.g.E_log = h->measure ? h->E_log + done : nullptr;
+            tp.g.M_log = h->measure ? h->M_log + done : nullptr;
             if (h->measure && tp.idle_ns > 200u) tp.idle_ns = 200u;     // every warp of every CTA is waited for after each update
             if (done != 0)        // the measurement's arrival counters count from zero in every launch
                 CHECK_CUDA(h, cudaMemsetAsync(&h->ctl->meas_arrive_a, 0, offsetof(Control, error) - offsetof(Control, meas_arrive_a), stream),
@@ -600,6 +628,7 @@ int wolff_run(wolff_handle h, uint64_t n_updates, void *cuda_stream)
     h->u += n_updates;
     h->last_n = n_updates;
     h->last_measured = h->measure != 0;
+    if (h->measure) h->meas_count += n_updates;
     h->em_valid = h->measure != 0;      // a measured run leaves E and M of the final lattice in the control block
     h->last_stream = stream;
     h->ran = true;
@@ -858,6 +887,7 @@ int wolff_reset_moments(wolff_handle h)
     if (rc) return rc;
     CHECK_CUDA(h, cudaMemsetAsync(h->ctl->moments, 0, sizeof(h->ctl->moments), h->last_stream), "clear moments");
     CHECK_CUDA(h, cudaStreamSynchronize(h->last_stream), "cudaStreamSynchronize");
+    h->meas_count = 0;
     return WOLFF_OK;
 }
 

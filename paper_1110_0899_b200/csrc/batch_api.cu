@@ -43,7 +43,9 @@ struct wolff_batch_ctx {
     uint32_t *lists = nullptr;
     uint32_t *sizes = nullptr;
     long long *E_log = nullptr, *M_log = nullptr;
-    uint64_t log_cap = 0;           // updates per chain the logs can hold
+    uint64_t log_cap = 0;           // updates per chain the size log can hold
+    uint64_t em_cap = 0;            // updates per chain E_log and M_log can hold (allocated by the first measured run)
+    uint64_t meas_count = 0;        // samples per chain in the moment accumulators (host-side count, for the overflow bound)
     uint2 *keys = nullptr;
     unsigned long long *thr_dev = nullptr;
     long long *EM = nullptr;
@@ -242,8 +244,8 @@ int run_clusters(wolff_batch_ctx *b, uint64_t n_updates, cudaStream_t stream)
         g.key0 = (uint32_t)b->seed[r]; g.key1 = (uint32_t)(b->seed[r] >> 32);
         g.thr = b->thr[r]; g.u0 = b->u; g.n_updates = n_updates;
         g.measure = measure ? 1u : 0u; g.claim_bits = 0xFEu;
-        g.E_log = b->E_log + (size_t)r * (size_t)n_updates;
-        g.M_log = b->M_log + (size_t)r * (size_t)n_updates;
+        g.E_log = measure ? b->E_log + (size_t)r * (size_t)n_updates : nullptr;      // the logs exist once a measured run has asked for them
+        g.M_log = measure ? b->M_log + (size_t)r * (size_t)n_updates : nullptr;
         g.ns_log = b->cl_ns + (size_t)r * (size_t)n_updates;
         if (measure) cp.idle_ns = 200;
         cp.thr32 = (uint32_t)b->thr[r];
@@ -382,22 +384,45 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
     }
     if (b->ran && (stream != b->last_stream || n_updates > b->log_cap))
         CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+    if (b->measure) {
+        // exact while samples * N^4 < 2^128 (see wolff_run): refuse what would wrap the accumulators silently
+        const unsigned __int128 n2 = (unsigned __int128)b->N * b->N, n4 = n2 * n2;
+        const unsigned __int128 limit = ~(unsigned __int128)0 / n4;
+        if ((unsigned __int128)b->meas_count + n_updates > limit) {
+            set_error("measured run refused: %llu + %llu samples of M^4 <= N^4 (N = %llu) would overflow the 128-bit moment "
+                      "accumulators; call wolff_batch_reset_moments first", (unsigned long long)b->meas_count,
+                      (unsigned long long)n_updates, (unsigned long long)b->N);
+            return WOLFF_EINVAL;
+        }
+    }
     if (n_updates > b->log_cap) {
         uint64_t cap = b->log_cap ? b->log_cap : 1024;
         while (cap < n_updates) cap *= 2;
         uint32_t *fresh = nullptr;
-        long long *fresh_E = nullptr, *fresh_M = nullptr;
         const size_t entries = (size_t)b->R * (size_t)cap;
-        if (cudaMalloc(&fresh, entries * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&fresh_E, entries * sizeof(long long)) != cudaSuccess ||
-            cudaMalloc(&fresh_M, entries * sizeof(long long)) != cudaSuccess) {
+        if (cudaMalloc(&fresh, entries * sizeof(uint32_t)) != cudaSuccess) {
             cudaGetLastError();
-            cudaFree(fresh); cudaFree(fresh_E); cudaFree(fresh_M);
-            set_error("cannot allocate the per-update logs for %u chains x %llu updates", b->R, (unsigned long long)n_updates);
+            set_error("cannot allocate the cluster-size log for %u chains x %llu updates", b->R, (unsigned long long)n_updates);
             return WOLFF_ENOMEM;
         }
-        cudaFree(b->sizes); cudaFree(b->E_log); cudaFree(b->M_log);
-        b->sizes = fresh; b->E_log = fresh_E; b->M_log = fresh_M;
+        cudaFree(b->sizes);
+        b->sizes = fresh;
         b->log_cap = cap;
+    }
+    if (b->measure && n_updates > b->em_cap) {
+        // E and M after every update of every chain: 16 R bytes per update, allocated only once a measured run asks for them
+        if (b->ran) CHECK_CUDA(b, cudaStreamSynchronize(b->last_stream), "cudaStreamSynchronize");
+        long long *fresh_E = nullptr, *fresh_M = nullptr;
+        const size_t entries = (size_t)b->R * (size_t)b->log_cap;
+        if (cudaMalloc(&fresh_E, entries * sizeof(long long)) != cudaSuccess || cudaMalloc(&fresh_M, entries * sizeof(long long)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(fresh_E); cudaFree(fresh_M);
+            set_error("cannot allocate the E / M logs for %u chains x %llu updates", b->R, (unsigned long long)n_updates);
+            return WOLFF_ENOMEM;
+        }
+        cudaFree(b->E_log); cudaFree(b->M_log);
+        b->E_log = fresh_E; b->M_log = fresh_M;
+        b->em_cap = b->log_cap;
     }
     if (b->resident == 3) {
         if (b->measure && b->L % 32 != 0) {
@@ -409,6 +434,7 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
         b->u += n_updates;
         b->last_n = n_updates;
         b->last_measured = b->measure != 0;
+        if (b->measure) b->meas_count += n_updates;
         b->em_valid = b->measure != 0;
         b->last_stream = stream;
         b->ran = true;
@@ -430,6 +456,7 @@ int wolff_batch_run(wolff_batch b, uint64_t n_updates, void *cuda_stream)
     b->u += n_updates;
     b->last_n = n_updates;
     b->last_measured = b->measure != 0;
+    if (b->measure) b->meas_count += n_updates;
     b->em_valid = b->measure != 0;       // a measured run leaves the running values in EM; an unmeasured one outdates them
     b->last_stream = stream;
     b->ran = true;
@@ -588,6 +615,7 @@ int wolff_batch_reset_moments(wolff_batch b)
     if (rc) return rc;
     DeviceScope scope(b);
     CHECK_CUDA(b, cudaMemsetAsync(b->moments, 0, 10 * (size_t)b->R * sizeof(unsigned long long), b->last_stream), "clear moments");
+    b->meas_count = 0;
     return sync_and_check(b);
 }
 

@@ -197,3 +197,34 @@ def test_running_energy_carries_over_in_a_batch():
             assert np.array_equal(raw[r], acc[r])
     tb.assert_same_lattices(gpu, refs, "after six measured batch runs without an evaluation in between")
     gpu.close()
+
+
+def test_measured_runs_that_would_wrap_the_moment_accumulators_are_refused():
+    """sum M^4 is kept in 128 bits and |M| <= N, so the accumulators are exact while samples x N^4 < 2^128.  At N = 2^28
+    that is 2^16 samples.  The oracle's accumulators would wrap in the same way, so parity cannot see an overflow: the
+    library refuses the run instead (wolff.h, wolff_get_moments)."""
+    L = 16384
+    gpu = binding.Wolff(2, L, 1.0, 2.4, seed=1)
+    gpu.set_option("measure", 1)
+    with pytest.raises(binding.WolffError) as info:
+        gpu.run(65537)
+    assert info.value.code == binding.WOLFF_EINVAL and "overflow" in str(info.value)
+    gpu.run(2)                                          # two samples in
+    assert int(gpu.moments()[0][0]) == 2
+    with pytest.raises(binding.WolffError):
+        gpu.run(65535)                                  # 2 + 65535 > 2^16
+    gpu.set_option("measure", 0)
+    gpu.run(3)                                          # unmeasured runs are not counted
+    gpu.set_option("measure", 1)
+    gpu.reset_moments()
+    gpu.run(65535)                                      # the count started again
+    assert int(gpu.moments()[0][0]) == 65535
+    with pytest.raises(binding.WolffError):
+        gpu.run(2)
+    gpu.close()
+    batch = binding.WolffBatch(2, L, 1.0, [2.4], [3])
+    batch.set_option("measure", 1)
+    with pytest.raises(binding.WolffError) as info:
+        batch.run(65537)
+    assert info.value.code == binding.WOLFF_EINVAL and "overflow" in str(info.value)
+    batch.close()
