@@ -173,6 +173,7 @@ def oracle_on_same_clusters(c, seed: int, lattice, update_index: int, budget_s: 
     ref.set_spins(lattice)
     ref.update_index = update_index
     flipped = n = 0
+    all_sizes = []
     t0 = time.perf_counter()
     while n < max_updates and time.perf_counter() - t0 < budget_s:
         if measured:
@@ -180,24 +181,28 @@ def oracle_on_same_clusters(c, seed: int, lattice, update_index: int, budget_s: 
         else:
             sizes = ref.run(1)
         flipped += int(sizes[0])
+        all_sizes.append(int(sizes[0]))
         n += 1
     dt = time.perf_counter() - t0
     ref.close()
-    return {"value": flipped / dt, "unit": UNIT, "updates_per_s": n / dt, "cores": 1, "kind": "oracle",
+    return {"sizes": all_sizes, "value": flipped / dt, "unit": UNIT, "updates_per_s": n / dt, "cores": 1, "kind": "oracle",
             "sample": "%s, the first %d updates of the GPU's timed region (from update index %d, same lattice, same seed): "
                       "%.1f s of CPU work, %d spins flipped%s" % (c.name, n, update_index, dt, flipped,
                                                                   ", E and M summed over the lattice after every update" if measured else ""),
             "host_cores_available": os.cpu_count()}
 
 
-def oracle_replicas(c, seeds, n_updates: int, budget_s: float, threads: int):
+def oracle_replicas(c, seeds, n_updates: int, budget_s: float, threads: int, equil: int = 0):
     """`threads` independent oracle chains side by side (one per host core; the ctypes calls release the GIL): the
-    aggregate the host can reach on replicas.  Literal start (the oracle's own seed-derived lattice)."""
+    aggregate the host can reach on replicas.  Literal start (the oracle's own seed-derived lattice), then the same
+    `equil` untimed updates the batch ran before its timed call, so that both sides time the same clusters."""
     import oracle
     from concurrent.futures import ThreadPoolExecutor
 
     def one(seed):
         ref = oracle.OracleWolff(c.dim, c.L, c.J, c.T, seed)
+        if equil:
+            ref.run(equil)
         t0 = time.perf_counter()
         n = f = 0
         while n < n_updates and time.perf_counter() - t0 < budget_s:
@@ -212,7 +217,8 @@ def oracle_replicas(c, seeds, n_updates: int, budget_s: float, threads: int):
     dt = max(r[2] for r in res)
     return {"updates_per_s": sum(r[0] for r in res) / dt, "value": sum(r[1] for r in res) / dt, "unit": UNIT, "cores": threads,
             "kind": "oracle", "one_core_updates_per_s": res[0][0] / res[0][2],
-            "sample": "%s literal random start, %d chains of up to %d updates side by side" % (c.name, threads, n_updates)}
+            "sample": "%s literal random start + %d untimed updates, %d chains of up to %d updates side by side (the updates the batch times)" % (
+                c.name, equil, threads, n_updates)}
 
 
 # ====================================================================== the CUDA arm
@@ -235,6 +241,7 @@ def run_b200(args, rank: int, world: int):
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     options = dict(args.opt)
     launches = [0]
+    parity_checks = []                  # one entry per leg whose oracle sample was compared with the kernel's size log
 
     def barrier():
         if world > 1:
@@ -268,7 +275,7 @@ def run_b200(args, rank: int, world: int):
         sizes_d = torch.zeros(updates, dtype=torch.int32, device=dev)
         ns_d = torch.zeros(updates, dtype=torch.int32, device=dev)
         res = {"cfg": c, "h": h, "seed": seed, "flipped": 0, "attempts": 0, "levels": 0, "depth_updates": 0, "updates": updates * steps,
-               "step_ms": [], "growth_ms": [], "update_ns": []}
+               "step_ms": [], "growth_ms": [], "update_ns": [], "sizes": []}
         # BFS depth of the clusters the timed steps grow (a property of the workload): the
         # level-synchronous kernel (mode 4) replays the same updates from the same lattice, untimed, and counts levels
         twin = None
@@ -302,6 +309,7 @@ def run_b200(args, rank: int, world: int):
                 res["kernel"] = kernel_of(st)
                 res["flipped"] += st["flipped"]; res["attempts"] += st["claim_attempts"]
                 assert int(sizes_d.sum().item()) == st["flipped"]
+                res["sizes"].append(sizes_d.cpu().numpy().astype(np.uint32))
                 h.series_into(None, None, ns_d)
                 res["update_ns"].append(ns_d.cpu().numpy().astype(np.uint32).astype(np.float64))
                 if replay:
@@ -345,7 +353,16 @@ def run_b200(args, rank: int, world: int):
             out["us_per_bfs_level"] = r["depth_growth_ms"] * 1e3 / max(r["levels"], 1)
             out["bfs_depth_sample"] = "the first %d timed updates, replayed untimed by the level-synchronous kernel" % r["depth_updates"]
         if rank == 0 and not args.no_cpu_baseline and oracle_budget > 0:
-            out["cpu_baseline"] = oracle_on_same_clusters(r["cfg"], r["seed"], r["start_lattice"], r["start_index"], oracle_budget, oracle_max)
+            base = oracle_on_same_clusters(r["cfg"], r["seed"], r["start_lattice"], r["start_index"], oracle_budget,
+                                           min(oracle_max, r["updates"]))
+            # the oracle ran the first n updates of the timed region from the same state: its cluster sizes must be the
+            # ones the kernel logged for those updates (north_star: bit-exact per-update cluster sizes)
+            ref_sizes = base.pop("sizes")
+            gpu_sizes = np.concatenate(r["sizes"])[:len(ref_sizes)].tolist() if r["sizes"] else []
+            out["parity_in_timed_region"] = {"updates": len(ref_sizes), "equal": gpu_sizes == ref_sizes,
+                                             "compared": "per-update cluster sizes, oracle vs the kernel's log, from update index %d" % r["start_index"]}
+            parity_checks.append(out["parity_in_timed_region"]["equal"])
+            out["cpu_baseline"] = base
             out["gpu_over_one_cpu_core"] = out["value"] / out["cpu_baseline"]["value"] if out["cpu_baseline"]["value"] else None
         return out
 
@@ -380,7 +397,9 @@ def run_b200(args, rank: int, world: int):
         def timed_run(measure: int, n: int):
             reset()
             h.set_option("measure", measure)
-            h.run(3, stream=stream); h.observables()       # the kernel choice of mode 0 and the tables settle
+            h.run(3, stream=stream); h.observables()       # first launch of this kernel variant (module load, attributes, logs)
+            # reset() loads the lattice again, which clears the handle's run history: the timed run below uses the kernel
+            # mode 0 picks WITHOUT a mean cluster size to go by.  Which one that was is read back and reported.
             reset()
             with torch.cuda.stream(stream):
                 e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
@@ -389,12 +408,13 @@ def run_b200(args, rank: int, world: int):
                 e1.record(stream)
             e1.synchronize()
             launches[0] += 1
-            return e0.elapsed_time(e1), h.stats()["flipped"]
+            st = h.stats()
+            return e0.elapsed_time(e1), st["flipped"], kernel_of(st)
 
         reset()
         cold_ms, warm_ms = timed_observables(True), timed_observables(False)
-        plain_ms, flipped = timed_run(0, n_updates)
-        meas_ms, flipped_m = timed_run(1, n_updates)
+        plain_ms, flipped, plain_kernel = timed_run(0, n_updates)
+        meas_ms, flipped_m, meas_kernel = timed_run(1, n_updates)
         assert flipped == flipped_m
         # host loop: one launch + one whole-lattice reduction per update
         h.set_option("measure", 0)
@@ -418,7 +438,7 @@ def run_b200(args, rank: int, world: int):
                                                    "itself: launch + kernel + one small read-back of the control block + one synchronise"},
                "with_measurement_every_update": {
                    "updates": n_updates, "same_updates_same_state": True,
-                   "update_only_ms_per_update": plain_ms / n_updates,
+                   "update_only_ms_per_update": plain_ms / n_updates, "update_only_kernel": plain_kernel, "in_kernel_kernel": meas_kernel,
                    "in_kernel_ms_per_update": meas_ms / n_updates, "in_kernel_over_update_only": meas_ms / plain_ms,
                    "in_kernel_value": flipped / (meas_ms * 1e-3), "unit": UNIT,
                    "in_kernel_protocol": "set_option('measure', 1); run(%d): ONE launch, E and M after every update on the device" % n_updates,
@@ -426,7 +446,9 @@ def run_b200(args, rank: int, world: int):
                    "host_loop_value": loop_flipped / loop_dt,
                    "host_loop_protocol": "run(1) + observables(E, M, size) per update, host wall clock"}}
         if rank == 0 and not args.no_cpu_baseline and oracle_budget > 0:
-            out["with_measurement_every_update"]["cpu_baseline"] = oracle_on_same_clusters(c, seed, lattice, index, oracle_budget, n_updates, measured=True)
+            base = oracle_on_same_clusters(c, seed, lattice, index, oracle_budget, n_updates, measured=True)
+            base.pop("sizes")
+            out["with_measurement_every_update"]["cpu_baseline"] = base
         h.close()
         return out
 
@@ -468,8 +490,8 @@ def run_b200(args, rank: int, world: int):
                "ms": ms}
         if rank == 0 and not args.no_cpu_baseline and oracle_budget > 0 and not cold:
             cores = os.cpu_count() or 1
-            out["cpu_baseline_one_core"] = oracle_replicas(c, seeds, 20000, oracle_budget, 1)
-            out["cpu_baseline_all_cores"] = oracle_replicas(c, seeds, 20000, oracle_budget, cores)
+            out["cpu_baseline_one_core"] = oracle_replicas(c, seeds, n, oracle_budget, 1, equil)
+            out["cpu_baseline_all_cores"] = oracle_replicas(c, seeds, n, oracle_budget, cores, equil)
         return out
 
     def reduce_sum(x):
@@ -542,7 +564,7 @@ def run_b200(args, rank: int, world: int):
                      "note": "the fraction is ~1e-3 by the nature of the path: a chain of dependent hops (BFS depth x hop latency) on a "
                              "lattice that lives in shared memory, not a stream; latency_roofline is the bound that describes it"},
     }
-    for key in ("bfs_depth_per_update", "us_per_bfs_level", "bfs_depth_sample", "cpu_baseline", "gpu_over_one_cpu_core"):
+    for key in ("bfs_depth_per_update", "us_per_bfs_level", "bfs_depth_sample", "cpu_baseline", "gpu_over_one_cpu_core", "parity_in_timed_region"):
         if key in summary:
             out[key] = summary[key]
 
@@ -609,7 +631,124 @@ def run_b200(args, rank: int, world: int):
             "C5a_equilibrated_one_cluster_per_chain": batch_leg("C5a", 14, 300, True, 300, 0.0, {"resident": 3}),
         }
     out["gpu_launches"] = launches[0]
+    out["parity_all_legs"] = {"legs_compared": len(parity_checks), "all_equal": all(parity_checks)}
     return out
+
+
+# ====================================================================== row A8 on its own (--a8)
+
+def run_a8(args):
+    """The one bandwidth-bound kernel of the path, the whole-lattice E/M reduction, at
+    the two headline lattices (16 MiB) and at sizes where the launch ramp no longer dominates (256 MiB, 1 GiB), two ways:
+    wolff_observables as a call (launch + kernel + read-back of the control block + one synchronise, device destinations)
+    and wolff_energy_magnetisation_noalloc on a copy of the same lattice (asynchronous: memset + kernel between the two
+    events).  Algorithmic bytes = N (every spin byte read once); the fraction is against the measured HBM peak.  Cold =
+    L2 flushed by a 256 MiB write before the timed call (the two large lattices do not fit L2 either way)."""
+    import torch
+    from paper_1110_0899_b200 import binding, build as cuda_build, workloads as wl
+    cuda_build.build()
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    stream = torch.cuda.Stream(device=dev)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    peak, peak_src = measured_peak_hbm()
+    out_d = torch.zeros(4, dtype=torch.int64, device=dev)
+
+    def timed(fn, cold: bool, reps: int = 7):
+        times = []
+        for _ in range(reps):
+            with torch.cuda.stream(stream):
+                if cold:
+                    flush.fill_(1)
+                e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                fn()
+                e1.record(stream)
+            e1.synchronize()
+            times.append(e0.elapsed_time(e1))
+        return min(times), statistics.median(times)
+
+    def figures(N, ms_pair):
+        best, med = ms_pair
+        return {"best_us": best * 1e3, "median_us": med * 1e3, "gbs": N / (best * 1e-3) / 1e9, "frac": N / (best * 1e-3) / 1e9 / peak}
+
+    rows = []
+    for dim, L in args.a8_lattices:
+        N = L ** dim
+        h = binding.Wolff(dim, L, 1.0, wl.TC_2D if dim == 2 else wl.TC_3D, 1)
+        call = lambda: h.observables_into(out_d[0:1], out_d[1:2], None)
+        call()
+        row = {"lattice": "%dD L=%d" % (dim, L), "bytes": N,
+               "wolff_observables_call": {"cold": figures(N, timed(call, True)), "warm": figures(N, timed(call, False))}}
+        if N <= binding.NOALLOC_MAX_SITES:
+            spins = torch.empty(N, dtype=torch.int8, device=dev)
+            h.get_spins_into(spins)
+            na = lambda: binding.energy_magnetisation_noalloc(spins, dim, L, out_d[2:3], out_d[3:4], stream)
+            na()
+            row["noalloc_kernel"] = {"cold": figures(N, timed(na, True)), "warm": figures(N, timed(na, False))}
+            torch.cuda.synchronize()
+            vals = out_d.cpu().tolist()
+            assert vals[0:2] == vals[2:4], vals
+            del spins
+        h.close()
+        rows.append(row)
+    return {"a8_only": True, "bound": "hbm", "peak": peak, "peak_source": peak_src, "unit": "GB/s", "algorithmic_bytes": "N (one byte per spin)",
+            "rows": rows}
+
+
+# ====================================================================== pass counters of a -DWOLFF_PROFILE build (--profile-counters)
+
+def run_profile_counters(args):
+    """What one warp pass of the barrier-free growth kernels costs, from counters compiled in with -DWOLFF_PROFILE
+    (libwolff_b200_profile.so, built here; main() points the binding at it).  Not a timing of the product: the counters
+    cost cycles themselves.  Per workload (equilibrated C3 and C5a): one launch of `updates` updates on the tiled kernel
+    and one on the cluster-resident kernel, and from wolff_get_stats the cycles spent inside passes, the passes, the
+    sites expanded, hand-overs / messages / spills, and the launch's prologue / growth / epilogue times."""
+    import torch
+    from paper_1110_0899_b200 import binding, workloads as wl
+    torch.cuda.set_device(0)
+    stream = torch.cuda.Stream()
+    rows = []
+    for name, updates in ((args.workload, args.updates), (args.secondary, args.secondary_updates)):
+        c = wl.CONFIGS[name]
+        for label, opts in (("growth_tiles_kernel", {"mode": 0, "small_cluster": 0}), ("growth_cluster_kernel", {"mode": 5})):
+            h = binding.Wolff(c.dim, c.L, c.J, c.T, c.seed)
+            for k, v in opts.items():
+                h.set_option(k, v)
+            h.set_spins(wl.cold(c.N))
+            h.run(args.equil, stream=stream)
+            h.observables()
+            e0 = torch.cuda.Event(enable_timing=True); e1 = torch.cuda.Event(enable_timing=True)
+            with torch.cuda.stream(stream):
+                e0.record(stream)
+                h.run(updates, stream=stream)
+                e1.record(stream)
+            e1.synchronize()
+            raw = (ctypes_stats(h))
+            row = {"workload": c.name, "kernel": label, "updates": raw[0], "flipped": raw[1], "launch_ms": e0.elapsed_time(e1),
+                   "warp_passes": raw[13], "cycles_in_passes": raw[2], "sites_expanded": raw[3],
+                   "cycles_per_pass": raw[2] / max(raw[13], 1), "sites_per_pass": raw[3] / max(raw[13], 1),
+                   "claim_attempts": raw[7], "ring_pushes": raw[12], "spills": raw[14]}
+            if label == "growth_tiles_kernel":
+                row.update({"messages": raw[11], "inline_philox_passes": raw[10], "prologue_us": raw[4] * 1e-3, "growth_us": raw[5] * 1e-3,
+                            "epilogue_us": raw[6] * 1e-3, "messages_per_spin": raw[11] / max(raw[1], 1)})
+            else:
+                row.update({"steals": raw[11], "hand_overs": raw[10], "cycles_per_hand_over": raw[4] / max(raw[10], 1),
+                            "takes": raw[8], "cycles_per_take": raw[6] / max(raw[8], 1)})
+            h.close()
+            rows.append(row)
+    return {"profile_counters": True, "build": "-DWOLFF_PROFILE (libwolff_b200_profile.so)", "equil": args.equil, "rows": rows}
+
+
+def ctypes_stats(h):
+    """The raw WOLFF_NSTATS words of wolff_get_stats (a profiling build reuses some slots, so no names here)."""
+    import ctypes
+    from paper_1110_0899_b200 import binding
+    buf = (ctypes.c_uint64 * binding.NSTATS)()
+    rc = binding.load().wolff_get_stats(h._h, buf)
+    if rc != binding.WOLFF_OK:
+        raise binding.WolffError(rc, binding.last_error())
+    return [int(x) for x in buf]
 
 
 # ====================================================================== the oracle arm (CPU)
@@ -696,6 +835,11 @@ def main():
     ap.add_argument("--no-secondary", action="store_true")
     ap.add_argument("--no-batch", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--profile-counters", action="store_true",
+                    help="build with -DWOLFF_PROFILE and print the pass counters of the growth kernels (not a timing of the product)")
+    ap.add_argument("--a8", action="store_true", help="only row A8 (the E/M reduction) on its own, at 16 MiB .. 1 GiB lattices")
+    ap.add_argument("--a8-lattices", type=lambda t: [tuple(int(x) for x in item.split(":")) for item in t.split(",")],
+                    default=[(2, 4096), (3, 256), (2, 16384), (3, 1024)], help="dim:L,dim:L,... for --a8")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         sys.stderr.write("note: fewer than 3 warm-up steps; the timing rules ask for W >= 3\n")
@@ -706,6 +850,16 @@ def main():
     if args.impl == "reference":
         if rank == 0:
             print(json.dumps(run_reference(args)), flush=True)
+        return 0
+    if args.profile_counters:
+        if rank == 0:
+            from paper_1110_0899_b200 import build as cuda_build
+            os.environ["WOLFF_B200_LIB"] = cuda_build.build(profile=True)      # before the binding is imported
+            print(json.dumps(run_profile_counters(args)), flush=True)
+        return 0
+    if args.a8:
+        if rank == 0:
+            print(json.dumps(run_a8(args)), flush=True)
         return 0
 
     if world > 1:
@@ -720,6 +874,9 @@ def main():
     if world > 1:
         import torch.distributed as dist
         dist.destroy_process_group()
+    if rank == 0 and not out["parity_all_legs"]["all_equal"]:
+        sys.stderr.write("bench: the oracle's cluster sizes differ from the kernel's inside a timed region\n")
+        return 1
     return 0
 
 

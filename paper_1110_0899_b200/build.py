@@ -13,6 +13,7 @@ LIB_NAME = "libwolff_b200.so"
 LIB_PATH = os.path.join(HERE, LIB_NAME)
 CHECKED_LIB_PATH = os.path.join(HERE, "libwolff_b200_checked.so")
 JITTER_LIB_PATH = os.path.join(HERE, "libwolff_b200_jitter.so")
+PROFILE_LIB_PATH = os.path.join(HERE, "libwolff_b200_profile.so")
 SOURCES = ["api.cu", "batch_api.cu", "growth.cu", "growth_batch.cu", "growth_cluster.cu", "growth_tiles.cu", "measure.cu", "microbench.cu", "noalloc.cu"]
 HEADERS = ["internal.h", "device_common.cuh", "expand.cuh", os.path.join(ROOT, "include", "wolff.h")]
 NVCC_COMPILE_FLAGS = [
@@ -42,7 +43,7 @@ def needs_build(lib_path: str = LIB_PATH) -> bool:
     return os.path.getmtime(lib_path) < max(os.path.getmtime(d) for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False, checked: bool = False, jitter: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, checked: bool = False, jitter: bool = False, profile: bool = False) -> str:
     """One nvcc per source file, side by side (the files share no device code, so there is no device link), then one
     link.  Objects are kept under paper_1110_0899_b200/build/ (git-ignored) and reused while they are newer than
     their source and every header.
@@ -50,8 +51,10 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False, jit
     checked=True builds libwolff_b200_checked.so with -DWOLFF_CHECKED (every queue, list, tile and bit-plane index is
     compared with its bound before use: device_common.cuh); load it with WOLFF_B200_LIB=<path> (binding.py).
     jitter=True builds libwolff_b200_jitter.so with -DWOLFF_CHECKED -DWOLFF_JITTER (random sleeps between the steps of the
-    lock-free protocols, device_common.cuh)."""
-    lib_path = JITTER_LIB_PATH if jitter else (CHECKED_LIB_PATH if checked else LIB_PATH)
+    lock-free protocols, device_common.cuh).
+    profile=True builds libwolff_b200_profile.so with -DWOLFF_PROFILE (cycle and pass counters inside the barrier-free growth
+    kernels, read through wolff_get_stats; `bench.py --profile-counters` prints them).  Never the measured path."""
+    lib_path = PROFILE_LIB_PATH if profile else (JITTER_LIB_PATH if jitter else (CHECKED_LIB_PATH if checked else LIB_PATH))
     if not force and not needs_build(lib_path):
         return lib_path
     nvcc = nvcc_path()
@@ -60,6 +63,8 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False, jit
         extra.append("-DWOLFF_CHECKED")
     if jitter:
         extra.append("-DWOLFF_JITTER")
+    if profile:
+        extra.append("-DWOLFF_PROFILE")
     os.makedirs(OBJ_DIR, exist_ok=True)
     tag = ("_" + "".join(c if c.isalnum() else "_" for c in " ".join(extra))) if extra else ""
     newest_header = max(os.path.getmtime(h) for h in _header_paths())
@@ -95,4 +100,5 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False, jit
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv, jitter="--jitter" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, checked="--checked" in sys.argv, jitter="--jitter" in sys.argv,
+                profile="--profile" in sys.argv))

@@ -129,12 +129,16 @@ __device__ __forceinline__ uint32_t merge4(uint32_t a, uint32_t b, uint32_t c, u
     return (a & kSignMask) | ((b & kSignMask) >> 1) | ((c & kSignMask) >> 2) | ((d & kSignMask) >> 3);
 }
 
-template <int DIM>
+// POW2: L is a power of two (>= 16), so the chunk's row and its position in the row are a shift and a mask instead of two
+// integer divisions per chunk and a third for z (profiles/r3_a8.md: at 1 GiB the divisions made the kernel issue-bound,
+// sm throughput 68 %, DRAM 35 %).
+template <int DIM, bool POW2>
 __global__ void __launch_bounds__(kThreads) energy_magnetisation_vec16(const int8_t *__restrict__ spins, Geometry g, Control *ctl,
                                                                        long long *E_dst, long long *M_dst)
 {
     const uint32_t chunks = g.N / 16u;
     const uint32_t chunks_per_row = g.L / 16u;
+    const uint32_t row_shift = POW2 ? g.logL - 4u : 0u;
     const uint32_t stride = gridDim.x * blockDim.x;
     unsigned long long unequal = 0, negative = 0;
     for (uint32_t c0 = blockIdx.x * blockDim.x + threadIdx.x; c0 < chunks; c0 += stride * kU) {
@@ -147,9 +151,9 @@ __global__ void __launch_bounds__(kThreads) energy_magnetisation_vec16(const int
             on[u] = c < chunks;
             const uint32_t cc = on[u] ? c : 0u;
             const uint32_t i = cc * 16u;
-            const uint32_t row = cc / chunks_per_row;          // y + L*z
+            const uint32_t row = POW2 ? cc >> row_shift : cc / chunks_per_row;      // y + L*z
             const uint32_t cx = cc - row * chunks_per_row;     // chunk index along x
-            const uint32_t y = (DIM == 3) ? row % g.L : row;
+            const uint32_t y = (DIM == 3) ? (POW2 ? row & (g.L - 1u) : row % g.L) : row;
             a[u] = *reinterpret_cast<const uint4 *>(spins + i);
             // +x: the 16 sites shifted by one byte; the 17th byte is the first site of the next chunk (wrapping)
             const uint32_t inext = (cx + 1u == chunks_per_row) ? i + 16u - g.L : i + 16u;
@@ -157,7 +161,7 @@ __global__ void __launch_bounds__(kThreads) energy_magnetisation_vec16(const int
             const uint32_t iy = (y + 1u == g.L) ? i - (g.LL - g.L) : i + g.L;
             by[u] = *reinterpret_cast<const uint4 *>(spins + iy);
             if (DIM == 3) {
-                const uint32_t z = row / g.L;
+                const uint32_t z = POW2 ? row >> g.logL : row / g.L;
                 const uint32_t iz = (z + 1u == g.L) ? i - (g.N - g.LL) : i + g.LL;
                 bz[u] = *reinterpret_cast<const uint4 *>(spins + iz);
             }
@@ -238,9 +242,16 @@ cudaError_t launch_energy_magnetisation(const int8_t *spins, const Geometry &geo
     if (geo.L % 16u == 0u) {
         // kU chunks in flight per thread, a few CTAs per SM (every CTA ends with two atomics on the same two words)
         // (measured on B200, 16 MiB, cold L2, ncu: 12.7 / 9.7 / 11.1 us with 2 / 4 / 8 CTAs per SM)
-        const int grid = grid_for((geo.N / 16u + kU - 1) / kU, num_sms, 4);
-        if (dim == 2) energy_magnetisation_vec16<2><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
-        else          energy_magnetisation_vec16<3><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
+        // lattices far beyond L2 (64 MiB and more) run long enough that the tail no longer matters and more loads in flight do:
+        // 8 CTAs per SM there (profiles/r3_a8.md)
+        const int grid = grid_for((geo.N / 16u + kU - 1) / kU, num_sms, geo.N >= (1u << 26) ? 8 : 4);
+        if (geo.pow2) {
+            if (dim == 2) energy_magnetisation_vec16<2, true><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
+            else          energy_magnetisation_vec16<3, true><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
+        } else {
+            if (dim == 2) energy_magnetisation_vec16<2, false><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
+            else          energy_magnetisation_vec16<3, false><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);
+        }
     } else {
         const int grid = grid_for(geo.N, num_sms, 8);
         if (dim == 2) energy_magnetisation_scalar<2><<<grid, kThreads, 0, stream>>>(spins, geo, ctl, E_dst, M_dst);

@@ -115,12 +115,14 @@ __device__ __forceinline__ uint32_t merge4(uint32_t a, uint32_t b, uint32_t c, u
 
 // L a multiple of 16: a 16-byte chunk never straddles a row.  CTA b takes chunks [1024 b, 1024 (b + 1)), thread t the
 // chunks 1024 b + t + 256 u, u = 0..3, all loads issued before any is used.
-template <int DIM>
-__global__ void __launch_bounds__(kThreads) noalloc_em_vec16(const int8_t *__restrict__ spins, uint32_t L, uint32_t N,
+// POW2: L = 2^logL (the host says so): rows and positions by shifts and masks instead of integer divisions.
+template <int DIM, bool POW2>
+__global__ void __launch_bounds__(kThreads) noalloc_em_vec16(const int8_t *__restrict__ spins, uint32_t L, uint32_t logL, uint32_t N,
                                                              unsigned long long *scratch, long long *E_dst, long long *M_dst)
 {
     constexpr int kU = (int)(kSitesPerCta / 16u) / kThreads;     // 4
     const uint32_t chunks = N / 16u, chunks_per_row = L / 16u, LL = L * L;
+    const uint32_t row_shift = POW2 ? logL - 4u : 0u;
     const uint32_t first = blockIdx.x * (kSitesPerCta / 16u) + threadIdx.x;
     uint4 a[kU], by[kU], bz[kU];
     uint32_t nb[kU];
@@ -131,15 +133,15 @@ __global__ void __launch_bounds__(kThreads) noalloc_em_vec16(const int8_t *__res
         on[u] = c < chunks;
         const uint32_t cc = on[u] ? c : 0u;
         const uint32_t i = cc * 16u;
-        const uint32_t row = cc / chunks_per_row;                // y + L z
+        const uint32_t row = POW2 ? cc >> row_shift : cc / chunks_per_row;       // y + L z
         const uint32_t cx = cc - row * chunks_per_row;
-        const uint32_t y = (DIM == 3) ? row % L : row;
+        const uint32_t y = (DIM == 3) ? (POW2 ? row & (L - 1u) : row % L) : row;
         a[u] = *reinterpret_cast<const uint4 *>(spins + i);
         // +x: the sixteen sites one byte on; the seventeenth is the first site of the next chunk, or of the row (wrap)
         nb[u] = (uint32_t)(uint8_t)spins[(cx + 1u == chunks_per_row) ? i + 16u - L : i + 16u];
         by[u] = *reinterpret_cast<const uint4 *>(spins + ((y + 1u == L) ? i - (LL - L) : i + L));
         if (DIM == 3) {
-            const uint32_t z = row / L;
+            const uint32_t z = POW2 ? row >> logL : row / L;
             bz[u] = *reinterpret_cast<const uint4 *>(spins + ((z + 1u == L) ? i - (N - LL) : i + LL));
         }
     }
@@ -274,8 +276,15 @@ extern "C" int wolff_energy_magnetisation_noalloc(const int8_t *spins_dev, int d
     const uint32_t n = (uint32_t)N, l = (uint32_t)L;
     const unsigned int grid = (unsigned int)((N + kSitesPerCta - 1u) / kSitesPerCta);       // <= kMaxCtas: one slot each
     if (L % 16 == 0) {
-        if (dim == 2) noalloc_em_vec16<2><<<grid, kThreads, 0, stream>>>(spins, l, n, scratch, E_dst, M_dst);
-        else          noalloc_em_vec16<3><<<grid, kThreads, 0, stream>>>(spins, l, n, scratch, E_dst, M_dst);
+        uint32_t logL = 0;
+        while ((1u << logL) < l) ++logL;
+        if ((1u << logL) == l) {
+            if (dim == 2) noalloc_em_vec16<2, true><<<grid, kThreads, 0, stream>>>(spins, l, logL, n, scratch, E_dst, M_dst);
+            else          noalloc_em_vec16<3, true><<<grid, kThreads, 0, stream>>>(spins, l, logL, n, scratch, E_dst, M_dst);
+        } else {
+            if (dim == 2) noalloc_em_vec16<2, false><<<grid, kThreads, 0, stream>>>(spins, l, 0u, n, scratch, E_dst, M_dst);
+            else          noalloc_em_vec16<3, false><<<grid, kThreads, 0, stream>>>(spins, l, 0u, n, scratch, E_dst, M_dst);
+        }
     } else {
         if (dim == 2) noalloc_em_scalar<2><<<grid, kThreads, 0, stream>>>(spins, l, n, scratch, E_dst, M_dst);
         else          noalloc_em_scalar<3><<<grid, kThreads, 0, stream>>>(spins, l, n, scratch, E_dst, M_dst);
