@@ -40,5 +40,5 @@ def pytest_collection_finish(session):
     if names:
         import protocol_farm
         # longest first: the pool runs them all at once, but start order decides who gets a core first on a small box
-        order = ["C3", "C3-stretch", "C5a", "C2", "C4", "C5b", "C5b-literal", "C2-literal"]
+        order = ["C3", "C3-stretch", "C5a", "C2", "C4", "C5b", "C5b-literal", "C2-literal", "C3-literal", "C4-literal", "C5a-literal"]
         protocol_farm.start([n for n in order if n in names])

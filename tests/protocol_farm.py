@@ -34,6 +34,11 @@ JOBS = {
     "C5b": dict(cfg="C5b", seed=None, cold=True, batches=[1000, 10000], stretch=0),
     "C5b-literal": dict(cfg="C5b", seed=None, cold=False, batches=[1000, 10000], stretch=0),
     "C2-literal": dict(cfg="C2", seed=None, cold=False, batches=[1000, 10000], stretch=0),
+    # BASELINE.json's configs 3-5 exactly as written (random start from the seed, 1,000 + 10,000 updates): the clusters
+    # stay at a handful of spins, so the oracle needs about a second per chain
+    "C3-literal": dict(cfg="C3", seed=None, cold=False, batches=[1000, 10000], stretch=0),
+    "C4-literal": dict(cfg="C4", seed=None, cold=False, batches=[1000, 10000], stretch=0),
+    "C5a-literal": dict(cfg="C5a", seed=None, cold=False, batches=[1000, 10000], stretch=0),
 }
 
 _lock = threading.Lock()

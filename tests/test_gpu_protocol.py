@@ -8,6 +8,10 @@ compared with the oracle after each batch: the regime the bench times (T_c-sized
 double-buffered across thousands of updates, 148 CTAs x 28 tile slots).  The oracle chains are computed by
 tests/protocol_farm.py in background threads while the other GPU tests run.
 """
+import hashlib
+import json
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -43,7 +47,7 @@ def check_batch(gpu, c, b, what, lattice_dev):
     assert gpu.update_index == b["u"]
 
 
-@pytest.mark.parametrize("name", ["C2", "C4", "C5b", "C5b-literal", "C2-literal", "C5a", "C3"])
+@pytest.mark.parametrize("name", ["C2", "C4", "C5b", "C5b-literal", "C2-literal", "C3-literal", "C4-literal", "C5a-literal", "C5a", "C3"])
 def test_protocol_batches(name):
     gpu, c = open_chain(name)
     stream = torch.cuda.Stream()
@@ -75,4 +79,53 @@ def test_protocol_energy_and_magnetisation_after_every_update(name):
         assert (E, M) == (int(st["E"][k]), int(st["M"][k])), "E/M differ at stretch update %d" % k
     assert np.array_equal(farm.pack(gpu.get_spins()), st["bits"])
     assert gpu.update_index == st["u"]
+    gpu.close()
+
+
+# ------------------------------------------------------------------ the whole protocol, and the region bench.py times
+# tests/golden/protocol_digests.json is written by tests/golden/make_protocol_digests.py from the oracle alone: the
+# equilibrated chains (cold start) of C3, C5a and C2 over run(1000) + 24 x run(500) = updates 0 .. 12,999, which contains
+# BASELINE.json's 1,000 + 10,000 and the updates bench.py times (2,500 .. 12,499 with its 3 warm-up steps), in the
+# bench's launch shape.  After every launch: E, M, the update index, the sum and the SHA-256 of the launch's cluster
+# sizes, the SHA-256 of the lattice as one bit per spin.
+DIGESTS_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "protocol_digests.json")
+
+
+def _digests():
+    with open(DIGESTS_PATH) as f:
+        return json.load(f)
+
+
+def _digest_chains():
+    """The chains the golden file holds (C3 takes the oracle about 1.5 hours of one host core; C5a and C2 minutes)."""
+    have = _digests() if os.path.exists(DIGESTS_PATH) else {}
+    return [name for name in ("C2", "C5a", "C3") if name in have]
+
+
+def test_the_golden_file_holds_the_secondary_headline_chain():
+    assert {"C2", "C5a"} <= set(_digest_chains())
+
+
+@pytest.mark.parametrize("chain", _digest_chains())
+def test_whole_protocol_against_the_oracle_digests(chain):
+    d = _digests()[chain]
+    c = wl.CONFIGS[chain]
+    assert (d["dim"], d["L"], d["J"], d["T"], d["seed"]) == (c.dim, c.L, c.J, c.T, c.seed)
+    assert len(d["batches"]) == len(d["checkpoints"]) and sum(d["batches"]) >= c.n_equil + c.n_meas
+    gpu = binding.Wolff(c.dim, c.L, c.J, c.T, c.seed)
+    assert gpu.threshold == d["threshold"]
+    gpu.set_spins(wl.cold(c.N))
+    stream = torch.cuda.Stream()
+    lattice_dev = torch.empty(c.N, dtype=torch.int8, device="cuda")
+    for k, (n, cp) in enumerate(zip(d["batches"], d["checkpoints"])):
+        what = "%s launch %d (updates %d..%d)" % (chain, k, cp["u"] - n, cp["u"] - 1)
+        gpu.run(n, stream=stream)                 # one persistent launch, as bench.py does
+        E, M, sz = gpu.observables(sizes=True)
+        assert int(sz.astype(np.int64).sum()) == cp["flipped"], what + ": flipped spins"
+        assert hashlib.sha256(np.ascontiguousarray(sz, dtype="<u4").tobytes()).hexdigest() == cp["sizes_sha256"], what + ": cluster sizes"
+        assert (E, M) == (cp["E"], cp["M"]), what + ": E/M"
+        gpu.get_spins_into(lattice_dev)
+        bits = np.packbits(lattice_dev.cpu().numpy().reshape(-1) > 0)
+        assert hashlib.sha256(bits.tobytes()).hexdigest() == cp["lattice_sha256"], what + ": lattice"
+        assert gpu.update_index == cp["u"], what
     gpu.close()
